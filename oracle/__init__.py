@@ -1,0 +1,315 @@
+"""Python face of the FP64 CPU oracle (TEST INFRASTRUCTURE, not the product).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+may import this package.  It never imports the CUDA package; the CUDA package never
+imports it.  The arithmetic of the SPH sums, gravity, keys and sort lives in
+sph_oracle.c; this file marshals arrays and writes out the O(N) formulas of the
+integration scheme (Eqs. 12-16) and the step sequence (DESIGN.md
+reading A11) in plain numpy FP64.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from dataclasses import dataclass
+
+import numpy as np
+
+from .build import build as _build
+
+_lib = None
+
+
+class _Grid(C.Structure):
+    _fields_ = [("origin", C.c_float * 3), ("cell", C.c_float), ("inv_cell", C.c_float), ("dims", C.c_int32 * 3)]
+
+
+class _Params(C.Structure):
+    _fields_ = [("h", C.c_double), ("gamma", C.c_double), ("alpha", C.c_double), ("beta", C.c_double),
+                ("eta", C.c_double)]
+
+
+@dataclass
+class Grid:
+    origin: tuple
+    cell: float
+    inv_cell: float
+    dims: tuple
+
+    @property
+    def M(self) -> int:
+        return int(self.dims[0]) * int(self.dims[1]) * int(self.dims[2])
+
+    def _c(self) -> _Grid:
+        g = _Grid()
+        for a in range(3):
+            g.origin[a] = self.origin[a]
+            g.dims[a] = self.dims[a]
+        g.cell = self.cell
+        g.inv_cell = self.inv_cell
+        return g
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build())
+        dp, fp, ip, up = (C.POINTER(C.c_double), C.POINTER(C.c_float), C.POINTER(C.c_int64), C.POINTER(C.c_uint32))
+        L.orc_num_threads.restype = C.c_int
+        L.orc_set_num_threads.argtypes = [C.c_int]
+        for f in (L.orc_W, L.orc_Wp, L.orc_dWp_dxi):
+            f.restype = C.c_double
+            f.argtypes = [C.c_double, C.c_double]
+        L.orc_gravity.argtypes = [dp, C.c_int64, C.c_double, C.c_double, ip, C.c_int64, dp]
+        L.orc_gravity.restype = None
+        L.orc_potential_energy.argtypes = [dp, C.c_int64, C.c_double, C.c_double]
+        L.orc_potential_energy.restype = C.c_double
+        L.orc_grid_from_bbox.argtypes = [dp, C.c_int64, C.c_float, C.POINTER(_Grid)]
+        L.orc_grid_from_bbox.restype = C.c_int
+        L.orc_cell_keys.argtypes = [dp, C.c_int64, C.POINTER(_Grid), up]
+        L.orc_cell_keys.restype = None
+        L.orc_counting_sort.argtypes = [up, C.c_int64, C.c_int64, up, up, up]
+        L.orc_counting_sort.restype = C.c_int
+        L.orc_rc2.argtypes = [C.c_float]
+        L.orc_rc2.restype = C.c_float
+        L.orc_neighbours_brute.argtypes = [dp, C.c_int64, C.c_float, ip, C.c_int64, up, ip, up]
+        L.orc_neighbours_brute.restype = None
+        L.orc_neighbours_grid.argtypes = [dp, C.c_int64, C.c_float, C.POINTER(_Grid), up, up, up, ip, C.c_int64,
+                                          up, ip, up]
+        L.orc_neighbours_grid.restype = None
+        L.orc_density.argtypes = [dp, C.c_double, ip, C.c_int64, ip, up, dp]
+        L.orc_density.restype = None
+        L.orc_forces.argtypes = [dp, dp, dp, C.POINTER(_Params), ip, C.c_int64, ip, up, dp]
+        L.orc_forces.restype = None
+        _lib = L
+    return _lib
+
+
+def _p(a, ct):
+    return a.ctypes.data_as(C.POINTER(ct)) if a is not None else None
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _tg(targets):
+    if targets is None:
+        return None
+    return np.ascontiguousarray(targets, dtype=np.int64)
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().orc_set_num_threads(int(n))
+
+
+# ------------------------------------------------------------------ kernels (Eqs. 8, 9)
+def W(xi, h):
+    return float(lib().orc_W(float(xi), float(h)))
+
+
+def Wp(xi, h):
+    return float(lib().orc_Wp(float(xi), float(h)))
+
+
+def dWp_dxi(xi, h):
+    return float(lib().orc_dWp_dxi(float(xi), float(h)))
+
+
+# ------------------------------------------------------------------ gravity (Eq. 4)
+def gravity(posm, G, delta, targets=None):
+    """a^g for `targets` (default all) against all N sources; returns float64 [nt,3]."""
+    posm = _f64(posm)
+    n = posm.shape[0]
+    tg = _tg(targets)
+    nt = n if tg is None else len(tg)
+    out = np.zeros((nt, 3), dtype=np.float64)
+    if nt and n:
+        lib().orc_gravity(_p(posm, C.c_double), n, float(G), float(delta), _p(tg, C.c_int64), nt, _p(out, C.c_double))
+    return out
+
+
+def potential_energy(posm, G, delta) -> float:
+    posm = _f64(posm)
+    return float(lib().orc_potential_energy(_p(posm, C.c_double), posm.shape[0], float(G), float(delta)))
+
+
+# ------------------------------------------------------------------ grid sort (a1-a5)
+def grid_from_bbox(posm, n_gas, h) -> Grid:
+    posm = _f64(posm)
+    g = _Grid()
+    rc = lib().orc_grid_from_bbox(_p(posm, C.c_double), int(n_gas), np.float32(h), C.byref(g))
+    if rc != 0:
+        raise ValueError("grid_from_bbox: invalid grid (dimension > 4096, M >= 2^31 or no gas)")
+    return Grid(tuple(g.origin), float(g.cell), float(g.inv_cell), tuple(g.dims))
+
+
+def cell_keys(posm, n_gas, grid: Grid):
+    posm = _f64(posm)
+    key = np.zeros(int(n_gas), dtype=np.uint32)
+    if n_gas:
+        lib().orc_cell_keys(_p(posm, C.c_double), int(n_gas), C.byref(grid._c()), _p(key, C.c_uint32))
+    return key
+
+
+def counting_sort(key, M):
+    """Returns (count[M], start[M+1], perm[n]) — perm maps sorted slot -> original index, stable."""
+    key = np.ascontiguousarray(key, dtype=np.uint32)
+    count = np.zeros(M, dtype=np.uint32)
+    start = np.zeros(M + 1, dtype=np.uint32)
+    perm = np.zeros(len(key), dtype=np.uint32)
+    rc = lib().orc_counting_sort(_p(key, C.c_uint32), len(key), int(M), _p(count, C.c_uint32), _p(start, C.c_uint32),
+                                 _p(perm, C.c_uint32))
+    if rc != 0:
+        raise ValueError("counting_sort: key out of range")
+    return count, start, perm
+
+
+def rc2(h) -> np.float32:
+    return np.float32(lib().orc_rc2(np.float32(h)))
+
+
+# ------------------------------------------------------------------ neighbour sets (O2)
+def neighbours(posm, n_gas, h, targets=None, method="brute", grid=None, sort=None):
+    """CSR neighbour lists (offsets int64[nt+1], index uint32[...]), each list ascending in j, j != i.
+    method "brute": definition, O(nt * n_gas).  method "grid": the oracle's own 3x3x3 search."""
+    posm = _f64(posm)
+    tg = _tg(targets)
+    nt = int(n_gas) if tg is None else len(tg)
+    cnt = np.zeros(nt, dtype=np.uint32)
+    L = lib()
+    if method == "grid":
+        if grid is None:
+            grid = grid_from_bbox(posm, n_gas, h)
+        if sort is None:
+            key = cell_keys(posm, n_gas, grid)
+            _, start, perm = counting_sort(key, grid.M)
+        else:
+            key, start, perm = sort
+        gc = grid._c()
+
+        def call(c, off, idx):
+            L.orc_neighbours_grid(_p(posm, C.c_double), int(n_gas), np.float32(h), C.byref(gc), _p(key, C.c_uint32),
+                                  _p(start, C.c_uint32), _p(perm, C.c_uint32), _p(tg, C.c_int64), nt, _p(c, C.c_uint32),
+                                  _p(off, C.c_int64), _p(idx, C.c_uint32))
+    else:
+        def call(c, off, idx):
+            L.orc_neighbours_brute(_p(posm, C.c_double), int(n_gas), np.float32(h), _p(tg, C.c_int64), nt,
+                                   _p(c, C.c_uint32), _p(off, C.c_int64), _p(idx, C.c_uint32))
+    if nt:
+        call(cnt, None, None)
+    off = np.zeros(nt + 1, dtype=np.int64)
+    np.cumsum(cnt, out=off[1:])
+    idx = np.zeros(max(int(off[-1]), 1), dtype=np.uint32)
+    if nt and off[-1] > 0:
+        call(cnt, off, idx)
+    return off, idx[: int(off[-1])]
+
+
+# ------------------------------------------------------------------ SPH sums (Eqs. 7, 10, 11)
+def density(posm, h, offsets, index, targets=None):
+    posm = _f64(posm)
+    tg = _tg(targets)
+    nt = len(offsets) - 1
+    rho = np.zeros(nt, dtype=np.float64)
+    idx = np.ascontiguousarray(index, dtype=np.uint32)
+    if len(idx) == 0:
+        idx = np.zeros(1, dtype=np.uint32)
+    off = np.ascontiguousarray(offsets, dtype=np.int64)
+    if nt:
+        lib().orc_density(_p(posm, C.c_double), float(h), _p(tg, C.c_int64), nt, _p(off, C.c_int64), _p(idx, C.c_uint32),
+                          _p(rho, C.c_double))
+    return rho
+
+
+def forces(posm, vele, rho_all, h, offsets, index, targets=None, gamma=5.0 / 3.0, alpha=0.5, beta=1.0, eta=0.1):
+    """(ax, ay, az, de/dt) of Eqs. 10-11 (hydro part) for `targets`; rho_all indexed by gas index."""
+    posm, vele, rho_all = _f64(posm), _f64(vele), _f64(rho_all)
+    tg = _tg(targets)
+    nt = len(offsets) - 1
+    out = np.zeros((nt, 4), dtype=np.float64)
+    idx = np.ascontiguousarray(index, dtype=np.uint32)
+    if len(idx) == 0:
+        idx = np.zeros(1, dtype=np.uint32)
+    off = np.ascontiguousarray(offsets, dtype=np.int64)
+    prm = _Params(float(h), float(gamma), float(alpha), float(beta), float(eta))
+    if nt:
+        lib().orc_forces(_p(posm, C.c_double), _p(vele, C.c_double), _p(rho_all, C.c_double), C.byref(prm),
+                         _p(tg, C.c_int64), nt, _p(off, C.c_int64), _p(idx, C.c_uint32), _p(out, C.c_double))
+    return out
+
+
+# ------------------------------------------------------------------ whole evaluation / step (O6)
+@dataclass
+class State:
+    """Carried state of the scheme (reading A11): r, v, e and the position-only
+    quantities at the current r (rho, a_grav)."""
+    posm: np.ndarray      # float64 [N,4]
+    vele: np.ndarray      # float64 [N,4]
+    n_gas: int
+    rho: np.ndarray = None       # float64 [n_gas]
+    acc_grav: np.ndarray = None  # float64 [N,3]
+
+
+def _nbr(posm, n_gas, h, method):
+    if n_gas == 0:
+        return np.zeros(1, dtype=np.int64), np.zeros(0, dtype=np.uint32)
+    return neighbours(posm, n_gas, h, method=method)
+
+
+def position_only(state: State, h, G, delta, method="grid"):
+    """SP + DC + GFC at the current positions (the quantities that depend on r only, L123)."""
+    off, idx = _nbr(state.posm, state.n_gas, h, method)
+    state.rho = density(state.posm, h, off, idx)
+    state.acc_grav = gravity(state.posm, G, delta) if G != 0.0 else np.zeros((len(state.posm), 3))
+    return off, idx
+
+
+def hydro(state: State, h, nbr, **visc):
+    if state.n_gas == 0:
+        return np.zeros((0, 4))
+    off, idx = nbr
+    return forces(state.posm, state.vele, state.rho, h, off, idx, **visc)
+
+
+def step(state: State, dt, h, G, delta, nbr=None, method="grid", **visc):
+    """One predictor-corrector step, Eqs. 12-16 (L103-121), sequence of DESIGN.md A11:
+    HFC(pred) -> SU(pred) -> SP, DC, GFC at r(t+dt) -> HFC(corr) -> SU(corr).
+    `state` must carry rho and acc_grav at the current r (call position_only first);
+    `nbr` are the neighbour lists at the current r (recomputed if None).
+    Returns (new_state, nbr_new, diagnostics)."""
+    ng = state.n_gas
+    if nbr is None:
+        nbr = _nbr(state.posm, ng, h, method)
+    Q = state.acc_grav.copy()                                  # halo: Q_i = a^g_i
+    hy = hydro(state, h, nbr, **visc)                          # HFC(predictor) at (r, v, e, rho)(t)
+    Q[:ng] += hy[:, :3]
+    E = hy[:, 3] if ng else np.zeros(0)
+    v0 = state.vele[:, :3].copy()
+    e0 = state.vele[:ng, 3].copy()
+    v_t = v0 + dt * Q                                          # Eq. 12
+    e_t = e0 + dt * E                                          # Eq. 13
+    new = State(state.posm.copy(), state.vele.copy(), ng)
+    new.posm[:, :3] = state.posm[:, :3] + 0.5 * dt * (v_t + v0)   # Eq. 14
+    new.vele[:, :3] = v_t
+    new.vele[:ng, 3] = e_t
+    nbr1 = position_only(new, h, G, delta, method)             # density "refined" (L115), gravity once (L123)
+    Q1 = new.acc_grav.copy()
+    hy1 = hydro(new, h, nbr1, **visc)                          # HFC(corrector) at (r(t+dt), v~, e~, rho(t+dt))
+    Q1[:ng] += hy1[:, :3]
+    E1 = hy1[:, 3] if ng else np.zeros(0)
+    new.vele[:, :3] = 0.5 * (v0 + v_t) + 0.5 * dt * Q1         # Eq. 15
+    new.vele[:ng, 3] = 0.5 * (e0 + e_t) + 0.5 * dt * E1        # Eq. 16
+    diag = dict(hydro_pred=hy, hydro_corr=hy1, v_pred=v_t, e_pred=e_t)
+    return new, nbr1, diag
+
+
+def total_energy(state: State, G, delta) -> float:
+    """E = sum 1/2 m v^2 + sum_gas m e + U (pin P7)."""
+    m = state.posm[:, 3]
+    ke = 0.5 * np.sum(m * np.sum(state.vele[:, :3] ** 2, axis=1))
+    ie = np.sum(m[: state.n_gas] * state.vele[: state.n_gas, 3])
+    return float(ke + ie + (potential_energy(state.posm, G, delta) if G != 0.0 else 0.0))
