@@ -1,0 +1,174 @@
+/*
+ * sph_b200.h — C ABI of the B200-native (sm_100a) hot path of
+ * Khrapov & Khoperskov, "Smoothed-Particle Hydrodynamics Models: Implementation Features
+ * on GPUs" (arXiv 1807.08116).  Citations "Lnn" are lines of the paper text;
+ * "A<n>" are the readings listed in DESIGN.md.
+ *
+ * Conventions (all entry points)
+ *   - extern "C"; every function returns an int status (0 = SPH_OK, negative = error);
+ *     no exceptions, no aborts, no printing.
+ *   - Unless a parameter says HOST, every array argument is a DEVICE pointer owned by the
+ *     caller, 16-byte aligned.  The library never allocates or frees device memory inside
+ *     these calls: scratch comes from the caller's workspace `ws` (DEVICE, >= the size
+ *     sph_workspace_bytes() reports, 256-byte aligned).  Only the *_host entry points, which
+ *     take HOST arrays, allocate (and free) device memory themselves.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Work
+ *     is enqueued on it and the call returns without synchronising, except where stated.
+ *   - Particle order: gas first [0, n_gas), halo [n_gas, n_total)  (the paper sums SPH
+ *     over 1..N_g and gravity over 1..N, L74, L91).
+ *       posm[i] = (x, y, z, m)        float4
+ *       vele[i] = (vx, vy, vz, e)     float4   (e ignored for halo particles)
+ *     All outputs are in the caller's ORIGINAL particle order.
+ *   - n_gas = 0 (collisionless, L150) and n_halo = 0 are legal.  Inputs must be finite.
+ *   - Counts are int64_t at the boundary; n_gas and n_total must be < 2^31.
+ */
+#ifndef SPH_B200_H
+#define SPH_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    SPH_OK = 0,
+    SPH_ERR_ARG = -1,         /* null / misaligned pointer, negative count, non-positive h */
+    SPH_ERR_GRID = -2,        /* a grid dimension > 4096, M >= 2^31, or cell < 2h */
+    SPH_ERR_WORKSPACE = -3,   /* workspace (or output capacity) too small */
+    SPH_ERR_CUDA = -4,        /* CUDA launch / runtime failure; see sph_last_cuda_error() */
+    SPH_ERR_UNSUPPORTED = -5  /* e.g. delta < 0 */
+};
+
+/* Dense grid covering the computational domain (L158 "covered by a grid Mx x My x Mz").
+ * Reading A7: cell = fl(fl(2h)(1+2^-9)), inv_cell = fl(1/cell); a particle's cell coordinate is
+ *   ix = (int) min(max(floor(fl(fl(x - origin_x) * inv_cell)), 0), Mx-1)
+ * (two separate FP32 RN operations, clamp in float before the cast), and its cell number is
+ *   k = ix + Mx (iy + My iz)                                                          (L161). */
+typedef struct {
+    float origin[3];
+    float cell;
+    float inv_cell;
+    int32_t dims[3];
+} sph_grid;
+
+/* h: smoothing length (one global value, L82 with h_i = h);  gamma: adiabatic index (Eq. 5);
+ * alpha, beta, eta: artificial-viscosity constants (L99: 0.5, 1, 0.1);  G, delta: Eq. 4 (L47-49). */
+typedef struct {
+    float h, gamma, alpha, beta, eta;
+    float G, delta;
+} sph_params;
+
+/* cudaError_t of the last failing CUDA call seen by this library in the calling thread (0 if none). */
+int sph_last_cuda_error(void);
+
+/* Grid descriptor from the bounding box of the gas particles (A7): origin = component-wise
+ * minimum, dims = (int)(fl(fl(max - origin) * inv_cell)) + 1.  SYNCHRONISES `stream` (it
+ * returns a HOST struct).  ws: >= 4096 bytes.  Errors: SPH_ERR_ARG, SPH_ERR_GRID.            */
+int sph_grid_from_bbox(const float* posm, int64_t n_gas, float h, sph_grid* out_host /*HOST*/,
+                       void* ws, size_t ws_bytes, void* stream);
+
+/* Bytes of workspace that any call below needs for these sizes (g may be NULL when n_gas = 0). */
+size_t sph_workspace_bytes(int64_t n_gas, int64_t n_total, const sph_grid* g /*HOST*/);
+
+/* (a1-a4) Grid sort, L158-173: per-particle cell number (indexPC[i].x), per-cell count
+ * (CellSPH[k].x), exclusive prefix cell_start[k] = CellSPH[k-1].y with cell_start[M] = n_gas
+ * (A13), and perm = indexPC[.].y : sorted slot -> original index.  Unlike the paper's atomic
+ * scatter (L204) the order inside a cell is STABLE (ascending original index, A16) and the
+ * whole result is deterministic.
+ *   key[n_gas], perm[n_gas], cell_count[M], cell_start[M+1]  — uint32, all written.          */
+int sph_build_grid(const float* posm, int64_t n_gas, const sph_grid* g /*HOST*/,
+                   uint32_t* key, uint32_t* perm, uint32_t* cell_count, uint32_t* cell_start,
+                   void* ws, size_t ws_bytes, void* stream);
+
+/* (a5) Ranges the neighbour loops of DC / HFC walk (L207):
+ *   cell_range[k]      = (start, end) of cell k in sorted order = (CellSPH[k-1].y, CellSPH[k].y) (L160, L203);
+ *   particle_runs[i][r] = (start, end) of the r-th x-run (r = (dy+1) + 3 (dz+1), dy,dz in -1..1)
+ *                         of the 3x3x3 stencil of ORIGINAL particle i: the three x-adjacent
+ *                         cells of a stencil row are contiguous in sorted order, so 9 runs cover
+ *                         the 27 cells; rows outside the grid give (0,0).
+ * Either output may be NULL.  Layout: uint32 pairs.                                          */
+int sph_neighbour_ranges(const sph_grid* g /*HOST*/, const uint32_t* key, const uint32_t* cell_start,
+                         int64_t n_gas, uint32_t* cell_range /*[M][2]*/, uint32_t* particle_runs /*[n_gas][9][2]*/,
+                         void* stream);
+
+/* (a6-a7) Density, Eq. 7 (L74) with the cubic spline of Eq. 8 (L79), self term included (A5):
+ *   rho_i = sum_{j gas, |r_ij| < 2h} m_j W(|r_ij|/h, h).   Cutoff predicate in FP32 (A8):
+ *   d2 = fma(dz,dz, fma(dy,dy, dx*dx)) < fl(fl(2h)^2).
+ * perm / cell_start are the outputs of sph_build_grid for the same posm and g.                */
+int sph_density(const float* posm, int64_t n_gas, const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/,
+                const uint32_t* perm, const uint32_t* cell_start, float* rho /*[n_gas]*/,
+                void* ws, size_t ws_bytes, void* stream);
+
+/* (a8-a9) Hydrodynamic force and energy rate, Eqs. 10-11 (L91-93) hydro part, with
+ * W_p of Eq. 9 (L86), Pi_ij and the Monaghan viscosity of L95-99 (A2: p_j/rho_j^2), EOS Eq. 5:
+ *   acc_sph[i] = (a_x, a_y, a_z, de/dt).   A coincident pair contributes nothing (A9).        */
+int sph_forces(const float* posm, const float* vele, const float* rho, int64_t n_gas,
+               const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/,
+               const uint32_t* perm, const uint32_t* cell_start, float* acc_sph /*[n_gas][4]*/,
+               void* ws, size_t ws_bytes, void* stream);
+
+/* (a10) Direct Particle-Particle gravity, Eq. 4 (L47) with Plummer softening (A1):
+ *   acc_grav[i] = -G sum_{j=1..N} m_j (r_i - r_j) / (|r_i - r_j|^2 + delta^2)^(3/2), w = 0.
+ * delta >= 0; with delta = 0 coincident pairs contribute 0.                                   */
+int nbody_pp_gravity(const float* posm, int64_t n_total, float G, float delta,
+                     float* acc_grav /*[n_total][4]*/, void* ws, size_t ws_bytes, void* stream);
+
+/* (a1-a11) One predictor-corrector "leapfrog" step, Eqs. 12-16 (L103-121), in the order
+ * HFC(pred) -> SU(pred) -> SP, DC, GFC at r(t+dt) -> HFC(corr) -> SU(corr)   (A11; gravity once
+ * per step, L123).  posm / vele are updated in place.  rho[n_gas], acc_sph[n_gas][4],
+ * acc_grav[n_total][4] and the grid arrays inside `ws` are CARRIED STATE between calls: the
+ * caller must not modify them, must pass the same buffers, and must pass first != 0 on the first
+ * call (or after changing posm by hand), which evaluates SP, DC, GFC at the current positions
+ * before stepping.  On return rho / acc_grav hold the values at the new positions and acc_sph
+ * the corrector's hydro terms.  The grid `g` is an input (fixed domain, L158); particles
+ * outside it are clamped into boundary cells, which keeps the search correct.                */
+int sph_step(float* posm, float* vele, int64_t n_gas, int64_t n_halo, const sph_params* p /*HOST*/,
+             const sph_grid* g /*HOST*/, float dt, int first,
+             float* rho, float* acc_sph, float* acc_grav, void* ws, size_t ws_bytes, void* stream);
+
+/* Force evaluation only (call stack (2) of DESIGN.md): SP, DC, GFC, HFC at the current state;
+ * fills rho, acc_sph, acc_grav and leaves the carried state valid for sph_step(first = 0).   */
+int sph_evaluate(const float* posm, const float* vele, int64_t n_gas, int64_t n_halo,
+                 const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/,
+                 float* rho, float* acc_sph, float* acc_grav, void* ws, size_t ws_bytes, void* stream);
+
+/* End-to-end entry point with HOST buffers: copies posm / vele to the device, derives the grid
+ * from the gas bounding box, runs `n_steps` steps (first = 1 on the first), copies posm, vele,
+ * rho, acc_sph, acc_grav back (any output pointer may be NULL) and synchronises.  Allocates and
+ * frees its own device memory.  All pointers HOST.                                           */
+int sph_step_host(float* posm /*HOST*/, float* vele /*HOST*/, int64_t n_gas, int64_t n_halo,
+                  const sph_params* p /*HOST*/, float dt, int n_steps,
+                  float* rho /*HOST*/, float* acc_sph /*HOST*/, float* acc_grav /*HOST*/);
+
+/* Persistent variant of the above for repeated end-to-end calls: device buffers are created once. */
+typedef struct sph_host_ctx sph_host_ctx;
+int sph_host_ctx_create(int64_t n_gas, int64_t n_halo, sph_host_ctx** out /*HOST*/);
+int sph_host_ctx_step(sph_host_ctx* ctx, float* posm /*HOST*/, float* vele /*HOST*/, const sph_params* p /*HOST*/,
+                      float dt, int n_steps, float* rho /*HOST*/, float* acc_sph /*HOST*/, float* acc_grav /*HOST*/);
+int sph_host_ctx_destroy(sph_host_ctx* ctx);
+
+/* Test helper: explicit neighbour sets N(i) = { j gas, j != i, d2 < (2h)^2 } in CSR form, every
+ * list ascending in original index.  nbr_count[n_gas], nbr_offset[n_gas+1] are always written;
+ * nbr_index only if nbr_capacity >= nbr_offset[n_gas], else SPH_ERR_WORKSPACE is returned and
+ * nbr_offset[n_gas] tells the needed capacity.  SYNCHRONISES `stream`.                        */
+int sph_neighbour_lists(const float* posm, int64_t n_gas, float h, const sph_grid* g /*HOST*/,
+                        const uint32_t* perm, const uint32_t* cell_start,
+                        uint32_t* nbr_count, uint64_t* nbr_offset, uint32_t* nbr_index, uint64_t nbr_capacity,
+                        void* ws, size_t ws_bytes, void* stream);
+
+/* Stage timing of the most recent sph_step / sph_evaluate on this thread when profiling was
+ * switched on with sph_set_profiling(1): milliseconds by CUDA events on the call's stream for
+ * {sort (a1-a6), density (a7), forces (a8-a9, summed over calls), gravity (a10), update (a11)}.
+ * Reading the times SYNCHRONISES.  Profiling adds event records only.                        */
+int sph_set_profiling(int on);
+int sph_get_stage_ms(float out_ms[5] /*HOST*/);
+
+/* Number of kernel launches this library has enqueued in the calling process since load. */
+int64_t sph_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPH_B200_H */

@@ -1,0 +1,261 @@
+// api.cu — the extern "C" boundary declared in include/sph_b200.h: argument checks, workspace
+// carving, stage sequencing and optional per-stage CUDA-event timing.  No arithmetic of the method.
+#include "common.cuh"
+
+using namespace sphb;
+
+namespace {
+
+// ---- per-stage timing (sph_set_profiling) -------------------------------------------------------
+enum Stage { ST_SORT = 0, ST_DENSITY, ST_FORCES, ST_GRAVITY, ST_UPDATE, ST_COUNT };
+constexpr int kMaxSpans = 16;
+struct Prof {
+    bool on = false;
+    cudaEvent_t ev[2 * kMaxSpans];
+    bool made = false;
+    int n = 0;
+    int stage[kMaxSpans];
+};
+thread_local Prof g_prof;
+
+struct Span {
+    cudaStream_t st;
+    int idx = -1;
+    Span(int stage, cudaStream_t s) : st(s) {
+        Prof& p = g_prof;
+        if (!p.on || p.n >= kMaxSpans) return;
+        if (!p.made) {
+            for (auto& e : p.ev) cudaEventCreate(&e);
+            p.made = true;
+        }
+        idx = p.n++;
+        p.stage[idx] = stage;
+        cudaEventRecord(p.ev[2 * idx], st);
+    }
+    ~Span() {
+        if (idx >= 0) cudaEventRecord(g_prof.ev[2 * idx + 1], st);
+    }
+};
+
+bool bad_count(int64_t n) { return n < 0 || n >= (1ll << 31); }
+
+int check_params(const sph_params* p, bool need_h) {
+    if (!p) return SPH_ERR_ARG;
+    if (need_h && !(p->h > 0.f)) return SPH_ERR_ARG;
+    if (p->delta < 0.f) return SPH_ERR_UNSUPPORTED;
+    return SPH_OK;
+}
+
+// SP + DC + GFC at the current positions: everything that depends on r only (L123, A11)
+int position_only(const float4* posm, int64_t n_gas, int64_t n_total, const sph_params* p, const sph_grid* g,
+                  float* rho, float4* acc_grav, const Workspace& w, cudaStream_t st) {
+    if (n_gas > 0) {
+        {
+            Span sp(ST_SORT, st);
+            SPHB_TRY(grid_build(posm, n_gas, g, w.key, w.perm, w.cell_count, w.cell_start, w.rank_u, w.tmp, w.tile_sums,
+                                w.posm_s, st));
+        }
+        {
+            Span sp(ST_DENSITY, st);
+            SPHB_TRY(density_sorted(w.posm_s, w.perm, w.cell_start, n_gas, p, g, rho, st));
+        }
+    }
+    {
+        Span sp(ST_GRAVITY, st);
+        SPHB_TRY(gravity(posm, n_total, p->G, p->delta, acc_grav, w.src_pk, w.grav_part, st));
+    }
+    return SPH_OK;
+}
+
+int hydro(const float4* vele, const float* rho, int64_t n_gas, const sph_params* p, const sph_grid* g, float4* acc_sph,
+          const Workspace& w, cudaStream_t st) {
+    if (n_gas <= 0) return SPH_OK;
+    Span sp(ST_FORCES, st);
+    return forces_sorted(w.posm_s, vele, rho, w.perm, w.cell_start, n_gas, p, g, w.velr_s, w.pc_s, acc_sph, st);
+}
+
+int check_state_args(const void* posm, const void* vele, int64_t n_gas, int64_t n_halo, const sph_params* p,
+                     const sph_grid* g, const void* rho, const void* acc_sph, const void* acc_grav, void* ws,
+                     size_t ws_bytes) {
+    if (bad_count(n_gas) || bad_count(n_halo) || bad_count(n_gas + n_halo)) return SPH_ERR_ARG;
+    SPHB_TRY(check_params(p, n_gas > 0));
+    if (n_gas + n_halo > 0 && (!posm || !vele || !acc_grav || !aligned16(posm) || !aligned16(vele) || !aligned16(acc_grav)))
+        return SPH_ERR_ARG;
+    if (n_gas > 0) {
+        if (!rho || !acc_sph || !aligned16(acc_sph)) return SPH_ERR_ARG;
+        SPHB_TRY(check_grid(g, p->h));
+    }
+    if (!ws || (reinterpret_cast<uintptr_t>(ws) & 255u)) return SPH_ERR_ARG;
+    if (ws_bytes < carve(nullptr, n_gas, n_gas + n_halo, n_gas > 0 ? g : nullptr).bytes) return SPH_ERR_WORKSPACE;
+    return SPH_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int sph_last_cuda_error(void) { return g_last_cuda_error; }
+int64_t sph_launch_count(void) { return g_launch_count; }
+
+int sph_set_profiling(int on) {
+    g_prof.on = on != 0;
+    g_prof.n = 0;
+    return SPH_OK;
+}
+
+int sph_get_stage_ms(float out_ms[5]) {
+    if (!out_ms) return SPH_ERR_ARG;
+    for (int s = 0; s < ST_COUNT; ++s) out_ms[s] = 0.f;
+    Prof& p = g_prof;
+    for (int i = 0; i < p.n; ++i) {
+        SPHB_CUDA(cudaEventSynchronize(p.ev[2 * i + 1]));
+        float ms = 0.f;
+        SPHB_CUDA(cudaEventElapsedTime(&ms, p.ev[2 * i], p.ev[2 * i + 1]));
+        out_ms[p.stage[i]] += ms;
+    }
+    return SPH_OK;
+}
+
+size_t sph_workspace_bytes(int64_t n_gas, int64_t n_total, const sph_grid* g) {
+    if (bad_count(n_gas) || bad_count(n_total) || n_gas > n_total) return 0;
+    if (n_gas > 0 && (!g || check_grid(g, 0.f) != SPH_OK)) return 0;
+    size_t b = carve(nullptr, n_gas, n_total, n_gas > 0 ? g : nullptr).bytes;
+    return b < 4096 ? 4096 : b;
+}
+
+int sph_grid_from_bbox(const float* posm, int64_t n_gas, float h, sph_grid* out, void* ws, size_t ws_bytes,
+                       void* stream) {
+    if (!posm || !out || !ws || n_gas <= 0 || bad_count(n_gas) || !(h > 0.f) || !aligned16(posm)) return SPH_ERR_ARG;
+    if (ws_bytes < 8 * sizeof(float)) return SPH_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    float* bb = static_cast<float*>(ws);
+    SPHB_TRY(bbox_gas(reinterpret_cast<const float4*>(posm), n_gas, bb, st));
+    float host[6];
+    SPHB_CUDA(cudaMemcpyAsync(host, bb, sizeof(host), cudaMemcpyDeviceToHost, st));
+    SPHB_CUDA(cudaStreamSynchronize(st));
+    // A7, FP32 with one rounding per operation (volatile keeps the host compiler from fusing)
+    volatile float two_h = 2.0f * h;
+    volatile float cell = two_h * 1.001953125f;   // 1 + 2^-9
+    volatile float inv = 1.0f / cell;
+    double m = 1.0;
+    for (int a = 0; a < 3; ++a) {
+        volatile float ext = host[3 + a] - host[a];
+        volatile float c = ext * inv;
+        if (!(c < 4096.0f)) return SPH_ERR_GRID;
+        out->origin[a] = host[a];
+        out->dims[a] = (int32_t)c + 1;
+        if (out->dims[a] > 4096) return SPH_ERR_GRID;
+        m *= out->dims[a];
+    }
+    if (m >= 2147483648.0) return SPH_ERR_GRID;
+    out->cell = cell;
+    out->inv_cell = inv;
+    return SPH_OK;
+}
+
+int sph_build_grid(const float* posm, int64_t n_gas, const sph_grid* g, uint32_t* key, uint32_t* perm,
+                   uint32_t* cell_count, uint32_t* cell_start, void* ws, size_t ws_bytes, void* stream) {
+    if (bad_count(n_gas) || !g || !cell_count || !cell_start || !ws) return SPH_ERR_ARG;
+    if (n_gas > 0 && (!posm || !key || !perm || !aligned16(posm))) return SPH_ERR_ARG;
+    SPHB_TRY(check_grid(g, 0.f));
+    if (reinterpret_cast<uintptr_t>(ws) & 255u) return SPH_ERR_ARG;
+    Workspace w = carve(ws, n_gas, n_gas, g);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    Span sp(ST_SORT, st);
+    return grid_build(reinterpret_cast<const float4*>(posm), n_gas, g, key, perm, cell_count, cell_start, w.rank_u, w.tmp,
+                      w.tile_sums, nullptr, st);
+}
+
+int sph_density(const float* posm, int64_t n_gas, const sph_params* p, const sph_grid* g, const uint32_t* perm,
+                const uint32_t* cell_start, float* rho, void* ws, size_t ws_bytes, void* stream) {
+    if (bad_count(n_gas)) return SPH_ERR_ARG;
+    SPHB_TRY(check_params(p, true));
+    if (n_gas == 0) return SPH_OK;
+    if (!posm || !perm || !cell_start || !rho || !ws || !aligned16(posm) || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return SPH_ERR_ARG;
+    SPHB_TRY(check_grid(g, p->h));
+    Workspace w = carve(ws, n_gas, n_gas, g);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
+    Span sp(ST_DENSITY, st);
+    return density_sorted(w.posm_s, perm, cell_start, n_gas, p, g, rho, st);
+}
+
+int sph_forces(const float* posm, const float* vele, const float* rho, int64_t n_gas, const sph_params* p,
+               const sph_grid* g, const uint32_t* perm, const uint32_t* cell_start, float* acc_sph, void* ws,
+               size_t ws_bytes, void* stream) {
+    if (bad_count(n_gas)) return SPH_ERR_ARG;
+    SPHB_TRY(check_params(p, true));
+    if (n_gas == 0) return SPH_OK;
+    if (!posm || !vele || !rho || !perm || !cell_start || !acc_sph || !ws || !aligned16(posm) || !aligned16(vele) ||
+        !aligned16(acc_sph) || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return SPH_ERR_ARG;
+    SPHB_TRY(check_grid(g, p->h));
+    Workspace w = carve(ws, n_gas, n_gas, g);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
+    Span sp(ST_FORCES, st);
+    return forces_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, perm, cell_start, n_gas, p, g, w.velr_s,
+                         w.pc_s, reinterpret_cast<float4*>(acc_sph), st);
+}
+
+int nbody_pp_gravity(const float* posm, int64_t n_total, float G, float delta, float* acc_grav, void* ws,
+                     size_t ws_bytes, void* stream) {
+    if (bad_count(n_total)) return SPH_ERR_ARG;
+    if (delta < 0.f) return SPH_ERR_UNSUPPORTED;
+    if (n_total == 0) return SPH_OK;
+    if (!posm || !acc_grav || !ws || !aligned16(posm) || !aligned16(acc_grav) || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return SPH_ERR_ARG;
+    Workspace w = carve(ws, 0, n_total, nullptr);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    Span sp(ST_GRAVITY, st);
+    return gravity(reinterpret_cast<const float4*>(posm), n_total, G, delta, reinterpret_cast<float4*>(acc_grav), w.src_pk,
+                   w.grav_part, st);
+}
+
+int sph_evaluate(const float* posm, const float* vele, int64_t n_gas, int64_t n_halo, const sph_params* p,
+                 const sph_grid* g, float* rho, float* acc_sph, float* acc_grav, void* ws, size_t ws_bytes,
+                 void* stream) {
+    SPHB_TRY(check_state_args(posm, vele, n_gas, n_halo, p, g, rho, acc_sph, acc_grav, ws, ws_bytes));
+    const int64_t n = n_gas + n_halo;
+    if (n == 0) return SPH_OK;
+    g_prof.n = 0;
+    Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
+    cudaStream_t st = (cudaStream_t)stream;
+    SPHB_TRY(position_only(reinterpret_cast<const float4*>(posm), n_gas, n, p, g, rho, reinterpret_cast<float4*>(acc_grav),
+                           w, st));
+    return hydro(reinterpret_cast<const float4*>(vele), rho, n_gas, p, g, reinterpret_cast<float4*>(acc_sph), w, st);
+}
+
+int sph_step(float* posm, float* vele, int64_t n_gas, int64_t n_halo, const sph_params* p, const sph_grid* g, float dt,
+             int first, float* rho, float* acc_sph, float* acc_grav, void* ws, size_t ws_bytes, void* stream) {
+    SPHB_TRY(check_state_args(posm, vele, n_gas, n_halo, p, g, rho, acc_sph, acc_grav, ws, ws_bytes));
+    const int64_t n = n_gas + n_halo;
+    if (n == 0) return SPH_OK;
+    g_prof.n = 0;
+    Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
+    cudaStream_t st = (cudaStream_t)stream;
+    float4* r4 = reinterpret_cast<float4*>(posm);
+    float4* v4 = reinterpret_cast<float4*>(vele);
+    float4* as4 = reinterpret_cast<float4*>(acc_sph);
+    float4* ag4 = reinterpret_cast<float4*>(acc_grav);
+    if (first) SPHB_TRY(position_only(r4, n_gas, n, p, g, rho, ag4, w, st));   // seed the carried state
+    SPHB_TRY(hydro(v4, rho, n_gas, p, g, as4, w, st));                          // HFC(predictor)
+    {
+        Span sp(ST_UPDATE, st);
+        SPHB_TRY(update_predictor(r4, v4, w.vele0, as4, ag4, n_gas, n, dt, st));   // SU(predictor): Eqs. 12-14
+    }
+    SPHB_TRY(position_only(r4, n_gas, n, p, g, rho, ag4, w, st));               // SP, DC, GFC at r(t+dt)
+    SPHB_TRY(hydro(v4, rho, n_gas, p, g, as4, w, st));                          // HFC(corrector)
+    {
+        Span sp(ST_UPDATE, st);
+        SPHB_TRY(update_corrector(v4, w.vele0, as4, ag4, n_gas, n, dt, st));       // SU(corrector): Eqs. 15-16
+    }
+    return SPH_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,103 @@
+// common.cuh — internal declarations shared by the CUDA translation units of libsph_b200.
+// Nothing here is visible at the C boundary (include/sph_b200.h) and nothing here is shared
+// with the oracle.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/sph_b200.h"
+
+namespace sphb {
+
+// ---- error plumbing ---------------------------------------------------------------------
+extern thread_local int g_last_cuda_error;
+extern long long g_launch_count;   // kernels enqueued by this library (sph_launch_count)
+
+inline int cuda_fail(cudaError_t e) {
+    g_last_cuda_error = (int)e;
+    return SPH_ERR_CUDA;
+}
+#define SPHB_CUDA(call)                                         \
+    do {                                                        \
+        cudaError_t e__ = (call);                               \
+        if (e__ != cudaSuccess) return ::sphb::cuda_fail(e__);  \
+    } while (0)
+// after a kernel launch: count it and surface launch-configuration errors
+#define SPHB_LAUNCHED()                                         \
+    do {                                                        \
+        ++::sphb::g_launch_count;                               \
+        cudaError_t e__ = cudaGetLastError();                   \
+        if (e__ != cudaSuccess) return ::sphb::cuda_fail(e__);  \
+    } while (0)
+#define SPHB_TRY(call)                 \
+    do {                               \
+        int rc__ = (call);             \
+        if (rc__ != SPH_OK) return rc__; \
+    } while (0)
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+inline size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+int num_sms();
+
+// ---- grid descriptor as the kernels see it -----------------------------------------------
+struct GridDev {
+    float ox, oy, oz, inv_cell;
+    int mx, my, mz;
+    float fx, fy, fz;   // (float)(M-1) per axis, the float clamp bound of reading A7
+};
+inline int64_t grid_cells(const sph_grid* g) { return (int64_t)g->dims[0] * g->dims[1] * g->dims[2]; }
+int check_grid(const sph_grid* g, float h);          // SPH_OK or SPH_ERR_GRID
+GridDev to_dev(const sph_grid* g);
+
+// ---- workspace layout (device scratch carved from the caller's ws) -------------------------
+struct Workspace {
+    // grid sort
+    uint32_t* key;         // [n_gas]   cell number of original particle i
+    uint32_t* rank_u;      // [n_gas]   unstable in-cell rank from the histogram atomics
+    uint32_t* tmp;         // [n_gas]   unstable scatter (original indices, cell order)
+    uint32_t* perm;        // [n_gas]   stable permutation: sorted slot -> original index
+    uint32_t* cell_count;  // [M]
+    uint32_t* cell_start;  // [M+1]
+    uint32_t* tile_sums;   // [n_scan_tiles + 1]
+    // sorted (cell-order) particle data
+    float4* posm_s;        // [n_gas] (x,y,z,m)
+    float4* velr_s;        // [n_gas] (vx,vy,vz,rho)
+    float2* pc_s;          // [n_gas] (p/rho^2, c)
+    // gravity
+    float4* src_pk;        // [n_pad] packed source pairs
+    float4* grav_part;     // [S][n_total] partial accelerations
+    // integrator
+    float4* vele0;         // [n_total] v(t), e(t) saved by the predictor
+    // bbox scratch
+    float* bbox;           // [8]
+    size_t bytes;          // total
+};
+// Lays the arrays out behind `base` (may be NULL to just measure).  g may be NULL if n_gas == 0.
+Workspace carve(void* base, int64_t n_gas, int64_t n_total, const sph_grid* g);
+
+// gravity decomposition (shared by carve and the launcher)
+constexpr int kGravTileSrc = 2048;                 // sources per shared-memory stage
+int grav_splits(int64_t n_total);                  // S: number of j-chunks
+int64_t grav_padded(int64_t n_total);              // sources padded to a whole number of tiles
+
+// ---- internal stage entry points (all enqueue on `st`, no synchronisation) -----------------
+int grid_build(const float4* posm, int64_t n_gas, const sph_grid* g, uint32_t* key, uint32_t* perm,
+               uint32_t* cell_count, uint32_t* cell_start, uint32_t* rank_u, uint32_t* tmp, uint32_t* tile_sums,
+               float4* posm_s /*may be NULL*/, cudaStream_t st);
+int gather_sorted_pos(const float4* posm, const uint32_t* perm, int64_t n_gas, float4* posm_s, cudaStream_t st);
+int density_sorted(const float4* posm_s, const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas,
+                   const sph_params* p, const sph_grid* g, float* rho, cudaStream_t st);
+int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const uint32_t* perm,
+                  const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
+                  float4* velr_s, float2* pc_s, float4* acc_sph, cudaStream_t st);
+int gravity(const float4* posm, int64_t n_total, float G, float delta, float4* acc_grav,
+            float4* src_pk, float4* grav_part, cudaStream_t st);
+int update_predictor(float4* posm, float4* vele, float4* vele0, const float4* acc_sph, const float4* acc_grav,
+                     int64_t n_gas, int64_t n_total, float dt, cudaStream_t st);
+int update_corrector(float4* vele, const float4* vele0, const float4* acc_sph, const float4* acc_grav,
+                     int64_t n_gas, int64_t n_total, float dt, cudaStream_t st);
+int bbox_gas(const float4* posm, int64_t n_gas, float* bbox_dev /*[8]*/, cudaStream_t st);
+
+}  // namespace sphb

@@ -1,0 +1,296 @@
+// gravity.cu — (a10) direct Particle-Particle softened gravity, Eq. 4 under
+// reading A1:  a_i = -G sum_j m_j (r_i - r_j) / (|r_i - r_j|^2 + delta^2)^(3/2).
+//
+// Design for sm_100a.  The kernel is bound by the FP32 FMA pipe
+// (128 lanes/clk/SM), not by memory.  One interaction is 12 FP32 operations + 1 MUFU.RSQ:
+//   3 sub (dx,dy,dz)  3 fma (r2 = dx^2+dy^2+dz^2+delta^2)  1 rsqrt
+//   3 mul (u^2, m u, m u^3)  3 fma (a += s dx).
+// Written with scalar FFMA the loop is ISSUE-bound (13 slots per interaction, measured
+// 7.8 interactions/clk/SM); Blackwell's packed FP32 instructions (add/mul/fma.f32x2, SASS
+// FADD2/FMUL2/FFMA2) do two lane-operations per issue slot, which moves the bound to the FMA
+// pipe itself (measured 10.3 of the 10.67 interactions/clk/SM that 12 flops allow).  The two
+// halves of every packed register are two consecutive SOURCES (j, j+1) for the same target, so
+// no operand has to be duplicated per interaction: sources are pre-packed once per evaluation
+// as (x_j, x_j+1, y_j, y_j+1), (z_j, z_j+1, m_j, m_j+1), staged in shared memory in 32 KB tiles
+// by TMA bulk copies (cp.async.bulk + mbarrier, double-buffered) and read back as broadcast
+// LDS.128.  Each thread keeps I targets in registers.
+//
+// Accuracy: two-level accumulation.  Per 2048-source tile each thread sums into packed FP32
+// partials (even / odd sources), which are flushed into FP32 tile accumulators; the j range is
+// split into S chunks whose partial accelerations go to a [S][N] buffer that a last kernel adds
+// in fixed order (deterministic; also gives S x more CTAs than i-tiles, so the grid is many
+// waves deep on 148 SMs and the tail is < 2 %).
+#include "common.cuh"
+
+namespace sphb {
+
+typedef unsigned long long u64;
+
+__device__ __forceinline__ u64 pk2(float lo, float hi) {
+    u64 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk2(u64 v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
+    u64 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ u64 mul2(u64 a, u64 b) {
+    u64 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ u64 sub2(u64 a, u64 b) {
+    u64 r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ float rsqrt_approx(float x) {
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// ---- mbarrier / bulk-copy helpers (TMA 1-D bulk copy, SASS UBLKCP) ---------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "W: mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@!p bra W;\n\t}" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// ---- source packing -----------------------------------------------------------------------
+// pk[2q] = (x_2q, x_2q+1, y_2q, y_2q+1), pk[2q+1] = (z_2q, z_2q+1, m_2q, m_2q+1); sources past
+// n are padded with mass 0 at the origin (they add exactly 0 when delta > 0 and are masked by
+// the r2 > 0 select of the delta = 0 variant when they coincide with a target).
+__global__ void __launch_bounds__(256) grav_pack_sources(const float4* __restrict__ posm, int n, int n_pad,
+                                                         float4* __restrict__ pk) {
+    int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (2 * q >= n_pad) return;
+    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+    if (2 * q < n) a = posm[2 * q];
+    if (2 * q + 1 < n) b = posm[2 * q + 1];
+    pk[2 * q] = make_float4(a.x, b.x, a.y, b.y);
+    pk[2 * q + 1] = make_float4(a.z, b.z, a.w, b.w);
+}
+
+constexpr int kTilePairs = kGravTileSrc / 2;           // 1024 source pairs = 32 KB per stage
+constexpr int kTileBytes = kTilePairs * 32;
+constexpr int kStages = 2;
+
+// One CTA: THREADS*I targets (i-tile blockIdx.x) against the sources of chunk blockIdx.y.
+template <int I, int THREADS, int MINB, bool ZERO_SOFT>
+__global__ void __launch_bounds__(THREADS, MINB)
+    grav_pp_kernel(const float4* __restrict__ posm, const float4* __restrict__ pk, int n, int tiles_total,
+                   int tiles_per_chunk, float eps2, float4* __restrict__ part) {
+    extern __shared__ __align__(128) float4 tiles[];   // [kStages][2 * kTilePairs]
+    __shared__ __align__(8) uint64_t full_bar[kStages];
+
+    const int tid = threadIdx.x;
+    const int tile0 = blockIdx.y * tiles_per_chunk;
+    const int ntiles = min(tiles_per_chunk, tiles_total - tile0);
+    if (ntiles <= 0) return;   // uniform per CTA
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kStages; ++s) mbar_init(&full_bar[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kStages; ++s)
+            if (s < ntiles) {
+                mbar_expect_tx(&full_bar[s], kTileBytes);
+                bulk_g2s(tiles + s * (2 * kTilePairs), pk + (size_t)(tile0 + s) * (2 * kTilePairs), kTileBytes, &full_bar[s]);
+            }
+    }
+
+    // targets: coalesced float4 loads; out-of-range lanes compute on a dummy and do not store
+    const int ibase = blockIdx.x * (THREADS * I);
+    u64 xi[I], yi[I], zi[I];
+    float ox[I], oy[I], oz[I];   // per-chunk (outer) accumulators
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        int i = ibase + k * THREADS + tid;
+        float4 t = (i < n) ? posm[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+        xi[k] = pk2(t.x, t.x);
+        yi[k] = pk2(t.y, t.y);
+        zi[k] = pk2(t.z, t.z);
+        ox[k] = oy[k] = oz[k] = 0.f;
+    }
+    const u64 e2 = pk2(eps2, eps2);
+
+    for (int t = 0; t < ntiles; ++t) {
+        const int s = t % kStages;
+        mbar_wait(&full_bar[s], (uint32_t)((t / kStages) & 1));
+        const float4* sp = tiles + s * (2 * kTilePairs);
+
+        u64 ax[I], ay[I], az[I];
+#pragma unroll
+        for (int k = 0; k < I; ++k) ax[k] = ay[k] = az[k] = 0ull;
+
+#pragma unroll 2
+        for (int q = 0; q < kTilePairs; ++q) {
+            const float4 A = sp[2 * q];       // (x0, x1, y0, y1)  broadcast LDS.128
+            const float4 B = sp[2 * q + 1];   // (z0, z1, m0, m1)
+            const u64 xj = pk2(A.x, A.y), yj = pk2(A.z, A.w), zj = pk2(B.x, B.y), mj = pk2(B.z, B.w);
+#pragma unroll
+            for (int k = 0; k < I; ++k) {
+                const u64 dx = sub2(xj, xi[k]);
+                const u64 dy = sub2(yj, yi[k]);
+                const u64 dz = sub2(zj, zi[k]);
+                u64 r2 = fma2(dx, dx, e2);
+                r2 = fma2(dy, dy, r2);
+                r2 = fma2(dz, dz, r2);
+                float r2a, r2b;
+                upk2(r2, r2a, r2b);
+                float ua = rsqrt_approx(r2a), ub = rsqrt_approx(r2b);
+                if (ZERO_SOFT) {   // delta = 0: coincident pair contributes 0 (Eq. 4 numerator is 0)
+                    ua = (r2a > 0.f) ? ua : 0.f;
+                    ub = (r2b > 0.f) ? ub : 0.f;
+                }
+                const u64 u = pk2(ua, ub);
+                const u64 u2 = mul2(u, u);
+                const u64 mu = mul2(mj, u);
+                const u64 sfac = mul2(mu, u2);     // m_j (r2)^(-3/2)
+                ax[k] = fma2(sfac, dx, ax[k]);
+                ay[k] = fma2(sfac, dy, ay[k]);
+                az[k] = fma2(sfac, dz, az[k]);
+            }
+        }
+        // flush the tile partials (even + odd sources) into the chunk accumulators
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            float a, b;
+            upk2(ax[k], a, b);
+            ox[k] += a + b;
+            upk2(ay[k], a, b);
+            oy[k] += a + b;
+            upk2(az[k], a, b);
+            oz[k] += a + b;
+        }
+        __syncthreads();   // every thread is done reading stage s
+        if (tid == 0 && t + kStages < ntiles) {
+            mbar_expect_tx(&full_bar[s], kTileBytes);
+            bulk_g2s(tiles + s * (2 * kTilePairs), pk + (size_t)(tile0 + t + kStages) * (2 * kTilePairs), kTileBytes,
+                     &full_bar[s]);
+        }
+    }
+
+    float4* __restrict__ out = part + (size_t)blockIdx.y * n;
+#pragma unroll
+    for (int k = 0; k < I; ++k) {
+        int i = ibase + k * THREADS + tid;
+        if (i < n) out[i] = make_float4(ox[k], oy[k], oz[k], 0.f);
+    }
+}
+
+// acc[i] = G * sum_s part[s][i]  in fixed order s = 0..S-1 (dx was r_j - r_i, so the sign of Eq. 4 is in).
+__global__ void __launch_bounds__(256) grav_reduce(const float4* __restrict__ part, int n, int S, float G,
+                                                   float4* __restrict__ acc) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float4 a = part[i];
+    for (int s = 1; s < S; ++s) {
+        float4 b = part[(size_t)s * n + i];
+        a.x += b.x;
+        a.y += b.y;
+        a.z += b.z;
+    }
+    acc[i] = make_float4(G * a.x, G * a.y, G * a.z, 0.f);
+}
+
+int64_t grav_padded(int64_t n_total) { return cdiv(n_total > 0 ? n_total : 1, kGravTileSrc) * kGravTileSrc; }
+
+// Targets per CTA and j-chunks.  Large N: 256 threads x 4 targets; small N: 128 threads x 1 target
+// so that there are CTAs to spread.  S is chosen so the grid is >= ~16 waves of 2 CTAs/SM deep
+// (tail < ~3 %) without making a chunk shorter than 4 tiles.
+static void grav_shape(int64_t n, int& I, int& threads, int& S) {
+    if (n > 65536) {
+        I = 4;
+        threads = 256;
+    } else {
+        I = 1;
+        threads = 128;
+    }
+    int64_t itiles = cdiv(n, (int64_t)I * threads);
+    int64_t tiles = grav_padded(n) / kGravTileSrc;
+    int64_t want = (int64_t)num_sms() * 2 * 16;
+    int64_t s = cdiv(want, itiles);
+    int64_t smax = tiles >= 4 ? tiles / 4 : 1;
+    if (s > smax) s = smax;
+    if (s > 64) s = 64;
+    if (s < 1) s = 1;
+    // make chunks equal: S = ceil(tiles / ceil(tiles / s))
+    int64_t tpc = cdiv(tiles, s);
+    S = (int)cdiv(tiles, tpc);
+}
+
+int grav_splits(int64_t n_total) {
+    int I, th, S;
+    grav_shape(n_total > 0 ? n_total : 1, I, th, S);
+    return S;
+}
+
+template <int I, int THREADS, int MINB>
+static int launch_grav(const float4* posm, const float4* pk, int n, int tiles, int tpc, int S, float eps2,
+                       bool zero_soft, float4* part, cudaStream_t st) {
+    dim3 grid((unsigned)cdiv(n, (int64_t)I * THREADS), (unsigned)S);
+    size_t smem = (size_t)kStages * kTileBytes;
+    if (zero_soft) {
+        auto kfn = grav_pp_kernel<I, THREADS, MINB, true>;
+        SPHB_CUDA(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kfn<<<grid, THREADS, smem, st>>>(posm, pk, n, tiles, tpc, eps2, part);
+    } else {
+        auto kfn = grav_pp_kernel<I, THREADS, MINB, false>;
+        SPHB_CUDA(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kfn<<<grid, THREADS, smem, st>>>(posm, pk, n, tiles, tpc, eps2, part);
+    }
+    SPHB_LAUNCHED();
+    return SPH_OK;
+}
+
+int gravity(const float4* posm, int64_t n_total, float G, float delta, float4* acc_grav, float4* src_pk,
+            float4* grav_part, cudaStream_t st) {
+    if (n_total <= 0) return SPH_OK;
+    const int n = (int)n_total;
+    const int n_pad = (int)grav_padded(n_total);
+    int I, threads, S;
+    grav_shape(n_total, I, threads, S);
+    const int tiles = n_pad / kGravTileSrc;
+    const int tpc = (int)cdiv(tiles, S);
+
+    grav_pack_sources<<<(unsigned)cdiv(n_pad / 2, 256), 256, 0, st>>>(posm, n, n_pad, src_pk);
+    SPHB_LAUNCHED();
+    const float eps2 = delta * delta;
+    const bool zero_soft = !(eps2 > 0.f);
+    if (I == 4)
+        SPHB_TRY((launch_grav<4, 256, 2>(posm, src_pk, n, tiles, tpc, S, eps2, zero_soft, grav_part, st)));
+    else
+        SPHB_TRY((launch_grav<1, 128, 4>(posm, src_pk, n, tiles, tpc, S, eps2, zero_soft, grav_part, st)));
+    grav_reduce<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(grav_part, n, S, G, acc_grav);
+    SPHB_LAUNCHED();
+    return SPH_OK;
+}
+
+}  // namespace sphb

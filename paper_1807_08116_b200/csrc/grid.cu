@@ -1,0 +1,342 @@
+// grid.cu — (a1-a6) the grid-sort neighbour search of PAPER.md L156-207, re-designed for sm_100a.
+//
+// Paper (Kepler): K0 zero, K1 key + atomic histogram, K2 Hillis-Steele scan per block + O(G^2)
+// atomics on block totals, K3 add block offsets, K4 atomic scatter (order inside a cell left to
+// the atomics: neither stable nor deterministic, L204).
+// Here:
+//   zero      cudaMemsetAsync of count[M]
+//   k_key_hist  per particle: cell number (A7, bit-exact FP32 op sequence) and
+//               rank_u[i] = atomicAdd(&count[k], 1) — the histogram atomics already hand every
+//               particle a unique (unstable) slot in its cell, so no second cursor array / pass
+//   k_scan_*    two-level exclusive scan ("in-block then across blocks", L171-172) with warp
+//               shuffles, 16 cells per thread through uint4 loads; 4 B read + 4 B read + 4 B
+//               written per cell
+//   k_scatter   tmp[start[k_i] + rank_u[i]] = i                          (unstable, like K4)
+//   k_stable    stable fix-up: slot s holding i moves to start[k] + #{t in cell : tmp[t] < i},
+//               i.e. ascending original index inside each cell (A16).  The count costs O(n_c)
+//               reads per particle, never more than the density pass's own-cell pair tests, so
+//               it is safe for any cell population.  Fused with (a6): writes perm and the
+//               cell-ordered copy posm_s.
+// All results are deterministic (integer atomics commute; the fix-up removes the only order
+// the atomics decide).
+#include "common.cuh"
+
+namespace sphb {
+
+// ---------------------------------------------------------------- bounding box (A7)
+__device__ __forceinline__ void atomic_min_f(float* addr, float v) {
+    // order-preserving for all finite floats: signed compare for >= 0, unsigned reversed for < 0
+    if (v >= 0.f) atomicMin(reinterpret_cast<int*>(addr), __float_as_int(v));
+    else atomicMax(reinterpret_cast<unsigned int*>(addr), __float_as_uint(v));
+}
+__device__ __forceinline__ void atomic_max_f(float* addr, float v) {
+    if (v >= 0.f) atomicMax(reinterpret_cast<int*>(addr), __float_as_int(v));
+    else atomicMin(reinterpret_cast<unsigned int*>(addr), __float_as_uint(v));
+}
+
+__global__ void k_bbox_init(float* bb) {
+    if (threadIdx.x < 3) bb[threadIdx.x] = __int_as_float(0x7f7fffff);        // +FLT_MAX
+    else if (threadIdx.x < 6) bb[threadIdx.x] = __int_as_float(0xff7fffff);   // -FLT_MAX
+}
+
+__global__ void __launch_bounds__(256) k_bbox(const float4* __restrict__ posm, int n, float* bb) {
+    float lo[3] = {3.4e38f, 3.4e38f, 3.4e38f}, hi[3] = {-3.4e38f, -3.4e38f, -3.4e38f};
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        float4 p = posm[i];
+        lo[0] = fminf(lo[0], p.x); hi[0] = fmaxf(hi[0], p.x);
+        lo[1] = fminf(lo[1], p.y); hi[1] = fmaxf(hi[1], p.y);
+        lo[2] = fminf(lo[2], p.z); hi[2] = fmaxf(hi[2], p.z);
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
+            hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+        }
+    if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            atomic_min_f(bb + a, lo[a]);
+            atomic_max_f(bb + 3 + a, hi[a]);
+        }
+    }
+}
+
+int bbox_gas(const float4* posm, int64_t n_gas, float* bb, cudaStream_t st) {
+    k_bbox_init<<<1, 32, 0, st>>>(bb);
+    SPHB_LAUNCHED();
+    int blocks = (int)(cdiv(n_gas, 256) < (int64_t)num_sms() * 8 ? cdiv(n_gas, 256) : (int64_t)num_sms() * 8);
+    k_bbox<<<blocks, 256, 0, st>>>(posm, (int)n_gas, bb);
+    SPHB_LAUNCHED();
+    return SPH_OK;
+}
+
+// ---------------------------------------------------------------- (a1) cell number, (a2) histogram
+__device__ __forceinline__ int cell_coord(float x, float o, float inv_cell, float fmax_) {
+    float c = __fmul_rn(__fsub_rn(x, o), inv_cell);   // two RN FP32 ops, never contracted (A7)
+    c = fminf(fmaxf(floorf(c), 0.0f), fmax_);         // clamp in float before the cast
+    return (int)c;
+}
+__device__ __forceinline__ uint32_t cell_key(const float4 p, const GridDev g) {
+    int ix = cell_coord(p.x, g.ox, g.inv_cell, g.fx);
+    int iy = cell_coord(p.y, g.oy, g.inv_cell, g.fy);
+    int iz = cell_coord(p.z, g.oz, g.inv_cell, g.fz);
+    return (uint32_t)ix + (uint32_t)g.mx * ((uint32_t)iy + (uint32_t)g.my * (uint32_t)iz);
+}
+
+__global__ void __launch_bounds__(256) k_key_hist(const float4* __restrict__ posm, int n, GridDev g,
+                                                  uint32_t* __restrict__ key, uint32_t* __restrict__ rank_u,
+                                                  uint32_t* __restrict__ count) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint32_t k = cell_key(posm[i], g);
+    key[i] = k;
+    rank_u[i] = atomicAdd(count + k, 1u);
+}
+
+// ---------------------------------------------------------------- (a3) two-level exclusive scan
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 16;
+constexpr int kScanTile = kScanThreads * kScanItems;   // 4096 cells per CTA
+
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* warp_sums, uint32_t& total) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    uint32_t inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) warp_sums[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        uint32_t s = lane < (kScanThreads / 32) ? warp_sums[lane] : 0u;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, s, o);
+            if (lane >= o) s += t;
+        }
+        if (lane < (kScanThreads / 32)) warp_sums[lane] = s;   // inclusive over warps
+    }
+    __syncthreads();
+    total = warp_sums[kScanThreads / 32 - 1];
+    uint32_t base = w > 0 ? warp_sums[w - 1] : 0u;
+    return base + inc - v;
+}
+
+// tile layout: thread t owns cells [tile*4096 + 16 t, +16) — four uint4 loads, fully coalesced per warp
+__device__ __forceinline__ void load_items(const uint32_t* __restrict__ count, int64_t base, int64_t M,
+                                           uint32_t (&c)[kScanItems]) {
+    if (base + kScanItems <= M && ((reinterpret_cast<uintptr_t>(count + base) & 15u) == 0)) {
+        const uint4* p = reinterpret_cast<const uint4*>(count + base);
+#pragma unroll
+        for (int q = 0; q < kScanItems / 4; ++q) {
+            uint4 v = p[q];
+            c[4 * q] = v.x; c[4 * q + 1] = v.y; c[4 * q + 2] = v.z; c[4 * q + 3] = v.w;
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < kScanItems; ++q) c[q] = (base + q < M) ? count[base + q] : 0u;
+    }
+}
+
+__global__ void __launch_bounds__(kScanThreads) k_scan_tile_sums(const uint32_t* __restrict__ count, int64_t M,
+                                                                 uint32_t* __restrict__ tile_sums) {
+    __shared__ uint32_t ws[kScanThreads / 32];
+    uint32_t c[kScanItems];
+    load_items(count, (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems, M, c);
+    uint32_t s = 0;
+#pragma unroll
+    for (int q = 0; q < kScanItems; ++q) s += c[q];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        uint32_t t = 0;
+#pragma unroll
+        for (int q = 0; q < kScanThreads / 32; ++q) t += ws[q];
+        tile_sums[blockIdx.x] = t;
+    }
+}
+
+// one CTA: exclusive scan of the tile sums in place (chunks of 256 with a running carry)
+__global__ void __launch_bounds__(kScanThreads) k_scan_tile_offsets(uint32_t* tile_sums, int n_tiles) {
+    __shared__ uint32_t ws[kScanThreads / 32];
+    uint32_t carry = 0;
+    for (int base = 0; base < n_tiles; base += kScanThreads) {
+        int i = base + threadIdx.x;
+        uint32_t v = i < n_tiles ? tile_sums[i] : 0u, total;
+        uint32_t ex = block_exclusive_scan(v, ws, total);
+        if (i < n_tiles) tile_sums[i] = carry + ex;
+        carry += total;
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(kScanThreads) k_scan_apply(const uint32_t* __restrict__ count, int64_t M,
+                                                             const uint32_t* __restrict__ tile_offsets,
+                                                             uint32_t* __restrict__ start, uint32_t n_gas) {
+    __shared__ uint32_t ws[kScanThreads / 32];
+    uint32_t c[kScanItems];
+    const int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
+    load_items(count, base, M, c);
+    uint32_t s = 0;
+#pragma unroll
+    for (int q = 0; q < kScanItems; ++q) s += c[q];
+    uint32_t total;
+    uint32_t run = tile_offsets[blockIdx.x] + block_exclusive_scan(s, ws, total);
+    uint32_t out[kScanItems];
+#pragma unroll
+    for (int q = 0; q < kScanItems; ++q) {
+        out[q] = run;
+        run += c[q];
+    }
+    if (base + kScanItems <= M && ((reinterpret_cast<uintptr_t>(start + base) & 15u) == 0)) {
+        uint4* p = reinterpret_cast<uint4*>(start + base);
+#pragma unroll
+        for (int q = 0; q < kScanItems / 4; ++q) p[q] = make_uint4(out[4 * q], out[4 * q + 1], out[4 * q + 2], out[4 * q + 3]);
+    } else {
+#pragma unroll
+        for (int q = 0; q < kScanItems; ++q)
+            if (base + q < M) start[base + q] = out[q];
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) start[M] = n_gas;   // A13: start[M] = N_g
+}
+
+// ---------------------------------------------------------------- (a4) scatter and stable fix-up
+__global__ void __launch_bounds__(256) k_scatter(const uint32_t* __restrict__ key, const uint32_t* __restrict__ rank_u,
+                                                 const uint32_t* __restrict__ start, int n, uint32_t* __restrict__ tmp) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    tmp[start[key[i]] + rank_u[i]] = (uint32_t)i;
+}
+
+// slot s of the unstable order holds i = tmp[s]; its stable slot is start[k] + #{t in cell k : tmp[t] < i}.
+// Consecutive threads share a cell, so the reads of tmp[a..b) are warp-broadcast / L1 hits.
+__global__ void __launch_bounds__(256) k_stable(const uint32_t* __restrict__ tmp, const uint32_t* __restrict__ key,
+                                                const uint32_t* __restrict__ start, const float4* __restrict__ posm,
+                                                int n, uint32_t* __restrict__ perm, float4* __restrict__ posm_s) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const uint32_t i = tmp[s];
+    const uint32_t k = key[i];
+    const uint32_t a = start[k], b = start[k + 1];
+    uint32_t r = 0;
+    for (uint32_t t = a; t < b; ++t) r += (tmp[t] < i) ? 1u : 0u;
+    perm[a + r] = i;
+    if (posm_s) posm_s[a + r] = posm[i];
+}
+
+__global__ void __launch_bounds__(256) k_gather_pos(const float4* __restrict__ posm, const uint32_t* __restrict__ perm,
+                                                    int n, float4* __restrict__ posm_s) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < n) posm_s[s] = posm[perm[s]];
+}
+
+int gather_sorted_pos(const float4* posm, const uint32_t* perm, int64_t n_gas, float4* posm_s, cudaStream_t st) {
+    if (n_gas <= 0) return SPH_OK;
+    k_gather_pos<<<(unsigned)cdiv(n_gas, 256), 256, 0, st>>>(posm, perm, (int)n_gas, posm_s);
+    SPHB_LAUNCHED();
+    return SPH_OK;
+}
+
+// ---------------------------------------------------------------- host side
+int check_grid(const sph_grid* g, float h) {
+    if (!g) return SPH_ERR_ARG;
+    double m = 1.0;
+    for (int a = 0; a < 3; ++a) {
+        if (g->dims[a] < 1 || g->dims[a] > 4096) return SPH_ERR_GRID;
+        m *= g->dims[a];
+    }
+    if (m >= 2147483648.0) return SPH_ERR_GRID;
+    if (!(g->cell > 0.f) || !(g->inv_cell > 0.f)) return SPH_ERR_GRID;
+    if (h > 0.f && g->cell < 2.0f * h) return SPH_ERR_GRID;   // 3x3x3 stencil needs cell >= 2h
+    return SPH_OK;
+}
+
+GridDev to_dev(const sph_grid* g) {
+    GridDev d;
+    d.ox = g->origin[0]; d.oy = g->origin[1]; d.oz = g->origin[2];
+    d.inv_cell = g->inv_cell;
+    d.mx = g->dims[0]; d.my = g->dims[1]; d.mz = g->dims[2];
+    d.fx = (float)(g->dims[0] - 1); d.fy = (float)(g->dims[1] - 1); d.fz = (float)(g->dims[2] - 1);
+    return d;
+}
+
+int grid_build(const float4* posm, int64_t n_gas, const sph_grid* g, uint32_t* key, uint32_t* perm,
+               uint32_t* cell_count, uint32_t* cell_start, uint32_t* rank_u, uint32_t* tmp, uint32_t* tile_sums,
+               float4* posm_s, cudaStream_t st) {
+    const int64_t M = grid_cells(g);
+    const int n = (int)n_gas;
+    SPHB_CUDA(cudaMemsetAsync(cell_count, 0, (size_t)M * sizeof(uint32_t), st));          // K0
+    if (n > 0) {
+        k_key_hist<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(posm, n, to_dev(g), key, rank_u, cell_count);   // K1
+        SPHB_LAUNCHED();
+    }
+    const int n_tiles = (int)cdiv(M, kScanTile);
+    k_scan_tile_sums<<<n_tiles, kScanThreads, 0, st>>>(cell_count, M, tile_sums);          // K2 (in-block)
+    SPHB_LAUNCHED();
+    k_scan_tile_offsets<<<1, kScanThreads, 0, st>>>(tile_sums, n_tiles);                   // K2 (across blocks)
+    SPHB_LAUNCHED();
+    k_scan_apply<<<n_tiles, kScanThreads, 0, st>>>(cell_count, M, tile_sums, cell_start, (uint32_t)n);   // K3
+    SPHB_LAUNCHED();
+    if (n > 0) {
+        k_scatter<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(key, rank_u, cell_start, n, tmp);                 // K4
+        SPHB_LAUNCHED();
+        k_stable<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(tmp, key, cell_start, posm, n, perm, posm_s);
+        SPHB_LAUNCHED();
+    }
+    return SPH_OK;
+}
+
+// ---------------------------------------------------------------- (a5) ranges
+__global__ void __launch_bounds__(256) k_cell_range(const uint32_t* __restrict__ start, int64_t M,
+                                                    uint2* __restrict__ range) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < M) range[k] = make_uint2(start[k], start[k + 1]);
+}
+
+__global__ void __launch_bounds__(256) k_particle_runs(const uint32_t* __restrict__ key,
+                                                       const uint32_t* __restrict__ start, int n, int mx, int my, int mz,
+                                                       uint2* __restrict__ runs) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint32_t k = key[i];
+    int ix = (int)(k % (uint32_t)mx), iy = (int)((k / (uint32_t)mx) % (uint32_t)my), iz = (int)(k / ((uint32_t)mx * my));
+    int x0 = max(ix - 1, 0), x1 = min(ix + 1, mx - 1);
+#pragma unroll
+    for (int r = 0; r < 9; ++r) {
+        int cy = iy + (r % 3) - 1, cz = iz + (r / 3) - 1;
+        uint2 v = make_uint2(0u, 0u);
+        if (cy >= 0 && cy < my && cz >= 0 && cz < mz) {
+            int64_t row = (int64_t)mx * (cy + (int64_t)my * cz);
+            v = make_uint2(start[row + x0], start[row + x1 + 1]);
+        }
+        runs[(size_t)i * 9 + r] = v;
+    }
+}
+
+}  // namespace sphb
+
+using namespace sphb;
+
+extern "C" int sph_neighbour_ranges(const sph_grid* g, const uint32_t* key, const uint32_t* cell_start, int64_t n_gas,
+                                    uint32_t* cell_range, uint32_t* particle_runs, void* stream) {
+    if (!g || !cell_start || n_gas < 0 || n_gas >= (1ll << 31)) return SPH_ERR_ARG;
+    SPHB_TRY(check_grid(g, 0.f));
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t M = grid_cells(g);
+    if (cell_range) {
+        k_cell_range<<<(unsigned)cdiv(M, 256), 256, 0, st>>>(cell_start, M, reinterpret_cast<uint2*>(cell_range));
+        SPHB_LAUNCHED();
+    }
+    if (particle_runs && n_gas > 0) {
+        if (!key) return SPH_ERR_ARG;
+        k_particle_runs<<<(unsigned)cdiv(n_gas, 256), 256, 0, st>>>(key, cell_start, (int)n_gas, g->dims[0], g->dims[1],
+                                                                    g->dims[2], reinterpret_cast<uint2*>(particle_runs));
+        SPHB_LAUNCHED();
+    }
+    return SPH_OK;
+}

@@ -1,0 +1,186 @@
+// sph.cu — (a7) density, (a8) EOS, (a9) hydro force / energy rate over the grid-sort ranges.
+//
+// Work is laid out in CELL ORDER (the sorted copy posm_s written by the grid build): thread s
+// owns sorted slot s, so the threads of a warp sit in the same or adjacent cells, walk nearly the
+// same candidate ranges, and their loads of posm_s[t] are warp-broadcasts / L1 hits.  The 27-cell
+// stencil is walked as 9 x-runs: the cells (cx-1, cx, cx+1) of one (y, z) row are contiguous in
+// sorted order, so each run is one [start, end) slot range (L160, L203, L207).
+// Candidates come out in ascending sorted slot, so every sum has a fixed order: results are
+// bitwise reproducible.
+//
+// Cutoff predicate (A8), identical op sequence to the oracle:
+//   dx = x_i (-) x_j ...  d2 = fma(dz,dz, fma(dy,dy, dx*dx))  neighbour iff d2 < fl(fl(2h)^2).
+#include "common.cuh"
+
+namespace sphb {
+
+struct RunCtx {
+    int mx, my, mz;
+};
+
+__device__ __forceinline__ float dist2_f32(const float4 a, const float4 b, float& dx, float& dy, float& dz) {
+    dx = __fsub_rn(a.x, b.x);
+    dy = __fsub_rn(a.y, b.y);
+    dz = __fsub_rn(a.z, b.z);
+    return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+}
+
+__device__ __forceinline__ uint32_t key_of(const float4 p, const GridDev g) {
+    float cx = fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.x, g.ox), g.inv_cell)), 0.0f), g.fx);
+    float cy = fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.y, g.oy), g.inv_cell)), 0.0f), g.fy);
+    float cz = fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.z, g.oz), g.inv_cell)), 0.0f), g.fz);
+    return (uint32_t)(int)cx + (uint32_t)g.mx * ((uint32_t)(int)cy + (uint32_t)g.my * (uint32_t)(int)cz);
+}
+
+// 9 x-runs of the stencil of the cell (ix,iy,iz): run r -> [lo, hi) sorted slots, (0,0) outside the grid
+__device__ __forceinline__ void stencil_run(const uint32_t* __restrict__ start, const GridDev g, int ix, int iy, int iz,
+                                            int r, uint32_t& lo, uint32_t& hi) {
+    const int cy = iy + (r % 3) - 1, cz = iz + (r / 3) - 1;
+    lo = hi = 0u;
+    if (cy >= 0 && cy < g.my && cz >= 0 && cz < g.mz) {
+        const int64_t row = (int64_t)g.mx * (cy + (int64_t)g.my * cz);
+        lo = start[row + max(ix - 1, 0)];
+        hi = start[row + min(ix + 1, g.mx - 1) + 1];
+    }
+}
+
+// ---------------------------------------------------------------- (a7) density, Eq. 7-8
+// W(xi,h) = 1/(pi h^3) { 1 - 3/2 xi^2 + 3/4 xi^3 (xi<=1) ; 1/4 (2-xi)^3 (1<=xi<=2) ; 0 }   (L79)
+__device__ __forceinline__ float w_spline_unnorm(float xi) {
+    float t = 2.0f - xi;
+    float outer = 0.25f * t * t * t;
+    float inner = fmaf(xi * xi, fmaf(0.75f, xi, -1.5f), 1.0f);
+    return xi <= 1.0f ? inner : fmaxf(outer, 0.0f);
+}
+
+__global__ void __launch_bounds__(128) k_density(const float4* __restrict__ posm_s, const uint32_t* __restrict__ perm,
+                                                 const uint32_t* __restrict__ start, int n, GridDev g, float rc2,
+                                                 float inv_h, float norm, float* __restrict__ rho) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const float4 pi = posm_s[s];
+    const uint32_t k = key_of(pi, g);
+    const int ix = (int)(k % (uint32_t)g.mx), iy = (int)((k / (uint32_t)g.mx) % (uint32_t)g.my),
+              iz = (int)(k / ((uint32_t)g.mx * (uint32_t)g.my));
+    float sum = 0.f;   // includes the self term m_i W(0): j = i passes the predicate with d2 = 0 (A5)
+#pragma unroll 1
+    for (int r = 0; r < 9; ++r) {
+        uint32_t lo, hi;
+        stencil_run(start, g, ix, iy, iz, r, lo, hi);
+        for (uint32_t t = lo; t < hi; ++t) {
+            const float4 pj = posm_s[t];
+            float dx, dy, dz;
+            const float d2 = dist2_f32(pi, pj, dx, dy, dz);
+            if (d2 < rc2) {
+                const float xi = sqrtf(d2) * inv_h;
+                sum = fmaf(pj.w, w_spline_unnorm(xi), sum);
+            }
+        }
+    }
+    rho[perm[s]] = sum * norm;
+}
+
+int density_sorted(const float4* posm_s, const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas,
+                   const sph_params* p, const sph_grid* g, float* rho, cudaStream_t st) {
+    if (n_gas <= 0) return SPH_OK;
+    const float two_h = 2.0f * p->h;
+    const float rc2 = two_h * two_h;
+    const float inv_h = 1.0f / p->h;
+    const float norm = (float)(1.0 / (3.14159265358979323846 * (double)p->h * (double)p->h * (double)p->h));
+    k_density<<<(unsigned)cdiv(n_gas, 128), 128, 0, st>>>(posm_s, perm, cell_start, (int)n_gas, to_dev(g), rc2, inv_h,
+                                                          norm, rho);
+    SPHB_LAUNCHED();
+    return SPH_OK;
+}
+
+// ---------------------------------------------------------------- (a8) EOS gather into cell order
+// velr_s[s] = (v_x, v_y, v_z, rho) ; pc_s[s] = (p/rho^2, c) with p = (gamma-1) rho e (Eq. 5),
+// c = sqrt(gamma p / rho) = sqrt(gamma (gamma-1) e) (L99).
+__global__ void __launch_bounds__(256) k_eos_gather(const float4* __restrict__ vele, const float* __restrict__ rho,
+                                                    const uint32_t* __restrict__ perm, int n, float gamma,
+                                                    float4* __restrict__ velr_s, float2* __restrict__ pc_s) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const uint32_t i = perm[s];
+    const float4 v = vele[i];
+    const float r = rho[i];
+    const float gm1 = gamma - 1.0f;
+    velr_s[s] = make_float4(v.x, v.y, v.z, r);
+    pc_s[s] = make_float2(gm1 * v.w / r, sqrtf(gamma * gm1 * v.w));
+}
+
+// ---------------------------------------------------------------- (a9) hydro force, Eqs. 10-11
+struct ViscDev {
+    float h, alpha, beta, eta_h2, gw;   // gw = -45 / (64 pi h^5): dWp/dxi / h per unit (2-xi)^2, times 1/h for xi
+};
+
+__global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_s, const float4* __restrict__ velr_s,
+                                                const float2* __restrict__ pc_s, const uint32_t* __restrict__ perm,
+                                                const uint32_t* __restrict__ start, int n, GridDev g, float rc2,
+                                                ViscDev q, float4* __restrict__ acc) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const float4 pi = posm_s[s];
+    const float4 vi = velr_s[s];
+    const float2 ci = pc_s[s];
+    const uint32_t k = key_of(pi, g);
+    const int ix = (int)(k % (uint32_t)g.mx), iy = (int)((k / (uint32_t)g.mx) % (uint32_t)g.my),
+              iz = (int)(k / ((uint32_t)g.mx * (uint32_t)g.my));
+    const float inv_h = 1.0f / q.h;
+    float ax = 0.f, ay = 0.f, az = 0.f, de = 0.f;
+#pragma unroll 1
+    for (int r = 0; r < 9; ++r) {
+        uint32_t lo, hi;
+        stencil_run(start, g, ix, iy, iz, r, lo, hi);
+        for (uint32_t t = lo; t < hi; ++t) {
+            const float4 pj = posm_s[t];
+            float dx, dy, dz;
+            const float d2 = dist2_f32(pi, pj, dx, dy, dz);
+            if (d2 < rc2 && d2 > 0.f) {   // d2 == 0: self, or a coincident pair (A9) — no contribution
+                const float4 vj = velr_s[t];
+                const float2 cj = pc_s[t];
+                const float rinv = rsqrtf(d2);
+                const float rr = d2 * rinv;                        // |dr|
+                const float tq = fmaxf(2.0f - rr * inv_h, 0.0f);   // 2 - xi
+                // grad W_p = dWp/dxi * dr/|dr| / h,  dWp/dxi = -45/(64 pi h^3) (2-xi)^2   (L95, Eq. 9, A3)
+                const float gmag = q.gw * tq * tq * rinv;          // grad W_p = gmag * dr
+                const float dvx = vi.x - vj.x, dvy = vi.y - vj.y, dvz = vi.z - vj.z;
+                const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
+                // mu_ij = h dr.dv / (|dr|^2 + eta h^2) if dr.dv < 0   (L97)
+                const float mu = rv < 0.f ? __fdividef(q.h * rv, d2 + q.eta_h2) : 0.f;
+                const float rho_ij = 0.5f * (vi.w + vj.w), c_ij = 0.5f * (ci.y + cj.y);
+                const float nu = __fdividef(mu * (q.beta * mu - q.alpha * c_ij), rho_ij);
+                const float Pi = ci.x + cj.x + nu;                 // p_i/rho_i^2 + p_j/rho_j^2 + nu  (L95, A2)
+                const float f = pj.w * Pi * gmag;                  // m_j Pi |grad Wp| / |dr|
+                ax = fmaf(-f, dx, ax);
+                ay = fmaf(-f, dy, ay);
+                az = fmaf(-f, dz, az);
+                de = fmaf(0.5f * f, rv, de);                       // 1/2 m_j Pi dv . grad W_p   (Eq. 11)
+            }
+        }
+    }
+    acc[perm[s]] = make_float4(ax, ay, az, de);
+}
+
+int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const uint32_t* perm,
+                  const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g, float4* velr_s,
+                  float2* pc_s, float4* acc_sph, cudaStream_t st) {
+    if (n_gas <= 0) return SPH_OK;
+    const int n = (int)n_gas;
+    k_eos_gather<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(vele, rho, perm, n, p->gamma, velr_s, pc_s);
+    SPHB_LAUNCHED();
+    const float two_h = 2.0f * p->h;
+    ViscDev q;
+    q.h = p->h;
+    q.alpha = p->alpha;
+    q.beta = p->beta;
+    q.eta_h2 = p->eta * p->h * p->h;
+    const double h = p->h;
+    q.gw = (float)(-45.0 / (64.0 * 3.14159265358979323846 * h * h * h * h));   // dWp/dxi scale / h
+    k_forces<<<(unsigned)cdiv(n, 128), 128, 0, st>>>(posm_s, velr_s, pc_s, perm, cell_start, n, to_dev(g),
+                                                     two_h * two_h, q, acc_sph);
+    SPHB_LAUNCHED();
+    return SPH_OK;
+}
+
+}  // namespace sphb

@@ -1,0 +1,401 @@
+"""GPU parity: the CUDA path (through the C ABI) against the FP64 oracle, element by element,
+on the same seeded inputs.  Integer / index work bit-exact; floating point at the north-star
+tolerances (tests/parity_util.py).  Run with -m gpu on a B200."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1807_08116_b200 import workloads as wl
+from parity_util import check_density, check_values
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+def _t(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _dense(n, seed, h, box=1.0):
+    rng = np.random.Generator(np.random.Philox(key=[seed, 0]))
+    posm = np.zeros((n, 4), np.float32)
+    vele = np.zeros((n, 4), np.float32)
+    posm[:, :3] = rng.random((n, 3)) * box
+    posm[:, 3] = (0.5 + rng.random(n)) / n
+    vele[:, :3] = 0.5 * rng.standard_normal((n, 3))
+    vele[:, 3] = 0.5 + 0.5 * rng.random(n)
+    return wl.Workload(f"dense{n}", posm, vele, n, 0, h, 0.01, 0.0, 1e-3, 1, seed)
+
+
+# ---------------------------------------------------------------- (a10) gravity
+@pytest.mark.parametrize("n", [1, 2, 3, 777, 2048, 2049, 5000])
+def test_gravity_small_and_ragged(cuda_lib, n):
+    b = cuda_lib
+    rng = np.random.Generator(np.random.Philox(key=[n, 1]))
+    posm = np.zeros((n, 4), np.float32)
+    posm[:, :3] = rng.standard_normal((n, 3))
+    posm[:, 3] = (0.2 + rng.random(n)) / n          # unequal masses
+    G, delta = 1.7, 0.05
+    d = _t(posm)
+    acc = torch.full((n, 4), 7.0, device="cuda")
+    ws = b.alloc_workspace(0, n)
+    b.nbody_pp_gravity(d, n, G, delta, acc, ws)
+    got = acc.cpu().numpy()
+    ref = oracle.gravity(posm, G, delta)
+    assert np.all(got[:, 3] == 0)
+    if n == 1:
+        assert np.all(got == 0)
+        return
+    check_values(got[:, :3], ref, f"a_grav n={n}")
+
+
+def test_gravity_config0_and_momentum(cuda_lib):
+    b = cuda_lib
+    w = wl.make_workload(0)
+    d = _t(w.posm)
+    acc = torch.zeros((w.n_total, 4), device="cuda")
+    ws = b.alloc_workspace(0, w.n_total)
+    b.nbody_pp_gravity(d, w.n_total, w.G, w.delta, acc, ws)
+    got = acc.cpu().numpy()[:, :3].astype(np.float64)
+    ref = oracle.gravity(w.posm, w.G, w.delta)
+    mx, med = check_values(got, ref, "a_grav config0")
+    m = w.posm[:, 3].astype(np.float64)
+    assert np.linalg.norm((m[:, None] * got).sum(0)) < 1e-5 * (m * np.linalg.norm(got, axis=1)).sum()
+    # deterministic: a second call is bitwise identical
+    acc2 = torch.zeros_like(acc)
+    b.nbody_pp_gravity(d, w.n_total, w.G, w.delta, acc2, ws)
+    assert torch.equal(acc, acc2)
+
+
+def test_gravity_zero_softening_and_duplicates(cuda_lib):
+    b = cuda_lib
+    n = 600
+    rng = np.random.Generator(np.random.Philox(key=[5, 5]))
+    posm = np.zeros((n, 4), np.float32)
+    posm[:, :3] = rng.standard_normal((n, 3))
+    posm[300:, :3] = posm[:300, :3]               # coincident pairs
+    posm[0, :3] = 0.0                             # a target at the origin (where padded sources sit)
+    posm[300, :3] = 0.0
+    posm[:, 3] = 1.0 / n
+    d = _t(posm)
+    acc = torch.zeros((n, 4), device="cuda")
+    ws = b.alloc_workspace(0, n)
+    b.nbody_pp_gravity(d, n, 1.0, 0.0, acc, ws)
+    got = acc.cpu().numpy()
+    assert np.all(np.isfinite(got))
+    check_values(got[:, :3], oracle.gravity(posm, 1.0, 0.0), "a_grav delta=0", max_tol=5e-4, med_tol=2e-5)
+
+
+def test_gravity_medium_subset(cuda_lib):
+    """N = 70001 (the 256x4 kernel, several j-chunks, ragged tail); oracle on a seeded subset."""
+    b = cuda_lib
+    w = wl.make_workload(1, scale=70001 / 2 ** 17)
+    n = w.n_total
+    d = _t(w.posm)
+    acc = torch.zeros((n, 4), device="cuda")
+    ws = b.alloc_workspace(0, n)
+    b.nbody_pp_gravity(d, n, w.G, w.delta, acc, ws)
+    g, h = wl.subset_indices(w.n_gas, w.n_halo, 77, n_each=512)
+    tg = np.concatenate([g, h, [0, n - 1]])
+    ref = oracle.gravity(w.posm, w.G, w.delta, targets=tg)
+    check_values(acc.cpu().numpy()[tg, :3], ref, "a_grav 70001 subset")
+
+
+# ---------------------------------------------------------------- (a1-a5) grid sort
+def _grid_case(case):
+    if case == "galaxy":
+        w = wl.make_workload(0)
+        return w, None
+    if case == "dense":
+        return _dense(20000, 3, 0.03), None
+    if case == "clumps":
+        return wl.make_workload(4, scale=2 ** -9), None
+    if case == "clamped":
+        w = wl.make_workload(0)
+        g = oracle.grid_from_bbox(w.posm, w.n_gas, w.h)
+        return w, oracle.Grid((-1.5, -1.0, -2.0), g.cell, g.inv_cell, (7, 5, 9))
+    if case == "one_cell":
+        w = _dense(5000, 4, 0.03)
+        w.h = 3.0
+        return w, None
+    if case == "ragged_M":
+        w = _dense(4099, 6, 0.031)
+        return w, None
+    raise KeyError(case)
+
+
+@pytest.mark.parametrize("case", ["galaxy", "dense", "clumps", "clamped", "one_cell", "ragged_M"])
+def test_grid_sort_bit_exact(cuda_lib, case):
+    b = cuda_lib
+    w, og = _grid_case(case)
+    n = w.n_gas
+    d = _t(w.posm)
+    if og is None:
+        g = b.sph_grid_from_bbox(d, n, w.h)
+        og = oracle.grid_from_bbox(w.posm, n, w.h)
+        assert tuple(g.dims) == tuple(og.dims) and tuple(g.origin) == tuple(np.float32(og.origin))
+        assert np.float32(g.cell) == np.float32(og.cell) and np.float32(g.inv_cell) == np.float32(og.inv_cell)
+    else:
+        g = b.sph_grid.make(og.origin, og.cell, og.inv_cell, og.dims)
+    M = g.M
+    key = torch.zeros(n, dtype=torch.int32, device="cuda")
+    perm = torch.zeros(n, dtype=torch.int32, device="cuda")
+    count = torch.full((M,), -1, dtype=torch.int32, device="cuda")
+    start = torch.full((M + 1,), -1, dtype=torch.int32, device="cuda")
+    ws = b.alloc_workspace(n, n, g)
+    b.sph_build_grid(d, n, g, key, perm, count, start, ws)
+    okey = oracle.cell_keys(w.posm, n, og)
+    ocount, ostart, operm = oracle.counting_sort(okey, M)
+    assert np.array_equal(key.cpu().numpy().view(np.uint32), okey)
+    assert np.array_equal(count.cpu().numpy().view(np.uint32), ocount)
+    assert np.array_equal(start.cpu().numpy().view(np.uint32), ostart)
+    assert np.array_equal(perm.cpu().numpy().view(np.uint32), operm)
+    # (a5) ranges
+    rng_ = torch.zeros((M, 2), dtype=torch.int32, device="cuda")
+    runs = torch.zeros((n, 9, 2), dtype=torch.int32, device="cuda")
+    b.sph_neighbour_ranges(g, key, start, n, rng_, runs)
+    r = rng_.cpu().numpy().view(np.uint32)
+    assert np.array_equal(r[:, 0], ostart[:-1]) and np.array_equal(r[:, 1], ostart[1:])
+    runs = runs.cpu().numpy().view(np.uint32)
+    mx, my, mz = og.dims
+    sel = np.random.Generator(np.random.Philox(key=[1, 2])).integers(0, n, 200)
+    for i in sel:
+        k = int(okey[i])
+        ix, iy, iz = k % mx, (k // mx) % my, k // (mx * my)
+        for rr in range(9):
+            cy, cz = iy + rr % 3 - 1, iz + rr // 3 - 1
+            if 0 <= cy < my and 0 <= cz < mz:
+                row = mx * (cy + my * cz)
+                want = (ostart[row + max(ix - 1, 0)], ostart[row + min(ix + 1, mx - 1) + 1])
+            else:
+                want = (0, 0)
+            assert tuple(runs[i, rr]) == want
+    # deterministic
+    perm2 = torch.zeros_like(perm)
+    b.sph_build_grid(d, n, g, key, perm2, count, start, ws)
+    assert torch.equal(perm, perm2)
+
+
+# ---------------------------------------------------------------- neighbour sets, density, forces
+def _build(b, w, og=None):
+    n = w.n_gas
+    d = _t(w.posm)
+    g = b.sph_grid_from_bbox(d, n, w.h) if og is None else b.sph_grid.make(og.origin, og.cell, og.inv_cell, og.dims)
+    key = torch.zeros(n, dtype=torch.int32, device="cuda")
+    perm = torch.zeros(n, dtype=torch.int32, device="cuda")
+    count = torch.zeros(g.M, dtype=torch.int32, device="cuda")
+    start = torch.zeros(g.M + 1, dtype=torch.int32, device="cuda")
+    ws = b.alloc_workspace(n, n, g)
+    b.sph_build_grid(d, n, g, key, perm, count, start, ws)
+    return d, g, perm, start, ws
+
+
+@pytest.mark.parametrize("case", ["galaxy", "dense", "clamped", "one_cell"])
+def test_neighbour_sets_bit_exact(cuda_lib, case):
+    b = cuda_lib
+    w, og = _grid_case(case)
+    if case == "one_cell":
+        w = _dense(1500, 4, 3.0)
+    n = w.n_gas
+    d, g, perm, start, ws = _build(b, w, og)
+    cnt, off, idx = b.sph_neighbour_lists(d, n, w.h, g, perm, start, ws)
+    ooff, oidx = oracle.neighbours(w.posm, n, w.h, method="brute" if n <= 6000 else "grid")
+    assert np.array_equal(off.cpu().numpy(), ooff)
+    assert np.array_equal(cnt.cpu().numpy().view(np.uint32), np.diff(ooff).astype(np.uint32))
+    assert np.array_equal(idx.cpu().numpy().view(np.uint32), oidx)
+
+
+@pytest.mark.parametrize("case", ["galaxy", "dense", "clumps", "clamped"])
+def test_density_and_forces_parity(cuda_lib, case):
+    b = cuda_lib
+    w, og = _grid_case(case)
+    n = w.n_gas
+    d, g, perm, start, ws = _build(b, w, og)
+    prm = b.sph_params.from_workload(w)
+    rho = torch.zeros(n, device="cuda")
+    b.sph_density(d, n, prm, g, perm, start, rho, ws)
+    ooff, oidx = oracle.neighbours(w.posm, n, w.h, method="grid")
+    orho = oracle.density(w.posm, w.h, ooff, oidx)
+    check_density(rho.cpu().numpy(), orho, f"rho {case}")
+    # forces from the GPU's own density (what the step does) against the oracle's chain
+    acc = torch.zeros((n, 4), device="cuda")
+    dv = _t(w.vele)
+    b.sph_forces(d, dv, rho, n, prm, g, perm, start, acc, ws)
+    of = oracle.forces(w.posm, w.vele, orho, w.h, ooff, oidx, gamma=w.gamma, alpha=w.alpha, beta=w.beta, eta=w.eta)
+    got = acc.cpu().numpy()
+    check_values(got[:, :3], of[:, :3], f"a_sph {case}")
+    check_values(got[:, 3], of[:, 3], f"de/dt {case}")
+    # invariants on the GPU result: momentum (P5) and energy-rate identity (P6) to FP32 round-off
+    m = w.posm[:n, 3].astype(np.float64)
+    a = got[:, :3].astype(np.float64)
+    v = w.vele[:n, :3].astype(np.float64)
+    scale = (m * np.linalg.norm(a, axis=1)).sum()
+    assert np.linalg.norm((m[:, None] * a).sum(0)) < 1e-5 * scale
+    resid = (m * got[:, 3]).sum() + (m * (v * a).sum(1)).sum()
+    assert abs(resid) < 1e-5 * ((m * np.abs(got[:, 3])).sum() + (m * np.abs((v * a).sum(1))).sum())
+    # deterministic
+    acc2 = torch.zeros_like(acc)
+    b.sph_forces(d, dv, rho, n, prm, g, perm, start, acc2, ws)
+    assert torch.equal(acc, acc2)
+
+
+def test_coincident_gas_particles(cuda_lib):
+    b = cuda_lib
+    w = _dense(2000, 8, 0.08)
+    w.posm[1000:, :3] = w.posm[:1000, :3]
+    n = w.n_gas
+    d, g, perm, start, ws = _build(b, w)
+    prm = b.sph_params.from_workload(w)
+    rho = torch.zeros(n, device="cuda")
+    acc = torch.zeros((n, 4), device="cuda")
+    b.sph_density(d, n, prm, g, perm, start, rho, ws)
+    b.sph_forces(d, _t(w.vele), rho, n, prm, g, perm, start, acc, ws)
+    ooff, oidx = oracle.neighbours(w.posm, n, w.h)
+    orho = oracle.density(w.posm, w.h, ooff, oidx)
+    of = oracle.forces(w.posm, w.vele, orho, w.h, ooff, oidx)
+    check_density(rho.cpu().numpy(), orho)
+    got = acc.cpu().numpy()
+    assert np.all(np.isfinite(got))
+    check_values(got[:, :3], of[:, :3], "a_sph duplicates")
+
+
+# ---------------------------------------------------------------- whole evaluation and step
+def _oracle_state(w):
+    return oracle.State(w.posm.astype(np.float64), w.vele.astype(np.float64), w.n_gas)
+
+
+def test_evaluate_config0(cuda_lib):
+    b = cuda_lib
+    w = wl.make_workload(0)
+    sim = b.Simulation(w)
+    sim.evaluate()
+    st = _oracle_state(w)
+    nbr = oracle.position_only(st, w.h, w.G, w.delta)
+    hy = oracle.hydro(st, w.h, nbr)
+    check_density(sim.rho.cpu().numpy(), st.rho)
+    check_values(sim.acc_grav.cpu().numpy()[:, :3], st.acc_grav, "a_grav")
+    a = sim.acc_sph.cpu().numpy()
+    check_values(a[:, :3], hy[:, :3], "a_sph")
+    check_values(a[:, 3], hy[:, 3], "de/dt")
+
+
+@pytest.mark.parametrize("cfg,scale,steps", [(0, 1.0, 1), (0, 1.0, 3), (1, 1 / 16, 4)])
+def test_step_parity_free_running(cuda_lib, cfg, scale, steps):
+    """Free-running multi-step trajectories: GPU FP32 state against the oracle's FP64 state."""
+    b = cuda_lib
+    w = wl.make_workload(cfg, scale=scale)
+    sim = b.Simulation(w)
+    og = oracle.grid_from_bbox(w.posm, w.n_gas, w.h)
+    assert tuple(sim.grid.dims) == tuple(og.dims)
+    st = _oracle_state(w)
+    nbr = oracle.position_only(st, w.h, w.G, w.delta)
+    for _ in range(steps):
+        sim.step()
+        st, nbr, _ = oracle.step(st, w.dt, w.h, w.G, w.delta, nbr=nbr)
+    pos = sim.posm.cpu().numpy()
+    vel = sim.vele.cpu().numpy()
+    ng = w.n_gas
+    # positions: absolute, a few FP32 ulps of the coordinate scale per step
+    assert np.abs(pos[:, :3] - st.posm[:, :3]).max() < 4e-6 * steps * max(1.0, np.abs(st.posm[:, :3]).max())
+    assert np.array_equal(pos[:, 3], w.posm[:, 3])
+    check_values(vel[:, :3], st.vele[:, :3], "v(t+dt)", max_tol=2e-5, med_tol=2e-6)
+    check_values(vel[:ng, 3], st.vele[:ng, 3], "e(t+dt)", max_tol=2e-5, med_tol=2e-6)
+    check_density(sim.rho.cpu().numpy()[:ng], st.rho, "rho(t+dt)") if steps == 1 else None
+    check_values(sim.acc_grav.cpu().numpy()[:, :3], st.acc_grav, "a_grav(t+dt)", max_tol=1e-3 if steps > 1 else 2e-4)
+
+
+def test_step_collisionless_and_gas_only(cuda_lib):
+    b = cuda_lib
+    w = wl.make_workload(0, scale=0.25)
+    # collisionless (L150): N_g = 0, SP/DC/HFC skipped
+    halo = wl.Workload("halo", w.posm[w.n_gas:].copy(), w.vele[w.n_gas:].copy(), 0, w.n_halo, w.h, w.delta, w.G, w.dt, 1, 0)
+    sim = b.Simulation(halo)
+    st = _oracle_state(halo)
+    nbr = oracle.position_only(st, w.h, w.G, w.delta)
+    for _ in range(2):
+        sim.step()
+        st, nbr, _ = oracle.step(st, w.dt, w.h, w.G, w.delta, nbr=nbr)
+    check_values(sim.vele.cpu().numpy()[:, :3], st.vele[:, :3], "v halo-only", max_tol=2e-5, med_tol=2e-6)
+    # gas only, no gravity (config 4 style): N_h = 0, G = 0
+    gas = _dense(6000, 12, 0.05)
+    sim = b.Simulation(gas)
+    st = _oracle_state(gas)
+    nbr = oracle.position_only(st, gas.h, 0.0, gas.delta)
+    sim.step()
+    st, nbr, _ = oracle.step(st, gas.dt, gas.h, 0.0, gas.delta, nbr=nbr)
+    check_values(sim.vele.cpu().numpy()[:, :3], st.vele[:, :3], "v gas-only", max_tol=2e-5, med_tol=2e-6)
+    check_values(sim.vele.cpu().numpy()[:, 3], st.vele[:, 3], "e gas-only", max_tol=2e-5, med_tol=2e-6)
+    assert np.all(sim.acc_grav.cpu().numpy() == 0)
+
+
+def test_step_host_matches_device_path(cuda_lib):
+    b = cuda_lib
+    w = wl.make_workload(0, scale=0.5)
+    sim = b.Simulation(w)
+    for _ in range(2):
+        sim.step()
+    posm, vele = w.posm.copy(), w.vele.copy()
+    rho = np.zeros(w.n_gas, np.float32)
+    ag = np.zeros((w.n_total, 4), np.float32)
+    b.sph_step_host(posm, vele, w.n_gas, w.n_halo, b.sph_params.from_workload(w), w.dt, 2, rho=rho, acc_grav=ag)
+    assert np.array_equal(posm, sim.posm.cpu().numpy())
+    assert np.array_equal(vele, sim.vele.cpu().numpy())
+    assert np.array_equal(rho, sim.rho.cpu().numpy()[: w.n_gas])
+    assert np.array_equal(ag, sim.acc_grav.cpu().numpy())
+    ctx = b.HostContext(w.n_gas, w.n_halo)
+    p2, v2 = w.posm.copy(), w.vele.copy()
+    ctx.step(p2, v2, b.sph_params.from_workload(w), w.dt, 2)
+    ctx.close()
+    assert np.array_equal(p2, posm) and np.array_equal(v2, vele)
+
+
+def test_energy_drift_gpu_state(cuda_lib):
+    """Pin P7 on the GPU trajectory: energy of the FP32 state, evaluated in FP64 by the oracle."""
+    b = cuda_lib
+    w = wl.make_workload(0)
+    sim = b.Simulation(w)
+    st0 = _oracle_state(w)
+    e0 = oracle.total_energy(st0, w.G, w.delta)
+    for _ in range(10):
+        sim.step()
+    st1 = oracle.State(sim.posm.cpu().numpy().astype(np.float64), sim.vele.cpu().numpy().astype(np.float64), w.n_gas)
+    e1 = oracle.total_energy(st1, w.G, w.delta)
+    assert abs((e1 - e0) / e0) <= 5e-6
+    m = w.posm[:, 3].astype(np.float64)
+    dp = (m[:, None] * (st1.vele[:, :3] - st0.vele[:, :3])).sum(0)
+    assert np.linalg.norm(dp) < 1e-6 * (m * np.linalg.norm(st0.vele[:, :3], axis=1)).sum()
+
+
+# ---------------------------------------------------------------- boundary behaviour
+def test_error_codes(cuda_lib):
+    b = cuda_lib
+    w = wl.make_workload(0, scale=0.1)
+    d = _t(w.posm)
+    acc = torch.zeros((w.n_total, 4), device="cuda")
+    small = torch.empty(256, dtype=torch.uint8, device="cuda")
+    with pytest.raises(b.SphError) as e:
+        b.nbody_pp_gravity(d, w.n_total, 1.0, 0.01, acc, small)
+    assert e.value.rc == b.SPH_ERR_WORKSPACE
+    ws = b.alloc_workspace(0, w.n_total)
+    with pytest.raises(b.SphError) as e:
+        b.nbody_pp_gravity(d, w.n_total, 1.0, -1.0, acc, ws)
+    assert e.value.rc == b.SPH_ERR_UNSUPPORTED
+    with pytest.raises(b.SphError) as e:
+        b.nbody_pp_gravity(d, -3, 1.0, 0.1, acc, ws)
+    assert e.value.rc == b.SPH_ERR_ARG
+    with pytest.raises(b.SphError) as e:                     # misaligned pointer
+        b.load().sph_build_grid  # noqa: B018
+        mis = torch.zeros(w.n_total * 4 + 1, device="cuda")[1:]
+        b.nbody_pp_gravity(mis, w.n_total, 1.0, 0.1, acc, ws)
+    assert e.value.rc == b.SPH_ERR_ARG
+    bad = b.sph_grid.make((0, 0, 0), 0.4, 2.5, (5000, 2, 2))
+    with pytest.raises(b.SphError) as e:
+        b.sph_build_grid(d, w.n_gas, bad, acc, acc, acc, acc, ws)
+    assert e.value.rc == b.SPH_ERR_GRID
+    tight = b.sph_grid.make((0, 0, 0), 0.1, 10.0, (4, 4, 4))      # cell < 2h
+    with pytest.raises(b.SphError) as e:
+        b.sph_density(d, w.n_gas, b.sph_params.make(w.h), tight, acc, acc, acc, ws)
+    assert e.value.rc == b.SPH_ERR_GRID
+    # n = 0 is legal everywhere
+    b.nbody_pp_gravity(d, 0, 1.0, 0.1, acc, ws)
+    assert b.sph_launch_count() > 0
