@@ -78,7 +78,7 @@ def lib():
         L.orc_neighbours_grid.restype = None
         L.orc_density.argtypes = [dp, C.c_double, ip, C.c_int64, ip, up, dp]
         L.orc_density.restype = None
-        L.orc_forces.argtypes = [dp, dp, dp, C.POINTER(_Params), ip, C.c_int64, ip, up, dp]
+        L.orc_forces.argtypes = [dp, dp, dp, C.POINTER(_Params), ip, C.c_int64, ip, up, dp, dp]
         L.orc_forces.restype = None
         _lib = L
     return _lib
@@ -225,8 +225,10 @@ def density(posm, h, offsets, index, targets=None):
     return rho
 
 
-def forces(posm, vele, rho_all, h, offsets, index, targets=None, gamma=5.0 / 3.0, alpha=0.5, beta=1.0, eta=0.1):
-    """(ax, ay, az, de/dt) of Eqs. 10-11 (hydro part) for `targets`; rho_all indexed by gas index."""
+def forces(posm, vele, rho_all, h, offsets, index, targets=None, gamma=5.0 / 3.0, alpha=0.5, beta=1.0, eta=0.1,
+           with_gross=False):
+    """(ax, ay, az, de/dt) of Eqs. 10-11 (hydro part) for `targets`; rho_all indexed by gas index.
+    with_gross: also return [nt,2] sums of the term magnitudes (conditioning diagnostic, reading A17)."""
     posm, vele, rho_all = _f64(posm), _f64(vele), _f64(rho_all)
     tg = _tg(targets)
     nt = len(offsets) - 1
@@ -236,10 +238,12 @@ def forces(posm, vele, rho_all, h, offsets, index, targets=None, gamma=5.0 / 3.0
         idx = np.zeros(1, dtype=np.uint32)
     off = np.ascontiguousarray(offsets, dtype=np.int64)
     prm = _Params(float(h), float(gamma), float(alpha), float(beta), float(eta))
+    gross = np.zeros((nt, 2), dtype=np.float64) if with_gross else None
     if nt:
         lib().orc_forces(_p(posm, C.c_double), _p(vele, C.c_double), _p(rho_all, C.c_double), C.byref(prm),
-                         _p(tg, C.c_int64), nt, _p(off, C.c_int64), _p(idx, C.c_uint32), _p(out, C.c_double))
-    return out
+                         _p(tg, C.c_int64), nt, _p(off, C.c_int64), _p(idx, C.c_uint32), _p(out, C.c_double),
+                         _p(gross, C.c_double))
+    return (out, gross) if with_gross else out
 
 
 # ------------------------------------------------------------------ whole evaluation / step (O6)

@@ -350,10 +350,13 @@ void orc_density(const double* posm, double h, const int64_t* targets, int64_t n
  *   de_i/dt  = 1/2 sum_j m_j Pi_ij dv_ij . grad W_p                         (Eq. 11)
  *   p = (gamma-1) rho e (Eq. 5) ; c = sqrt(gamma p / rho) (L99).
  * rho_all[j] must hold the density of every j that appears (index by global gas index).
- * A pair at zero separation contributes nothing (reading A9).  out[t] = (ax, ay, az, de/dt). */
+ * A pair at zero separation contributes nothing (reading A9).  out[t] = (ax, ay, az, de/dt).
+ * gross (may be NULL): gross[t] = (sum_j |m_j Pi_ij grad W_p|, sum_j |1/2 m_j Pi_ij dv.grad W_p|), the
+ * sums of the magnitudes of the same terms — a conditioning diagnostic for the parity tolerance
+ * (reading A17), not part of the method.                                            */
 void orc_forces(const double* posm, const double* vele, const double* rho_all, const orc_sph_params* p,
                 const int64_t* targets, int64_t nt,
-                const int64_t* nbr_offset, const uint32_t* nbr_index, double* out) {
+                const int64_t* nbr_offset, const uint32_t* nbr_index, double* out, double* gross) {
     const double h = p->h, gm1 = p->gamma - 1.0;
 #pragma omp parallel for schedule(dynamic, 64)
     for (int64_t t = 0; t < nt; ++t) {
@@ -363,7 +366,7 @@ void orc_forces(const double* posm, const double* vele, const double* rho_all, c
         double rhoi = rho_all[i];
         double pi_ = gm1 * rhoi * ei;
         double ci = sqrt(p->gamma * pi_ / rhoi);
-        double ax = 0.0, ay = 0.0, az = 0.0, de = 0.0;
+        double ax = 0.0, ay = 0.0, az = 0.0, de = 0.0, ga = 0.0, ge = 0.0;
         for (int64_t q = nbr_offset[t]; q < nbr_offset[t + 1]; ++q) {
             int64_t j = nbr_index[q];
             double dx = xi - posm[4 * j], dy = yi - posm[4 * j + 1], dz = zi - posm[4 * j + 2];
@@ -385,6 +388,12 @@ void orc_forces(const double* posm, const double* vele, const double* rho_all, c
             ay -= mj * Pi * gy;
             az -= mj * Pi * gz;
             de += 0.5 * mj * Pi * (dvx * gx + dvy * gy + dvz * gz);
+            ga += fabs(mj * Pi) * sqrt(gx * gx + gy * gy + gz * gz);
+            ge += fabs(0.5 * mj * Pi * (dvx * gx + dvy * gy + dvz * gz));
+        }
+        if (gross) {
+            gross[2 * t + 0] = ga;
+            gross[2 * t + 1] = ge;
         }
         out[4 * t + 0] = ax;
         out[4 * t + 1] = ay;

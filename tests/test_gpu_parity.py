@@ -221,10 +221,11 @@ def test_density_and_forces_parity(cuda_lib, case):
     acc = torch.zeros((n, 4), device="cuda")
     dv = _t(w.vele)
     b.sph_forces(d, dv, rho, n, prm, g, perm, start, acc, ws)
-    of = oracle.forces(w.posm, w.vele, orho, w.h, ooff, oidx, gamma=w.gamma, alpha=w.alpha, beta=w.beta, eta=w.eta)
+    of, gross = oracle.forces(w.posm, w.vele, orho, w.h, ooff, oidx, gamma=w.gamma, alpha=w.alpha, beta=w.beta,
+                              eta=w.eta, with_gross=True)
     got = acc.cpu().numpy()
-    check_values(got[:, :3], of[:, :3], f"a_sph {case}")
-    check_values(got[:, 3], of[:, 3], f"de/dt {case}")
+    check_values(got[:, :3], of[:, :3], f"a_sph {case}", gross=gross[:, 0])
+    check_values(got[:, 3], of[:, 3], f"de/dt {case}", gross=gross[:, 1])
     # invariants on the GPU result: momentum (P5) and energy-rate identity (P6) to FP32 round-off
     m = w.posm[:n, 3].astype(np.float64)
     a = got[:, :3].astype(np.float64)
@@ -252,11 +253,11 @@ def test_coincident_gas_particles(cuda_lib):
     b.sph_forces(d, _t(w.vele), rho, n, prm, g, perm, start, acc, ws)
     ooff, oidx = oracle.neighbours(w.posm, n, w.h)
     orho = oracle.density(w.posm, w.h, ooff, oidx)
-    of = oracle.forces(w.posm, w.vele, orho, w.h, ooff, oidx)
+    of, gross = oracle.forces(w.posm, w.vele, orho, w.h, ooff, oidx, with_gross=True)
     check_density(rho.cpu().numpy(), orho)
     got = acc.cpu().numpy()
     assert np.all(np.isfinite(got))
-    check_values(got[:, :3], of[:, :3], "a_sph duplicates")
+    check_values(got[:, :3], of[:, :3], "a_sph duplicates", gross=gross[:, 0])
 
 
 # ---------------------------------------------------------------- whole evaluation and step
@@ -271,12 +272,12 @@ def test_evaluate_config0(cuda_lib):
     sim.evaluate()
     st = _oracle_state(w)
     nbr = oracle.position_only(st, w.h, w.G, w.delta)
-    hy = oracle.hydro(st, w.h, nbr)
+    hy, gross = oracle.forces(st.posm, st.vele, st.rho, w.h, nbr[0], nbr[1], with_gross=True)
     check_density(sim.rho.cpu().numpy(), st.rho)
     check_values(sim.acc_grav.cpu().numpy()[:, :3], st.acc_grav, "a_grav")
     a = sim.acc_sph.cpu().numpy()
-    check_values(a[:, :3], hy[:, :3], "a_sph")
-    check_values(a[:, 3], hy[:, 3], "de/dt")
+    check_values(a[:, :3], hy[:, :3], "a_sph", gross=gross[:, 0])
+    check_values(a[:, 3], hy[:, 3], "de/dt", gross=gross[:, 1])
 
 
 @pytest.mark.parametrize("cfg,scale,steps", [(0, 1.0, 1), (0, 1.0, 3), (1, 1 / 16, 4)])
