@@ -111,7 +111,22 @@ __global__ void __launch_bounds__(256) k_eos_gather(const float4* __restrict__ v
 
 // ---------------------------------------------------------------- (a9) hydro force, Eqs. 10-11
 struct ViscDev {
-    float h, alpha, beta, eta_h2, gw;   // gw = -45 / (64 pi h^5): dWp/dxi / h per unit (2-xi)^2, times 1/h for xi
+    float h, alpha, beta, eta_h2, gw;   // gw = -45 / (64 pi h^4): grad W_p = gw (2-xi)^2 dr/|dr|
+    float inv_h2;                       // 1 / h^2
+    double rc2_64;                      // 4 h^2 in FP64 (h as given, widened)
+};
+
+// Compensated (Kahan) accumulation.  The hydro terms of one particle routinely cancel by 10^2-10^3
+// and dense cells sum hundreds of them; a plain FP32 running sum loses ~sqrt(n) ulps of the GROSS
+// sum, which is what broke the 2e-4 parity bar on the clumpy configs.  Cost: 3 extra FADD per add.
+struct KSum {
+    float s = 0.f, c = 0.f;
+    __device__ __forceinline__ void add(float x) {
+        const float y = __fsub_rn(x, c);
+        const float t = __fadd_rn(s, y);
+        c = __fsub_rn(__fsub_rn(t, s), y);
+        s = t;
+    }
 };
 
 __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_s, const float4* __restrict__ velr_s,
@@ -127,7 +142,7 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
     const int ix = (int)(k % (uint32_t)g.mx), iy = (int)((k / (uint32_t)g.mx) % (uint32_t)g.my),
               iz = (int)(k / ((uint32_t)g.mx * (uint32_t)g.my));
     const float inv_h = 1.0f / q.h;
-    float ax = 0.f, ay = 0.f, az = 0.f, de = 0.f;
+    KSum ax, ay, az, de;
 #pragma unroll 1
     for (int r = 0; r < 9; ++r) {
         uint32_t lo, hi;
@@ -139,27 +154,32 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
             if (d2 < rc2 && d2 > 0.f) {   // d2 == 0: self, or a coincident pair (A9) — no contribution
                 const float4 vj = velr_s[t];
                 const float2 cj = pc_s[t];
-                const float rinv = rsqrtf(d2);
+                float rinv = rsqrtf(d2);
+                rinv = rinv * fmaf(-0.5f * d2 * rinv, rinv, 1.5f);   // one Newton step: ~1 ulp
                 const float rr = d2 * rinv;                        // |dr|
-                const float tq = fmaxf(2.0f - rr * inv_h, 0.0f);   // 2 - xi
+                // 2 - xi = (4h^2 - |dr|^2) / (h^2 (2 + xi)).  Formed as 2 - rr/h in FP32 it loses a factor
+                // xi/(2-xi) of relative accuracy near the kernel edge (every term of a sparsely surrounded
+                // particle sits there), so the numerator alone is taken in FP64: 3 cvt + 3 DFMA per pair.
+                const double num = fma(-(double)dz, (double)dz, fma(-(double)dy, (double)dy, fma(-(double)dx, (double)dx, q.rc2_64)));
+                const float tq = fmaxf((float)num, 0.0f) * q.inv_h2 / (2.0f + rr * inv_h);   // 2 - xi
                 // grad W_p = dWp/dxi * dr/|dr| / h,  dWp/dxi = -45/(64 pi h^3) (2-xi)^2   (L95, Eq. 9, A3)
                 const float gmag = q.gw * tq * tq * rinv;          // grad W_p = gmag * dr
                 const float dvx = vi.x - vj.x, dvy = vi.y - vj.y, dvz = vi.z - vj.z;
                 const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
                 // mu_ij = h dr.dv / (|dr|^2 + eta h^2) if dr.dv < 0   (L97)
-                const float mu = rv < 0.f ? __fdividef(q.h * rv, d2 + q.eta_h2) : 0.f;
+                const float mu = rv < 0.f ? (q.h * rv) / (d2 + q.eta_h2) : 0.f;       // IEEE division
                 const float rho_ij = 0.5f * (vi.w + vj.w), c_ij = 0.5f * (ci.y + cj.y);
-                const float nu = __fdividef(mu * (q.beta * mu - q.alpha * c_ij), rho_ij);
+                const float nu = (mu * (q.beta * mu - q.alpha * c_ij)) / rho_ij;
                 const float Pi = ci.x + cj.x + nu;                 // p_i/rho_i^2 + p_j/rho_j^2 + nu  (L95, A2)
                 const float f = pj.w * Pi * gmag;                  // m_j Pi |grad Wp| / |dr|
-                ax = fmaf(-f, dx, ax);
-                ay = fmaf(-f, dy, ay);
-                az = fmaf(-f, dz, az);
-                de = fmaf(0.5f * f, rv, de);                       // 1/2 m_j Pi dv . grad W_p   (Eq. 11)
+                ax.add(-f * dx);
+                ay.add(-f * dy);
+                az.add(-f * dz);
+                de.add(0.5f * f * rv);                             // 1/2 m_j Pi dv . grad W_p   (Eq. 11)
             }
         }
     }
-    acc[perm[s]] = make_float4(ax, ay, az, de);
+    acc[perm[s]] = make_float4(ax.s, ay.s, az.s, de.s);
 }
 
 int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const uint32_t* perm,
@@ -177,6 +197,8 @@ int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, co
     q.eta_h2 = p->eta * p->h * p->h;
     const double h = p->h;
     q.gw = (float)(-45.0 / (64.0 * 3.14159265358979323846 * h * h * h * h));   // dWp/dxi scale / h
+    q.inv_h2 = (float)(1.0 / (h * h));
+    q.rc2_64 = 4.0 * h * h;
     k_forces<<<(unsigned)cdiv(n, 128), 128, 0, st>>>(posm_s, velr_s, pc_s, perm, cell_start, n, to_dev(g),
                                                      two_h * two_h, q, acc_sph);
     SPHB_LAUNCHED();

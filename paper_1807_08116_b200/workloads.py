@@ -43,6 +43,17 @@ class Workload:
     eta: float = 0.1
     meta: dict = field(default_factory=dict)
 
+    def __post_init__(self):
+        # the boundary carries every parameter as FP32 (sph_params, dt): round them once here so
+        # the oracle (FP64) and the CUDA path see bit-identical parameter values
+        for k in ("h", "delta", "G", "dt", "gamma", "alpha", "beta", "eta"):
+            object.__setattr__(self, k, float(np.float32(getattr(self, k))))
+
+    def __setattr__(self, k, v):
+        if k in ("h", "delta", "G", "dt", "gamma", "alpha", "beta", "eta"):
+            v = float(np.float32(v))
+        object.__setattr__(self, k, v)
+
     @property
     def n_total(self) -> int:
         return self.n_gas + self.n_halo
