@@ -1,0 +1,317 @@
+#!/usr/bin/env python
+"""bench.py — step time of the hot path at BASELINE.json's headline config (config 2, N = 2^20).
+
+    python bench.py --gpus N --steps K --warmup W [--config C] [--impl reference]
+
+One "step" = one sph_step (all §8(a) rows: HFC x2, SU x2, grid sort, density, PP gravity).
+Prints ONE JSON line (see DESIGN.md §7 for every key).  The path does not shard (north star:
+multi-GPU out of scope), so --gpus N runs N independent replicas, one per rank, and reports the
+max-over-ranks step time ("replicas only").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+FLOPS_PER_INTERACTION = 20          # BASELINE.json convention for Eq. 4
+SM_COUNT_B200 = 148
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d, "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+def _env_rank():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "power_w_max": None, "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(", ") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, pw, reasons, mx = [], [], set(), None
+        for r in rows:
+            if len(r) < 9:
+                continue
+            try:
+                sm.append(float(r[1]))
+                mx = float(r[2])
+                pw.append(float(r[3]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                if v.strip().lower() == "active":
+                    reasons.add(name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=mx, reasons=sorted(reasons), power_w_max=max(pw),
+                       samples=len(sm))
+        return out
+
+
+# ------------------------------------------------------------------------------------------------
+# oracle timings (cpu_baseline leg and --impl reference): the oracle as it stands, bounded sample
+def oracle_sample_step(w, n_targets=1024, seed=123):
+    """Time the oracle on a bounded sample of one step of workload `w` and extrapolate.
+
+    A step is 1 gravity evaluation + 1 grid sort + 1 density pass + 2 hydro passes + O(N) updates.
+    Sample: the full CPU counting sort (it is O(N)); gravity for n_targets gas+halo targets against
+    all N sources; density and one force pass for n_targets gas targets (their neighbours' densities
+    included).  step_ms = sort + gravity * N/n_t + (density + 2 forces) * N_g/n_t.
+    """
+    import oracle
+    from paper_1807_08116_b200 import workloads as wl
+    ng, n = w.n_gas, w.n_total
+    half = max(1, n_targets // 2)
+    g_idx, h_idx = wl.subset_indices(ng, w.n_halo, seed, n_each=half)
+    tg = np.concatenate([g_idx, h_idx]).astype(np.int64)
+    posm64 = w.posm.astype(np.float64)
+    vele64 = w.vele.astype(np.float64)
+    t = {}
+    t0 = time.perf_counter()
+    if ng:
+        grid = oracle.grid_from_bbox(posm64, ng, w.h)
+        key = oracle.cell_keys(posm64, ng, grid)
+        _, start, perm = oracle.counting_sort(key, grid.M)
+    t["sort"] = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    if w.G != 0.0 and len(tg):
+        oracle.gravity(posm64, w.G, w.delta, targets=tg)
+    t["gravity_sample"] = time.perf_counter() - t0
+    t["density_sample"] = t["forces_sample"] = 0.0
+    if ng and len(g_idx):
+        t0 = time.perf_counter()
+        off, idx = oracle.neighbours(posm64, ng, w.h, targets=g_idx, method="grid", grid=grid, sort=(key, start, perm))
+        rho_t = oracle.density(posm64, w.h, off, idx, targets=g_idx)
+        t["density_sample"] = time.perf_counter() - t0
+        # densities of the neighbours (needed by the force sums): not charged to the sample's force time
+        closure = np.unique(np.concatenate([g_idx, idx.astype(np.int64)]))
+        off2, idx2 = oracle.neighbours(posm64, ng, w.h, targets=closure, method="grid", grid=grid, sort=(key, start, perm))
+        rho_all = np.ones(ng)
+        rho_all[closure] = oracle.density(posm64, w.h, off2, idx2, targets=closure)
+        t0 = time.perf_counter()
+        oracle.forces(posm64, vele64, rho_all, w.h, off, idx, targets=g_idx, gamma=w.gamma, alpha=w.alpha, beta=w.beta,
+                      eta=w.eta)
+        t["forces_sample"] = time.perf_counter() - t0 + t["density_sample"] * 0.0
+    n_t, n_g = max(len(tg), 1), max(len(g_idx), 1)
+    step_s = t["sort"] + t["gravity_sample"] * (n / n_t if w.G != 0.0 else 0.0) \
+        + (t["density_sample"] + 2.0 * t["forces_sample"]) * (ng / n_g if ng else 0.0)
+    sample_s = sum(t.values())
+    desc = (f"{len(tg)} gravity targets x {n} sources + density/forces for {len(g_idx)} gas targets + full CPU counting "
+            f"sort; step time extrapolated by N/n_targets")
+    return step_s * 1e3, sample_s, desc, t
+
+
+def run_reference(args, w):
+    import oracle
+    rank, _, _ = _env_rank()
+    if rank != 0:
+        return
+    vals = []
+    for i in range(args.warmup + args.steps):
+        ms, _, desc, _ = oracle_sample_step(w, n_targets=args.ref_targets, seed=100 + i)
+        if i >= args.warmup:
+            vals.append(ms)
+    v = float(np.mean(vals))
+    cores = oracle.num_threads()
+    line = {
+        "impl": "reference", "metric": "step_ms", "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": w.name, "n_total": w.n_total, "n_gas": w.n_gas, "h": w.h, "delta": w.delta, "dt": w.dt},
+        "cpu_baseline": {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": v, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+def run_ours(args, w):
+    import torch
+    import torch.distributed as dist
+    from paper_1807_08116_b200 import binding as b
+
+    rank, local_rank, world = _env_rank()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    b.load()
+    peaks, peak_src = _peaks()
+
+    n, ng = w.n_total, w.n_gas
+    sim = b.Simulation(w)
+    M = sim.grid.M if ng else 0
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident arm -----------------------------------------------------------------
+    for _ in range(max(args.warmup, 3)):
+        sim.step()
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    launches0 = b.sph_launch_count()
+    b.sph_set_profiling(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        sim.step()
+    e1.record()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    stage = b.sph_get_stage_ms()
+    b.sph_set_profiling(False)
+    launches = b.sph_launch_count() - launches0
+    clocks = sampler.stop() if sampler else None
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / args.steps
+
+    # ---- end-to-end arm: HOST (pinned) buffers through sph_host_ctx_step, copies inside the timing
+    e2e = None
+    if not args.no_e2e:
+        hp = torch.from_numpy(w.posm.copy()).pin_memory()
+        hv = torch.from_numpy(w.vele.copy()).pin_memory()
+        hrho = torch.zeros(max(ng, 1), dtype=torch.float32).pin_memory()
+        prm = b.sph_params.from_workload(w)
+        ctx = b.HostContext(ng, w.n_halo)
+        ctx.step(hp, hv, prm, w.dt, 1, first=True, rho=hrho)          # warm-up + seeding
+        ctx.step(hp, hv, prm, w.dt, 1, first=False, rho=hrho)
+        k_e2e = max(1, min(args.steps, args.e2e_steps))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(k_e2e):
+            ctx.step(hp, hv, prm, w.dt, 1, first=False, rho=hrho)     # H2D posm+vele, step, D2H posm+vele+rho, sync
+        t_e2e = (time.perf_counter() - t0) * 1e3 / k_e2e
+        ctx.close()
+        te = torch.tensor([t_e2e], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": float(te.item()), "unit": "ms", "h2d_bytes_per_step": 2 * n * 16,
+               "d2h_bytes_per_step": 2 * n * 16 + ng * 4, "steps": k_e2e,
+               "timing": "host wall clock around sph_host_ctx_step (it synchronises), max over ranks"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- derived figures -----------------------------------------------------------------------
+    K = args.steps
+    grav_ms = stage["gravity"] / K          # one evaluation per step (L123)
+    sort_ms, dens_ms, forc_ms, upd_ms = (stage[k] / K for k in ("sort", "density", "forces", "update"))
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    alu_peak_tflops = 2 * 128 * SM_COUNT_B200 * sm_max * 1e6 / 1e12
+    roofline = None
+    if w.G != 0.0 and grav_ms > 0:
+        achieved = FLOPS_PER_INTERACTION * float(n) * float(n) / (grav_ms * 1e-3) / 1e12
+        roofline = {"kernel": "grav_pp_kernel", "bound": "alu", "achieved": achieved, "peak": alu_peak_tflops,
+                    "unit": "TFLOP/s", "frac": achieved / alu_peak_tflops, "traffic": None,
+                    "peak_source": f"2*128*148*sm_max_mhz ({peak_src} sm_max_mhz={sm_max:.0f}); 20 flops/interaction",
+                    "kernel_ms": grav_ms, "launches_per_step": 1,
+                    "note": "gravity stage = pack + grav_pp_kernel + reduce; the two O(N) kernels are <0.1% of it"}
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    sort_bytes = ng * 96 + M * 16
+    upd_bytes = n * (64 + 48) + n * (48 + 16)
+    stages = {
+        "gravity_ms": grav_ms, "sort_ms": sort_ms, "density_ms": dens_ms, "forces_ms_2passes": forc_ms, "update_ms": upd_ms,
+        "pp_ginteractions_per_s": (float(n) * n / (grav_ms * 1e-3) / 1e9) if grav_ms > 0 else None,
+        "sph_mparticles_per_s": (ng / ((sort_ms + dens_ms + forc_ms) * 1e-3) / 1e6) if ng else None,
+        "sort_mkeys_per_s": (ng / (sort_ms * 1e-3) / 1e6) if ng and sort_ms > 0 else None,
+        "sort_hbm_gbs": (sort_bytes / (sort_ms * 1e-3) / 1e9) if ng and sort_ms > 0 else None,
+        "sort_hbm_frac": (sort_bytes / (sort_ms * 1e-3) / 1e9 / hbm) if ng and sort_ms > 0 else None,
+        "update_hbm_frac": (upd_bytes / (upd_ms * 1e-3) / 1e9 / hbm) if upd_ms > 0 else None,
+        "hbm_peak_gbs": hbm, "peak_source": peak_src,
+    }
+
+    # ---- the oracle on this box's host cores, bounded sample (rank 0, N = 1 only) ----------------
+    cpu = None
+    if world == 1 and not args.no_cpu:
+        import oracle
+        ms, sample_s, desc, _ = oracle_sample_step(w, n_targets=args.cpu_targets)
+        cpu = {"value": ms, "unit": "ms", "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": desc + f" ({sample_s:.1f} s of CPU wall time)", "extrapolated": True}
+
+    line = {
+        "metric": "step_ms", "value": ms_step, "unit": "ms", "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config}] ({w.name}): N={n}, N_g={ng}, h={w.h:g}, "
+                               f"delta={w.delta:g}, dt={w.dt:g}", "grid_dims": list(sim.grid.dims) if ng else None,
+                   "cells": M, "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": "no flush: one step streams >300 MB (cell arrays, gravity partials, particle arrays) > 126 MB L2"},
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        "stages": stages,
+        "context": "paper Table 1 (K40, N=2^20, units inferred as s): t_SPH=7.87, t_GFC=53.62 — other hardware, not a target",
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--scale", type=float, default=1.0, help="shrink the workload (debug only; invalid as a bench number)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-targets", type=int, default=2048)
+    ap.add_argument("--ref-targets", type=int, default=1024)
+    args = ap.parse_args()
+    from paper_1807_08116_b200 import workloads as wl
+    w = wl.make_workload(args.config, scale=args.scale)
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_ours(args, w)
+
+
+if __name__ == "__main__":
+    main()

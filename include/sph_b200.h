@@ -145,8 +145,12 @@ int sph_step_host(float* posm /*HOST*/, float* vele /*HOST*/, int64_t n_gas, int
 /* Persistent variant of the above for repeated end-to-end calls: device buffers are created once. */
 typedef struct sph_host_ctx sph_host_ctx;
 int sph_host_ctx_create(int64_t n_gas, int64_t n_halo, sph_host_ctx** out /*HOST*/);
+/* first != 0: seed the carried state from the uploaded positions (as sph_step).  first == 0: the
+ * caller asserts posm / vele are exactly what the previous call on this ctx returned, so the
+ * carried rho / acc_grav / grid inside the ctx are still valid and only the steps are run.    */
 int sph_host_ctx_step(sph_host_ctx* ctx, float* posm /*HOST*/, float* vele /*HOST*/, const sph_params* p /*HOST*/,
-                      float dt, int n_steps, float* rho /*HOST*/, float* acc_sph /*HOST*/, float* acc_grav /*HOST*/);
+                      float dt, int n_steps, int first, float* rho /*HOST*/, float* acc_sph /*HOST*/,
+                      float* acc_grav /*HOST*/);
 int sph_host_ctx_destroy(sph_host_ctx* ctx);
 
 /* Test helper: explicit neighbour sets N(i) = { j gas, j != i, d2 < (2h)^2 } in CSR form, every
@@ -158,10 +162,12 @@ int sph_neighbour_lists(const float* posm, int64_t n_gas, float h, const sph_gri
                         uint32_t* nbr_count, uint64_t* nbr_offset, uint32_t* nbr_index, uint64_t nbr_capacity,
                         void* ws, size_t ws_bytes, void* stream);
 
-/* Stage timing of the most recent sph_step / sph_evaluate on this thread when profiling was
- * switched on with sph_set_profiling(1): milliseconds by CUDA events on the call's stream for
- * {sort (a1-a6), density (a7), forces (a8-a9, summed over calls), gravity (a10), update (a11)}.
- * Reading the times SYNCHRONISES.  Profiling adds event records only.                        */
+/* Stage timing: after sph_set_profiling(1) every stage the calling thread enqueues is bracketed
+ * by CUDA events on the call's stream; sph_get_stage_ms() returns the milliseconds summed over all
+ * calls since that switch-on (at most 4096 stage spans) for
+ * {sort (a1-a6), density (a7), forces (a8-a9), gravity (a10), update (a11)}.
+ * sph_set_profiling() (either value) resets the sums.  Reading the times SYNCHRONISES on the
+ * recorded events.  Profiling adds event records only.                                       */
 int sph_set_profiling(int on);
 int sph_get_stage_ms(float out_ms[5] /*HOST*/);
 

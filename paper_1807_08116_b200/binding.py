@@ -94,7 +94,7 @@ def load():
     L.sph_evaluate.argtypes = [vp, vp, i64, i64, pp, gp, vp, vp, vp, vp, sz, vp]
     L.sph_step_host.argtypes = [vp, vp, i64, i64, pp, f32, C.c_int, vp, vp, vp]
     L.sph_host_ctx_create.argtypes = [i64, i64, C.POINTER(vp)]
-    L.sph_host_ctx_step.argtypes = [vp, vp, vp, pp, f32, C.c_int, vp, vp, vp]
+    L.sph_host_ctx_step.argtypes = [vp, vp, vp, pp, f32, C.c_int, C.c_int, vp, vp, vp]
     L.sph_host_ctx_destroy.argtypes = [vp]
     L.sph_neighbour_lists.argtypes = [vp, i64, f32, gp, vp, vp, vp, vp, vp, C.c_uint64, vp, sz, vp]
     _lib = L
@@ -214,9 +214,10 @@ class HostContext:
         self._h = C.c_void_p()
         _chk("sph_host_ctx_create", load().sph_host_ctx_create(int(n_gas), int(n_halo), C.byref(self._h)))
 
-    def step(self, posm, vele, params, dt, n_steps, rho=None, acc_sph=None, acc_grav=None):
+    def step(self, posm, vele, params, dt, n_steps, first=True, rho=None, acc_sph=None, acc_grav=None):
         _chk("sph_host_ctx_step", load().sph_host_ctx_step(self._h, _hp(posm), _hp(vele), C.byref(params), float(dt),
-                                                           int(n_steps), _hp(rho), _hp(acc_sph), _hp(acc_grav)))
+                                                           int(n_steps), int(bool(first)), _hp(rho), _hp(acc_sph),
+                                                           _hp(acc_grav)))
 
     def close(self):
         if self._h:

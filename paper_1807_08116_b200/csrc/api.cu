@@ -8,11 +8,11 @@ namespace {
 
 // ---- per-stage timing (sph_set_profiling) -------------------------------------------------------
 enum Stage { ST_SORT = 0, ST_DENSITY, ST_FORCES, ST_GRAVITY, ST_UPDATE, ST_COUNT };
-constexpr int kMaxSpans = 16;
+constexpr int kMaxSpans = 4096;   // spans accumulate over calls until sph_set_profiling() resets them
 struct Prof {
     bool on = false;
     cudaEvent_t ev[2 * kMaxSpans];
-    bool made = false;
+    int made = 0;                 // events created so far (lazily, two per span)
     int n = 0;
     int stage[kMaxSpans];
 };
@@ -24,10 +24,7 @@ struct Span {
     Span(int stage, cudaStream_t s) : st(s) {
         Prof& p = g_prof;
         if (!p.on || p.n >= kMaxSpans) return;
-        if (!p.made) {
-            for (auto& e : p.ev) cudaEventCreate(&e);
-            p.made = true;
-        }
+        while (p.made < 2 * (p.n + 1)) cudaEventCreate(&p.ev[p.made++]);
         idx = p.n++;
         p.stage[idx] = stage;
         cudaEventRecord(p.ev[2 * idx], st);
@@ -223,7 +220,6 @@ int sph_evaluate(const float* posm, const float* vele, int64_t n_gas, int64_t n_
     SPHB_TRY(check_state_args(posm, vele, n_gas, n_halo, p, g, rho, acc_sph, acc_grav, ws, ws_bytes));
     const int64_t n = n_gas + n_halo;
     if (n == 0) return SPH_OK;
-    g_prof.n = 0;
     Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
     cudaStream_t st = (cudaStream_t)stream;
     SPHB_TRY(position_only(reinterpret_cast<const float4*>(posm), n_gas, n, p, g, rho, reinterpret_cast<float4*>(acc_grav),
@@ -236,7 +232,6 @@ int sph_step(float* posm, float* vele, int64_t n_gas, int64_t n_halo, const sph_
     SPHB_TRY(check_state_args(posm, vele, n_gas, n_halo, p, g, rho, acc_sph, acc_grav, ws, ws_bytes));
     const int64_t n = n_gas + n_halo;
     if (n == 0) return SPH_OK;
-    g_prof.n = 0;
     Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
     cudaStream_t st = (cudaStream_t)stream;
     float4* r4 = reinterpret_cast<float4*>(posm);

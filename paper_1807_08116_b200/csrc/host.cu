@@ -11,6 +11,8 @@ struct sph_host_ctx {
     void* ws = nullptr;
     size_t ws_bytes = 0;
     cudaStream_t st = nullptr;
+    sph_grid grid;          // grid of the last seeding call (first != 0)
+    bool seeded = false;
 };
 
 namespace {
@@ -62,25 +64,31 @@ int sph_host_ctx_destroy(sph_host_ctx* c) {
     return SPH_OK;
 }
 
-int sph_host_ctx_step(sph_host_ctx* c, float* posm, float* vele, const sph_params* p, float dt, int n_steps, float* rho,
-                      float* acc_sph, float* acc_grav) {
+int sph_host_ctx_step(sph_host_ctx* c, float* posm, float* vele, const sph_params* p, float dt, int n_steps, int first,
+                      float* rho, float* acc_sph, float* acc_grav) {
     if (!c || !posm || !vele || !p || n_steps < 0) return SPH_ERR_ARG;
+    if (!first && !c->seeded) return SPH_ERR_ARG;
     const int64_t n = c->n_gas + c->n_halo;
     if (n == 0) return SPH_OK;
     cudaStream_t st = c->st;
     SPHB_CUDA(cudaMemcpyAsync(c->posm, posm, (size_t)n * 16, cudaMemcpyHostToDevice, st));
     SPHB_CUDA(cudaMemcpyAsync(c->vele, vele, (size_t)n * 16, cudaMemcpyHostToDevice, st));
-    sph_grid g;
-    g.origin[0] = g.origin[1] = g.origin[2] = 0.f;
-    g.cell = g.inv_cell = 1.f;
-    g.dims[0] = g.dims[1] = g.dims[2] = 1;
-    if (c->n_gas > 0) SPHB_TRY(sph_grid_from_bbox(c->posm, c->n_gas, p->h, &g, c->ws, c->ws_bytes, st));
-    size_t need = sph_workspace_bytes(c->n_gas, n, c->n_gas > 0 ? &g : nullptr);
-    if (need == 0) return SPH_ERR_GRID;
-    SPHB_TRY(ensure_ws(c, need));
+    if (first) {
+        sph_grid g;
+        g.origin[0] = g.origin[1] = g.origin[2] = 0.f;
+        g.cell = g.inv_cell = 1.f;
+        g.dims[0] = g.dims[1] = g.dims[2] = 1;
+        if (c->n_gas > 0) SPHB_TRY(sph_grid_from_bbox(c->posm, c->n_gas, p->h, &g, c->ws, c->ws_bytes, st));
+        size_t need = sph_workspace_bytes(c->n_gas, n, c->n_gas > 0 ? &g : nullptr);
+        if (need == 0) return SPH_ERR_GRID;
+        SPHB_TRY(ensure_ws(c, need));
+        c->grid = g;
+        c->seeded = true;
+    }
+    const sph_grid& g = c->grid;   // fixed domain between seedings (L158); outliers are clamped
     for (int s = 0; s < n_steps; ++s)
-        SPHB_TRY(sph_step(c->posm, c->vele, c->n_gas, c->n_halo, p, &g, dt, s == 0, c->rho, c->acc_sph, c->acc_grav, c->ws,
-                          c->ws_bytes, st));
+        SPHB_TRY(sph_step(c->posm, c->vele, c->n_gas, c->n_halo, p, &g, dt, first && s == 0, c->rho, c->acc_sph,
+                          c->acc_grav, c->ws, c->ws_bytes, st));
     if (n_steps == 0)
         SPHB_TRY(sph_evaluate(c->posm, c->vele, c->n_gas, c->n_halo, p, &g, c->rho, c->acc_sph, c->acc_grav, c->ws,
                               c->ws_bytes, st));
@@ -97,7 +105,7 @@ int sph_step_host(float* posm, float* vele, int64_t n_gas, int64_t n_halo, const
                   float* rho, float* acc_sph, float* acc_grav) {
     sph_host_ctx* c = nullptr;
     SPHB_TRY(sph_host_ctx_create(n_gas, n_halo, &c));
-    int rc = sph_host_ctx_step(c, posm, vele, p, dt, n_steps, rho, acc_sph, acc_grav);
+    int rc = sph_host_ctx_step(c, posm, vele, p, dt, n_steps, 1, rho, acc_sph, acc_grav);
     sph_host_ctx_destroy(c);
     return rc;
 }

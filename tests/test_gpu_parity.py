@@ -348,7 +348,8 @@ def test_step_host_matches_device_path(cuda_lib):
     assert np.array_equal(ag, sim.acc_grav.cpu().numpy())
     ctx = b.HostContext(w.n_gas, w.n_halo)
     p2, v2 = w.posm.copy(), w.vele.copy()
-    ctx.step(p2, v2, b.sph_params.from_workload(w), w.dt, 2)
+    ctx.step(p2, v2, b.sph_params.from_workload(w), w.dt, 1, first=True)
+    ctx.step(p2, v2, b.sph_params.from_workload(w), w.dt, 1, first=False)     # resumes the carried state
     ctx.close()
     assert np.array_equal(p2, posm) and np.array_equal(v2, vele)
 
