@@ -1,0 +1,127 @@
+"""Large-N protocol: BASELINE.json's full-size configs in the launch configuration
+bench.py times.  O(N) structures (keys, perm, ranges) and the O(N) update formulas are checked
+on ALL particles; gravity and the SPH sums on a seeded 4096-particle subset (2048 gas + 2048
+halo, plus forced members), stage by stage (teacher-forced: each stage's oracle input is the
+GPU's verified output of the previous stage)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1807_08116_b200 import workloads as wl
+from parity_util import check_density, check_values
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+
+def _subset(w, key, count):
+    g_idx, h_idx = wl.subset_indices(w.n_gas, w.n_halo, w.seed, n_each=2048)
+    forced = []
+    if w.n_gas:
+        gas = w.posm[: w.n_gas, :3]
+        forced += [int(gas[:, a].argmin()) for a in range(3)] + [int(gas[:, a].argmax()) for a in range(3)]
+        forced.append(int(np.flatnonzero(key == np.argmax(count))[0]))      # a particle of the fullest cell
+    g_idx = np.unique(np.concatenate([g_idx, np.array(forced, dtype=np.int64)])) if w.n_gas else g_idx
+    return g_idx.astype(np.int64), h_idx.astype(np.int64)
+
+
+def _check_structures(b, sim, w):
+    """keys / perm / start inside the workspace against the oracle's sequential counting sort: ALL particles."""
+    ng = w.n_gas
+    og = oracle.grid_from_bbox(w.posm, ng, w.h)
+    assert tuple(og.dims) == tuple(sim.grid.dims)
+    d = sim.posm
+    M = sim.grid.M
+    key = torch.zeros(ng, dtype=torch.int32, device="cuda")
+    perm = torch.zeros(ng, dtype=torch.int32, device="cuda")
+    count = torch.zeros(M, dtype=torch.int32, device="cuda")
+    start = torch.zeros(M + 1, dtype=torch.int32, device="cuda")
+    b.sph_build_grid(d, ng, sim.grid, key, perm, count, start, sim.ws)
+    okey = oracle.cell_keys(w.posm, ng, og)
+    ocount, ostart, operm = oracle.counting_sort(okey, M)
+    assert np.array_equal(key.cpu().numpy().view(np.uint32), okey)
+    assert np.array_equal(start.cpu().numpy().view(np.uint32), ostart)
+    assert np.array_equal(perm.cpu().numpy().view(np.uint32), operm)
+    assert np.array_equal(count.cpu().numpy().view(np.uint32), ocount)
+    return og, okey, ocount, ostart, operm
+
+
+def _check_sph_subset(w, posm, vele, rho_gpu, acc_sph_gpu, g_idx, og, sort):
+    """density for the subset, forces for the subset with the GPU's verified rho as input."""
+    off, idx = oracle.neighbours(posm, w.n_gas, w.h, targets=g_idx, method="grid", grid=og, sort=sort)
+    orho = oracle.density(posm, w.h, off, idx, targets=g_idx)
+    check_density(rho_gpu[g_idx], orho, "rho subset")
+    # every neighbour's density is also checked (two-hop closure): a wrong rho_j would otherwise hide
+    closure = np.unique(idx.astype(np.int64))
+    if len(closure):
+        off2, idx2 = oracle.neighbours(posm, w.n_gas, w.h, targets=closure, method="grid", grid=og, sort=sort)
+        check_density(rho_gpu[closure], oracle.density(posm, w.h, off2, idx2, targets=closure), "rho closure")
+    of, gross = oracle.forces(posm, vele, rho_gpu.astype(np.float64), w.h, off, idx, targets=g_idx, gamma=w.gamma,
+                              alpha=w.alpha, beta=w.beta, eta=w.eta, with_gross=True)
+    check_values(acc_sph_gpu[g_idx, :3], of[:, :3], "a_sph subset", gross=gross[:, 0])
+    check_values(acc_sph_gpu[g_idx, 3], of[:, 3], "de/dt subset", gross=gross[:, 1])
+    return np.diff(off)
+
+
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_full_size_collision(cuda_lib, cfg):
+    b = cuda_lib
+    w = wl.make_workload(cfg)
+    ng, n = w.n_gas, w.n_total
+    sim = b.Simulation(w)
+    og, okey, ocount, ostart, operm = _check_structures(b, sim, w)
+    g_idx, h_idx = _subset(w, okey, ocount)
+    tg = np.concatenate([g_idx, h_idx])
+    # ---- force evaluation at t = 0
+    sim.evaluate()
+    rho0 = sim.rho.cpu().numpy()
+    as0 = sim.acc_sph.cpu().numpy()
+    ag0 = sim.acc_grav.cpu().numpy()
+    check_values(ag0[tg, :3], oracle.gravity(w.posm, w.G, w.delta, targets=tg), f"a_grav cfg{cfg} subset")
+    assert np.all(ag0[:, 3] == 0)
+    nn = _check_sph_subset(w, w.posm, w.vele, rho0, as0, g_idx, og, (okey, ostart, operm))
+    assert nn.max() > 10
+    if cfg == 3:
+        return                      # one evaluation at N = 2^22 is enough for the suite's time budget
+    # ---- one step; O(N) update formulas on ALL particles from the GPU's own stage outputs (FP64 restatement)
+    sim.step()
+    p1 = sim.posm.cpu().numpy()
+    v1 = sim.vele.cpu().numpy()
+    ag1 = sim.acc_grav.cpu().numpy().astype(np.float64)
+    as1 = sim.acc_sph.cpu().numpy().astype(np.float64)
+    dt = w.dt
+    Q0 = ag0[:, :3].astype(np.float64)
+    Q0[:ng] += as0[:, :3]
+    v0 = w.vele[:, :3].astype(np.float64)
+    e0 = w.vele[:ng, 3].astype(np.float64)
+    vt = v0 + dt * Q0                                                # Eq. 12
+    et = e0 + dt * as0[:, 3].astype(np.float64)                      # Eq. 13
+    r1 = w.posm[:, :3].astype(np.float64) + 0.5 * dt * (vt + v0)     # Eq. 14
+    assert np.abs(p1[:, :3] - r1).max() <= 2e-6 * max(1.0, np.abs(r1).max())
+    assert np.array_equal(p1[:, 3], w.posm[:, 3])
+    Q1 = ag1[:, :3].copy()
+    Q1[:ng] += as1[:, :3]
+    check_values(v1[:, :3], 0.5 * (v0 + vt) + 0.5 * dt * Q1, "v(t+dt) all", max_tol=2e-6, med_tol=2e-7)     # Eq. 15
+    check_values(v1[:ng, 3], 0.5 * (e0 + et) + 0.5 * dt * as1[:, 3], "e(t+dt) all", max_tol=2e-6, med_tol=2e-7)  # Eq. 16
+    # ---- the position-only quantities and the corrector's hydro terms at r(t+dt), subset
+    check_values(ag1[tg, :3], oracle.gravity(p1, w.G, w.delta, targets=tg), "a_grav(t+dt) subset")
+    key1 = oracle.cell_keys(p1, ng, og)
+    _, start1, perm1 = oracle.counting_sort(key1, og.M)
+    vele_t = np.zeros((n, 4))
+    vele_t[:, :3] = vt
+    vele_t[:ng, 3] = et
+    _check_sph_subset(w, p1, vele_t, sim.rho.cpu().numpy(), sim.acc_sph.cpu().numpy(), g_idx, og, (key1, start1, perm1))
+
+
+def test_full_size_sph_only_config4(cuda_lib):
+    """config 4: N_g = 2^24 gas, no gravity — grid sort on all particles, density / forces on the subset."""
+    b = cuda_lib
+    w = wl.make_workload(4)
+    sim = b.Simulation(w)
+    og, okey, ocount, ostart, operm = _check_structures(b, sim, w)
+    g_idx, _ = _subset(w, okey, ocount)
+    sim.evaluate()
+    assert torch.count_nonzero(sim.acc_grav).item() == 0
+    nn = _check_sph_subset(w, w.posm, w.vele, sim.rho.cpu().numpy(), sim.acc_sph.cpu().numpy(), g_idx, og,
+                           (okey, ostart, operm))
+    assert nn.max() > 500           # the clump cores
