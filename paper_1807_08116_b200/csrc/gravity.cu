@@ -276,6 +276,10 @@ static int launch_grav(const float4* posm, const float4* pk, int n, int tiles, i
 int gravity(const float4* posm, int64_t n_total, float G, float delta, float4* acc_grav, float4* src_pk,
             float4* grav_part, cudaStream_t st) {
     if (n_total <= 0) return SPH_OK;
+    if (G == 0.0f) {   // no self-gravity (BASELINE config 4, "SPH-only"): Eq. 4 is identically 0
+        SPHB_CUDA(cudaMemsetAsync(acc_grav, 0, (size_t)n_total * sizeof(float4), st));
+        return SPH_OK;
+    }
     const int n = (int)n_total;
     const int n_pad = (int)grav_padded(n_total);
     int I, threads, S;
