@@ -161,17 +161,40 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_tile_sums(const uint32_t*
     }
 }
 
-// one CTA: exclusive scan of the tile sums in place (chunks of 256 with a running carry)
-__global__ void __launch_bounds__(kScanThreads) k_scan_tile_offsets(uint32_t* tile_sums, int n_tiles) {
-    __shared__ uint32_t ws[kScanThreads / 32];
-    uint32_t carry = 0;
-    for (int base = 0; base < n_tiles; base += kScanThreads) {
-        int i = base + threadIdx.x;
-        uint32_t v = i < n_tiles ? tile_sums[i] : 0u, total;
-        uint32_t ex = block_exclusive_scan(v, ws, total);
-        if (i < n_tiles) tile_sums[i] = carry + ex;
-        carry += total;
-        __syncthreads();
+// one CTA of 1024 threads: exclusive scan of the tile sums in place.  Thread t owns the contiguous
+// slice [t*per, (t+1)*per): local sum, one block scan over the 1024 slice sums, local rescan —
+// a single pass whatever n_tiles is (the chunked version needed n_tiles/256 dependent block scans).
+constexpr int kOffThreads = 1024;
+__global__ void __launch_bounds__(kOffThreads) k_scan_tile_offsets(uint32_t* tile_sums, int n_tiles) {
+    __shared__ uint32_t ws[32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int per = (n_tiles + kOffThreads - 1) / kOffThreads;
+    const int lo = min(threadIdx.x * per, n_tiles), hi = min(lo + per, n_tiles);
+    uint32_t s = 0;
+    for (int i = lo; i < hi; ++i) s += tile_sums[i];
+    uint32_t inc = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) ws[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        uint32_t v = ws[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, v, o);
+            if (lane >= o) v += t;
+        }
+        ws[lane] = v;
+    }
+    __syncthreads();
+    uint32_t run = (w > 0 ? ws[w - 1] : 0u) + inc - s;
+    for (int i = lo; i < hi; ++i) {
+        const uint32_t v = tile_sums[i];
+        tile_sums[i] = run;
+        run += v;
     }
 }
 
@@ -223,8 +246,14 @@ __global__ void __launch_bounds__(256) k_stable(const uint32_t* __restrict__ tmp
     const uint32_t i = tmp[s];
     const uint32_t k = key[i];
     const uint32_t a = start[k], b = start[k + 1];
-    uint32_t r = 0;
-    for (uint32_t t = a; t < b; ++t) r += (tmp[t] < i) ? 1u : 0u;
+    uint32_t r = 0, t = a;
+    // tmp is 16-byte aligned (workspace carve): scalar head to a multiple of 4, uint4 body, scalar tail
+    for (; t < b && (t & 3u); ++t) r += (tmp[t] < i) ? 1u : 0u;
+    for (; t + 4u <= b; t += 4u) {
+        const uint4 v = *reinterpret_cast<const uint4*>(tmp + t);
+        r += (v.x < i ? 1u : 0u) + (v.y < i ? 1u : 0u) + (v.z < i ? 1u : 0u) + (v.w < i ? 1u : 0u);
+    }
+    for (; t < b; ++t) r += (tmp[t] < i) ? 1u : 0u;
     perm[a + r] = i;
     if (posm_s) posm_s[a + r] = posm[i];
 }
@@ -278,7 +307,7 @@ int grid_build(const float4* posm, int64_t n_gas, const sph_grid* g, uint32_t* k
     const int n_tiles = (int)cdiv(M, kScanTile);
     k_scan_tile_sums<<<n_tiles, kScanThreads, 0, st>>>(cell_count, M, tile_sums);          // K2 (in-block)
     SPHB_LAUNCHED();
-    k_scan_tile_offsets<<<1, kScanThreads, 0, st>>>(tile_sums, n_tiles);                   // K2 (across blocks)
+    k_scan_tile_offsets<<<1, kOffThreads, 0, st>>>(tile_sums, n_tiles);                   // K2 (across blocks)
     SPHB_LAUNCHED();
     k_scan_apply<<<n_tiles, kScanThreads, 0, st>>>(cell_count, M, tile_sums, cell_start, (uint32_t)n);   // K3
     SPHB_LAUNCHED();
