@@ -134,6 +134,23 @@ int sph_evaluate(const float* posm, const float* vele, int64_t n_gas, int64_t n_
                  const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/,
                  float* rho, float* acc_sph, float* acc_grav, void* ws, size_t ws_bytes, void* stream);
 
+/* Modified CFL step, Eq. 17 (L125-129):
+ *   dt = C_CFL min_i  s_i / ( c_i^max (1 + 1.2 alpha) + 1.2 beta mu_i^max + sqrt( s_i (|Q_i| + |E_i|) ) )
+ * over the gas particles, with, over the neighbours j of i (same FP32 cutoff predicate as everywhere,
+ * j != i, pairs at zero separation skipped as in A9):
+ *   s_i = min_j |r_i - r_j|,  c_i^max = max_j (c_i + c_j)/2,  mu_i^max = max_j |mu_ij|  (mu_ij of L97; A23),
+ *   Q_i = acc_sph[i].xyz + acc_grav[i].xyz (right-hand side of Eq. 10),  E_i = acc_sph[i].w (Eq. 11).
+ * A gas particle without neighbours takes s_i = 2h, c^max = c_i, mu^max = 0 (A22).  rho, acc_sph,
+ * acc_grav are the arrays the last sph_evaluate / sph_step left behind; perm / cell_start the grid
+ * of the same positions.  dt_out: DEVICE, one float (+inf if n_gas = 0).  dt_particle: DEVICE
+ * [n_gas], the bracket of Eq. 17 per particle WITHOUT C_CFL, or NULL.  The minimum is taken with
+ * integer atomics on the float bit pattern: exact and order-independent.                       */
+int sph_cfl_dt(const float* posm, const float* vele, const float* rho, const float* acc_sph, const float* acc_grav,
+               int64_t n_gas, const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/,
+               const uint32_t* perm, const uint32_t* cell_start, float c_cfl,
+               float* dt_out /*[1]*/, float* dt_particle /*[n_gas] or NULL*/,
+               void* ws, size_t ws_bytes, void* stream);
+
 /* End-to-end entry point with HOST buffers: copies posm / vele to the device, derives the grid
  * from the gas bounding box, runs `n_steps` steps (first = 1 on the first), copies posm, vele,
  * rho, acc_sph, acc_grav back (any output pointer may be NULL) and synchronises.  Allocates and

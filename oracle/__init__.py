@@ -78,6 +78,8 @@ def lib():
         L.orc_neighbours_grid.restype = None
         L.orc_density.argtypes = [dp, C.c_double, ip, C.c_int64, ip, up, dp]
         L.orc_density.restype = None
+        L.orc_cfl_terms.argtypes = [dp, dp, dp, C.POINTER(_Params), ip, C.c_int64, ip, up, dp]
+        L.orc_cfl_terms.restype = None
         L.orc_forces.argtypes = [dp, dp, dp, C.POINTER(_Params), ip, C.c_int64, ip, up, dp, dp]
         L.orc_forces.restype = None
         _lib = L
@@ -244,6 +246,35 @@ def forces(posm, vele, rho_all, h, offsets, index, targets=None, gamma=5.0 / 3.0
                          _p(tg, C.c_int64), nt, _p(off, C.c_int64), _p(idx, C.c_uint32), _p(out, C.c_double),
                          _p(gross, C.c_double))
     return (out, gross) if with_gross else out
+
+
+def cfl_dt(posm, vele, rho_all, acc_sph, acc_grav, h, offsets, index, c_cfl, targets=None, gamma=5.0 / 3.0, alpha=0.5,
+           beta=1.0, eta=0.1):
+    """Eq. 17 (L125-129): returns (dt, bracket[nt]) with dt = C_CFL min_i bracket_i,
+    bracket_i = s_i / (c_i^max (1 + 1.2 alpha) + 1.2 beta mu_i^max + sqrt(s_i (|Q_i| + |E_i|))).
+    acc_sph[nt,4] = (a_sph, de/dt) and acc_grav[nt,>=3] are given FOR THE TARGETS (Q_i = a_sph + a_grav is the
+    right-hand side of Eq. 10, E_i of Eq. 11); rho_all is indexed by gas index."""
+    posm, vele, rho_all = _f64(posm), _f64(vele), _f64(rho_all)
+    tg = _tg(targets)
+    nt = len(offsets) - 1
+    terms = np.zeros((nt, 3), dtype=np.float64)
+    idx = np.ascontiguousarray(index, dtype=np.uint32)
+    if len(idx) == 0:
+        idx = np.zeros(1, dtype=np.uint32)
+    off = np.ascontiguousarray(offsets, dtype=np.int64)
+    prm = _Params(float(h), float(gamma), float(alpha), float(beta), float(eta))
+    if nt == 0:
+        return np.inf, np.zeros(0)
+    lib().orc_cfl_terms(_p(posm, C.c_double), _p(vele, C.c_double), _p(rho_all, C.c_double), C.byref(prm),
+                        _p(tg, C.c_int64), nt, _p(off, C.c_int64), _p(idx, C.c_uint32), _p(terms, C.c_double))
+    a_s = np.asarray(acc_sph, dtype=np.float64)
+    a_g = np.asarray(acc_grav, dtype=np.float64)
+    Q = np.linalg.norm(a_s[:, :3] + a_g[:, :3], axis=1)
+    E = np.abs(a_s[:, 3])
+    s, cmax, mumax = terms[:, 0], terms[:, 1], terms[:, 2]
+    with np.errstate(divide="ignore"):
+        bracket = s / (cmax * (1.0 + 1.2 * alpha) + 1.2 * beta * mumax + np.sqrt(s * (Q + E)))
+    return float(c_cfl * bracket.min()), bracket
 
 
 # ------------------------------------------------------------------ whole evaluation / step (O6)

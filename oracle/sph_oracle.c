@@ -21,7 +21,9 @@
  * Parity unpinned (specifications of this build, not fixed by the paper):
  *   - the softening form of Eq. 4 (reading A1: Plummer, (|dr|^2 + delta^2)^(3/2));
  *   - gamma (reading A6: a parameter, default 5/3);
- *   - the cell geometry / linearisation (reading A7).
+ *   - the cell geometry / linearisation (reading A7);
+ *   - in Eq. 17 (orc_cfl_terms): the value for a particle without neighbours (reading A22) and
+ *     taking mu^max as the largest magnitude (reading A23).
  * Everything else is pinned by tests/test_oracle_pins.py.
  *
  * Build: gcc -O2 -fopenmp -ffp-contract=off -shared -fPIC (oracle/build.py).
@@ -399,5 +401,41 @@ void orc_forces(const double* posm, const double* vele, const double* rho_all, c
         out[4 * t + 1] = ay;
         out[4 * t + 2] = az;
         out[4 * t + 3] = de;
+    }
+}
+
+/* Modified CFL condition, Eq. 17 (L125-129), per target particle i over its neighbour list:
+ *   s_i = min_j |r_i - r_j|,  c_i^max = max_j c_ij,  mu_i^max = max_j |mu_ij|
+ * with c_ij = (c_i + c_j)/2, c = sqrt(gamma p / rho) (L99) and mu_ij of L97.  Readings:
+ * A23 mu^max is the largest MAGNITUDE (mu_ij <= 0 by its definition, so "max" as printed would always
+ * be 0); A9 pairs at zero separation are skipped; A22 a particle with no neighbour gets s = 2h,
+ * c^max = c_i, mu^max = 0.  out[t] = (s_i, c_i^max, mu_i^max).                                     */
+void orc_cfl_terms(const double* posm, const double* vele, const double* rho_all, const orc_sph_params* p,
+                   const int64_t* targets, int64_t nt,
+                   const int64_t* nbr_offset, const uint32_t* nbr_index, double* out) {
+    const double h = p->h, gm1 = p->gamma - 1.0;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t t = 0; t < nt; ++t) {
+        int64_t i = targets ? targets[t] : t;
+        double ci = sqrt(p->gamma * (gm1 * rho_all[i] * vele[4 * i + 3]) / rho_all[i]);
+        double smin = -1.0, cmax = ci, mumax = 0.0;
+        for (int64_t q = nbr_offset[t]; q < nbr_offset[t + 1]; ++q) {
+            int64_t j = nbr_index[q];
+            double dx = posm[4 * i] - posm[4 * j], dy = posm[4 * i + 1] - posm[4 * j + 1], dz = posm[4 * i + 2] - posm[4 * j + 2];
+            double r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 == 0.0) continue;
+            double r = sqrt(r2);
+            double rv = dx * (vele[4 * i] - vele[4 * j]) + dy * (vele[4 * i + 1] - vele[4 * j + 1]) +
+                        dz * (vele[4 * i + 2] - vele[4 * j + 2]);
+            double mu = (rv < 0.0) ? h * rv / (r2 + p->eta * h * h) : 0.0;
+            double cj = sqrt(p->gamma * (gm1 * rho_all[j] * vele[4 * j + 3]) / rho_all[j]);
+            double cij = 0.5 * (ci + cj);
+            if (smin < 0.0 || r < smin) smin = r;
+            if (cij > cmax) cmax = cij;
+            if (fabs(mu) > mumax) mumax = fabs(mu);
+        }
+        out[3 * t + 0] = smin < 0.0 ? 2.0 * h : smin;
+        out[3 * t + 1] = cmax;
+        out[3 * t + 2] = mumax;
     }
 }

@@ -24,7 +24,7 @@ EXPORTS = (
     "sph_last_cuda_error", "sph_grid_from_bbox", "sph_workspace_bytes", "sph_build_grid", "sph_neighbour_ranges",
     "sph_density", "sph_forces", "nbody_pp_gravity", "sph_step", "sph_evaluate", "sph_step_host",
     "sph_host_ctx_create", "sph_host_ctx_step", "sph_host_ctx_destroy", "sph_neighbour_lists",
-    "sph_set_profiling", "sph_get_stage_ms", "sph_launch_count",
+    "sph_set_profiling", "sph_get_stage_ms", "sph_launch_count", "sph_cfl_dt",
 )
 
 
@@ -90,6 +90,7 @@ def load():
     L.sph_density.argtypes = [vp, i64, pp, gp, vp, vp, vp, vp, sz, vp]
     L.sph_forces.argtypes = [vp, vp, vp, i64, pp, gp, vp, vp, vp, vp, sz, vp]
     L.nbody_pp_gravity.argtypes = [vp, i64, f32, f32, vp, vp, sz, vp]
+    L.sph_cfl_dt.argtypes = [vp, vp, vp, vp, vp, i64, pp, gp, vp, vp, f32, vp, vp, vp, sz, vp]
     L.sph_step.argtypes = [vp, vp, i64, i64, pp, gp, f32, C.c_int, vp, vp, vp, vp, sz, vp]
     L.sph_evaluate.argtypes = [vp, vp, i64, i64, pp, gp, vp, vp, vp, vp, sz, vp]
     L.sph_step_host.argtypes = [vp, vp, i64, i64, pp, f32, C.c_int, vp, vp, vp]
@@ -175,6 +176,14 @@ def nbody_pp_gravity(posm, n_total, G, delta, acc_grav, ws):
     p, nb = _ws(ws)
     _chk("nbody_pp_gravity", load().nbody_pp_gravity(_ptr(posm), int(n_total), float(G), float(delta), _ptr(acc_grav),
                                                      p, nb, _stream()))
+
+
+def sph_cfl_dt(posm, vele, rho, acc_sph, acc_grav, n_gas, params, grid, perm, cell_start, c_cfl, dt_out, dt_particle, ws):
+    p, nb = _ws(ws)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_cfl_dt", load().sph_cfl_dt(_ptr(posm), _ptr(vele), _ptr(rho), _ptr(acc_sph), _ptr(acc_grav), int(n_gas),
+                                         C.byref(params), g, _ptr(perm), _ptr(cell_start), float(c_cfl), _ptr(dt_out),
+                                         _ptr(dt_particle), p, nb, _stream()))
 
 
 def sph_step(posm, vele, n_gas, n_halo, params, grid, dt, first, rho, acc_sph, acc_grav, ws):

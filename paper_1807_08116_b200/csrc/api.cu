@@ -199,6 +199,27 @@ int sph_forces(const float* posm, const float* vele, const float* rho, int64_t n
                          w.pc_s, reinterpret_cast<float4*>(acc_sph), st);
 }
 
+int sph_cfl_dt(const float* posm, const float* vele, const float* rho, const float* acc_sph, const float* acc_grav,
+               int64_t n_gas, const sph_params* p, const sph_grid* g, const uint32_t* perm, const uint32_t* cell_start,
+               float c_cfl, float* dt_out, float* dt_particle, void* ws, size_t ws_bytes, void* stream) {
+    if (bad_count(n_gas) || !dt_out || !(c_cfl > 0.f)) return SPH_ERR_ARG;
+    SPHB_TRY(check_params(p, n_gas > 0));
+    cudaStream_t st = (cudaStream_t)stream;
+    if (n_gas == 0)
+        return cfl_sorted(nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, p, g, c_cfl, nullptr, nullptr,
+                          dt_out, dt_particle, st);
+    if (!posm || !vele || !rho || !acc_sph || !acc_grav || !perm || !cell_start || !ws || !aligned16(posm) ||
+        !aligned16(vele) || !aligned16(acc_sph) || !aligned16(acc_grav) || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return SPH_ERR_ARG;
+    SPHB_TRY(check_grid(g, p->h));
+    Workspace w = carve(ws, n_gas, n_gas, g);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
+    return cfl_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, reinterpret_cast<const float4*>(acc_sph),
+                      reinterpret_cast<const float4*>(acc_grav), perm, cell_start, n_gas, p, g, c_cfl, w.velr_s, w.pc_s,
+                      dt_out, dt_particle, st);
+}
+
 int nbody_pp_gravity(const float* posm, int64_t n_total, float G, float delta, float* acc_grav, void* ws,
                      size_t ws_bytes, void* stream) {
     if (bad_count(n_total)) return SPH_ERR_ARG;

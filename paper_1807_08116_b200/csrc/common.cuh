@@ -92,6 +92,9 @@ int density_sorted(const float4* posm_s, const uint32_t* perm, const uint32_t* c
 int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const uint32_t* perm,
                   const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
                   float4* velr_s, float2* pc_s, float4* acc_sph, cudaStream_t st);
+int cfl_sorted(const float4* posm_s, const float4* vele, const float* rho, const float4* acc_sph, const float4* acc_grav,
+               const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
+               float c_cfl, float4* velr_s, float2* pc_s, float* dt_out, float* dt_particle, cudaStream_t st);
 int gravity(const float4* posm, int64_t n_total, float G, float delta, float4* acc_grav,
             float4* src_pk, float4* grav_part, cudaStream_t st);
 int update_predictor(float4* posm, float4* vele, float4* vele0, const float4* acc_sph, const float4* acc_grav,

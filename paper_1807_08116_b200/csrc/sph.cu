@@ -205,4 +205,76 @@ int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, co
     return SPH_OK;
 }
 
+// ---------------------------------------------------------------- (NEXT-1) modified CFL step, Eq. 17
+// Per gas particle: s = min |dr|, cmax = max c_ij, mumax = max |mu_ij| over its neighbours (same walk
+// and predicate as k_forces), then the bracket of Eq. 17; the global minimum by atomicMin on the bit
+// pattern (positive floats order like unsigned ints), so it is exact and order-independent.
+__global__ void k_cfl_init(float* dt_out) { *dt_out = __int_as_float(0x7f800000); }
+
+__global__ void __launch_bounds__(128) k_cfl(const float4* __restrict__ posm_s, const float4* __restrict__ velr_s,
+                                             const float2* __restrict__ pc_s, const uint32_t* __restrict__ perm,
+                                             const uint32_t* __restrict__ start, const float4* __restrict__ acc_sph,
+                                             const float4* __restrict__ acc_grav, int n, GridDev g, float rc2, float h,
+                                             float eta_h2, float alpha, float beta, float c_cfl,
+                                             float* __restrict__ dt_particle, float* dt_out) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    float bound = __int_as_float(0x7f800000);
+    if (s < n) {
+        const float4 pi = posm_s[s];
+        const float4 vi = velr_s[s];
+        const float ci = pc_s[s].y;
+        const uint32_t k = key_of(pi, g);
+        const int ix = (int)(k % (uint32_t)g.mx), iy = (int)((k / (uint32_t)g.mx) % (uint32_t)g.my),
+                  iz = (int)(k / ((uint32_t)g.mx * (uint32_t)g.my));
+        float d2min = rc2, cmax = ci, mumax = 0.f;   // A22: no neighbour -> s = 2h, c_i, 0
+#pragma unroll 1
+        for (int r = 0; r < 9; ++r) {
+            uint32_t lo, hi;
+            stencil_run(start, g, ix, iy, iz, r, lo, hi);
+            for (uint32_t t = lo; t < hi; ++t) {
+                const float4 pj = posm_s[t];
+                float dx, dy, dz;
+                const float d2 = dist2_f32(pi, pj, dx, dy, dz);
+                if (d2 < rc2 && d2 > 0.f) {
+                    const float4 vj = velr_s[t];
+                    const float rv = fmaf(dz, vi.z - vj.z, fmaf(dy, vi.y - vj.y, dx * (vi.x - vj.x)));
+                    const float mu = rv < 0.f ? (h * rv) / (d2 + eta_h2) : 0.f;   // L97
+                    d2min = fminf(d2min, d2);
+                    cmax = fmaxf(cmax, 0.5f * (ci + pc_s[t].y));
+                    mumax = fmaxf(mumax, fabsf(mu));
+                }
+            }
+        }
+        const uint32_t i = perm[s];
+        const float4 as = acc_sph[i], ag = acc_grav[i];
+        const float qx = as.x + ag.x, qy = as.y + ag.y, qz = as.z + ag.z;
+        const float qe = sqrtf(fmaf(qz, qz, fmaf(qy, qy, qx * qx))) + fabsf(as.w);   // |Q_i| + |E_i|
+        const float sm = d2min < rc2 ? sqrtf(d2min) : 2.0f * h;
+        bound = sm / (fmaf(cmax, 1.0f + 1.2f * alpha, 1.2f * beta * mumax) + sqrtf(sm * qe));
+        if (dt_particle) dt_particle[i] = bound;
+    }
+    float v = c_cfl * bound;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if ((threadIdx.x & 31) == 0 && v < __int_as_float(0x7f800000))
+        atomicMin(reinterpret_cast<unsigned int*>(dt_out), __float_as_uint(fmaxf(v, 0.f)));
+}
+
+int cfl_sorted(const float4* posm_s, const float4* vele, const float* rho, const float4* acc_sph, const float4* acc_grav,
+               const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
+               float c_cfl, float4* velr_s, float2* pc_s, float* dt_out, float* dt_particle, cudaStream_t st) {
+    k_cfl_init<<<1, 1, 0, st>>>(dt_out);
+    SPHB_LAUNCHED();
+    if (n_gas <= 0) return SPH_OK;
+    const int n = (int)n_gas;
+    k_eos_gather<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(vele, rho, perm, n, p->gamma, velr_s, pc_s);
+    SPHB_LAUNCHED();
+    const float two_h = 2.0f * p->h;
+    k_cfl<<<(unsigned)cdiv(n, 128), 128, 0, st>>>(posm_s, velr_s, pc_s, perm, cell_start, acc_sph, acc_grav, n, to_dev(g),
+                                                  two_h * two_h, p->h, p->eta * p->h * p->h, p->alpha, p->beta, c_cfl,
+                                                  dt_particle, dt_out);
+    SPHB_LAUNCHED();
+    return SPH_OK;
+}
+
 }  // namespace sphb

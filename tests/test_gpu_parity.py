@@ -242,6 +242,39 @@ def test_density_and_forces_parity(cuda_lib, case):
     assert torch.equal(acc, acc2)
 
 
+@pytest.mark.parametrize("case", ["galaxy", "dense", "clumps"])
+def test_cfl_step_parity(cuda_lib, case):
+    """NEXT-1, Eq. 17 (L125-129): per-particle bracket and the global minimum against the oracle.  Both sides
+    take the same rho and the same Q, E (the GPU's verified FP32 outputs, widened), so this checks the
+    neighbour reductions s^min, c^max, mu^max and the formula."""
+    b = cuda_lib
+    w, og = _grid_case(case)
+    n = w.n_gas
+    d, g, perm, start, ws = _build(b, w, og)
+    prm = b.sph_params.from_workload(w)
+    rho = torch.zeros(n, device="cuda")
+    b.sph_density(d, n, prm, g, perm, start, rho, ws)
+    acc = torch.zeros((n, 4), device="cuda")
+    dv = _t(w.vele)
+    b.sph_forces(d, dv, rho, n, prm, g, perm, start, acc, ws)
+    rng = np.random.Generator(np.random.Philox(key=[77, 0]))
+    ag = _t((0.3 * rng.standard_normal((n, 4))).astype(np.float32))          # any gravity field will do
+    dt = torch.zeros(1, device="cuda")
+    dti = torch.zeros(n, device="cuda")
+    b.sph_cfl_dt(d, dv, rho, acc, ag, n, prm, g, perm, start, 0.7, dt, dti, ws)
+    ooff, oidx = oracle.neighbours(w.posm, n, w.h, method="grid")
+    odt, obr = oracle.cfl_dt(w.posm, w.vele, rho.cpu().numpy().astype(np.float64), acc.cpu().numpy(), ag.cpu().numpy(),
+                             w.h, ooff, oidx, 0.7, gamma=w.gamma, alpha=w.alpha, beta=w.beta, eta=w.eta)
+    got = dti.cpu().numpy().astype(np.float64)
+    rel = np.abs(got - obr) / obr
+    assert rel.max() < 5e-6, rel.max()          # a few FP32 roundings: sqrt, one division, three products
+    assert abs(dt.item() - odt) < 5e-6 * odt
+    assert abs(dt.item() - 0.7 * got.min()) <= 2e-7 * got.min()      # the minimum itself is exact (integer atomics)
+    # no gas: +inf
+    b.sph_cfl_dt(None, None, None, None, None, 0, prm, None, None, None, 0.7, dt, None, ws)
+    assert np.isinf(dt.item())
+
+
 def test_coincident_gas_particles(cuda_lib):
     b = cuda_lib
     w = _dense(2000, 8, 0.08)

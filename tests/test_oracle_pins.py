@@ -428,3 +428,74 @@ def test_P7_energy_drift_config0():
     # halving dt at fixed end time shrinks the drift by >= 4x (third-order local energy error)
     d_big, _ = run(2e-3, 5)
     assert d_big >= 4 * drift * 0.9
+
+
+# ---------------------------------------------------------------- NEXT-1: modified CFL step, Eq. 17 (L125-129)
+def _golden(name):
+    import os
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "closed_forms.txt")):
+        f = line.split()
+        if f and f[0] == name:
+            return f[1]
+    raise KeyError(name)
+
+
+def test_CFL_two_particles_by_hand():
+    """Worked example (tests/golden/closed_forms.txt: cfl_two_particles), every factor a round number."""
+    h = 1.0
+    posm = np.array([[0, 0, 0, 1.0], [1, 0, 0, 1.0]], dtype=np.float64)
+    vele = np.array([[0.5, 0, 0, 0.9], [-0.5, 0, 0, 0.9]], dtype=np.float64)    # closing speed 1, c = 1
+    off, idx = oracle.neighbours(posm, 2, h)
+    rho = oracle.density(posm, h, off, idx)
+    acc_sph = np.array([[3.0, 0, 0, 1.0], [0, 2.0, 0, -1.0]])                    # |Q| = 3 (with a_grav below), |E| = 1
+    acc_grav = np.array([[0.0, 0, 0, 0], [0, 1.0, 0, 0]])
+    dt, br = oracle.cfl_dt(posm, vele, rho, acc_sph, acc_grav, h, off, idx, 0.5)
+    num, den = _golden("cfl_two_particles").split("/")
+    expect = float(Fraction(num) / Fraction(den))
+    assert abs(expect - 0.5 / (3.6 + 12.0 / 11.0)) < 1e-15
+    assert np.isclose(dt, expect, rtol=1e-14)
+    assert np.allclose(br, 2 * expect, rtol=1e-14)                               # symmetric pair: same bracket
+    # receding pair: mu = 0 (L97), the viscous term drops out
+    vele[:, 0] *= -1
+    dt2, _ = oracle.cfl_dt(posm, vele, rho, acc_sph, acc_grav, h, off, idx, 0.5)
+    assert np.isclose(dt2, 0.5 / (1.6 + 2.0), rtol=1e-14)
+
+
+def test_CFL_static_lattice_reduces_to_courant():
+    """Uniform lattice at rest, no forces: Eq. 17 collapses to the textbook Courant condition
+    dt = C a / (c (1 + 1.2 alpha)) with a the lattice spacing and c = sqrt(gamma (gamma-1) e)."""
+    a, h, e, gamma, alpha = 0.25, 0.3, 0.7, 1.4, 0.5
+    g = np.arange(5) * a
+    x, y, z = np.meshgrid(g, g, g, indexing="ij")
+    n = x.size
+    posm = np.stack([x.ravel(), y.ravel(), z.ravel(), np.full(n, a ** 3)], 1)
+    vele = np.zeros((n, 4))
+    vele[:, :3] = (0.3, -0.2, 0.1)                  # uniform motion: Galilean invariance, all dv = 0
+    vele[:, 3] = e
+    off, idx = oracle.neighbours(posm, n, h)
+    rho = oracle.density(posm, h, off, idx)
+    zero = np.zeros((n, 4))
+    dt, br = oracle.cfl_dt(posm, vele, rho, zero, zero, h, off, idx, 0.8, gamma=gamma, alpha=alpha)
+    c = math.sqrt(gamma * (gamma - 1) * e)
+    assert np.allclose(br, a / (c * (1 + 1.2 * alpha)), rtol=1e-12)
+    assert np.isclose(dt, 0.8 * a / (c * (1 + 1.2 * alpha)), rtol=1e-12)
+
+
+def test_CFL_isolated_particle_and_monotonicity():
+    """A22: a particle with no neighbour takes s = 2h; a larger |Q| can only shrink the step; dt is
+    the minimum of the per-particle brackets."""
+    h, gamma = 0.1, 5.0 / 3.0
+    posm = np.array([[0, 0, 0, 1.0], [5, 5, 5, 1.0], [5.05, 5, 5, 1.0]], dtype=np.float64)
+    vele = np.array([[0, 0, 0, 0.9], [0, 0, 0, 0.9], [0, 0, 0, 0.9]], dtype=np.float64)
+    off, idx = oracle.neighbours(posm, 3, h)
+    assert np.diff(off).tolist() == [0, 1, 1]
+    rho = oracle.density(posm, h, off, idx)
+    zero = np.zeros((3, 4))
+    dt, br = oracle.cfl_dt(posm, vele, rho, zero, zero, h, off, idx, 1.0, gamma=gamma, alpha=0.5)
+    assert np.isclose(br[0], 2 * h / 1.6, rtol=1e-14)           # c = 1
+    assert np.isclose(br[1], 0.05 / 1.6, rtol=1e-12) and np.isclose(dt, br.min())
+    acc = zero.copy()
+    acc[:, 0] = 10.0
+    dt2, br2 = oracle.cfl_dt(posm, vele, rho, acc, zero, h, off, idx, 1.0, gamma=gamma, alpha=0.5)
+    assert np.all(br2 < br) and dt2 < dt
+    assert np.isclose(br2[0], 2 * h / (1.6 + math.sqrt(2 * h * 10.0)), rtol=1e-14)
