@@ -35,6 +35,42 @@ def _peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
+def workload_config(args, w, grid_dims=None, cells=None, world=1):
+    """The `config` object of the JSON line: identical for both arms (ours / reference)."""
+    src = f"BASELINE.json configs[{args.config}]" if args.config <= 4 else "SURVEY.md 8(f) NEXT-3 (collisionless, not a BASELINE config)"
+    return {"workload": f"{src} ({w.name}): N={w.n_total}, N_g={w.n_gas}, h={w.h:g}, delta={w.delta:g}, dt={w.dt:g}",
+            "grid_dims": grid_dims, "cells": cells, "parallelism": "replicas only" if world > 1 else "single GPU",
+            "l2": "no flush: one step streams >300 MB (cell arrays, gravity partials, particle arrays) > 126 MB L2"}
+
+
+def reduce_max_ms(ms: float, world: int, device: str = "cuda") -> float:
+    """Max over ranks of a per-rank duration (the contract's timing rule); identity for one rank.
+    Works on any initialised process group (NCCL on the GPUs, gloo in the CPU test)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def ncu_traffic(kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed ncu --set full
+    summary profiles/traffic_r01.csv (kernel,n_total,dram_read_bytes,dram_write_bytes); None if absent."""
+    p = os.path.join(ROOT, "profiles", "traffic_r01.csv")
+    if not os.path.exists(p):
+        return None
+    for line in open(p):
+        f = line.strip().split(",")
+        if len(f) >= 4 and f[0] == kernel:
+            try:
+                return {"n_total": int(f[1]), "bytes": float(f[2]) + float(f[3])}
+            except ValueError:
+                continue
+    return None
+
+
 def _env_rank():
     return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
 
@@ -150,12 +186,16 @@ def run_reference(args, w):
             vals.append(ms)
     v = float(np.mean(vals))
     cores = oracle.num_threads()
+    grid_dims = cells = None
+    if w.n_gas:
+        og = oracle.grid_from_bbox(w.posm.astype(np.float64), w.n_gas, w.h)
+        grid_dims, cells = [int(d) for d in og.dims], int(og.M)
     line = {
         "impl": "reference", "metric": "step_ms", "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "n_total": w.n_total, "n_gas": w.n_gas, "h": w.h, "delta": w.delta, "dt": w.dt},
-        "cpu_baseline": {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": desc},
+        "config": workload_config(args, w, grid_dims, cells, 1),
+        "cpu_baseline": {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": desc, "extrapolated": True},
         "e2e": {"value": v, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -204,10 +244,7 @@ def run_ours(args, w):
     b.sph_set_profiling(False)
     launches = b.sph_launch_count() - launches0
     clocks = sampler.stop() if sampler else None
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step = float(t.item()) / args.steps
+    ms_step = reduce_max_ms(ms_total, world) / args.steps
 
     # ---- end-to-end arm: HOST (pinned) buffers through sph_host_ctx_step, copies inside the timing
     e2e = None
@@ -226,10 +263,7 @@ def run_ours(args, w):
             ctx.step(hp, hv, prm, w.dt, 1, first=False, rho=hrho)     # H2D posm+vele, step, D2H posm+vele+rho, sync
         t_e2e = (time.perf_counter() - t0) * 1e3 / k_e2e
         ctx.close()
-        te = torch.tensor([t_e2e], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e2e = {"value": float(te.item()), "unit": "ms", "h2d_bytes_per_step": 2 * n * 16,
+        e2e = {"value": reduce_max_ms(t_e2e, world), "unit": "ms", "h2d_bytes_per_step": 2 * n * 16,
                "d2h_bytes_per_step": 2 * n * 16 + ng * 4, "steps": k_e2e,
                "timing": "host wall clock around sph_host_ctx_step (it synchronises), max over ranks"}
 
@@ -247,8 +281,11 @@ def run_ours(args, w):
     roofline = None
     if w.G != 0.0 and grav_ms > 0:
         achieved = FLOPS_PER_INTERACTION * float(n) * float(n) / (grav_ms * 1e-3) / 1e12
+        tr = ncu_traffic("grav_pp_kernel")
+        traffic = tr["bytes"] if tr and tr["n_total"] == n else None   # the capture is of this workload only
         roofline = {"kernel": "grav_pp_kernel", "bound": "alu", "achieved": achieved, "peak": alu_peak_tflops,
-                    "unit": "TFLOP/s", "frac": achieved / alu_peak_tflops, "traffic": None,
+                    "unit": "TFLOP/s", "frac": achieved / alu_peak_tflops, "traffic": traffic,
+                    "traffic_note": "DRAM bytes per launch (ncu --set full, profiles/traffic_r01.csv); irrelevant to an ALU-bound kernel",
                     "peak_source": f"2*128*148*sm_max_mhz ({peak_src} sm_max_mhz={sm_max:.0f}); 20 flops/interaction",
                     "kernel_ms": grav_ms, "launches_per_step": 1,
                     "note": "gravity stage = pack + grav_pp_kernel + reduce; the two O(N) kernels are <0.1% of it"}
@@ -278,10 +315,7 @@ def run_ours(args, w):
         "metric": "step_ms", "value": ms_step, "unit": "ms", "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[{args.config}] ({w.name}): N={n}, N_g={ng}, h={w.h:g}, "
-                               f"delta={w.delta:g}, dt={w.dt:g}", "grid_dims": list(sim.grid.dims) if ng else None,
-                   "cells": M, "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "l2": "no flush: one step streams >300 MB (cell arrays, gravity partials, particle arrays) > 126 MB L2"},
+        "config": workload_config(args, w, list(sim.grid.dims) if ng else None, M, world),
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "stages": stages,
         "context": "paper Table 1 (K40, N=2^20, units inferred as s): t_SPH=7.87, t_GFC=53.62 — other hardware, not a target",
@@ -302,8 +336,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--cpu-targets", type=int, default=2048)
-    ap.add_argument("--ref-targets", type=int, default=1024)
+    ap.add_argument("--cpu-targets", type=int, default=32768)
+    ap.add_argument("--ref-targets", type=int, default=8192)
     args = ap.parse_args()
     from paper_1807_08116_b200 import workloads as wl
     w = wl.make_workload(args.config, scale=args.scale)

@@ -158,6 +158,9 @@ CONFIGS = {
     3: dict(kind="collision", n_gas=2 ** 21, n_halo=2 ** 21, h=0.02, delta=0.001, dt=1e-4, steps=5, seed=4,
             gas_core=0.2, halo_core=0.5),
     4: dict(kind="clumps", n_gas=2 ** 24, h=0.004, seed=5),
+    # not a BASELINE.json config: SURVEY §8(f) NEXT-3, the collisionless mode (N_g = 0; SP, DC, HFC skipped,
+    # PAPER.md L150) at N = 2^22, inside the paper's range of N (L213); same halo profile and orbits as config 2
+    5: dict(kind="collision", n_gas=0, n_halo=2 ** 22, h=0.05, delta=0.001, dt=1e-4, steps=5, seed=6),
 }
 
 
@@ -169,8 +172,8 @@ def make_workload(config: int, scale: float = 1.0) -> Workload:
     name = f"config{config}" + ("" if scale == 1.0 else f"@{scale:g}")
     if kind == "clumps":
         return _clumps(name, max(2, int(c["n_gas"] * scale)), c["h"], c["seed"])
-    c["n_gas"] = max(2, int(c["n_gas"] * scale))
-    c["n_halo"] = max(2, int(c["n_halo"] * scale))
+    c["n_gas"] = max(2, int(c["n_gas"] * scale)) if c["n_gas"] else 0
+    c["n_halo"] = max(2, int(c["n_halo"] * scale)) if c["n_halo"] else 0
     if kind == "single":
         return _single_galaxy(name, **c)
     return _collision(name, **c)

@@ -125,3 +125,29 @@ def test_full_size_sph_only_config4(cuda_lib):
     nn = _check_sph_subset(w, w.posm, w.vele, sim.rho.cpu().numpy(), sim.acc_sph.cpu().numpy(), g_idx, og,
                            (okey, ostart, operm))
     assert nn.max() > 500           # the clump cores
+
+
+def test_full_size_collisionless_next3(cuda_lib):
+    """N_g = 0 (SP, DC, HFC skipped, L150) at N = 2^22.  One step: Eqs. 12-16 reduce to
+    velocity Verlet (pin P8), checked on ALL particles from the GPU's own accelerations; the accelerations
+    themselves on the seeded subset against the oracle, before and after the step."""
+    b = cuda_lib
+    w = wl.make_workload(5)
+    assert w.n_gas == 0 and w.n_total == 2 ** 22
+    _, h_idx = wl.subset_indices(0, w.n_halo, w.seed, n_each=2048)
+    sim = b.Simulation(w)
+    sim.evaluate()
+    a0 = sim.acc_grav.cpu().numpy().astype(np.float64)[:, :3]
+    check_values(a0[h_idx], oracle.gravity(w.posm, w.G, w.delta, targets=h_idx), "a_grav cfg5 subset")
+    sim.first = True
+    sim.step()
+    p1 = sim.posm.cpu().numpy()
+    v1 = sim.vele.cpu().numpy()
+    a1 = sim.acc_grav.cpu().numpy().astype(np.float64)[:, :3]
+    dt = w.dt
+    r0 = w.posm[:, :3].astype(np.float64)
+    v0 = w.vele[:, :3].astype(np.float64)
+    r1 = r0 + dt * v0 + 0.5 * dt * dt * a0                               # velocity Verlet
+    assert np.abs(p1[:, :3] - r1).max() <= 2e-6 * max(1.0, np.abs(r1).max())
+    check_values(v1[:, :3], v0 + 0.5 * dt * (a0 + a1), "v(t+dt) cfg5 all", max_tol=2e-6, med_tol=2e-7)
+    check_values(a1[h_idx], oracle.gravity(p1, w.G, w.delta, targets=h_idx), "a_grav(t+dt) cfg5 subset")
