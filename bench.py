@@ -290,11 +290,12 @@ def run_ours(args, w):
                     "kernel_ms": grav_ms, "launches_per_step": 1,
                     "note": "gravity stage = pack + grav_pp_kernel + reduce; the two O(N) kernels are <0.1% of it"}
     hbm = float(peaks.get("hbm_gbs", 6650.0))
-    sort_bytes = ng * 96 + M * 16
-    upd_bytes = n * (64 + 48) + n * (48 + 16)
+    sort_bytes = ng * 92 + M * 16
+    # gas: predictor 64 B read + 48 B written, corrector 64 + 16; halo particles never touch acc_sph: 48 + 48, 48 + 16
+    upd_bytes = ng * (112 + 80) + (n - ng) * (96 + 64)
     stages = {
         "gravity_ms": grav_ms, "sort_ms": sort_ms, "density_ms": dens_ms, "forces_ms_2passes": forc_ms, "update_ms": upd_ms,
-        "pp_ginteractions_per_s": (float(n) * n / (grav_ms * 1e-3) / 1e9) if grav_ms > 0 else None,
+        "pp_ginteractions_per_s": (float(n) * n / (grav_ms * 1e-3) / 1e9) if (grav_ms > 0 and w.G != 0.0) else None,
         "sph_mparticles_per_s": (ng / ((sort_ms + dens_ms + forc_ms) * 1e-3) / 1e6) if ng else None,
         "sort_mkeys_per_s": (ng / (sort_ms * 1e-3) / 1e6) if ng and sort_ms > 0 else None,
         "sort_hbm_gbs": (sort_bytes / (sort_ms * 1e-3) / 1e9) if ng and sort_ms > 0 else None,

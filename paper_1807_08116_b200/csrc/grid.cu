@@ -238,13 +238,16 @@ __global__ void __launch_bounds__(256) k_scatter(const uint32_t* __restrict__ ke
 
 // slot s of the unstable order holds i = tmp[s]; its stable slot is start[k] + #{t in cell k : tmp[t] < i}.
 // Consecutive threads share a cell, so the reads of tmp[a..b) are warp-broadcast / L1 hits.
-__global__ void __launch_bounds__(256) k_stable(const uint32_t* __restrict__ tmp, const uint32_t* __restrict__ key,
+// The cell number is recomputed from posm[i] (needed anyway for the reorder) instead of gathering key[i]:
+// one random 32-byte sector less per particle.
+__global__ void __launch_bounds__(256) k_stable(const uint32_t* __restrict__ tmp, const GridDev g,
                                                 const uint32_t* __restrict__ start, const float4* __restrict__ posm,
                                                 int n, uint32_t* __restrict__ perm, float4* __restrict__ posm_s) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
     const uint32_t i = tmp[s];
-    const uint32_t k = key[i];
+    const float4 p = posm[i];
+    const uint32_t k = cell_key(p, g);
     const uint32_t a = start[k], b = start[k + 1];
     uint32_t r = 0, t = a;
     // tmp is 16-byte aligned (workspace carve): scalar head to a multiple of 4, uint4 body, scalar tail
@@ -255,7 +258,7 @@ __global__ void __launch_bounds__(256) k_stable(const uint32_t* __restrict__ tmp
     }
     for (; t < b; ++t) r += (tmp[t] < i) ? 1u : 0u;
     perm[a + r] = i;
-    if (posm_s) posm_s[a + r] = posm[i];
+    if (posm_s) posm_s[a + r] = p;
 }
 
 __global__ void __launch_bounds__(256) k_gather_pos(const float4* __restrict__ posm, const uint32_t* __restrict__ perm,
@@ -314,7 +317,7 @@ int grid_build(const float4* posm, int64_t n_gas, const sph_grid* g, uint32_t* k
     if (n > 0) {
         k_scatter<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(key, rank_u, cell_start, n, tmp);                 // K4
         SPHB_LAUNCHED();
-        k_stable<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(tmp, key, cell_start, posm, n, perm, posm_s);
+        k_stable<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(tmp, to_dev(g), cell_start, posm, n, perm, posm_s);
         SPHB_LAUNCHED();
     }
     return SPH_OK;
