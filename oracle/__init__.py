@@ -71,16 +71,16 @@ def lib():
         L.orc_counting_sort.restype = C.c_int
         L.orc_rc2.argtypes = [C.c_float]
         L.orc_rc2.restype = C.c_float
-        L.orc_neighbours_brute.argtypes = [dp, C.c_int64, C.c_float, ip, C.c_int64, up, ip, up]
+        L.orc_neighbours_brute.argtypes = [dp, C.c_int64, C.c_float, fp, ip, C.c_int64, up, ip, up]
         L.orc_neighbours_brute.restype = None
-        L.orc_neighbours_grid.argtypes = [dp, C.c_int64, C.c_float, C.POINTER(_Grid), up, up, up, ip, C.c_int64,
+        L.orc_neighbours_grid.argtypes = [dp, C.c_int64, C.c_float, fp, C.POINTER(_Grid), up, up, up, ip, C.c_int64,
                                           up, ip, up]
         L.orc_neighbours_grid.restype = None
-        L.orc_density.argtypes = [dp, C.c_double, ip, C.c_int64, ip, up, dp]
+        L.orc_density.argtypes = [dp, C.c_double, dp, ip, C.c_int64, ip, up, dp]
         L.orc_density.restype = None
         L.orc_cfl_terms.argtypes = [dp, dp, dp, C.POINTER(_Params), ip, C.c_int64, ip, up, dp]
         L.orc_cfl_terms.restype = None
-        L.orc_forces.argtypes = [dp, dp, dp, C.POINTER(_Params), ip, C.c_int64, ip, up, dp, dp]
+        L.orc_forces.argtypes = [dp, dp, dp, C.POINTER(_Params), dp, ip, C.c_int64, ip, up, dp, dp]
         L.orc_forces.restype = None
         _lib = L
     return _lib
@@ -175,10 +175,27 @@ def rc2(h) -> np.float32:
 
 
 # ------------------------------------------------------------------ neighbour sets (O2)
-def neighbours(posm, n_gas, h, targets=None, method="brute", grid=None, sort=None):
+def _hs32(hs):
+    return None if hs is None else np.ascontiguousarray(hs, dtype=np.float32)
+
+
+def _hs64(hs):
+    return None if hs is None else np.ascontiguousarray(np.asarray(hs, dtype=np.float32), dtype=np.float64)
+
+
+def smoothing_lengths(posm, rho, sigma, h_max):
+    """L82: h_i = sigma (m_i / rho_i)^(1/3), capped at h_max (reading A25: the grid's cells are 2 h_max wide,
+    so no pair farther apart than that can be found).  Returned as FP32, the type both sides carry h in."""
+    m = _f64(posm)[: len(rho), 3]
+    return np.minimum(float(sigma) * np.cbrt(m / np.asarray(rho, dtype=np.float64)), float(h_max)).astype(np.float32)
+
+
+def neighbours(posm, n_gas, h, targets=None, method="brute", grid=None, sort=None, hs=None):
     """CSR neighbour lists (offsets int64[nt+1], index uint32[...]), each list ascending in j, j != i.
-    method "brute": definition, O(nt * n_gas).  method "grid": the oracle's own 3x3x3 search."""
+    method "brute": definition, O(nt * n_gas).  method "grid": the oracle's own 3x3x3 search.
+    hs: per-particle smoothing lengths (FP32, all <= h): pair cutoff fl(fl(h_i + h_j)^2) (reading A24)."""
     posm = _f64(posm)
+    hs = _hs32(hs)
     tg = _tg(targets)
     nt = int(n_gas) if tg is None else len(tg)
     cnt = np.zeros(nt, dtype=np.uint32)
@@ -194,12 +211,12 @@ def neighbours(posm, n_gas, h, targets=None, method="brute", grid=None, sort=Non
         gc = grid._c()
 
         def call(c, off, idx):
-            L.orc_neighbours_grid(_p(posm, C.c_double), int(n_gas), np.float32(h), C.byref(gc), _p(key, C.c_uint32),
+            L.orc_neighbours_grid(_p(posm, C.c_double), int(n_gas), np.float32(h), _p(hs, C.c_float), C.byref(gc), _p(key, C.c_uint32),
                                   _p(start, C.c_uint32), _p(perm, C.c_uint32), _p(tg, C.c_int64), nt, _p(c, C.c_uint32),
                                   _p(off, C.c_int64), _p(idx, C.c_uint32))
     else:
         def call(c, off, idx):
-            L.orc_neighbours_brute(_p(posm, C.c_double), int(n_gas), np.float32(h), _p(tg, C.c_int64), nt,
+            L.orc_neighbours_brute(_p(posm, C.c_double), int(n_gas), np.float32(h), _p(hs, C.c_float), _p(tg, C.c_int64), nt,
                                    _p(c, C.c_uint32), _p(off, C.c_int64), _p(idx, C.c_uint32))
     if nt:
         call(cnt, None, None)
@@ -212,8 +229,9 @@ def neighbours(posm, n_gas, h, targets=None, method="brute", grid=None, sort=Non
 
 
 # ------------------------------------------------------------------ SPH sums (Eqs. 7, 10, 11)
-def density(posm, h, offsets, index, targets=None):
+def density(posm, h, offsets, index, targets=None, hs=None):
     posm = _f64(posm)
+    hs = _hs64(hs)
     tg = _tg(targets)
     nt = len(offsets) - 1
     rho = np.zeros(nt, dtype=np.float64)
@@ -222,13 +240,13 @@ def density(posm, h, offsets, index, targets=None):
         idx = np.zeros(1, dtype=np.uint32)
     off = np.ascontiguousarray(offsets, dtype=np.int64)
     if nt:
-        lib().orc_density(_p(posm, C.c_double), float(h), _p(tg, C.c_int64), nt, _p(off, C.c_int64), _p(idx, C.c_uint32),
+        lib().orc_density(_p(posm, C.c_double), float(h), _p(hs, C.c_double), _p(tg, C.c_int64), nt, _p(off, C.c_int64), _p(idx, C.c_uint32),
                           _p(rho, C.c_double))
     return rho
 
 
 def forces(posm, vele, rho_all, h, offsets, index, targets=None, gamma=5.0 / 3.0, alpha=0.5, beta=1.0, eta=0.1,
-           with_gross=False):
+           with_gross=False, hs=None):
     """(ax, ay, az, de/dt) of Eqs. 10-11 (hydro part) for `targets`; rho_all indexed by gas index.
     with_gross: also return [nt,2] sums of the term magnitudes (conditioning diagnostic, reading A17)."""
     posm, vele, rho_all = _f64(posm), _f64(vele), _f64(rho_all)
@@ -241,9 +259,10 @@ def forces(posm, vele, rho_all, h, offsets, index, targets=None, gamma=5.0 / 3.0
     off = np.ascontiguousarray(offsets, dtype=np.int64)
     prm = _Params(float(h), float(gamma), float(alpha), float(beta), float(eta))
     gross = np.zeros((nt, 2), dtype=np.float64) if with_gross else None
+    hs = _hs64(hs)
     if nt:
         lib().orc_forces(_p(posm, C.c_double), _p(vele, C.c_double), _p(rho_all, C.c_double), C.byref(prm),
-                         _p(tg, C.c_int64), nt, _p(off, C.c_int64), _p(idx, C.c_uint32), _p(out, C.c_double),
+                         _p(hs, C.c_double), _p(tg, C.c_int64), nt, _p(off, C.c_int64), _p(idx, C.c_uint32), _p(out, C.c_double),
                          _p(gross, C.c_double))
     return (out, gross) if with_gross else out
 
@@ -289,38 +308,43 @@ class State:
     acc_grav: np.ndarray = None  # float64 [N,3]
 
 
-def _nbr(posm, n_gas, h, method):
+def _nbr(posm, n_gas, h, method, hs=None):
     if n_gas == 0:
         return np.zeros(1, dtype=np.int64), np.zeros(0, dtype=np.uint32)
-    return neighbours(posm, n_gas, h, method=method)
+    return neighbours(posm, n_gas, h, method=method, hs=hs)
 
 
-def position_only(state: State, h, G, delta, method="grid"):
-    """SP + DC + GFC at the current positions (the quantities that depend on r only, L123)."""
-    off, idx = _nbr(state.posm, state.n_gas, h, method)
-    state.rho = density(state.posm, h, off, idx)
+def position_only(state: State, h, G, delta, method="grid", hs=None):
+    """SP + DC + GFC at the current positions (the quantities that depend on r only, L123).
+    hs: per-particle smoothing lengths (then h is their cap h_max, which sizes the grid)."""
+    off, idx = _nbr(state.posm, state.n_gas, h, method, hs)
+    state.rho = density(state.posm, h, off, idx, hs=hs)
     state.acc_grav = gravity(state.posm, G, delta) if G != 0.0 else np.zeros((len(state.posm), 3))
     return off, idx
 
 
-def hydro(state: State, h, nbr, **visc):
+def hydro(state: State, h, nbr, hs=None, **visc):
     if state.n_gas == 0:
         return np.zeros((0, 4))
     off, idx = nbr
-    return forces(state.posm, state.vele, state.rho, h, off, idx, **visc)
+    return forces(state.posm, state.vele, state.rho, h, off, idx, hs=hs, **visc)
 
 
-def step(state: State, dt, h, G, delta, nbr=None, method="grid", **visc):
+def step(state: State, dt, h, G, delta, nbr=None, method="grid", hs=None, sigma=0.0, **visc):
     """One predictor-corrector step, Eqs. 12-16 (L103-121), sequence of DESIGN.md A11:
     HFC(pred) -> SU(pred) -> SP, DC, GFC at r(t+dt) -> HFC(corr) -> SU(corr).
     `state` must carry rho and acc_grav at the current r (call position_only first);
     `nbr` are the neighbour lists at the current r (recomputed if None).
-    Returns (new_state, nbr_new, diagnostics)."""
+    Returns (new_state, nbr_new, diagnostics).
+    Per-particle smoothing lengths (L82, reading A26): with `hs` the pair length is h_ij = (h_i + h_j)/2 and h is the
+    cap h_max; with sigma > 0 the lengths are renewed from the refined density, h_i = min(sigma (m_i/rho_i)^(1/3), h_max),
+    right after DC at r(t+dt) — the density itself was summed with the old lengths — and used by the corrector and by
+    the next step (diag["hs"])."""
     ng = state.n_gas
     if nbr is None:
-        nbr = _nbr(state.posm, ng, h, method)
+        nbr = _nbr(state.posm, ng, h, method, hs)
     Q = state.acc_grav.copy()                                  # halo: Q_i = a^g_i
-    hy = hydro(state, h, nbr, **visc)                          # HFC(predictor) at (r, v, e, rho)(t)
+    hy = hydro(state, h, nbr, hs=hs, **visc)                   # HFC(predictor) at (r, v, e, rho)(t)
     Q[:ng] += hy[:, :3]
     E = hy[:, 3] if ng else np.zeros(0)
     v0 = state.vele[:, :3].copy()
@@ -331,14 +355,18 @@ def step(state: State, dt, h, G, delta, nbr=None, method="grid", **visc):
     new.posm[:, :3] = state.posm[:, :3] + 0.5 * dt * (v_t + v0)   # Eq. 14
     new.vele[:, :3] = v_t
     new.vele[:ng, 3] = e_t
-    nbr1 = position_only(new, h, G, delta, method)             # density "refined" (L115), gravity once (L123)
+    nbr1 = position_only(new, h, G, delta, method, hs=hs)      # density "refined" (L115), gravity once (L123)
+    hs1 = hs
+    if hs is not None and sigma > 0.0 and ng:
+        hs1 = smoothing_lengths(new.posm, new.rho, sigma, h)
+        nbr1 = _nbr(new.posm, ng, h, method, hs1)              # the pair cutoff follows the lengths
     Q1 = new.acc_grav.copy()
-    hy1 = hydro(new, h, nbr1, **visc)                          # HFC(corrector) at (r(t+dt), v~, e~, rho(t+dt))
+    hy1 = hydro(new, h, nbr1, hs=hs1, **visc)                  # HFC(corrector) at (r(t+dt), v~, e~, rho(t+dt))
     Q1[:ng] += hy1[:, :3]
     E1 = hy1[:, 3] if ng else np.zeros(0)
     new.vele[:, :3] = 0.5 * (v0 + v_t) + 0.5 * dt * Q1         # Eq. 15
     new.vele[:ng, 3] = 0.5 * (e0 + e_t) + 0.5 * dt * E1        # Eq. 16
-    diag = dict(hydro_pred=hy, hydro_corr=hy1, v_pred=v_t, e_pred=e_t)
+    diag = dict(hydro_pred=hy, hydro_corr=hy1, v_pred=v_t, e_pred=e_t, hs=hs1)
     return new, nbr1, diag
 
 

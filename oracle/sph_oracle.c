@@ -252,6 +252,16 @@ float orc_rc2(float h) {
     return rc2;
 }
 
+/* Per-particle smoothing lengths (L82: h_ij = (h_i + h_j)/2; reading A24): the pair (i,j) is a
+ * neighbour pair iff d2 < rc2_ij with rc2_ij = fl(fl(h_i + h_j)^2) in FP32 (2 h_ij = h_i + h_j exactly).
+ * hs == NULL: one global h, rc2 = orc_rc2(h).  With h_i = h_j = h both give the same number.        */
+static inline float orc_rc2_pair(float rc2_global, const float* hs, int64_t i, int64_t j) {
+    if (!hs) return rc2_global;
+    volatile float sum = hs[i] + hs[j];
+    volatile float rc2 = sum * sum;
+    return rc2;
+}
+
 static int orc_cmp_u32(const void* a, const void* b) {
     uint32_t x = *(const uint32_t*)a, y = *(const uint32_t*)b;
     return (x > y) - (x < y);
@@ -261,7 +271,7 @@ static int orc_cmp_u32(const void* a, const void* b) {
  * Two-call protocol: with nbr_index == NULL only nbr_count[t] is written.  Otherwise
  * nbr_offset[nt+1] (exclusive prefix of the counts) must be given and lists are written
  * ascending in j.                                                                        */
-void orc_neighbours_brute(const double* posm, int64_t n_gas, float h,
+void orc_neighbours_brute(const double* posm, int64_t n_gas, float h, const float* hs /*[n_gas] or NULL*/,
                           const int64_t* targets, int64_t nt,
                           uint32_t* nbr_count, const int64_t* nbr_offset, uint32_t* nbr_index) {
     const float rc2 = orc_rc2(h);
@@ -271,7 +281,7 @@ void orc_neighbours_brute(const double* posm, int64_t n_gas, float h,
         uint32_t c = 0;
         for (int64_t j = 0; j < n_gas; ++j) {
             if (j == i) continue;
-            if (orc_d2_f32(posm + 4 * i, posm + 4 * j) < rc2) {
+            if (orc_d2_f32(posm + 4 * i, posm + 4 * j) < orc_rc2_pair(rc2, hs, i, j)) {
                 if (nbr_index) nbr_index[nbr_offset[t] + c] = (uint32_t)j;
                 ++c;
             }
@@ -282,7 +292,8 @@ void orc_neighbours_brute(const double* posm, int64_t n_gas, float h,
 
 /* Same sets through the oracle's own grid (3x3x3 stencil over the counting-sort ranges).
  * Proven equal to the brute-force sets by pin P1.                                       */
-void orc_neighbours_grid(const double* posm, int64_t n_gas, float h, const orc_grid* g,
+void orc_neighbours_grid(const double* posm, int64_t n_gas, float h, const float* hs /*[n_gas] or NULL; all <= h*/,
+                         const orc_grid* g,
                          const uint32_t* key, const uint32_t* start, const uint32_t* perm,
                          const int64_t* targets, int64_t nt,
                          uint32_t* nbr_count, const int64_t* nbr_offset, uint32_t* nbr_index) {
@@ -307,7 +318,7 @@ void orc_neighbours_grid(const double* posm, int64_t n_gas, float h, const orc_g
                     for (uint32_t s = start[cc]; s < start[cc + 1]; ++s) {
                         int64_t j = perm[s];
                         if (j == i) continue;
-                        if (orc_d2_f32(posm + 4 * i, posm + 4 * j) < rc2) {
+                        if (orc_d2_f32(posm + 4 * i, posm + 4 * j) < orc_rc2_pair(rc2, hs, i, j)) {
                             if (nbr_index) nbr_index[nbr_offset[t] + c] = (uint32_t)j;
                             ++c;
                         }
@@ -325,19 +336,21 @@ void orc_neighbours_grid(const double* posm, int64_t n_gas, float h, const orc_g
 /* ------------------------------------------------------------ SPH sums ---- */
 
 /* Eq. 7 (L74) with the self term (reading A5):
- *   rho_i = m_i W(0,h) + sum_{j in N(i)} m_j W(|r_i - r_j|/h, h)        (distances in FP64). */
-void orc_density(const double* posm, double h, const int64_t* targets, int64_t nt,
+ *   rho_i = m_i W(0,h_ii) + sum_{j in N(i)} m_j W(|r_i - r_j|/h_ij, h_ij)   (distances in FP64),
+ * h_ij = (h_i + h_j)/2 (L82) when hs is given, else the global h.                                */
+void orc_density(const double* posm, double h, const double* hs /*[n_gas] or NULL*/, const int64_t* targets, int64_t nt,
                  const int64_t* nbr_offset, const uint32_t* nbr_index, double* rho) {
 #pragma omp parallel for schedule(dynamic, 64)
     for (int64_t t = 0; t < nt; ++t) {
         int64_t i = targets ? targets[t] : t;
         double xi = posm[4 * i], yi = posm[4 * i + 1], zi = posm[4 * i + 2];
-        double r = posm[4 * i + 3] * orc_W(0.0, h);
+        double r = posm[4 * i + 3] * orc_W(0.0, hs ? hs[i] : h);
         for (int64_t q = nbr_offset[t]; q < nbr_offset[t + 1]; ++q) {
             int64_t j = nbr_index[q];
             double dx = xi - posm[4 * j], dy = yi - posm[4 * j + 1], dz = zi - posm[4 * j + 2];
             double d = sqrt(dx * dx + dy * dy + dz * dz);
-            r += posm[4 * j + 3] * orc_W(d / h, h);
+            double hij = hs ? 0.5 * (hs[i] + hs[j]) : h;
+            r += posm[4 * j + 3] * orc_W(d / hij, hij);
         }
         rho[t] = r;
     }
@@ -357,9 +370,10 @@ void orc_density(const double* posm, double h, const int64_t* targets, int64_t n
  * sums of the magnitudes of the same terms — a conditioning diagnostic for the parity tolerance
  * (reading A17), not part of the method.                                            */
 void orc_forces(const double* posm, const double* vele, const double* rho_all, const orc_sph_params* p,
+                const double* hs /*[n_gas] or NULL: h_ij = (h_i + h_j)/2 in grad W_p and mu_ij (L82, L95-97)*/,
                 const int64_t* targets, int64_t nt,
                 const int64_t* nbr_offset, const uint32_t* nbr_index, double* out, double* gross) {
-    const double h = p->h, gm1 = p->gamma - 1.0;
+    const double gm1 = p->gamma - 1.0;
 #pragma omp parallel for schedule(dynamic, 64)
     for (int64_t t = 0; t < nt; ++t) {
         int64_t i = targets ? targets[t] : t;
@@ -375,6 +389,7 @@ void orc_forces(const double* posm, const double* vele, const double* rho_all, c
             double r2 = dx * dx + dy * dy + dz * dz;
             if (r2 == 0.0) continue;
             double r = sqrt(r2);
+            double h = hs ? 0.5 * (hs[i] + hs[j]) : p->h;
             double dwp = orc_dWp_dxi(r / h, h);
             double gx = dwp * dx / r / h, gy = dwp * dy / r / h, gz = dwp * dz / r / h;
             double dvx = vxi - vele[4 * j], dvy = vyi - vele[4 * j + 1], dvz = vzi - vele[4 * j + 2];

@@ -499,3 +499,110 @@ def test_CFL_isolated_particle_and_monotonicity():
     dt2, br2 = oracle.cfl_dt(posm, vele, rho, acc, zero, h, off, idx, 1.0, gamma=gamma, alpha=0.5)
     assert np.all(br2 < br) and dt2 < dt
     assert np.isclose(br2[0], 2 * h / (1.6 + math.sqrt(2 * h * 10.0)), rtol=1e-14)
+
+
+# ---------------------------------------------------------------- NEXT-2: per-particle smoothing lengths (L82)
+def _varh_case(n=1500, seed=11, h_max=0.08):
+    rng = np.random.Generator(np.random.Philox(key=[seed, 0]))
+    posm = np.zeros((n, 4), np.float32)
+    vele = np.zeros((n, 4), np.float32)
+    posm[:, :3] = rng.random((n, 3)) * 0.6
+    posm[:, 3] = (0.5 + rng.random(n)) / n
+    vele[:, :3] = 0.5 * rng.standard_normal((n, 3))
+    vele[:, 3] = 0.5 + 0.5 * rng.random(n)
+    hs = (h_max * (0.45 + 0.55 * rng.random(n))).astype(np.float32)
+    return posm, vele, hs
+
+
+def test_VARH_equal_lengths_reduce_to_global_h():
+    """h_i = h for all i: h_ij = h, so sets, density and forces must equal the (pinned) global-h results."""
+    posm, vele, _ = _varh_case()
+    n, h = len(posm), np.float32(0.06)
+    hs = np.full(n, h, np.float32)
+    o0, i0 = oracle.neighbours(posm, n, h)
+    o1, i1 = oracle.neighbours(posm, n, h, hs=hs)
+    assert np.array_equal(o0, o1) and np.array_equal(i0, i1)
+    r0 = oracle.density(posm, h, o0, i0)
+    r1 = oracle.density(posm, h, o1, i1, hs=hs)
+    assert np.allclose(r0, r1, rtol=1e-14)
+    f0 = oracle.forces(posm, vele, r0, h, o0, i0)
+    f1 = oracle.forces(posm, vele, r0, h, o1, i1, hs=hs)
+    assert np.allclose(f0, f1, rtol=1e-12, atol=1e-14 * np.abs(f0).max())
+
+
+def test_VARH_grid_sets_equal_brute_force_and_are_symmetric():
+    posm, _, hs = _varh_case()
+    n, h_max = len(posm), 0.08
+    ob, ib = oracle.neighbours(posm, n, h_max, hs=hs, method="brute")
+    og, ig = oracle.neighbours(posm, n, h_max, hs=hs, method="grid")
+    assert np.array_equal(ob, og) and np.array_equal(ib, ig)
+    pairs = set()
+    for i in range(n):
+        for j in ib[ob[i]:ob[i + 1]]:
+            pairs.add((i, int(j)))
+    assert all((j, i) in pairs for (i, j) in pairs)               # h_ij is symmetric, so is the relation
+    # the cutoff really is h_i + h_j: every listed pair is inside it, and some pair is outside 2 min(h_i, h_j)
+    d = np.array([np.linalg.norm(posm[i, :3].astype(np.float64) - posm[j, :3]) for (i, j) in pairs])
+    lim = np.array([float(hs[i]) + float(hs[j]) for (i, j) in pairs])
+    small = np.array([2.0 * min(float(hs[i]), float(hs[j])) for (i, j) in pairs])
+    assert np.all(d < lim * (1 + 1e-6)) and np.any(d > small)
+
+
+def test_VARH_momentum_and_energy_identity():
+    """h_ij symmetric => Pi_ij symmetric and grad W_p antisymmetric as before: P5 and P6 must still hold."""
+    posm, vele, hs = _varh_case()
+    n, h_max = len(posm), 0.08
+    off, idx = oracle.neighbours(posm, n, h_max, hs=hs)
+    rho = oracle.density(posm, h_max, off, idx, hs=hs)
+    f = oracle.forces(posm, vele, rho, h_max, off, idx, hs=hs)
+    m = posm[:, 3].astype(np.float64)
+    v = vele[:, :3].astype(np.float64)
+    scale = (m * np.linalg.norm(f[:, :3], axis=1)).sum()
+    assert np.linalg.norm((m[:, None] * f[:, :3]).sum(0)) < 1e-13 * scale
+    resid = (m * f[:, 3]).sum() + (m * (v * f[:, :3]).sum(1)).sum()
+    assert abs(resid) < 1e-13 * ((m * np.abs(f[:, 3])).sum() + (m * np.abs((v * f[:, :3]).sum(1))).sum())
+
+
+def test_VARH_single_pair_by_hand():
+    gamma, alpha, beta, eta = 1.4, 0.5, 1.0, 0.1
+    h1, h2, d = 0.5, 0.3, 0.6                    # h_12 = 0.4, xi = 1.5 (outer branch); 2 h_12 = 0.8 > d
+    m1, m2, e1, e2 = 0.3, 0.7, 1.2, 0.8
+    posm = np.array([[0, 0, 0, m1], [d, 0, 0, m2]], dtype=np.float64)
+    vele = np.array([[0.4, 0.1, 0, e1], [-0.2, 0.0, 0, e2]], dtype=np.float64)
+    hs = np.array([h1, h2], dtype=np.float32)
+    h1, h2 = float(hs[0]), float(hs[1])          # the FP32 values both sides carry
+    h12 = 0.5 * (h1 + h2)
+    off, idx = oracle.neighbours(posm, 2, 0.5, hs=hs)
+    assert off.tolist() == [0, 1, 2]
+    rho = oracle.density(posm, 0.5, off, idx, hs=hs)
+    xi = d / h12
+    w12 = 0.25 * (2 - xi) ** 3 / (PI * h12 ** 3)
+    assert np.allclose(rho, [m1 / (PI * h1 ** 3) + m2 * w12, m2 / (PI * h2 ** 3) + m1 * w12], rtol=1e-14)
+    f = oracle.forces(posm, vele, rho, 0.5, off, idx, gamma=gamma, alpha=alpha, beta=beta, eta=eta, hs=hs)
+    p1, p2 = (gamma - 1) * rho[0] * e1, (gamma - 1) * rho[1] * e2
+    c1, c2 = math.sqrt(gamma * p1 / rho[0]), math.sqrt(gamma * p2 / rho[1])
+    dr, dv = np.array([-d, 0, 0]), np.array([0.6, 0.1, 0])
+    mu = h12 * (dr @ dv) / (d * d + eta * h12 * h12)
+    nu = mu * (beta * mu - alpha * 0.5 * (c1 + c2)) / (0.5 * (rho[0] + rho[1]))
+    Pi = p1 / rho[0] ** 2 + p2 / rho[1] ** 2 + nu
+    gradWp = (-45 / (64 * PI * h12 ** 3) * (2 - xi) ** 2) * (dr / d) / h12
+    assert np.allclose(f[0, :3], -m2 * Pi * gradWp, rtol=1e-13)
+    assert np.isclose(f[1, 3], 0.5 * m1 * Pi * (dv @ gradWp), rtol=1e-13)
+    # farther apart than h_1 + h_2 = 0.8 but closer than 2 h_1 = 1.0: not neighbours (the pair length decides)
+    posm[1, 0] = 0.9
+    off, _ = oracle.neighbours(posm, 2, 0.5, hs=hs)
+    assert off.tolist() == [0, 0, 0]
+
+
+def test_VARH_smoothing_lengths_on_lattice():
+    """L82 on a uniform lattice with m = rho0 a^3: (m/rho)^(1/3) = a (rho0/rho)^(1/3); capped at h_max (A25)."""
+    w = wl.lattice(7, 0.1, rho0=2.0)
+    n = w.n_gas
+    off, idx = oracle.neighbours(w.posm, n, 0.1)
+    rho = oracle.density(w.posm, 0.1, off, idx)
+    hs = oracle.smoothing_lengths(w.posm, rho, 1.3, 1.0)
+    assert hs.dtype == np.float32
+    assert np.allclose(hs, 1.3 * 0.1 * np.cbrt(2.0 / rho), rtol=2e-7)
+    centre = n // 2
+    assert abs(hs[centre] / (1.3 * 0.1) - 1) < 1e-4              # interior rho = 0.99997 rho0 (pin P3)
+    assert np.all(oracle.smoothing_lengths(w.posm, rho, 1.3, 0.12) <= np.float32(0.12))
