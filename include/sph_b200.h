@@ -179,6 +179,38 @@ int sph_neighbour_lists(const float* posm, int64_t n_gas, float h, const sph_gri
                         uint32_t* nbr_count, uint64_t* nbr_offset, uint32_t* nbr_index, uint64_t nbr_capacity,
                         void* ws, size_t ws_bytes, void* stream);
 
+/* ---- per-particle smoothing lengths (L82) ---------------------------------------
+ * hsml[n_gas] (DEVICE, float): h_i.  The effective length of a pair is h_ij = (h_i + h_j)/2 (L82) in W (Eq. 7-8),
+ * in grad W_p (L95) and in mu_ij (L97); (i, j) is a neighbour pair iff d2 < fl(fl(h_i + h_j)^2), FP32 like the
+ * global cutoff (reading A24; equal to it when h_i = h_j = h).  In these calls p->h is the CAP h_max of the
+ * lengths: the grid needs cell >= 2 h_max for the 3x3x3 stencil (that is what the paper's per-cell hmaxCell
+ * array, L164, provides for a finer grid), and every hsml[i] must be <= p->h — not checked (it would need a
+ * device reduction and a synchronisation); a larger value silently loses neighbours.
+ *
+ * sph_smoothing_lengths: hsml[i] = min(sigma (m_i / rho_i)^(1/3), h_max)        (L82; reading A25)
+ * sph_density_h / sph_forces_h / sph_evaluate_h / sph_neighbour_lists_h: as the calls without _h.
+ * sph_step_h: as sph_step; additionally, if sigma > 0, hsml is renewed from the refined density right after DC at
+ *   r(t+dt) (which itself used the old lengths) and the new lengths serve the corrector and the next step
+ *   (reading A26); sigma = 0 keeps hsml fixed.  hsml = NULL is exactly sph_step.                            */
+int sph_smoothing_lengths(const float* posm, const float* rho, int64_t n_gas, float sigma, float h_max,
+                          float* hsml /*[n_gas]*/, void* stream);
+int sph_density_h(const float* posm, const float* hsml, int64_t n_gas, const sph_params* p /*HOST*/,
+                  const sph_grid* g /*HOST*/, const uint32_t* perm, const uint32_t* cell_start, float* rho,
+                  void* ws, size_t ws_bytes, void* stream);
+int sph_forces_h(const float* posm, const float* vele, const float* rho, const float* hsml, int64_t n_gas,
+                 const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/, const uint32_t* perm,
+                 const uint32_t* cell_start, float* acc_sph, void* ws, size_t ws_bytes, void* stream);
+int sph_evaluate_h(const float* posm, const float* vele, const float* hsml, int64_t n_gas, int64_t n_halo,
+                   const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/, float* rho, float* acc_sph,
+                   float* acc_grav, void* ws, size_t ws_bytes, void* stream);
+int sph_step_h(float* posm, float* vele, float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p /*HOST*/,
+               const sph_grid* g /*HOST*/, float sigma, float dt, int first, float* rho, float* acc_sph,
+               float* acc_grav, void* ws, size_t ws_bytes, void* stream);
+int sph_neighbour_lists_h(const float* posm, const float* hsml, int64_t n_gas, float h_max, const sph_grid* g /*HOST*/,
+                          const uint32_t* perm, const uint32_t* cell_start, uint32_t* nbr_count,
+                          uint64_t* nbr_offset, uint32_t* nbr_index, uint64_t nbr_capacity,
+                          void* ws, size_t ws_bytes, void* stream);
+
 /* Stage timing: after sph_set_profiling(1) every stage the calling thread enqueues is bracketed
  * by CUDA events on the call's stream; sph_get_stage_ms() returns the milliseconds summed over all
  * calls since that switch-on (at most 4096 stage spans) for

@@ -25,6 +25,7 @@ EXPORTS = (
     "sph_density", "sph_forces", "nbody_pp_gravity", "sph_step", "sph_evaluate", "sph_step_host",
     "sph_host_ctx_create", "sph_host_ctx_step", "sph_host_ctx_destroy", "sph_neighbour_lists",
     "sph_set_profiling", "sph_get_stage_ms", "sph_launch_count", "sph_cfl_dt",
+    "sph_smoothing_lengths", "sph_density_h", "sph_forces_h", "sph_evaluate_h", "sph_step_h", "sph_neighbour_lists_h",
 )
 
 
@@ -98,6 +99,12 @@ def load():
     L.sph_host_ctx_step.argtypes = [vp, vp, vp, pp, f32, C.c_int, C.c_int, vp, vp, vp]
     L.sph_host_ctx_destroy.argtypes = [vp]
     L.sph_neighbour_lists.argtypes = [vp, i64, f32, gp, vp, vp, vp, vp, vp, C.c_uint64, vp, sz, vp]
+    L.sph_neighbour_lists_h.argtypes = [vp, vp, i64, f32, gp, vp, vp, vp, vp, vp, C.c_uint64, vp, sz, vp]
+    L.sph_smoothing_lengths.argtypes = [vp, vp, i64, f32, f32, vp, vp]
+    L.sph_density_h.argtypes = [vp, vp, i64, pp, gp, vp, vp, vp, vp, sz, vp]
+    L.sph_forces_h.argtypes = [vp, vp, vp, vp, i64, pp, gp, vp, vp, vp, vp, sz, vp]
+    L.sph_evaluate_h.argtypes = [vp, vp, vp, i64, i64, pp, gp, vp, vp, vp, vp, sz, vp]
+    L.sph_step_h.argtypes = [vp, vp, vp, i64, i64, pp, gp, f32, f32, C.c_int, vp, vp, vp, vp, sz, vp]
     _lib = L
     return L
 
@@ -200,6 +207,40 @@ def sph_evaluate(posm, vele, n_gas, n_halo, params, grid, rho, acc_sph, acc_grav
                                              _ptr(rho), _ptr(acc_sph), _ptr(acc_grav), p, nb, _stream()))
 
 
+# ------------------------------------------------------------------ NEXT-2: per-particle smoothing lengths
+def sph_smoothing_lengths(posm, rho, n_gas, sigma, h_max, hsml):
+    _chk("sph_smoothing_lengths", load().sph_smoothing_lengths(_ptr(posm), _ptr(rho), int(n_gas), float(sigma),
+                                                               float(h_max), _ptr(hsml), _stream()))
+
+
+def sph_density_h(posm, hsml, n_gas, params, grid, perm, cell_start, rho, ws):
+    p, nb = _ws(ws)
+    _chk("sph_density_h", load().sph_density_h(_ptr(posm), _ptr(hsml), int(n_gas), C.byref(params), C.byref(grid),
+                                               _ptr(perm), _ptr(cell_start), _ptr(rho), p, nb, _stream()))
+
+
+def sph_forces_h(posm, vele, rho, hsml, n_gas, params, grid, perm, cell_start, acc_sph, ws):
+    p, nb = _ws(ws)
+    _chk("sph_forces_h", load().sph_forces_h(_ptr(posm), _ptr(vele), _ptr(rho), _ptr(hsml), int(n_gas), C.byref(params),
+                                             C.byref(grid), _ptr(perm), _ptr(cell_start), _ptr(acc_sph), p, nb, _stream()))
+
+
+def sph_evaluate_h(posm, vele, hsml, n_gas, n_halo, params, grid, rho, acc_sph, acc_grav, ws):
+    p, nb = _ws(ws)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_evaluate_h", load().sph_evaluate_h(_ptr(posm), _ptr(vele), _ptr(hsml), int(n_gas), int(n_halo),
+                                                 C.byref(params), g, _ptr(rho), _ptr(acc_sph), _ptr(acc_grav), p, nb,
+                                                 _stream()))
+
+
+def sph_step_h(posm, vele, hsml, n_gas, n_halo, params, grid, sigma, dt, first, rho, acc_sph, acc_grav, ws):
+    p, nb = _ws(ws)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_step_h", load().sph_step_h(_ptr(posm), _ptr(vele), _ptr(hsml), int(n_gas), int(n_halo), C.byref(params), g,
+                                         float(sigma), float(dt), int(bool(first)), _ptr(rho), _ptr(acc_sph),
+                                         _ptr(acc_grav), p, nb, _stream()))
+
+
 def _hp(a):
     if a is None:
         return None
@@ -240,24 +281,25 @@ class HostContext:
             pass
 
 
-def sph_neighbour_lists(posm, n_gas, h, grid, perm, cell_start, ws):
-    """Returns (count[n] uint32, offset[n+1] uint64 as int64 tensor, index[total] uint32) on the device."""
+def sph_neighbour_lists(posm, n_gas, h, grid, perm, cell_start, ws, hsml=None):
+    """Returns (count[n] uint32, offset[n+1] uint64 as int64 tensor, index[total] uint32) on the device.
+    hsml: per-particle smoothing lengths (sph_neighbour_lists_h; h is then their cap)."""
     L = load()
     n = int(n_gas)
     cnt = torch.zeros(max(n, 1), dtype=torch.int32, device="cuda")
     off = torch.zeros(n + 1, dtype=torch.int64, device="cuda")
     p, nb = _ws(ws)
-    rc = L.sph_neighbour_lists(_ptr(posm), n, float(h), C.byref(grid), _ptr(perm), _ptr(cell_start), _ptr(cnt), _ptr(off),
-                               None, 0, p, nb, _stream())
+    rc = L.sph_neighbour_lists_h(_ptr(posm), _ptr(hsml), n, float(h), C.byref(grid), _ptr(perm), _ptr(cell_start),
+                                 _ptr(cnt), _ptr(off), None, 0, p, nb, _stream())
     total = int(off[n].item())
     if rc == SPH_OK and total == 0:
         return cnt[:n], off, torch.zeros(0, dtype=torch.int32, device="cuda")
     if rc != SPH_ERR_WORKSPACE:
         _chk("sph_neighbour_lists", rc)
     idx = torch.zeros(total, dtype=torch.int32, device="cuda")
-    _chk("sph_neighbour_lists", L.sph_neighbour_lists(_ptr(posm), n, float(h), C.byref(grid), _ptr(perm),
-                                                      _ptr(cell_start), _ptr(cnt), _ptr(off), _ptr(idx), total, p, nb,
-                                                      _stream()))
+    _chk("sph_neighbour_lists", L.sph_neighbour_lists_h(_ptr(posm), _ptr(hsml), n, float(h), C.byref(grid), _ptr(perm),
+                                                        _ptr(cell_start), _ptr(cnt), _ptr(off), _ptr(idx), total, p, nb,
+                                                        _stream()))
     return cnt[:n], off, idx
 
 

@@ -43,18 +43,25 @@ int check_params(const sph_params* p, bool need_h) {
     return SPH_OK;
 }
 
-// SP + DC + GFC at the current positions: everything that depends on r only (L123, A11)
-int position_only(const float4* posm, int64_t n_gas, int64_t n_total, const sph_params* p, const sph_grid* g,
-                  float* rho, float4* acc_grav, const Workspace& w, cudaStream_t st) {
+// SP + DC + GFC at the current positions: everything that depends on r only (L123, A11).
+// hsml != NULL (NEXT-2): per-particle smoothing lengths; with sigma > 0 they are renewed from the refined density
+// right after DC, h_i = min(sigma (m_i/rho_i)^(1/3), p->h) (L82, readings A25/A26), and re-gathered into cell order.
+int position_only(const float4* posm, float* hsml, float sigma, int64_t n_gas, int64_t n_total, const sph_params* p,
+                  const sph_grid* g, float* rho, float4* acc_grav, const Workspace& w, cudaStream_t st) {
     if (n_gas > 0) {
         {
             Span sp(ST_SORT, st);
             SPHB_TRY(grid_build(posm, n_gas, g, w.key, w.perm, w.cell_count, w.cell_start, w.rank_u, w.tmp, w.tile_sums,
                                 w.posm_s, st));
+            if (hsml) SPHB_TRY(gather_sorted_h(hsml, w.perm, n_gas, w.h_s, st));
         }
         {
             Span sp(ST_DENSITY, st);
-            SPHB_TRY(density_sorted(w.posm_s, w.perm, w.cell_start, n_gas, p, g, rho, st));
+            SPHB_TRY(density_sorted(w.posm_s, hsml ? w.h_s : nullptr, w.perm, w.cell_start, n_gas, p, g, rho, st));
+            if (hsml && sigma > 0.f) {
+                SPHB_TRY(smoothing_lengths(posm, rho, n_gas, sigma, p->h, hsml, st));
+                SPHB_TRY(gather_sorted_h(hsml, w.perm, n_gas, w.h_s, st));
+            }
         }
     }
     {
@@ -64,11 +71,12 @@ int position_only(const float4* posm, int64_t n_gas, int64_t n_total, const sph_
     return SPH_OK;
 }
 
-int hydro(const float4* vele, const float* rho, int64_t n_gas, const sph_params* p, const sph_grid* g, float4* acc_sph,
-          const Workspace& w, cudaStream_t st) {
+int hydro(const float4* vele, const float* rho, bool varh, int64_t n_gas, const sph_params* p, const sph_grid* g,
+          float4* acc_sph, const Workspace& w, cudaStream_t st) {
     if (n_gas <= 0) return SPH_OK;
     Span sp(ST_FORCES, st);
-    return forces_sorted(w.posm_s, vele, rho, w.perm, w.cell_start, n_gas, p, g, w.velr_s, w.pc_s, acc_sph, st);
+    return forces_sorted(w.posm_s, vele, rho, varh ? w.h_s : nullptr, w.perm, w.cell_start, n_gas, p, g, w.velr_s, w.pc_s,
+                         acc_sph, st);
 }
 
 int check_state_args(const void* posm, const void* vele, int64_t n_gas, int64_t n_halo, const sph_params* p,
@@ -177,7 +185,7 @@ int sph_density(const float* posm, int64_t n_gas, const sph_params* p, const sph
     cudaStream_t st = (cudaStream_t)stream;
     SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
     Span sp(ST_DENSITY, st);
-    return density_sorted(w.posm_s, perm, cell_start, n_gas, p, g, rho, st);
+    return density_sorted(w.posm_s, nullptr, perm, cell_start, n_gas, p, g, rho, st);
 }
 
 int sph_forces(const float* posm, const float* vele, const float* rho, int64_t n_gas, const sph_params* p,
@@ -195,7 +203,7 @@ int sph_forces(const float* posm, const float* vele, const float* rho, int64_t n
     cudaStream_t st = (cudaStream_t)stream;
     SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
     Span sp(ST_FORCES, st);
-    return forces_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, perm, cell_start, n_gas, p, g, w.velr_s,
+    return forces_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, nullptr, perm, cell_start, n_gas, p, g, w.velr_s,
                          w.pc_s, reinterpret_cast<float4*>(acc_sph), st);
 }
 
@@ -235,22 +243,32 @@ int nbody_pp_gravity(const float* posm, int64_t n_total, float G, float delta, f
                    w.grav_part, st);
 }
 
-int sph_evaluate(const float* posm, const float* vele, int64_t n_gas, int64_t n_halo, const sph_params* p,
-                 const sph_grid* g, float* rho, float* acc_sph, float* acc_grav, void* ws, size_t ws_bytes,
-                 void* stream) {
+int sph_evaluate_h(const float* posm, const float* vele, const float* hsml, int64_t n_gas, int64_t n_halo,
+                   const sph_params* p, const sph_grid* g, float* rho, float* acc_sph, float* acc_grav, void* ws,
+                   size_t ws_bytes, void* stream) {
     SPHB_TRY(check_state_args(posm, vele, n_gas, n_halo, p, g, rho, acc_sph, acc_grav, ws, ws_bytes));
     const int64_t n = n_gas + n_halo;
     if (n == 0) return SPH_OK;
     Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
     cudaStream_t st = (cudaStream_t)stream;
-    SPHB_TRY(position_only(reinterpret_cast<const float4*>(posm), n_gas, n, p, g, rho, reinterpret_cast<float4*>(acc_grav),
-                           w, st));
-    return hydro(reinterpret_cast<const float4*>(vele), rho, n_gas, p, g, reinterpret_cast<float4*>(acc_sph), w, st);
+    float* hs = n_gas > 0 ? const_cast<float*>(hsml) : nullptr;   // sigma = 0: never written
+    SPHB_TRY(position_only(reinterpret_cast<const float4*>(posm), hs, 0.f, n_gas, n, p, g, rho,
+                           reinterpret_cast<float4*>(acc_grav), w, st));
+    return hydro(reinterpret_cast<const float4*>(vele), rho, hs != nullptr, n_gas, p, g, reinterpret_cast<float4*>(acc_sph),
+                 w, st);
 }
 
-int sph_step(float* posm, float* vele, int64_t n_gas, int64_t n_halo, const sph_params* p, const sph_grid* g, float dt,
-             int first, float* rho, float* acc_sph, float* acc_grav, void* ws, size_t ws_bytes, void* stream) {
+int sph_evaluate(const float* posm, const float* vele, int64_t n_gas, int64_t n_halo, const sph_params* p,
+                 const sph_grid* g, float* rho, float* acc_sph, float* acc_grav, void* ws, size_t ws_bytes,
+                 void* stream) {
+    return sph_evaluate_h(posm, vele, nullptr, n_gas, n_halo, p, g, rho, acc_sph, acc_grav, ws, ws_bytes, stream);
+}
+
+int sph_step_h(float* posm, float* vele, float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p,
+               const sph_grid* g, float sigma, float dt, int first, float* rho, float* acc_sph, float* acc_grav, void* ws,
+               size_t ws_bytes, void* stream) {
     SPHB_TRY(check_state_args(posm, vele, n_gas, n_halo, p, g, rho, acc_sph, acc_grav, ws, ws_bytes));
+    if (sigma < 0.f) return SPH_ERR_ARG;
     const int64_t n = n_gas + n_halo;
     if (n == 0) return SPH_OK;
     Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
@@ -259,19 +277,73 @@ int sph_step(float* posm, float* vele, int64_t n_gas, int64_t n_halo, const sph_
     float4* v4 = reinterpret_cast<float4*>(vele);
     float4* as4 = reinterpret_cast<float4*>(acc_sph);
     float4* ag4 = reinterpret_cast<float4*>(acc_grav);
-    if (first) SPHB_TRY(position_only(r4, n_gas, n, p, g, rho, ag4, w, st));   // seed the carried state
-    SPHB_TRY(hydro(v4, rho, n_gas, p, g, as4, w, st));                          // HFC(predictor)
+    float* hs = n_gas > 0 ? hsml : nullptr;
+    const bool varh = hs != nullptr;
+    if (first) SPHB_TRY(position_only(r4, hs, 0.f, n_gas, n, p, g, rho, ag4, w, st));   // seed the carried state
+    SPHB_TRY(hydro(v4, rho, varh, n_gas, p, g, as4, w, st));                             // HFC(predictor)
     {
         Span sp(ST_UPDATE, st);
         SPHB_TRY(update_predictor(r4, v4, w.vele0, as4, ag4, n_gas, n, dt, st));   // SU(predictor): Eqs. 12-14
     }
-    SPHB_TRY(position_only(r4, n_gas, n, p, g, rho, ag4, w, st));               // SP, DC, GFC at r(t+dt)
-    SPHB_TRY(hydro(v4, rho, n_gas, p, g, as4, w, st));                          // HFC(corrector)
+    SPHB_TRY(position_only(r4, hs, sigma, n_gas, n, p, g, rho, ag4, w, st));      // SP, DC (+ new h), GFC at r(t+dt)
+    SPHB_TRY(hydro(v4, rho, varh, n_gas, p, g, as4, w, st));                      // HFC(corrector)
     {
         Span sp(ST_UPDATE, st);
         SPHB_TRY(update_corrector(v4, w.vele0, as4, ag4, n_gas, n, dt, st));       // SU(corrector): Eqs. 15-16
     }
     return SPH_OK;
+}
+
+int sph_step(float* posm, float* vele, int64_t n_gas, int64_t n_halo, const sph_params* p, const sph_grid* g, float dt,
+             int first, float* rho, float* acc_sph, float* acc_grav, void* ws, size_t ws_bytes, void* stream) {
+    return sph_step_h(posm, vele, nullptr, n_gas, n_halo, p, g, 0.f, dt, first, rho, acc_sph, acc_grav, ws, ws_bytes,
+                      stream);
+}
+
+int sph_smoothing_lengths(const float* posm, const float* rho, int64_t n_gas, float sigma, float h_max, float* hsml,
+                          void* stream) {
+    if (bad_count(n_gas) || !(sigma > 0.f) || !(h_max > 0.f)) return SPH_ERR_ARG;
+    if (n_gas == 0) return SPH_OK;
+    if (!posm || !rho || !hsml || !aligned16(posm)) return SPH_ERR_ARG;
+    return smoothing_lengths(reinterpret_cast<const float4*>(posm), rho, n_gas, sigma, h_max, hsml, (cudaStream_t)stream);
+}
+
+int sph_density_h(const float* posm, const float* hsml, int64_t n_gas, const sph_params* p, const sph_grid* g,
+                  const uint32_t* perm, const uint32_t* cell_start, float* rho, void* ws, size_t ws_bytes, void* stream) {
+    if (bad_count(n_gas)) return SPH_ERR_ARG;
+    SPHB_TRY(check_params(p, true));
+    if (n_gas == 0) return SPH_OK;
+    if (!posm || !hsml || !perm || !cell_start || !rho || !ws || !aligned16(posm) ||
+        (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return SPH_ERR_ARG;
+    SPHB_TRY(check_grid(g, p->h));
+    Workspace w = carve(ws, n_gas, n_gas, g);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
+    SPHB_TRY(gather_sorted_h(hsml, perm, n_gas, w.h_s, st));
+    Span sp(ST_DENSITY, st);
+    return density_sorted(w.posm_s, w.h_s, perm, cell_start, n_gas, p, g, rho, st);
+}
+
+int sph_forces_h(const float* posm, const float* vele, const float* rho, const float* hsml, int64_t n_gas,
+                 const sph_params* p, const sph_grid* g, const uint32_t* perm, const uint32_t* cell_start, float* acc_sph,
+                 void* ws, size_t ws_bytes, void* stream) {
+    if (bad_count(n_gas)) return SPH_ERR_ARG;
+    SPHB_TRY(check_params(p, true));
+    if (n_gas == 0) return SPH_OK;
+    if (!posm || !vele || !rho || !hsml || !perm || !cell_start || !acc_sph || !ws || !aligned16(posm) ||
+        !aligned16(vele) || !aligned16(acc_sph) || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return SPH_ERR_ARG;
+    SPHB_TRY(check_grid(g, p->h));
+    Workspace w = carve(ws, n_gas, n_gas, g);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
+    SPHB_TRY(gather_sorted_h(hsml, perm, n_gas, w.h_s, st));
+    Span sp(ST_FORCES, st);
+    return forces_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, w.h_s, perm, cell_start, n_gas, p, g,
+                         w.velr_s, w.pc_s, reinterpret_cast<float4*>(acc_sph), st);
 }
 
 }  // extern "C"

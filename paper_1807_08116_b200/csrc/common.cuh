@@ -65,6 +65,7 @@ struct Workspace {
     float4* posm_s;        // [n_gas] (x,y,z,m)
     float4* velr_s;        // [n_gas] (vx,vy,vz,rho)
     float2* pc_s;          // [n_gas] (p/rho^2, c)
+    float* h_s;            // [n_gas] per-particle smoothing lengths in cell order (NEXT-2)
     // gravity
     float4* src_pk;        // [n_pad] packed source pairs
     float4* grav_part;     // [S][n_total] partial accelerations
@@ -87,11 +88,15 @@ int grid_build(const float4* posm, int64_t n_gas, const sph_grid* g, uint32_t* k
                uint32_t* cell_count, uint32_t* cell_start, uint32_t* rank_u, uint32_t* tmp, uint32_t* tile_sums,
                float4* posm_s /*may be NULL*/, cudaStream_t st);
 int gather_sorted_pos(const float4* posm, const uint32_t* perm, int64_t n_gas, float4* posm_s, cudaStream_t st);
-int density_sorted(const float4* posm_s, const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas,
-                   const sph_params* p, const sph_grid* g, float* rho, cudaStream_t st);
-int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const uint32_t* perm,
+// h_s: per-particle smoothing lengths in cell order (NEXT-2), or NULL for the one global p->h
+int density_sorted(const float4* posm_s, const float* h_s, const uint32_t* perm, const uint32_t* cell_start,
+                   int64_t n_gas, const sph_params* p, const sph_grid* g, float* rho, cudaStream_t st);
+int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const float* h_s, const uint32_t* perm,
                   const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
                   float4* velr_s, float2* pc_s, float4* acc_sph, cudaStream_t st);
+int smoothing_lengths(const float4* posm, const float* rho, int64_t n_gas, float sigma, float h_max, float* hsml,
+                      cudaStream_t st);
+int gather_sorted_h(const float* hsml, const uint32_t* perm, int64_t n_gas, float* h_s, cudaStream_t st);
 int cfl_sorted(const float4* posm_s, const float4* vele, const float* rho, const float4* acc_sph, const float4* acc_grav,
                const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
                float c_cfl, float4* velr_s, float2* pc_s, float* dt_out, float* dt_particle, cudaStream_t st);

@@ -13,6 +13,7 @@ __device__ __forceinline__ float nl_d2(const float4 a, const float4 b) {
 template <int PASS>
 __global__ void __launch_bounds__(128) k_nbr(const float4* __restrict__ posm_s, const uint32_t* __restrict__ perm,
                                              const uint32_t* __restrict__ start, int n, GridDev g, float rc2,
+                                             const float* __restrict__ h_s /*cell order, or NULL (global h)*/,
                                              uint32_t* __restrict__ cnt, const uint64_t* __restrict__ off,
                                              uint32_t* __restrict__ idx) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
@@ -31,7 +32,12 @@ __global__ void __launch_bounds__(128) k_nbr(const float4* __restrict__ posm_s, 
         const uint32_t lo = start[row + max(ix - 1, 0)], hi = start[row + min(ix + 1, g.mx - 1) + 1];
         for (uint32_t t = lo; t < hi; ++t) {
             if ((int)t == s) continue;
-            if (nl_d2(pi, posm_s[t]) < rc2) {
+            float lim = rc2;
+            if (h_s) {   // reading A24: pair cutoff fl(fl(h_i + h_j)^2)
+                const float hsum = __fadd_rn(h_s[s], h_s[t]);
+                lim = __fmul_rn(hsum, hsum);
+            }
+            if (nl_d2(pi, posm_s[t]) < lim) {
                 if (PASS) idx[base + c] = perm[t];
                 ++c;
             }
@@ -96,9 +102,10 @@ __global__ void __launch_bounds__(128) k_nbr_sort(const uint64_t* __restrict__ o
 
 using namespace sphb;
 
-extern "C" int sph_neighbour_lists(const float* posm, int64_t n_gas, float h, const sph_grid* g, const uint32_t* perm,
-                                   const uint32_t* cell_start, uint32_t* nbr_count, uint64_t* nbr_offset,
-                                   uint32_t* nbr_index, uint64_t nbr_capacity, void* ws, size_t ws_bytes, void* stream) {
+extern "C" int sph_neighbour_lists_h(const float* posm, const float* hsml, int64_t n_gas, float h, const sph_grid* g,
+                                     const uint32_t* perm, const uint32_t* cell_start, uint32_t* nbr_count,
+                                     uint64_t* nbr_offset, uint32_t* nbr_index, uint64_t nbr_capacity, void* ws,
+                                     size_t ws_bytes, void* stream) {
     if (n_gas < 0 || n_gas >= (1ll << 31) || !(h > 0.f) || !nbr_offset) return SPH_ERR_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     if (n_gas == 0) {
@@ -116,7 +123,13 @@ extern "C" int sph_neighbour_lists(const float* posm, int64_t n_gas, float h, co
     const float rc2 = two_h * two_h;
     const GridDev gd = to_dev(g);
     SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
-    k_nbr<0><<<(unsigned)cdiv(n, 128), 128, 0, st>>>(w.posm_s, perm, cell_start, n, gd, rc2, nbr_count, nullptr, nullptr);
+    const float* h_s = nullptr;
+    if (hsml) {
+        SPHB_TRY(gather_sorted_h(hsml, perm, n_gas, w.h_s, st));
+        h_s = w.h_s;
+    }
+    k_nbr<0><<<(unsigned)cdiv(n, 128), 128, 0, st>>>(w.posm_s, perm, cell_start, n, gd, rc2, h_s, nbr_count, nullptr,
+                                                    nullptr);
     SPHB_LAUNCHED();
     k_nbr_scan<<<1, 1024, 0, st>>>(nbr_count, n, nbr_offset);
     SPHB_LAUNCHED();
@@ -125,7 +138,7 @@ extern "C" int sph_neighbour_lists(const float* posm, int64_t n_gas, float h, co
     SPHB_CUDA(cudaStreamSynchronize(st));
     if (total > nbr_capacity || (total > 0 && !nbr_index)) return SPH_ERR_WORKSPACE;
     if (total > 0) {
-        k_nbr<1><<<(unsigned)cdiv(n, 128), 128, 0, st>>>(w.posm_s, perm, cell_start, n, gd, rc2, nbr_count, nbr_offset,
+        k_nbr<1><<<(unsigned)cdiv(n, 128), 128, 0, st>>>(w.posm_s, perm, cell_start, n, gd, rc2, h_s, nbr_count, nbr_offset,
                                                         nbr_index);
         SPHB_LAUNCHED();
         k_nbr_sort<<<(unsigned)cdiv(n, 128), 128, 0, st>>>(nbr_offset, n, nbr_index);
@@ -133,4 +146,11 @@ extern "C" int sph_neighbour_lists(const float* posm, int64_t n_gas, float h, co
     }
     SPHB_CUDA(cudaStreamSynchronize(st));
     return SPH_OK;
+}
+
+extern "C" int sph_neighbour_lists(const float* posm, int64_t n_gas, float h, const sph_grid* g, const uint32_t* perm,
+                                   const uint32_t* cell_start, uint32_t* nbr_count, uint64_t* nbr_offset,
+                                   uint32_t* nbr_index, uint64_t nbr_capacity, void* ws, size_t ws_bytes, void* stream) {
+    return sph_neighbour_lists_h(posm, nullptr, n_gas, h, g, perm, cell_start, nbr_count, nbr_offset, nbr_index,
+                                 nbr_capacity, ws, ws_bytes, stream);
 }

@@ -53,12 +53,18 @@ __device__ __forceinline__ float w_spline_unnorm(float xi) {
     return xi <= 1.0f ? inner : fmaxf(outer, 0.0f);
 }
 
-__global__ void __launch_bounds__(128) k_density(const float4* __restrict__ posm_s, const uint32_t* __restrict__ perm,
-                                                 const uint32_t* __restrict__ start, int n, GridDev g, float rc2,
-                                                 float inv_h, float norm, float* __restrict__ rho) {
+// VARH: per-particle smoothing lengths h_s[] in cell order; the pair length is
+// h_ij = (h_i + h_j)/2, the pair is a neighbour pair iff d2 < fl(fl(h_i + h_j)^2) (reading A24, FP32 like A8),
+// and W(|dr|/h_ij, h_ij) carries its own 1/(pi h_ij^3).  VARH = false is the global-h kernel, unchanged.
+template <bool VARH>
+__global__ void __launch_bounds__(128) k_density(const float4* __restrict__ posm_s, const float* __restrict__ h_s,
+                                                 const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start,
+                                                 int n, GridDev g, float rc2, float inv_h, float norm,
+                                                 float* __restrict__ rho) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
     const float4 pi = posm_s[s];
+    const float h_i = VARH ? h_s[s] : 0.f;
     const uint32_t k = key_of(pi, g);
     const int ix = (int)(k % (uint32_t)g.mx), iy = (int)((k / (uint32_t)g.mx) % (uint32_t)g.my),
               iz = (int)(k / ((uint32_t)g.mx * (uint32_t)g.my));
@@ -71,7 +77,14 @@ __global__ void __launch_bounds__(128) k_density(const float4* __restrict__ posm
             const float4 pj = posm_s[t];
             float dx, dy, dz;
             const float d2 = dist2_f32(pi, pj, dx, dy, dz);
-            if (d2 < rc2) {
+            if (VARH) {
+                const float hsum = __fadd_rn(h_i, h_s[t]);         // 2 h_ij
+                if (d2 < __fmul_rn(hsum, hsum)) {
+                    const float inv = 1.0f / (0.5f * hsum);        // IEEE division
+                    const float xi = sqrtf(d2) * inv;
+                    sum = fmaf(pj.w, w_spline_unnorm(xi) * (inv * inv * inv), sum);
+                }
+            } else if (d2 < rc2) {
                 const float xi = sqrtf(d2) * inv_h;
                 sum = fmaf(pj.w, w_spline_unnorm(xi), sum);
             }
@@ -80,15 +93,50 @@ __global__ void __launch_bounds__(128) k_density(const float4* __restrict__ posm
     rho[perm[s]] = sum * norm;
 }
 
-int density_sorted(const float4* posm_s, const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas,
-                   const sph_params* p, const sph_grid* g, float* rho, cudaStream_t st) {
+__global__ void __launch_bounds__(256) k_gather_f32(const float* __restrict__ a, const uint32_t* __restrict__ perm, int n,
+                                                    float* __restrict__ a_s) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < n) a_s[s] = a[perm[s]];
+}
+
+// L82: h_i = sigma (m_i / rho_i)^(1/3), capped at h_max (reading A25).  cbrtf is within 1 ulp.
+__global__ void __launch_bounds__(256) k_smoothing_lengths(const float4* __restrict__ posm, const float* __restrict__ rho,
+                                                           int n, float sigma, float h_max, float* __restrict__ hsml) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) hsml[i] = fminf(sigma * cbrtf(posm[i].w / rho[i]), h_max);
+}
+
+int smoothing_lengths(const float4* posm, const float* rho, int64_t n_gas, float sigma, float h_max, float* hsml,
+                      cudaStream_t st) {
+    if (n_gas <= 0) return SPH_OK;
+    k_smoothing_lengths<<<(unsigned)cdiv(n_gas, 256), 256, 0, st>>>(posm, rho, (int)n_gas, sigma, h_max, hsml);
+    SPHB_LAUNCHED();
+    return SPH_OK;
+}
+
+int gather_sorted_h(const float* hsml, const uint32_t* perm, int64_t n_gas, float* h_s, cudaStream_t st) {
+    if (n_gas <= 0) return SPH_OK;
+    k_gather_f32<<<(unsigned)cdiv(n_gas, 256), 256, 0, st>>>(hsml, perm, (int)n_gas, h_s);
+    SPHB_LAUNCHED();
+    return SPH_OK;
+}
+
+int density_sorted(const float4* posm_s, const float* h_s /*cell order, or NULL: global h*/, const uint32_t* perm,
+                   const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g, float* rho,
+                   cudaStream_t st) {
     if (n_gas <= 0) return SPH_OK;
     const float two_h = 2.0f * p->h;
     const float rc2 = two_h * two_h;
     const float inv_h = 1.0f / p->h;
-    const float norm = (float)(1.0 / (3.14159265358979323846 * (double)p->h * (double)p->h * (double)p->h));
-    k_density<<<(unsigned)cdiv(n_gas, 128), 128, 0, st>>>(posm_s, perm, cell_start, (int)n_gas, to_dev(g), rc2, inv_h,
-                                                          norm, rho);
+    const unsigned blocks = (unsigned)cdiv(n_gas, 128);
+    if (h_s) {
+        k_density<true><<<blocks, 128, 0, st>>>(posm_s, h_s, perm, cell_start, (int)n_gas, to_dev(g), rc2, inv_h,
+                                                (float)(1.0 / 3.14159265358979323846), rho);
+    } else {
+        const float norm = (float)(1.0 / (3.14159265358979323846 * (double)p->h * (double)p->h * (double)p->h));
+        k_density<false><<<blocks, 128, 0, st>>>(posm_s, nullptr, perm, cell_start, (int)n_gas, to_dev(g), rc2, inv_h,
+                                                 norm, rho);
+    }
     SPHB_LAUNCHED();
     return SPH_OK;
 }
@@ -114,6 +162,7 @@ struct ViscDev {
     float h, alpha, beta, eta_h2, gw;   // gw = -45 / (64 pi h^4): grad W_p = gw (2-xi)^2 dr/|dr|
     float inv_h2;                       // 1 / h^2
     double rc2_64;                      // 4 h^2 in FP64 (h as given, widened)
+    float eta, gw_unit;                 // VARH: eta and -45 / (64 pi); the h powers are applied per pair
 };
 
 // Compensated (Kahan) accumulation.  The hydro terms of one particle routinely cancel by 10^2-10^3
@@ -129,29 +178,39 @@ struct KSum {
     }
 };
 
+// VARH: as k_density<true> — pair length h_ij = (h_i + h_j)/2 in the cutoff, in grad W_p and in mu_ij (L82, L95-97).
+template <bool VARH>
 __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_s, const float4* __restrict__ velr_s,
-                                                const float2* __restrict__ pc_s, const uint32_t* __restrict__ perm,
-                                                const uint32_t* __restrict__ start, int n, GridDev g, float rc2,
-                                                ViscDev q, float4* __restrict__ acc) {
+                                                const float2* __restrict__ pc_s, const float* __restrict__ h_s,
+                                                const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start,
+                                                int n, GridDev g, float rc2, ViscDev q, float4* __restrict__ acc) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
     const float4 pi = posm_s[s];
     const float4 vi = velr_s[s];
     const float2 ci = pc_s[s];
+    const float h_i = VARH ? h_s[s] : 0.f;
     const uint32_t k = key_of(pi, g);
     const int ix = (int)(k % (uint32_t)g.mx), iy = (int)((k / (uint32_t)g.mx) % (uint32_t)g.my),
               iz = (int)(k / ((uint32_t)g.mx * (uint32_t)g.my));
-    const float inv_h = 1.0f / q.h;
+    const float inv_h_glob = 1.0f / q.h;
     KSum ax, ay, az, de;
 #pragma unroll 1
     for (int r = 0; r < 9; ++r) {
-        uint32_t lo, hi;
-        stencil_run(start, g, ix, iy, iz, r, lo, hi);
-        for (uint32_t t = lo; t < hi; ++t) {
+        uint32_t lo, hi_;
+        stencil_run(start, g, ix, iy, iz, r, lo, hi_);
+        for (uint32_t t = lo; t < hi_; ++t) {
             const float4 pj = posm_s[t];
             float dx, dy, dz;
             const float d2 = dist2_f32(pi, pj, dx, dy, dz);
-            if (d2 < rc2 && d2 > 0.f) {   // d2 == 0: self, or a coincident pair (A9) — no contribution
+            // pair constants: global h, or the pair length h_ij
+            float rc2p = rc2, hh = q.h, eta_h2 = q.eta_h2;
+            float hsum = 0.f;
+            if (VARH) {
+                hsum = __fadd_rn(h_i, h_s[t]);                     // 2 h_ij
+                rc2p = __fmul_rn(hsum, hsum);
+            }
+            if (d2 < rc2p && d2 > 0.f) {   // d2 == 0: self, or a coincident pair (A9) — no contribution
                 const float4 vj = velr_s[t];
                 const float2 cj = pc_s[t];
                 float rinv = rsqrtf(d2);
@@ -160,14 +219,26 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
                 // 2 - xi = (4h^2 - |dr|^2) / (h^2 (2 + xi)).  Formed as 2 - rr/h in FP32 it loses a factor
                 // xi/(2-xi) of relative accuracy near the kernel edge (every term of a sparsely surrounded
                 // particle sits there), so the numerator alone is taken in FP64: 3 cvt + 3 DFMA per pair.
-                const double num = fma(-(double)dz, (double)dz, fma(-(double)dy, (double)dy, fma(-(double)dx, (double)dx, q.rc2_64)));
-                const float tq = fmaxf((float)num, 0.0f) * q.inv_h2 / (2.0f + rr * inv_h);   // 2 - xi
                 // grad W_p = dWp/dxi * dr/|dr| / h,  dWp/dxi = -45/(64 pi h^3) (2-xi)^2   (L95, Eq. 9, A3)
-                const float gmag = q.gw * tq * tq * rinv;          // grad W_p = gmag * dr
+                float gmag;                                        // grad W_p = gmag * dr
+                if (VARH) {
+                    // the pair factor goes like h_ij^-8: with a per-pair h its roundings no longer cancel as a
+                    // common factor of the particle's sum, so it is formed in FP64 and rounded once
+                    const double hd = 0.5 * (double)hsum, ihd = 1.0 / hd, ih2 = ihd * ihd;
+                    const double num = fma(-(double)dz, (double)dz, fma(-(double)dy, (double)dy, fma(-(double)dx, (double)dx, (double)hsum * (double)hsum)));
+                    const double tqd = fmax(num, 0.0) * ih2 / (2.0 + (double)rr * ihd);       // 2 - xi
+                    gmag = (float)((double)q.gw_unit * ih2 * ih2 * tqd * tqd) * rinv;
+                    hh = 0.5f * hsum;
+                    eta_h2 = q.eta * hh * hh;
+                } else {
+                    const double num = fma(-(double)dz, (double)dz, fma(-(double)dy, (double)dy, fma(-(double)dx, (double)dx, q.rc2_64)));
+                    const float tq = fmaxf((float)num, 0.0f) * q.inv_h2 / (2.0f + rr * inv_h_glob);   // 2 - xi
+                    gmag = q.gw * tq * tq * rinv;
+                }
                 const float dvx = vi.x - vj.x, dvy = vi.y - vj.y, dvz = vi.z - vj.z;
                 const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
                 // mu_ij = h dr.dv / (|dr|^2 + eta h^2) if dr.dv < 0   (L97)
-                const float mu = rv < 0.f ? (q.h * rv) / (d2 + q.eta_h2) : 0.f;       // IEEE division
+                const float mu = rv < 0.f ? (hh * rv) / (d2 + eta_h2) : 0.f;       // IEEE division
                 const float rho_ij = 0.5f * (vi.w + vj.w), c_ij = 0.5f * (ci.y + cj.y);
                 const float nu = (mu * (q.beta * mu - q.alpha * c_ij)) / rho_ij;
                 const float Pi = ci.x + cj.x + nu;                 // p_i/rho_i^2 + p_j/rho_j^2 + nu  (L95, A2)
@@ -182,9 +253,9 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
     acc[perm[s]] = make_float4(ax.s, ay.s, az.s, de.s);
 }
 
-int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const uint32_t* perm,
-                  const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g, float4* velr_s,
-                  float2* pc_s, float4* acc_sph, cudaStream_t st) {
+int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const float* h_s /*or NULL*/,
+                  const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
+                  float4* velr_s, float2* pc_s, float4* acc_sph, cudaStream_t st) {
     if (n_gas <= 0) return SPH_OK;
     const int n = (int)n_gas;
     k_eos_gather<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(vele, rho, perm, n, p->gamma, velr_s, pc_s);
@@ -199,8 +270,14 @@ int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, co
     q.gw = (float)(-45.0 / (64.0 * 3.14159265358979323846 * h * h * h * h));   // dWp/dxi scale / h
     q.inv_h2 = (float)(1.0 / (h * h));
     q.rc2_64 = 4.0 * h * h;
-    k_forces<<<(unsigned)cdiv(n, 128), 128, 0, st>>>(posm_s, velr_s, pc_s, perm, cell_start, n, to_dev(g),
-                                                     two_h * two_h, q, acc_sph);
+    q.eta = p->eta;
+    q.gw_unit = (float)(-45.0 / (64.0 * 3.14159265358979323846));
+    if (h_s)
+        k_forces<true><<<(unsigned)cdiv(n, 128), 128, 0, st>>>(posm_s, velr_s, pc_s, h_s, perm, cell_start, n, to_dev(g),
+                                                               two_h * two_h, q, acc_sph);
+    else
+        k_forces<false><<<(unsigned)cdiv(n, 128), 128, 0, st>>>(posm_s, velr_s, pc_s, nullptr, perm, cell_start, n,
+                                                                to_dev(g), two_h * two_h, q, acc_sph);
     SPHB_LAUNCHED();
     return SPH_OK;
 }

@@ -39,6 +39,7 @@ Workspace carve(void* base, int64_t n_gas, int64_t n_total, const sph_grid* g) {
     w.posm_s = (float4*)take(ng * 16);
     w.velr_s = (float4*)take(ng * 16);
     w.pc_s = (float2*)take(ng * 8);
+    w.h_s = (float*)take(ng * 4);
     w.src_pk = (float4*)take((size_t)grav_padded(n_total) * 16);
     w.grav_part = (float4*)take((size_t)grav_splits(n_total) * nt * 16);
     w.vele0 = (float4*)take(nt * 16);

@@ -437,3 +437,86 @@ def test_error_codes(cuda_lib):
     # n = 0 is legal everywhere
     b.nbody_pp_gravity(d, 0, 1.0, 0.1, acc, ws)
     assert b.sph_launch_count() > 0
+
+
+# ---------------------------------------------------------------- NEXT-2: per-particle smoothing lengths (L82)
+def _hs_for(w, seed=5):
+    """Seeded lengths in [0.45, 1] h_max (FP32), spatially uncorrelated: the hardest case for the pair cutoff."""
+    rng = np.random.Generator(np.random.Philox(key=[seed, 9]))
+    return (np.float32(w.h) * (0.45 + 0.55 * rng.random(w.n_gas))).astype(np.float32)
+
+
+@pytest.mark.parametrize("case", ["galaxy", "dense", "clumps"])
+def test_varh_sets_density_forces_parity(cuda_lib, case):
+    b = cuda_lib
+    w, og = _grid_case(case)
+    n = w.n_gas
+    hs = _hs_for(w)
+    d, g, perm, start, ws = _build(b, w, og)
+    dh = _t(hs)
+    prm = b.sph_params.from_workload(w)                       # prm.h is the cap h_max: it sizes the cells
+    # neighbour sets: bit-exact
+    cnt, off, idx = b.sph_neighbour_lists(d, n, w.h, g, perm, start, ws, hsml=dh)
+    ooff, oidx = oracle.neighbours(w.posm, n, w.h, method="grid", hs=hs)
+    assert np.array_equal(off.cpu().numpy(), ooff)
+    assert np.array_equal(idx.cpu().numpy().view(np.uint32), oidx)
+    g_off, _ = oracle.neighbours(w.posm, n, w.h, method="grid")
+    assert ooff[-1] < g_off[-1]                                # the pair lengths really cut pairs the cap would keep
+    # density
+    rho = torch.zeros(n, device="cuda")
+    b.sph_density_h(d, dh, n, prm, g, perm, start, rho, ws)
+    orho = oracle.density(w.posm, w.h, ooff, oidx, hs=hs)
+    check_density(rho.cpu().numpy(), orho, f"rho varh {case}")
+    # forces, teacher-forced on the GPU's verified rho
+    acc = torch.zeros((n, 4), device="cuda")
+    dv = _t(w.vele)
+    b.sph_forces_h(d, dv, rho, dh, n, prm, g, perm, start, acc, ws)
+    of, gross = oracle.forces(w.posm, w.vele, rho.cpu().numpy().astype(np.float64), w.h, ooff, oidx, gamma=w.gamma,
+                              alpha=w.alpha, beta=w.beta, eta=w.eta, with_gross=True, hs=hs)
+    got = acc.cpu().numpy()
+    check_values(got[:, :3], of[:, :3], f"a_sph varh {case}", gross=gross[:, 0])
+    check_values(got[:, 3], of[:, 3], f"de/dt varh {case}", gross=gross[:, 1])
+    m = w.posm[:n, 3].astype(np.float64)
+    a = got[:, :3].astype(np.float64)
+    assert np.linalg.norm((m[:, None] * a).sum(0)) < 1e-5 * (m * np.linalg.norm(a, axis=1)).sum()   # P5 survives h_ij
+    # equal lengths reproduce the global-h kernels bit for bit
+    dh_eq = torch.full((n,), float(np.float32(w.h)), device="cuda")
+    rho_eq, rho_g = torch.zeros(n, device="cuda"), torch.zeros(n, device="cuda")
+    b.sph_density_h(d, dh_eq, n, prm, g, perm, start, rho_eq, ws)
+    b.sph_density(d, n, prm, g, perm, start, rho_g, ws)
+    assert (rho_eq - rho_g).abs().max().item() <= 2e-6 * rho_g.max().item()
+
+
+def test_varh_smoothing_lengths_and_step(cuda_lib):
+    """sph_smoothing_lengths against L82, then sph_step_h (lengths renewed after DC, reading A26) against the
+    oracle's step, free-running for 2 steps on config 0."""
+    b = cuda_lib
+    w = wl.make_workload(0, scale=0.5)
+    n, ng = w.n_total, w.n_gas
+    sigma = 0.8         # config 0 is sparse (~4 neighbours inside 2h): a smaller sigma than the paper's 1.2-1.3 so that
+                        # both the formula and the cap h_max = w.h (which sizes the cells) are exercised
+    sim = b.Simulation(w)
+    sim.evaluate()
+    hs_dev = torch.zeros(ng, device="cuda")
+    b.sph_smoothing_lengths(sim.posm, sim.rho, ng, sigma, w.h, hs_dev)
+    hs0 = oracle.smoothing_lengths(w.posm, sim.rho.cpu().numpy().astype(np.float64), sigma, w.h)
+    got = hs_dev.cpu().numpy()
+    assert np.abs(got - hs0).max() <= 3e-7 * hs0.max()          # cbrtf: 1 ulp
+    assert (got < np.float32(w.h)).any() and (got == np.float32(w.h)).any()   # both branches of the cap
+    # oracle side starts from the GPU's own FP32 lengths (an input of the step)
+    st = oracle.State(w.posm.astype(np.float64), w.vele.astype(np.float64), ng)
+    hs = got.copy()
+    nbr = oracle.position_only(st, w.h, w.G, w.delta, hs=hs)
+    sim.first = True
+    for k in range(2):
+        b.sph_step_h(sim.posm, sim.vele, hs_dev, ng, w.n_halo, sim.params, sim.grid, sigma, w.dt, k == 0, sim.rho,
+                     sim.acc_sph, sim.acc_grav, sim.ws)
+        st, nbr, diag = oracle.step(st, w.dt, w.h, w.G, w.delta, nbr=nbr, hs=hs, sigma=sigma)
+        hs = diag["hs"]
+    p = sim.posm.cpu().numpy()
+    v = sim.vele.cpu().numpy()
+    assert np.abs(p[:, :3] - st.posm[:, :3]).max() < 1e-5
+    check_values(v[:, :3], st.vele[:, :3], "v after 2 varh steps", max_tol=2e-5, med_tol=1e-6)
+    check_values(v[:ng, 3], st.vele[:ng, 3], "e after 2 varh steps", max_tol=2e-5, med_tol=1e-6)
+    check_density(sim.rho.cpu().numpy()[:ng], st.rho, "rho after 2 varh steps")
+    assert np.abs(hs_dev.cpu().numpy() - hs).max() <= 1e-5 * hs.max()
