@@ -218,7 +218,7 @@ def run_ours(args, w):
     peaks, peak_src = _peaks()
 
     n, ng = w.n_total, w.n_gas
-    sim = b.Simulation(w)
+    sim = b.Simulation(w, sigma=args.sigma)
     M = sim.grid.M if ng else 0
 
     def barrier():
@@ -316,7 +316,8 @@ def run_ours(args, w):
         "metric": "step_ms", "value": ms_step, "unit": "ms", "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "config": workload_config(args, w, list(sim.grid.dims) if ng else None, M, world),
+        "config": dict(workload_config(args, w, list(sim.grid.dims) if ng else None, M, world),
+                       **({"smoothing_lengths": f"per particle, sigma={args.sigma:g}, cap h"} if args.sigma is not None else {})),
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "stages": stages,
         "context": "paper Table 1 (K40, N=2^20, units inferred as s): t_SPH=7.87, t_GFC=53.62 — other hardware, not a target",
@@ -334,6 +335,8 @@ def main():
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--scale", type=float, default=1.0, help="shrink the workload (debug only; invalid as a bench number)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--sigma", type=float, default=None,
+                    help="per-particle smoothing lengths (NEXT-2): h_i = min(sigma (m/rho)^(1/3), h), renewed every step")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)

@@ -320,7 +320,9 @@ def sph_launch_count() -> int:
 class Simulation:
     """Convenience holder of the device buffers one run needs (no arithmetic: allocation and calls only)."""
 
-    def __init__(self, workload, grid=None):
+    def __init__(self, workload, grid=None, sigma=None):
+        """sigma: None = one global h (sph_step); a float = per-particle smoothing lengths (sph_step_h), started at
+        the cap h_max = workload.h and renewed every step with that sigma (0 keeps them fixed)."""
         w = workload
         self.w = w
         self.n_gas, self.n_halo, self.n = w.n_gas, w.n_halo, w.n_total
@@ -335,13 +337,18 @@ class Simulation:
             self.grid = sph_grid_from_bbox(self.posm, self.n_gas, w.h)
         self.ws = alloc_workspace(self.n_gas, self.n, self.grid)
         self.first = True
+        self.sigma = sigma
+        self.hsml = None
+        if sigma is not None and self.n_gas > 0:
+            self.hsml = torch.full((self.n_gas,), float(np.float32(w.h)), dtype=torch.float32, device="cuda")
 
     def evaluate(self):
-        sph_evaluate(self.posm, self.vele, self.n_gas, self.n_halo, self.params, self.grid, self.rho, self.acc_sph,
-                     self.acc_grav, self.ws)
+        sph_evaluate_h(self.posm, self.vele, self.hsml, self.n_gas, self.n_halo, self.params, self.grid, self.rho,
+                       self.acc_sph, self.acc_grav, self.ws)
         self.first = False
 
     def step(self, dt=None):
-        sph_step(self.posm, self.vele, self.n_gas, self.n_halo, self.params, self.grid,
-                 self.w.dt if dt is None else dt, self.first, self.rho, self.acc_sph, self.acc_grav, self.ws)
+        sph_step_h(self.posm, self.vele, self.hsml, self.n_gas, self.n_halo, self.params, self.grid,
+                   self.sigma or 0.0, self.w.dt if dt is None else dt, self.first, self.rho, self.acc_sph, self.acc_grav,
+                   self.ws)
         self.first = False
