@@ -25,11 +25,11 @@ __device__ __forceinline__ float dist2_f32(const float4 a, const float4 b, float
     return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
 }
 
-__device__ __forceinline__ uint32_t key_of(const float4 p, const GridDev g) {
-    float cx = fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.x, g.ox), g.inv_cell)), 0.0f), g.fx);
-    float cy = fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.y, g.oy), g.inv_cell)), 0.0f), g.fy);
-    float cz = fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.z, g.oz), g.inv_cell)), 0.0f), g.fz);
-    return (uint32_t)(int)cx + (uint32_t)g.mx * ((uint32_t)(int)cy + (uint32_t)g.my * (uint32_t)(int)cz);
+// cell coordinates of a particle (reading A7, same FP32 op sequence as the key kernel); no div / mod needed
+__device__ __forceinline__ void cell_of(const float4 p, const GridDev g, int& ix, int& iy, int& iz) {
+    ix = (int)fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.x, g.ox), g.inv_cell)), 0.0f), g.fx);
+    iy = (int)fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.y, g.oy), g.inv_cell)), 0.0f), g.fy);
+    iz = (int)fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.z, g.oz), g.inv_cell)), 0.0f), g.fz);
 }
 
 // 9 x-runs of the stencil of the cell (ix,iy,iz): run r -> [lo, hi) sorted slots, (0,0) outside the grid
@@ -38,9 +38,9 @@ __device__ __forceinline__ void stencil_run(const uint32_t* __restrict__ start, 
     const int cy = iy + (r % 3) - 1, cz = iz + (r / 3) - 1;
     lo = hi = 0u;
     if (cy >= 0 && cy < g.my && cz >= 0 && cz < g.mz) {
-        const int64_t row = (int64_t)g.mx * (cy + (int64_t)g.my * cz);
-        lo = start[row + max(ix - 1, 0)];
-        hi = start[row + min(ix + 1, g.mx - 1) + 1];
+        const uint32_t row = (uint32_t)g.mx * ((uint32_t)cy + (uint32_t)g.my * (uint32_t)cz);   // M < 2^31 (check_grid)
+        lo = start[row + (uint32_t)max(ix - 1, 0)];
+        hi = start[row + (uint32_t)min(ix + 1, g.mx - 1) + 1u];
     }
 }
 
@@ -65,9 +65,8 @@ __global__ void __launch_bounds__(128) k_density(const float4* __restrict__ posm
     if (s >= n) return;
     const float4 pi = posm_s[s];
     const float h_i = VARH ? h_s[s] : 0.f;
-    const uint32_t k = key_of(pi, g);
-    const int ix = (int)(k % (uint32_t)g.mx), iy = (int)((k / (uint32_t)g.mx) % (uint32_t)g.my),
-              iz = (int)(k / ((uint32_t)g.mx * (uint32_t)g.my));
+    int ix, iy, iz;
+    cell_of(pi, g, ix, iy, iz);
     float sum = 0.f;   // includes the self term m_i W(0): j = i passes the predicate with d2 = 0 (A5)
 #pragma unroll 1
     for (int r = 0; r < 9; ++r) {
@@ -190,9 +189,8 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
     const float4 vi = velr_s[s];
     const float2 ci = pc_s[s];
     const float h_i = VARH ? h_s[s] : 0.f;
-    const uint32_t k = key_of(pi, g);
-    const int ix = (int)(k % (uint32_t)g.mx), iy = (int)((k / (uint32_t)g.mx) % (uint32_t)g.my),
-              iz = (int)(k / ((uint32_t)g.mx * (uint32_t)g.my));
+    int ix, iy, iz;
+    cell_of(pi, g, ix, iy, iz);
     const float inv_h_glob = 1.0f / q.h;
     KSum ax, ay, az, de;
 #pragma unroll 1
@@ -300,9 +298,8 @@ __global__ void __launch_bounds__(128) k_cfl(const float4* __restrict__ posm_s, 
         const float4 pi = posm_s[s];
         const float4 vi = velr_s[s];
         const float ci = pc_s[s].y;
-        const uint32_t k = key_of(pi, g);
-        const int ix = (int)(k % (uint32_t)g.mx), iy = (int)((k / (uint32_t)g.mx) % (uint32_t)g.my),
-                  iz = (int)(k / ((uint32_t)g.mx * (uint32_t)g.my));
+        int ix, iy, iz;
+        cell_of(pi, g, ix, iy, iz);
         float d2min = rc2, cmax = ci, mumax = 0.f;   // A22: no neighbour -> s = 2h, c_i, 0
 #pragma unroll 1
         for (int r = 0; r < 9; ++r) {
