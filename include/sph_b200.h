@@ -211,6 +211,34 @@ int sph_neighbour_lists_h(const float* posm, const float* hsml, int64_t n_gas, f
                           uint64_t* nbr_offset, uint32_t* nbr_index, uint64_t nbr_capacity,
                           void* ws, size_t ws_bytes, void* stream);
 
+/* ---- the stages of a step, and target slices, for the N/k-per-GPU decomposition (L133-139) ----
+ * The paper gives each of k GPUs N/k particles and copies the other GPUs' particles over before GFC (L139).  Here every
+ * GPU keeps the whole (replicated) state and computes the O(N^2) stage — gravity, 99.9 % of the step — only for its own
+ * TARGET slice [i0, i1) against all N sources; the caller then exchanges the acc_grav slices (one all-gather of
+ * 16 B x N/k per GPU; paper_1807_08116_b200/binding.py ShardedSimulation does it with torch.distributed / NCCL) and all
+ * GPUs run the O(N) and SPH stages redundantly — they are deterministic, so the replicas stay bitwise identical.
+ *
+ * nbody_pp_gravity_slice: Eq. 4 for targets [i0, i1) only; rows outside the slice of acc_grav are not touched.
+ * sph_position_slice:     SP, DC (+ renewal of hsml if sigma > 0, as in sph_step_h), GFC for targets [i0, i1):
+ *                         everything that depends on r only (L123).  hsml may be NULL (global h).
+ * sph_predict:            HFC(predictor) + SU(predictor), Eqs. 10-14; needs rho and the COMPLETE acc_grav at r(t).
+ * sph_correct:            HFC(corrector) + SU(corrector), Eqs. 10-11, 15-16; needs rho and the COMPLETE acc_grav at
+ *                         r(t+dt).
+ * sph_step_h(first) == [first: sph_position_slice(sigma = 0, 0, N)] ; sph_predict ; sph_position_slice(sigma, 0, N) ;
+ *                      sph_correct  — the same code path, so one GPU with the full slice reproduces sph_step bit for bit.
+ * The workspace is the carried state between these calls exactly as for sph_step.                                    */
+int nbody_pp_gravity_slice(const float* posm, int64_t n_total, int64_t i0, int64_t i1, float G, float delta,
+                           float* acc_grav /*[n_total][4]*/, void* ws, size_t ws_bytes, void* stream);
+int sph_position_slice(const float* posm, float* hsml /*or NULL*/, float sigma, int64_t n_gas, int64_t n_halo,
+                       int64_t i0, int64_t i1, const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/,
+                       float* rho, float* acc_grav, void* ws, size_t ws_bytes, void* stream);
+int sph_predict(float* posm, float* vele, const float* hsml /*or NULL*/, int64_t n_gas, int64_t n_halo,
+                const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/, float dt,
+                const float* rho, float* acc_sph, const float* acc_grav, void* ws, size_t ws_bytes, void* stream);
+int sph_correct(float* vele, const float* hsml /*or NULL*/, int64_t n_gas, int64_t n_halo,
+                const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/, float dt,
+                const float* rho, float* acc_sph, const float* acc_grav, void* ws, size_t ws_bytes, void* stream);
+
 /* Stage timing: after sph_set_profiling(1) every stage the calling thread enqueues is bracketed
  * by CUDA events on the call's stream; sph_get_stage_ms() returns the milliseconds summed over all
  * calls since that switch-on (at most 4096 stage spans) for

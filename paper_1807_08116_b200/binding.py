@@ -25,6 +25,7 @@ EXPORTS = (
     "sph_density", "sph_forces", "nbody_pp_gravity", "sph_step", "sph_evaluate", "sph_step_host",
     "sph_host_ctx_create", "sph_host_ctx_step", "sph_host_ctx_destroy", "sph_neighbour_lists",
     "sph_set_profiling", "sph_get_stage_ms", "sph_launch_count", "sph_cfl_dt",
+    "nbody_pp_gravity_slice", "sph_position_slice", "sph_predict", "sph_correct",
     "sph_smoothing_lengths", "sph_density_h", "sph_forces_h", "sph_evaluate_h", "sph_step_h", "sph_neighbour_lists_h",
 )
 
@@ -101,6 +102,10 @@ def load():
     L.sph_neighbour_lists.argtypes = [vp, i64, f32, gp, vp, vp, vp, vp, vp, C.c_uint64, vp, sz, vp]
     L.sph_neighbour_lists_h.argtypes = [vp, vp, i64, f32, gp, vp, vp, vp, vp, vp, C.c_uint64, vp, sz, vp]
     L.sph_smoothing_lengths.argtypes = [vp, vp, i64, f32, f32, vp, vp]
+    L.nbody_pp_gravity_slice.argtypes = [vp, i64, i64, i64, f32, f32, vp, vp, sz, vp]
+    L.sph_position_slice.argtypes = [vp, vp, f32, i64, i64, i64, i64, pp, gp, vp, vp, vp, sz, vp]
+    L.sph_predict.argtypes = [vp, vp, vp, i64, i64, pp, gp, f32, vp, vp, vp, vp, sz, vp]
+    L.sph_correct.argtypes = [vp, vp, i64, i64, pp, gp, f32, vp, vp, vp, vp, sz, vp]
     L.sph_density_h.argtypes = [vp, vp, i64, pp, gp, vp, vp, vp, vp, sz, vp]
     L.sph_forces_h.argtypes = [vp, vp, vp, vp, i64, pp, gp, vp, vp, vp, vp, sz, vp]
     L.sph_evaluate_h.argtypes = [vp, vp, vp, i64, i64, pp, gp, vp, vp, vp, vp, sz, vp]
@@ -205,6 +210,35 @@ def sph_evaluate(posm, vele, n_gas, n_halo, params, grid, rho, acc_sph, acc_grav
     g = C.byref(grid) if grid is not None else None
     _chk("sph_evaluate", load().sph_evaluate(_ptr(posm), _ptr(vele), int(n_gas), int(n_halo), C.byref(params), g,
                                              _ptr(rho), _ptr(acc_sph), _ptr(acc_grav), p, nb, _stream()))
+
+
+# ------------------------------------------------------------------ NEXT-4: stages of a step, target slices
+def nbody_pp_gravity_slice(posm, n_total, i0, i1, G, delta, acc_grav, ws):
+    p, nb = _ws(ws)
+    _chk("nbody_pp_gravity_slice", load().nbody_pp_gravity_slice(_ptr(posm), int(n_total), int(i0), int(i1), float(G),
+                                                                 float(delta), _ptr(acc_grav), p, nb, _stream()))
+
+
+def sph_position_slice(posm, hsml, sigma, n_gas, n_halo, i0, i1, params, grid, rho, acc_grav, ws):
+    p, nb = _ws(ws)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_position_slice", load().sph_position_slice(_ptr(posm), _ptr(hsml), float(sigma), int(n_gas), int(n_halo),
+                                                         int(i0), int(i1), C.byref(params), g, _ptr(rho), _ptr(acc_grav),
+                                                         p, nb, _stream()))
+
+
+def sph_predict(posm, vele, hsml, n_gas, n_halo, params, grid, dt, rho, acc_sph, acc_grav, ws):
+    p, nb = _ws(ws)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_predict", load().sph_predict(_ptr(posm), _ptr(vele), _ptr(hsml), int(n_gas), int(n_halo), C.byref(params), g,
+                                           float(dt), _ptr(rho), _ptr(acc_sph), _ptr(acc_grav), p, nb, _stream()))
+
+
+def sph_correct(vele, hsml, n_gas, n_halo, params, grid, dt, rho, acc_sph, acc_grav, ws):
+    p, nb = _ws(ws)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_correct", load().sph_correct(_ptr(vele), _ptr(hsml), int(n_gas), int(n_halo), C.byref(params), g, float(dt),
+                                           _ptr(rho), _ptr(acc_sph), _ptr(acc_grav), p, nb, _stream()))
 
 
 # ------------------------------------------------------------------ NEXT-2: per-particle smoothing lengths

@@ -46,8 +46,9 @@ int check_params(const sph_params* p, bool need_h) {
 // SP + DC + GFC at the current positions: everything that depends on r only (L123, A11).
 // hsml != NULL (NEXT-2): per-particle smoothing lengths; with sigma > 0 they are renewed from the refined density
 // right after DC, h_i = min(sigma (m_i/rho_i)^(1/3), p->h) (L82, readings A25/A26), and re-gathered into cell order.
-int position_only(const float4* posm, float* hsml, float sigma, int64_t n_gas, int64_t n_total, const sph_params* p,
-                  const sph_grid* g, float* rho, float4* acc_grav, const Workspace& w, cudaStream_t st) {
+int position_only(const float4* posm, float* hsml, float sigma, int64_t n_gas, int64_t n_total, int64_t i0, int64_t i1,
+                  const sph_params* p, const sph_grid* g, float* rho, float4* acc_grav, const Workspace& w,
+                  cudaStream_t st) {
     if (n_gas > 0) {
         {
             Span sp(ST_SORT, st);
@@ -66,7 +67,7 @@ int position_only(const float4* posm, float* hsml, float sigma, int64_t n_gas, i
     }
     {
         Span sp(ST_GRAVITY, st);
-        SPHB_TRY(gravity(posm, n_total, p->G, p->delta, acc_grav, w.src_pk, w.grav_part, st));
+        SPHB_TRY(gravity(posm, n_total, i0, i1, p->G, p->delta, acc_grav, w.src_pk, w.grav_part, st));   // GFC, targets [i0, i1)
     }
     return SPH_OK;
 }
@@ -228,9 +229,9 @@ int sph_cfl_dt(const float* posm, const float* vele, const float* rho, const flo
                       dt_out, dt_particle, st);
 }
 
-int nbody_pp_gravity(const float* posm, int64_t n_total, float G, float delta, float* acc_grav, void* ws,
-                     size_t ws_bytes, void* stream) {
-    if (bad_count(n_total)) return SPH_ERR_ARG;
+int nbody_pp_gravity_slice(const float* posm, int64_t n_total, int64_t i0, int64_t i1, float G, float delta,
+                           float* acc_grav, void* ws, size_t ws_bytes, void* stream) {
+    if (bad_count(n_total) || i0 < 0 || i1 < i0 || i1 > n_total) return SPH_ERR_ARG;
     if (delta < 0.f) return SPH_ERR_UNSUPPORTED;
     if (n_total == 0) return SPH_OK;
     if (!posm || !acc_grav || !ws || !aligned16(posm) || !aligned16(acc_grav) || (reinterpret_cast<uintptr_t>(ws) & 255u))
@@ -239,8 +240,13 @@ int nbody_pp_gravity(const float* posm, int64_t n_total, float G, float delta, f
     if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     Span sp(ST_GRAVITY, st);
-    return gravity(reinterpret_cast<const float4*>(posm), n_total, G, delta, reinterpret_cast<float4*>(acc_grav), w.src_pk,
-                   w.grav_part, st);
+    return gravity(reinterpret_cast<const float4*>(posm), n_total, i0, i1, G, delta, reinterpret_cast<float4*>(acc_grav),
+                   w.src_pk, w.grav_part, st);
+}
+
+int nbody_pp_gravity(const float* posm, int64_t n_total, float G, float delta, float* acc_grav, void* ws,
+                     size_t ws_bytes, void* stream) {
+    return nbody_pp_gravity_slice(posm, n_total, 0, n_total, G, delta, acc_grav, ws, ws_bytes, stream);
 }
 
 int sph_evaluate_h(const float* posm, const float* vele, const float* hsml, int64_t n_gas, int64_t n_halo,
@@ -252,7 +258,7 @@ int sph_evaluate_h(const float* posm, const float* vele, const float* hsml, int6
     Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
     cudaStream_t st = (cudaStream_t)stream;
     float* hs = n_gas > 0 ? const_cast<float*>(hsml) : nullptr;   // sigma = 0: never written
-    SPHB_TRY(position_only(reinterpret_cast<const float4*>(posm), hs, 0.f, n_gas, n, p, g, rho,
+    SPHB_TRY(position_only(reinterpret_cast<const float4*>(posm), hs, 0.f, n_gas, n, 0, n, p, g, rho,
                            reinterpret_cast<float4*>(acc_grav), w, st));
     return hydro(reinterpret_cast<const float4*>(vele), rho, hs != nullptr, n_gas, p, g, reinterpret_cast<float4*>(acc_sph),
                  w, st);
@@ -264,6 +270,55 @@ int sph_evaluate(const float* posm, const float* vele, int64_t n_gas, int64_t n_
     return sph_evaluate_h(posm, vele, nullptr, n_gas, n_halo, p, g, rho, acc_sph, acc_grav, ws, ws_bytes, stream);
 }
 
+// ---- the three stages of a step (exposed so that a caller owning several GPUs can put its
+// exchange of acc_grav between them); sph_step_h is their composition on one GPU.
+int sph_position_slice(const float* posm, float* hsml, float sigma, int64_t n_gas, int64_t n_halo, int64_t i0,
+                       int64_t i1, const sph_params* p, const sph_grid* g, float* rho, float* acc_grav, void* ws,
+                       size_t ws_bytes, void* stream) {
+    if (bad_count(n_gas) || bad_count(n_halo) || bad_count(n_gas + n_halo)) return SPH_ERR_ARG;
+    const int64_t n = n_gas + n_halo;
+    if (i0 < 0 || i1 < i0 || i1 > n || sigma < 0.f) return SPH_ERR_ARG;
+    SPHB_TRY(check_params(p, n_gas > 0));
+    if (n == 0) return SPH_OK;
+    if (!posm || !acc_grav || !aligned16(posm) || !aligned16(acc_grav) || (n_gas > 0 && !rho)) return SPH_ERR_ARG;
+    if (n_gas > 0) SPHB_TRY(check_grid(g, p->h));
+    if (!ws || (reinterpret_cast<uintptr_t>(ws) & 255u)) return SPH_ERR_ARG;
+    Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    return position_only(reinterpret_cast<const float4*>(posm), n_gas > 0 ? hsml : nullptr, sigma, n_gas, n, i0, i1, p, g,
+                         rho, reinterpret_cast<float4*>(acc_grav), w, (cudaStream_t)stream);
+}
+
+int sph_predict(float* posm, float* vele, const float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p,
+                const sph_grid* g, float dt, const float* rho, float* acc_sph, const float* acc_grav, void* ws,
+                size_t ws_bytes, void* stream) {
+    SPHB_TRY(check_state_args(posm, vele, n_gas, n_halo, p, g, rho, acc_sph, acc_grav, ws, ws_bytes));
+    const int64_t n = n_gas + n_halo;
+    if (n == 0) return SPH_OK;
+    Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
+    cudaStream_t st = (cudaStream_t)stream;
+    float4* as4 = reinterpret_cast<float4*>(acc_sph);
+    SPHB_TRY(hydro(reinterpret_cast<const float4*>(vele), rho, hsml != nullptr && n_gas > 0, n_gas, p, g, as4, w, st));
+    Span sp(ST_UPDATE, st);
+    return update_predictor(reinterpret_cast<float4*>(posm), reinterpret_cast<float4*>(vele), w.vele0, as4,
+                            reinterpret_cast<const float4*>(acc_grav), n_gas, n, dt, st);   // Eqs. 12-14
+}
+
+int sph_correct(float* vele, const float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p, const sph_grid* g,
+                float dt, const float* rho, float* acc_sph, const float* acc_grav, void* ws, size_t ws_bytes,
+                void* stream) {
+    SPHB_TRY(check_state_args(vele, vele, n_gas, n_halo, p, g, rho, acc_sph, acc_grav, ws, ws_bytes));
+    const int64_t n = n_gas + n_halo;
+    if (n == 0) return SPH_OK;
+    Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
+    cudaStream_t st = (cudaStream_t)stream;
+    float4* as4 = reinterpret_cast<float4*>(acc_sph);
+    SPHB_TRY(hydro(reinterpret_cast<const float4*>(vele), rho, hsml != nullptr && n_gas > 0, n_gas, p, g, as4, w, st));
+    Span sp(ST_UPDATE, st);
+    return update_corrector(reinterpret_cast<float4*>(vele), w.vele0, as4, reinterpret_cast<const float4*>(acc_grav),
+                            n_gas, n, dt, st);                                               // Eqs. 15-16
+}
+
 int sph_step_h(float* posm, float* vele, float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p,
                const sph_grid* g, float sigma, float dt, int first, float* rho, float* acc_sph, float* acc_grav, void* ws,
                size_t ws_bytes, void* stream) {
@@ -271,27 +326,11 @@ int sph_step_h(float* posm, float* vele, float* hsml, int64_t n_gas, int64_t n_h
     if (sigma < 0.f) return SPH_ERR_ARG;
     const int64_t n = n_gas + n_halo;
     if (n == 0) return SPH_OK;
-    Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
-    cudaStream_t st = (cudaStream_t)stream;
-    float4* r4 = reinterpret_cast<float4*>(posm);
-    float4* v4 = reinterpret_cast<float4*>(vele);
-    float4* as4 = reinterpret_cast<float4*>(acc_sph);
-    float4* ag4 = reinterpret_cast<float4*>(acc_grav);
-    float* hs = n_gas > 0 ? hsml : nullptr;
-    const bool varh = hs != nullptr;
-    if (first) SPHB_TRY(position_only(r4, hs, 0.f, n_gas, n, p, g, rho, ag4, w, st));   // seed the carried state
-    SPHB_TRY(hydro(v4, rho, varh, n_gas, p, g, as4, w, st));                             // HFC(predictor)
-    {
-        Span sp(ST_UPDATE, st);
-        SPHB_TRY(update_predictor(r4, v4, w.vele0, as4, ag4, n_gas, n, dt, st));   // SU(predictor): Eqs. 12-14
-    }
-    SPHB_TRY(position_only(r4, hs, sigma, n_gas, n, p, g, rho, ag4, w, st));      // SP, DC (+ new h), GFC at r(t+dt)
-    SPHB_TRY(hydro(v4, rho, varh, n_gas, p, g, as4, w, st));                      // HFC(corrector)
-    {
-        Span sp(ST_UPDATE, st);
-        SPHB_TRY(update_corrector(v4, w.vele0, as4, ag4, n_gas, n, dt, st));       // SU(corrector): Eqs. 15-16
-    }
-    return SPH_OK;
+    if (first)   // seed the carried state: SP, DC, GFC at the current positions
+        SPHB_TRY(sph_position_slice(posm, hsml, 0.f, n_gas, n_halo, 0, n, p, g, rho, acc_grav, ws, ws_bytes, stream));
+    SPHB_TRY(sph_predict(posm, vele, hsml, n_gas, n_halo, p, g, dt, rho, acc_sph, acc_grav, ws, ws_bytes, stream));
+    SPHB_TRY(sph_position_slice(posm, hsml, sigma, n_gas, n_halo, 0, n, p, g, rho, acc_grav, ws, ws_bytes, stream));
+    return sph_correct(vele, hsml, n_gas, n_halo, p, g, dt, rho, acc_sph, acc_grav, ws, ws_bytes, stream);
 }
 
 int sph_step(float* posm, float* vele, int64_t n_gas, int64_t n_halo, const sph_params* p, const sph_grid* g, float dt,

@@ -100,7 +100,7 @@ constexpr int kStages = 2;
 // One CTA: THREADS*I targets (i-tile blockIdx.x) against the sources of chunk blockIdx.y.
 template <int I, int THREADS, int MINB, bool ZERO_SOFT, int UNROLL = 2>
 __global__ void __launch_bounds__(THREADS, MINB)
-    grav_pp_kernel(const float4* __restrict__ posm, const float4* __restrict__ pk, int n, int tiles_total,
+    grav_pp_kernel(const float4* __restrict__ posm, const float4* __restrict__ pk, int i0, int i1, int tiles_total,
                    int tiles_per_chunk, float eps2, float4* __restrict__ part) {
     extern __shared__ __align__(128) float4 tiles[];   // [kStages][2 * kTilePairs]
     __shared__ __align__(8) uint64_t full_bar[kStages];
@@ -126,13 +126,13 @@ __global__ void __launch_bounds__(THREADS, MINB)
     }
 
     // targets: coalesced float4 loads; out-of-range lanes compute on a dummy and do not store
-    const int ibase = blockIdx.x * (THREADS * I);
+    const int ibase = i0 + blockIdx.x * (THREADS * I);   // targets [i0, i1): the whole range, or one GPU's slice
     u64 xi[I], yi[I], zi[I];
     float ox[I], oy[I], oz[I];   // per-chunk (outer) accumulators
 #pragma unroll
     for (int k = 0; k < I; ++k) {
         int i = ibase + k * THREADS + tid;
-        float4 t = (i < n) ? posm[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+        float4 t = (i < i1) ? posm[i] : make_float4(0.f, 0.f, 0.f, 0.f);
         xi[k] = pk2(t.x, t.x);
         yi[k] = pk2(t.y, t.y);
         zi[k] = pk2(t.z, t.z);
@@ -197,18 +197,18 @@ __global__ void __launch_bounds__(THREADS, MINB)
         }
     }
 
-    float4* __restrict__ out = part + (size_t)blockIdx.y * n;
+    float4* __restrict__ out = part + (size_t)blockIdx.y * (i1 - i0);
 #pragma unroll
     for (int k = 0; k < I; ++k) {
         int i = ibase + k * THREADS + tid;
-        if (i < n) out[i] = make_float4(ox[k], oy[k], oz[k], 0.f);
+        if (i < i1) out[i - i0] = make_float4(ox[k], oy[k], oz[k], 0.f);
     }
 }
 
 // acc[i] = G * sum_s part[s][i]  in fixed order s = 0..S-1 (dx was r_j - r_i, so the sign of Eq. 4 is in).
-__global__ void __launch_bounds__(256) grav_reduce(const float4* __restrict__ part, int n, int S, float G,
+__global__ void __launch_bounds__(256) grav_reduce(const float4* __restrict__ part, int i0, int n, int S, float G,
                                                    float4* __restrict__ acc) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;   // slice-local target
     if (i >= n) return;
     float4 a = part[i];
     for (int s = 1; s < S; ++s) {
@@ -217,7 +217,7 @@ __global__ void __launch_bounds__(256) grav_reduce(const float4* __restrict__ pa
         a.y += b.y;
         a.z += b.z;
     }
-    acc[i] = make_float4(G * a.x, G * a.y, G * a.z, 0.f);
+    acc[i0 + i] = make_float4(G * a.x, G * a.y, G * a.z, 0.f);
 }
 
 int64_t grav_padded(int64_t n_total) { return cdiv(n_total > 0 ? n_total : 1, kGravTileSrc) * kGravTileSrc; }
@@ -228,7 +228,7 @@ int64_t grav_padded(int64_t n_total) { return cdiv(n_total > 0 ? n_total : 1, kG
 // distinct 64-bit registers and the register file delivers two per FFMA2 slot); small N: 128
 // threads x 1 target so that there are CTAs to spread.  S is chosen so the grid is >= ~16 waves of 2 CTAs/SM deep
 // (tail < ~3 %) without making a chunk shorter than 4 tiles.
-static void grav_shape(int64_t n, int& I, int& threads, int& S) {
+static void grav_shape(int64_t n, int64_t n_src, int& I, int& threads, int& S) {   // n targets, n_src sources
     if (n > 65536) {
         I = 8;
         threads = 128;
@@ -237,7 +237,7 @@ static void grav_shape(int64_t n, int& I, int& threads, int& S) {
         threads = 128;
     }
     int64_t itiles = cdiv(n, (int64_t)I * threads);
-    int64_t tiles = grav_padded(n) / kGravTileSrc;
+    int64_t tiles = grav_padded(n_src) / kGravTileSrc;
     int64_t want = (int64_t)num_sms() * 2 * 16;
     int64_t s = cdiv(want, itiles);
     int64_t smax = tiles >= 4 ? tiles / 4 : 1;
@@ -251,51 +251,59 @@ static void grav_shape(int64_t n, int& I, int& threads, int& S) {
 
 int grav_splits(int64_t n_total) {
     int I, th, S;
-    grav_shape(n_total > 0 ? n_total : 1, I, th, S);
+    grav_shape(n_total > 0 ? n_total : 1, n_total > 0 ? n_total : 1, I, th, S);
     return S;
 }
 
 template <int I, int THREADS, int MINB, int UNROLL>
-static int launch_grav(const float4* posm, const float4* pk, int n, int tiles, int tpc, int S, float eps2,
+static int launch_grav(const float4* posm, const float4* pk, int i0, int i1, int tiles, int tpc, int S, float eps2,
                        bool zero_soft, float4* part, cudaStream_t st) {
-    dim3 grid((unsigned)cdiv(n, (int64_t)I * THREADS), (unsigned)S);
+    dim3 grid((unsigned)cdiv(i1 - i0, (int64_t)I * THREADS), (unsigned)S);
     size_t smem = (size_t)kStages * kTileBytes;
     if (zero_soft) {
         auto kfn = grav_pp_kernel<I, THREADS, MINB, true, UNROLL>;
         SPHB_CUDA(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kfn<<<grid, THREADS, smem, st>>>(posm, pk, n, tiles, tpc, eps2, part);
+        kfn<<<grid, THREADS, smem, st>>>(posm, pk, i0, i1, tiles, tpc, eps2, part);
     } else {
         auto kfn = grav_pp_kernel<I, THREADS, MINB, false, UNROLL>;
         SPHB_CUDA(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kfn<<<grid, THREADS, smem, st>>>(posm, pk, n, tiles, tpc, eps2, part);
+        kfn<<<grid, THREADS, smem, st>>>(posm, pk, i0, i1, tiles, tpc, eps2, part);
     }
     SPHB_LAUNCHED();
     return SPH_OK;
 }
 
-int gravity(const float4* posm, int64_t n_total, float G, float delta, float4* acc_grav, float4* src_pk,
-            float4* grav_part, cudaStream_t st) {
-    if (n_total <= 0) return SPH_OK;
+// Targets [i0, i1) against all n_total sources (i0 = 0, i1 = n_total: the whole evaluation; a proper sub-range:
+// one GPU's share in the paper's N/k-per-GPU decomposition, L139).  Rows outside [i0, i1) of acc_grav are untouched.
+// The partial buffer holds grav_splits(n_total) * n_total float4; a slice may use more, shorter j-chunks (to keep
+// the grid many waves deep) as long as S * (i1 - i0) fits in it.
+int gravity(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, float G, float delta, float4* acc_grav,
+            float4* src_pk, float4* grav_part, cudaStream_t st) {
+    if (n_total <= 0 || i1 <= i0) return SPH_OK;
+    const int nt = (int)(i1 - i0);
     if (G == 0.0f) {   // no self-gravity (BASELINE config 4, "SPH-only"): Eq. 4 is identically 0
-        SPHB_CUDA(cudaMemsetAsync(acc_grav, 0, (size_t)n_total * sizeof(float4), st));
+        SPHB_CUDA(cudaMemsetAsync(acc_grav + i0, 0, (size_t)nt * sizeof(float4), st));
         return SPH_OK;
     }
     const int n = (int)n_total;
     const int n_pad = (int)grav_padded(n_total);
     int I, threads, S;
-    grav_shape(n_total, I, threads, S);
+    grav_shape(nt, n_total, I, threads, S);
+    const int64_t cap = (int64_t)grav_splits(n_total) * n_total / nt;   // chunks the partial buffer can hold
+    if (S > cap) S = (int)cap;
     const int tiles = n_pad / kGravTileSrc;
     const int tpc = (int)cdiv(tiles, S);
+    S = (int)cdiv(tiles, tpc);
 
     grav_pack_sources<<<(unsigned)cdiv(n_pad / 2, 256), 256, 0, st>>>(posm, n, n_pad, src_pk);
     SPHB_LAUNCHED();
     const float eps2 = delta * delta;
     const bool zero_soft = !(eps2 > 0.f);
     if (I == 8)
-        SPHB_TRY((launch_grav<8, 128, 2, 1>(posm, src_pk, n, tiles, tpc, S, eps2, zero_soft, grav_part, st)));
+        SPHB_TRY((launch_grav<8, 128, 2, 1>(posm, src_pk, (int)i0, (int)i1, tiles, tpc, S, eps2, zero_soft, grav_part, st)));
     else
-        SPHB_TRY((launch_grav<1, 128, 4, 2>(posm, src_pk, n, tiles, tpc, S, eps2, zero_soft, grav_part, st)));
-    grav_reduce<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(grav_part, n, S, G, acc_grav);
+        SPHB_TRY((launch_grav<1, 128, 4, 2>(posm, src_pk, (int)i0, (int)i1, tiles, tpc, S, eps2, zero_soft, grav_part, st)));
+    grav_reduce<<<(unsigned)cdiv(nt, 256), 256, 0, st>>>(grav_part, (int)i0, nt, S, G, acc_grav);
     SPHB_LAUNCHED();
     return SPH_OK;
 }

@@ -57,3 +57,50 @@ def test_config_is_shared_by_both_arms():
     c2 = bench.workload_config(a, w, [3, 4, 5], 60, 2)
     assert c1["workload"] == c2["workload"] and "configs[0]" in c1["workload"]
     assert c1["parallelism"] == "single GPU" and c2["parallelism"] == "replicas only"
+
+
+# ---------------------------------------------------------------- NEXT-4: slices and the exchange (host logic)
+def test_slice_bounds_cover_and_align():
+    sys.path.insert(0, ROOT)
+    from paper_1807_08116_b200.sharded import slice_bounds, SLICE_ALIGN
+    for n in (0, 1, 1023, 1024, 1025, 8192, 2 ** 20, 2 ** 20 + 7, 4194304):
+        for world in (1, 2, 3, 4, 8):
+            covered, chunk0 = 0, None
+            for r in range(world):
+                i0, i1, chunk = slice_bounds(n, r, world)
+                chunk0 = chunk0 or chunk
+                assert chunk == chunk0 and chunk % SLICE_ALIGN == 0 and world * chunk >= n
+                assert i0 == min(r * chunk, n) and i0 <= i1 <= n and i1 - i0 <= chunk
+                assert i0 == covered                     # contiguous, in rank order, no gaps, no overlap
+                covered = i1
+            assert covered == n
+    with pytest.raises(ValueError):
+        slice_bounds(10, 2, 2)
+
+
+def _gather_worker(rank, world, port, out):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    from paper_1807_08116_b200.sharded import slice_bounds, allgather_rows
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        n = 2500                                          # ragged: rank 1's slice is short
+        i0, i1, chunk = slice_bounds(n, rank, world)
+        full = torch.full((world * chunk, 4), -1.0)       # stale values everywhere
+        rows = torch.arange(i0, i1, dtype=torch.float32)
+        full[i0:i1] = torch.stack([rows, 2 * rows, 3 * rows, torch.zeros_like(rows)], 1)   # "my slice of acc_grav"
+        allgather_rows(full, rank, world, chunk)
+        out[rank] = full[:n].clone().numpy()
+    finally:
+        dist.destroy_process_group()
+
+
+def test_allgather_rows_gloo_world2():
+    import numpy as np
+    world, port = 2, _free_port()
+    mgr = mp.Manager()
+    out = mgr.dict()
+    mp.spawn(_gather_worker, args=(world, port, out), nprocs=world, join=True)
+    rows = np.arange(2500, dtype=np.float32)
+    expect = np.stack([rows, 2 * rows, 3 * rows, np.zeros_like(rows)], 1)
+    assert np.array_equal(out[0], expect) and np.array_equal(out[1], expect)     # every rank holds every row

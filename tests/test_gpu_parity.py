@@ -520,3 +520,100 @@ def test_varh_smoothing_lengths_and_step(cuda_lib):
     check_values(v[:ng, 3], st.vele[:ng, 3], "e after 2 varh steps", max_tol=2e-5, med_tol=1e-6)
     check_density(sim.rho.cpu().numpy()[:ng], st.rho, "rho after 2 varh steps")
     assert np.abs(hs_dev.cpu().numpy() - hs).max() <= 1e-5 * hs.max()
+
+
+def test_step_bitwise_reproducible(cuda_lib):
+    """Run twice, compare bits: the histogram atomics hand out in-cell slots in a run-dependent
+    order, the stable fix-up removes it, every floating-point sum has a fixed order (gravity partials are
+    reduced in chunk order) — so two runs of the same steps must agree bit for bit, with and without
+    per-particle smoothing lengths."""
+    b = cuda_lib
+    w = wl.make_workload(1, scale=1 / 8)
+    for sigma in (None, 1.0):
+        outs = []
+        for _ in range(2):
+            sim = b.Simulation(w, sigma=sigma)
+            for _ in range(3):
+                sim.step()
+            torch.cuda.synchronize()
+            outs.append([t.clone() for t in (sim.posm, sim.vele, sim.rho, sim.acc_sph, sim.acc_grav)])
+        for x, y in zip(*outs):
+            assert torch.equal(x, y)
+
+
+# ---------------------------------------------------------------- NEXT-4: target slices and the staged step
+def test_gravity_slices_equal_full(cuda_lib):
+    b = cuda_lib
+    w = wl.make_workload(1, scale=0.75)                  # N = 98304 > 65536: the 8-targets-per-thread shape
+    n = w.n_total
+    d = _t(w.posm)
+    ws = b.alloc_workspace(0, n)
+    full = torch.zeros((n, 4), device="cuda")
+    b.nbody_pp_gravity(d, n, w.G, w.delta, full, ws)
+    whole = torch.full((n, 4), 7.0, device="cuda")
+    b.nbody_pp_gravity_slice(d, n, 0, n, w.G, w.delta, whole, ws)
+    assert torch.equal(whole, full)                      # the full slice IS the full call
+    from paper_1807_08116_b200.sharded import slice_bounds
+    for world in (2, 3, 8):
+        acc = torch.full((n, 4), 7.0, device="cuda")
+        for r in range(world):
+            i0, i1, _ = slice_bounds(n, r, world)
+            before = acc.clone()
+            b.nbody_pp_gravity_slice(d, n, i0, i1, w.G, w.delta, acc, ws)
+            assert torch.equal(acc[:i0], before[:i0]) and torch.equal(acc[i1:], before[i1:])   # rows outside untouched
+        # a slice may use more, shorter j-chunks: same sums in another (fixed) order
+        err = (acc[:, :3] - full[:, :3]).norm(dim=1) / full[:, :3].norm(dim=1).clamp_min(1e-3)
+        assert err.max().item() < 2e-6
+    tg = np.arange(0, n, 97)
+    check_values(acc.cpu().numpy()[tg, :3], oracle.gravity(w.posm, w.G, w.delta, targets=tg), "a_grav 8 slices")
+    # ragged and degenerate slices
+    b.nbody_pp_gravity_slice(d, n, 5, 5, w.G, w.delta, acc, ws)
+    one = torch.zeros((n, 4), device="cuda")
+    b.nbody_pp_gravity_slice(d, n, 12345, 12346, w.G, w.delta, one, ws)
+    assert torch.count_nonzero(one[:12345]).item() == 0 and torch.count_nonzero(one[12346:]).item() == 0
+    assert (one[12345, :3] - full[12345, :3]).norm().item() < 2e-6 * full[12345, :3].norm().item()
+    with pytest.raises(b.SphError):
+        b.nbody_pp_gravity_slice(d, n, 10, n + 1, w.G, w.delta, acc, ws)
+
+
+def test_staged_step_two_slices_sequential(cuda_lib):
+    """Two replicas of the state, each doing the gravity of its own slice, exchanging acc_grav by a plain copy
+    between the stages (what the all-gather does), run one after the other on this one GPU: both replicas must
+    stay bitwise identical and match the single-GPU step."""
+    b = cuda_lib
+    from paper_1807_08116_b200.sharded import ShardedSimulation, slice_bounds
+    w = wl.make_workload(1, scale=0.75)
+    n, ng, nh = w.n_total, w.n_gas, w.n_halo
+    ref = b.Simulation(w)
+    ref.step()
+    ref.step()
+    # world = 1 through the class (same calls, no collective): bit for bit the plain step
+    one = ShardedSimulation(w, 0, 1)
+    one.step()
+    one.step()
+    for x, y in ((one.posm, ref.posm), (one.vele, ref.vele), (one.rho, ref.rho), (one.acc_grav[:n], ref.acc_grav)):
+        assert torch.equal(x, y)
+    world = 2
+    reps = [ShardedSimulation(w, r, world) for r in range(world)]
+
+    def position(sigma):
+        for s in reps:
+            b.sph_position_slice(s.posm, s.hsml, sigma, ng, nh, s.i0, s.i1, s.params, s.grid, s.rho, s.acc_grav, s.ws)
+        for s in reps:                                    # the exchange: every replica receives every slice
+            for o in reps:
+                if o is not s:
+                    s.acc_grav[o.i0:o.i1] = o.acc_grav[o.i0:o.i1]
+
+    position(0.0)
+    for _ in range(2):
+        for s in reps:
+            b.sph_predict(s.posm, s.vele, s.hsml, ng, nh, s.params, s.grid, w.dt, s.rho, s.acc_sph, s.acc_grav, s.ws)
+        position(0.0)
+        for s in reps:
+            b.sph_correct(s.vele, s.hsml, ng, nh, s.params, s.grid, w.dt, s.rho, s.acc_sph, s.acc_grav, s.ws)
+    a, c = reps
+    for x, y in ((a.posm, c.posm), (a.vele, c.vele), (a.rho, c.rho), (a.acc_sph, c.acc_sph), (a.acc_grav, c.acc_grav)):
+        assert torch.equal(x, y)
+    assert (a.posm - ref.posm).abs().max().item() < 1e-6
+    check_values(a.vele.cpu().numpy()[:, :3], ref.vele.cpu().numpy()[:, :3].astype(np.float64), "v sliced vs single",
+                 max_tol=2e-6, med_tol=2e-7)
