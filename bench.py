@@ -4,9 +4,9 @@
     python bench.py --gpus N --steps K --warmup W [--config C] [--impl reference]
 
 One "step" = one sph_step (all §8(a) rows: HFC x2, SU x2, grid sort, density, PP gravity).
-Prints ONE JSON line (see DESIGN.md §7 for every key).  The path does not shard (north star:
-multi-GPU out of scope), so --gpus N runs N independent replicas, one per rank, and reports the
-max-over-ranks step time ("replicas only").
+Prints ONE JSON line (see DESIGN.md §7 for every key).  --gpus N (under torchrun, one rank per GPU) splits
+the O(N^2) gravity stage by target slices (the paper's N/k-per-GPU decomposition, L139) with one NCCL
+all-gather of the acceleration slices per force evaluation; total work is fixed ("scaling": "strong").
 """
 from __future__ import annotations
 
@@ -39,7 +39,8 @@ def workload_config(args, w, grid_dims=None, cells=None, world=1):
     """The `config` object of the JSON line: identical for both arms (ours / reference)."""
     src = f"BASELINE.json configs[{args.config}]" if args.config <= 4 else "SURVEY.md 8(f) NEXT-3 (collisionless, not a BASELINE config)"
     return {"workload": f"{src} ({w.name}): N={w.n_total}, N_g={w.n_gas}, h={w.h:g}, delta={w.delta:g}, dt={w.dt:g}",
-            "grid_dims": grid_dims, "cells": cells, "parallelism": "replicas only" if world > 1 else "single GPU",
+            "grid_dims": grid_dims, "cells": cells, "parallelism": (f"gravity targets sliced N/{world} per GPU + 1 all-gather of acc_grav per evaluation; O(N) and SPH stages replicated"
+                            if world > 1 else "single GPU"),
             "l2": "no flush: one step streams >300 MB (cell arrays, gravity partials, particle arrays) > 126 MB L2"}
 
 
@@ -192,7 +193,7 @@ def run_reference(args, w):
         grid_dims, cells = [int(d) for d in og.dims], int(og.M)
     line = {
         "impl": "reference", "metric": "step_ms", "value": v, "unit": "ms", "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "warmup": args.warmup, "ms_per_step": v, "higher_is_better": False, "scaling": "strong", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": workload_config(args, w, grid_dims, cells, 1),
         "cpu_baseline": {"value": v, "unit": "ms", "cores": cores, "kind": "oracle", "sample": desc, "extrapolated": True},
@@ -212,17 +213,25 @@ def run_ours(args, w):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device — the product path has no CPU fallback")
     torch.cuda.set_device(local_rank)
-    if world > 1:
+    # under torchrun (any world size, also 1) the sharded path runs, collective included; plain `python bench.py` is
+    # the single-GPU sph_step path
+    use_dist = "RANK" in os.environ and "WORLD_SIZE" in os.environ
+    if use_dist:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     b.load()
     peaks, peak_src = _peaks()
 
     n, ng = w.n_total, w.n_gas
-    sim = b.Simulation(w, sigma=args.sigma)
+    if use_dist:
+        from paper_1807_08116_b200.sharded import ShardedSimulation
+        sim = ShardedSimulation(w, rank, world, sigma=args.sigma)
+    else:
+        sim = b.Simulation(w, sigma=args.sigma)
+    n_slice = (sim.i1 - sim.i0) if use_dist else n           # this rank's gravity targets
     M = sim.grid.M if ng else 0
 
     def barrier():
-        if world > 1:
+        if use_dist:
             dist.barrier()
         torch.cuda.synchronize()
 
@@ -253,23 +262,44 @@ def run_ours(args, w):
         hv = torch.from_numpy(w.vele.copy()).pin_memory()
         hrho = torch.zeros(max(ng, 1), dtype=torch.float32).pin_memory()
         prm = b.sph_params.from_workload(w)
-        ctx = b.HostContext(ng, w.n_halo)
-        ctx.step(hp, hv, prm, w.dt, 1, first=True, rho=hrho)          # warm-up + seeding
-        ctx.step(hp, hv, prm, w.dt, 1, first=False, rho=hrho)
         k_e2e = max(1, min(args.steps, args.e2e_steps))
+        if not use_dist:
+            ctx = b.HostContext(ng, w.n_halo)
+            ctx.step(hp, hv, prm, w.dt, 1, first=True, rho=hrho)          # warm-up + seeding
+            ctx.step(hp, hv, prm, w.dt, 1, first=False, rho=hrho)
+
+            def e2e_step():                                               # H2D posm+vele, step, D2H posm+vele+rho, sync
+                ctx.step(hp, hv, prm, w.dt, 1, first=False, rho=hrho)
+            how = "host wall clock around sph_host_ctx_step (it synchronises)"
+        else:
+            sim_e = ShardedSimulation(w, rank, world, sigma=args.sigma)
+            sim_e.step()
+            hp.copy_(sim_e.posm)
+            hv.copy_(sim_e.vele)
+
+            def e2e_step():                                               # the same copies around the sharded step
+                sim_e.posm.copy_(hp, non_blocking=True)
+                sim_e.vele.copy_(hv, non_blocking=True)
+                sim_e.step()
+                hp.copy_(sim_e.posm, non_blocking=True)
+                hv.copy_(sim_e.vele, non_blocking=True)
+                if ng:
+                    hrho.copy_(sim_e.rho[:ng], non_blocking=True)
+                torch.cuda.synchronize()
+            e2e_step()
+            how = "host wall clock around pinned H2D + ShardedSimulation.step + D2H + synchronise"
         barrier()
         t0 = time.perf_counter()
         for _ in range(k_e2e):
-            ctx.step(hp, hv, prm, w.dt, 1, first=False, rho=hrho)     # H2D posm+vele, step, D2H posm+vele+rho, sync
+            e2e_step()
         t_e2e = (time.perf_counter() - t0) * 1e3 / k_e2e
-        ctx.close()
+        if not use_dist:
+            ctx.close()
         e2e = {"value": reduce_max_ms(t_e2e, world), "unit": "ms", "h2d_bytes_per_step": 2 * n * 16,
-               "d2h_bytes_per_step": 2 * n * 16 + ng * 4, "steps": k_e2e,
-               "timing": "host wall clock around sph_host_ctx_step (it synchronises), max over ranks"}
+               "d2h_bytes_per_step": 2 * n * 16 + ng * 4, "steps": k_e2e, "timing": how + ", max over ranks"}
 
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        dist.destroy_process_group()
         return
 
     # ---- derived figures -----------------------------------------------------------------------
@@ -280,7 +310,7 @@ def run_ours(args, w):
     alu_peak_tflops = 2 * 128 * SM_COUNT_B200 * sm_max * 1e6 / 1e12
     roofline = None
     if w.G != 0.0 and grav_ms > 0:
-        achieved = FLOPS_PER_INTERACTION * float(n) * float(n) / (grav_ms * 1e-3) / 1e12
+        achieved = FLOPS_PER_INTERACTION * float(n_slice) * float(n) / (grav_ms * 1e-3) / 1e12   # per GPU (rank 0's slice)
         tr = ncu_traffic("grav_pp_kernel")
         traffic = tr["bytes"] if tr and tr["n_total"] == n else None   # the capture is of this workload only
         roofline = {"kernel": "grav_pp_kernel", "bound": "alu", "achieved": achieved, "peak": alu_peak_tflops,
@@ -295,7 +325,7 @@ def run_ours(args, w):
     upd_bytes = ng * (112 + 80) + (n - ng) * (96 + 64)
     stages = {
         "gravity_ms": grav_ms, "sort_ms": sort_ms, "density_ms": dens_ms, "forces_ms_2passes": forc_ms, "update_ms": upd_ms,
-        "pp_ginteractions_per_s": (float(n) * n / (grav_ms * 1e-3) / 1e9) if (grav_ms > 0 and w.G != 0.0) else None,
+        "pp_ginteractions_per_s": (float(n) * n / (grav_ms * 1e-3) / 1e9) if (grav_ms > 0 and w.G != 0.0) else None,   # whole job: all slices run concurrently
         "sph_mparticles_per_s": (ng / ((sort_ms + dens_ms + forc_ms) * 1e-3) / 1e6) if ng else None,
         "sort_mkeys_per_s": (ng / (sort_ms * 1e-3) / 1e6) if ng and sort_ms > 0 else None,
         "sort_hbm_gbs": (sort_bytes / (sort_ms * 1e-3) / 1e9) if ng and sort_ms > 0 else None,
@@ -314,7 +344,7 @@ def run_ours(args, w):
 
     line = {
         "metric": "step_ms", "value": ms_step, "unit": "ms", "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
-        "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "ms_per_step": ms_step, "higher_is_better": False, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": dict(workload_config(args, w, list(sim.grid.dims) if ng else None, M, world),
                        **({"smoothing_lengths": f"per particle, sigma={args.sigma:g}, cap h"} if args.sigma is not None else {})),
@@ -323,7 +353,7 @@ def run_ours(args, w):
         "context": "paper Table 1 (K40, N=2^20, units inferred as s): t_SPH=7.87, t_GFC=53.62 — other hardware, not a target",
     }
     print(json.dumps(line), flush=True)
-    if world > 1:
+    if use_dist:
         dist.destroy_process_group()
 
 

@@ -35,8 +35,8 @@ def slice_bounds(n: int, rank: int, world: int, align: int = SLICE_ALIGN):
 def allgather_rows(full: torch.Tensor, rank: int, world: int, chunk: int, group=None) -> None:
     """`full` has world * chunk rows; rank r has written rows [r * chunk, (r+1) * chunk).  After the call every
     rank holds all rows.  Works for any backend (NCCL on the GPUs, gloo in the CPU tests)."""
-    if world == 1:
-        return
+    if world == 1 and not dist.is_initialized():
+        return                                   # no process group: plain single-GPU use of the staged calls
     assert full.shape[0] == world * chunk and full.is_contiguous()
     send = full[rank * chunk:(rank + 1) * chunk].clone()
     dist.all_gather_into_tensor(full, send, group=group)

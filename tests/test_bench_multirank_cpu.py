@@ -1,6 +1,6 @@
-"""The N > 1 path of bench.py on CPU: world_size-2 gloo.  The path does not shard (DESIGN.md §10,
-"replicas only"), so what N > 1 adds is the rendezvous, the barrier and the max-over-ranks of the
-per-rank step time; those are exercised here without a GPU."""
+"""The N > 1 path on CPU: world_size-2 gloo.  What N > 1 adds to the single-GPU path is the
+rendezvous, the barrier, the max-over-ranks of the per-rank step time, the target-slice bookkeeping and the
+all-gather of the acceleration slices; those are exercised here without a GPU."""
 import os
 import socket
 import sys
@@ -56,7 +56,7 @@ def test_config_is_shared_by_both_arms():
     c1 = bench.workload_config(a, w, [3, 4, 5], 60, 1)
     c2 = bench.workload_config(a, w, [3, 4, 5], 60, 2)
     assert c1["workload"] == c2["workload"] and "configs[0]" in c1["workload"]
-    assert c1["parallelism"] == "single GPU" and c2["parallelism"] == "replicas only"
+    assert c1["parallelism"] == "single GPU" and "N/2 per GPU" in c2["parallelism"]
 
 
 # ---------------------------------------------------------------- NEXT-4: slices and the exchange (host logic)
