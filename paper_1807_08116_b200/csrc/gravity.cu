@@ -100,7 +100,7 @@ constexpr int kStages = 2;
 // One CTA: THREADS*I targets (i-tile blockIdx.x) against the sources of chunk blockIdx.y.
 template <int I, int THREADS, int MINB, bool ZERO_SOFT, int UNROLL = 2>
 __global__ void __launch_bounds__(THREADS, MINB)
-    grav_pp_kernel(const float4* __restrict__ posm, const float4* __restrict__ pk, int i0, int i1, int tiles_total,
+    grav_pp_kernel(const float4* __restrict__ posm /*targets*/, const float4* __restrict__ pk, int n, int tiles_total,
                    int tiles_per_chunk, float eps2, float4* __restrict__ part) {
     extern __shared__ __align__(128) float4 tiles[];   // [kStages][2 * kTilePairs]
     __shared__ __align__(8) uint64_t full_bar[kStages];
@@ -126,13 +126,13 @@ __global__ void __launch_bounds__(THREADS, MINB)
     }
 
     // targets: coalesced float4 loads; out-of-range lanes compute on a dummy and do not store
-    const int ibase = i0 + blockIdx.x * (THREADS * I);   // targets [i0, i1): the whole range, or one GPU's slice
+    const int ibase = blockIdx.x * (THREADS * I);   // `posm` points at the first target (the whole range or one GPU's slice)
     u64 xi[I], yi[I], zi[I];
     float ox[I], oy[I], oz[I];   // per-chunk (outer) accumulators
 #pragma unroll
     for (int k = 0; k < I; ++k) {
         int i = ibase + k * THREADS + tid;
-        float4 t = (i < i1) ? posm[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+        float4 t = (i < n) ? posm[i] : make_float4(0.f, 0.f, 0.f, 0.f);
         xi[k] = pk2(t.x, t.x);
         yi[k] = pk2(t.y, t.y);
         zi[k] = pk2(t.z, t.z);
@@ -197,11 +197,11 @@ __global__ void __launch_bounds__(THREADS, MINB)
         }
     }
 
-    float4* __restrict__ out = part + (size_t)blockIdx.y * (i1 - i0);
+    float4* __restrict__ out = part + (size_t)blockIdx.y * n;
 #pragma unroll
     for (int k = 0; k < I; ++k) {
         int i = ibase + k * THREADS + tid;
-        if (i < i1) out[i - i0] = make_float4(ox[k], oy[k], oz[k], 0.f);
+        if (i < n) out[i] = make_float4(ox[k], oy[k], oz[k], 0.f);
     }
 }
 
@@ -256,18 +256,18 @@ int grav_splits(int64_t n_total) {
 }
 
 template <int I, int THREADS, int MINB, int UNROLL>
-static int launch_grav(const float4* posm, const float4* pk, int i0, int i1, int tiles, int tpc, int S, float eps2,
+static int launch_grav(const float4* targets, const float4* pk, int n, int tiles, int tpc, int S, float eps2,
                        bool zero_soft, float4* part, cudaStream_t st) {
-    dim3 grid((unsigned)cdiv(i1 - i0, (int64_t)I * THREADS), (unsigned)S);
+    dim3 grid((unsigned)cdiv(n, (int64_t)I * THREADS), (unsigned)S);
     size_t smem = (size_t)kStages * kTileBytes;
     if (zero_soft) {
         auto kfn = grav_pp_kernel<I, THREADS, MINB, true, UNROLL>;
         SPHB_CUDA(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kfn<<<grid, THREADS, smem, st>>>(posm, pk, i0, i1, tiles, tpc, eps2, part);
+        kfn<<<grid, THREADS, smem, st>>>(targets, pk, n, tiles, tpc, eps2, part);
     } else {
         auto kfn = grav_pp_kernel<I, THREADS, MINB, false, UNROLL>;
         SPHB_CUDA(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kfn<<<grid, THREADS, smem, st>>>(posm, pk, i0, i1, tiles, tpc, eps2, part);
+        kfn<<<grid, THREADS, smem, st>>>(targets, pk, n, tiles, tpc, eps2, part);
     }
     SPHB_LAUNCHED();
     return SPH_OK;
@@ -300,9 +300,9 @@ int gravity(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, float G
     const float eps2 = delta * delta;
     const bool zero_soft = !(eps2 > 0.f);
     if (I == 8)
-        SPHB_TRY((launch_grav<8, 128, 2, 1>(posm, src_pk, (int)i0, (int)i1, tiles, tpc, S, eps2, zero_soft, grav_part, st)));
+        SPHB_TRY((launch_grav<8, 128, 2, 1>(posm + i0, src_pk, nt, tiles, tpc, S, eps2, zero_soft, grav_part, st)));
     else
-        SPHB_TRY((launch_grav<1, 128, 4, 2>(posm, src_pk, (int)i0, (int)i1, tiles, tpc, S, eps2, zero_soft, grav_part, st)));
+        SPHB_TRY((launch_grav<1, 128, 4, 2>(posm + i0, src_pk, nt, tiles, tpc, S, eps2, zero_soft, grav_part, st)));
     grav_reduce<<<(unsigned)cdiv(nt, 256), 256, 0, st>>>(grav_part, (int)i0, nt, S, G, acc_grav);
     SPHB_LAUNCHED();
     return SPH_OK;
