@@ -617,3 +617,39 @@ def test_staged_step_two_slices_sequential(cuda_lib):
     assert (a.posm - ref.posm).abs().max().item() < 1e-6
     check_values(a.vele.cpu().numpy()[:, :3], ref.vele.cpu().numpy()[:, :3].astype(np.float64), "v sliced vs single",
                  max_tol=2e-6, med_tol=2e-7)
+
+
+@pytest.mark.parametrize("masses", ["equal", "one_differs_last", "one_differs_first", "random", "equal_zero"])
+def test_gravity_mass_variants_large_shape(cuda_lib, masses):
+    """The uniform-mass variant (m_j left out of the loop) and the general one, chosen on the device by the flag the
+    pack pass sets; N > 65536 so the 8-targets-per-thread kernel runs, ragged tail so the padded sources matter."""
+    b = cuda_lib
+    w = wl.make_workload(1, scale=70001 / 2 ** 17)
+    n = w.n_total
+    posm = w.posm.copy()
+    rng = np.random.Generator(np.random.Philox(key=[21, 3]))
+    if masses == "one_differs_last":
+        posm[n - 1, 3] *= 3.0
+    elif masses == "one_differs_first":
+        posm[0, 3] *= 0.25                       # m_0 is the reference mass of the flag
+    elif masses == "random":
+        posm[:, 3] = ((0.2 + rng.random(n)) / n).astype(np.float32)
+    elif masses == "equal_zero":
+        posm[:, 3] = 0.0
+    posm[7, :3] = (1.0e3, -2.0e3, 5.0e2)         # a far-away target: the pads at 1e18 must still add exactly 0
+    d = _t(posm)
+    acc = torch.full((n, 4), 7.0, device="cuda")
+    ws = b.alloc_workspace(0, n)
+    b.nbody_pp_gravity(d, n, w.G, w.delta, acc, ws)
+    got = acc.cpu().numpy()
+    assert np.all(np.isfinite(got)) and np.all(got[:, 3] == 0)
+    if masses == "equal_zero":
+        assert np.all(got == 0)
+        return
+    tg = np.concatenate([np.arange(0, n, 61), [0, 7, n - 1]])
+    check_values(got[tg, :3], oracle.gravity(posm, w.G, w.delta, targets=tg), f"a_grav masses={masses}")
+    # delta = 0 goes through the same two variants
+    b.nbody_pp_gravity(d, n, w.G, 0.0, acc, ws)
+    got0 = acc.cpu().numpy()
+    check_values(got0[tg, :3], oracle.gravity(posm, w.G, 0.0, targets=tg), f"a_grav delta=0 masses={masses}",
+                 max_tol=5e-4, med_tol=2e-5)
