@@ -67,7 +67,7 @@ int position_only(const float4* posm, float* hsml, float sigma, int64_t n_gas, i
     }
     {
         Span sp(ST_GRAVITY, st);
-        SPHB_TRY(gravity(posm, n_total, i0, i1, p->G, p->delta, acc_grav, w.src_pk, w.grav_part, w.grav_flag, st));   // GFC
+        SPHB_TRY(gravity(posm, n_total, i0, i1, p->G, p->delta, acc_grav, w.src_pk, w.grav_part, w.grav_acc64, w.grav_flag, st));   // GFC
     }
     return SPH_OK;
 }
@@ -241,7 +241,7 @@ int nbody_pp_gravity_slice(const float* posm, int64_t n_total, int64_t i0, int64
     cudaStream_t st = (cudaStream_t)stream;
     Span sp(ST_GRAVITY, st);
     return gravity(reinterpret_cast<const float4*>(posm), n_total, i0, i1, G, delta, reinterpret_cast<float4*>(acc_grav),
-                   w.src_pk, w.grav_part, w.grav_flag, st);
+                   w.src_pk, w.grav_part, w.grav_acc64, w.grav_flag, st);
 }
 
 int nbody_pp_gravity(const float* posm, int64_t n_total, float G, float delta, float* acc_grav, void* ws,

@@ -69,7 +69,8 @@ struct Workspace {
     // gravity
     float4* src_pk;        // [n_pad] packed source pairs
     float4* grav_part;     // [S][n_total] partial accelerations
-    unsigned int* grav_flag;   // [1] set by the pack pass if the masses are not all equal
+    long long* grav_acc64;     // [n_pad][3] fixed-point accumulators of the pair-symmetric gravity kernel
+    unsigned int* grav_flag;   // 256-byte device control block of one gravity evaluation (GravCtl, grav_dev.cuh)
     // integrator
     float4* vele0;         // [n_total] v(t), e(t) saved by the predictor
     // bbox scratch
@@ -102,7 +103,7 @@ int cfl_sorted(const float4* posm_s, const float4* vele, const float* rho, const
                const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
                float c_cfl, float4* velr_s, float2* pc_s, float* dt_out, float* dt_particle, cudaStream_t st);
 int gravity(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, float G, float delta, float4* acc_grav,
-            float4* src_pk, float4* grav_part, unsigned int* grav_flag, cudaStream_t st);   // targets [i0, i1) against all sources
+            float4* src_pk, float4* grav_part, long long* grav_acc64, unsigned int* grav_flag, cudaStream_t st);   // targets [i0, i1) against all sources
 int update_predictor(float4* posm, float4* vele, float4* vele0, const float4* acc_sph, const float4* acc_grav,
                      int64_t n_gas, int64_t n_total, float dt, cudaStream_t st);
 int update_corrector(float4* vele, const float4* vele0, const float4* acc_sph, const float4* acc_grav,

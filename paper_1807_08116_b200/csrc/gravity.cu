@@ -20,92 +20,100 @@
 // split into S chunks whose partial accelerations go to a [S][N] buffer that a last kernel adds
 // in fixed order (deterministic; also gives S x more CTAs than i-tiles, so the grid is many
 // waves deep on 148 SMs and the tail is < 2 %).
-#include "common.cuh"
+#include "grav_dev.cuh"
 
 namespace sphb {
-
-typedef unsigned long long u64;
-
-__device__ __forceinline__ u64 pk2(float lo, float hi) {
-    u64 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void upk2(u64 v, float& lo, float& hi) {
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) {
-    u64 r;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
-    return r;
-}
-__device__ __forceinline__ u64 mul2(u64 a, u64 b) {
-    u64 r;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-    return r;
-}
-__device__ __forceinline__ u64 sub2(u64 a, u64 b) {
-    u64 r;
-    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-    return r;
-}
-__device__ __forceinline__ float rsqrt_approx(float x) {
-    float r;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-
-// ---- mbarrier / bulk-copy helpers (TMA 1-D bulk copy, SASS UBLKCP) ---------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "W: mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@!p bra W;\n\t}" ::"r"(smem_u32(bar)),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(dst_smem)),
-                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
 
 // ---- source packing -----------------------------------------------------------------------
 // pk[2q] = (x_2q, x_2q+1, y_2q, y_2q+1), pk[2q+1] = (z_2q, z_2q+1, m_2q, m_2q+1); sources past n are padded with
 // mass 0 at (1e18, 1e18, 1e18): r2 ~ 3e36 stays finite and u^3 ~ 2e-55 underflows to exactly 0, so a pad adds
 // exactly 0 whether or not the kernel multiplies by its mass.
-// The same pass finds out whether all masses are equal (every BASELINE.json config has m = 1/N): *nonuniform is
-// set (it was zeroed before the launch) as soon as one mass differs from m_0.  No host read-back: both kernel
-// variants are launched and the one that does not apply returns at once (see grav_pp_kernel).
-constexpr float kPadCoord = 1.0e18f;
+// The same pass finds out whether all masses are equal (every BASELINE.json config has m = 1/N): ctl->nonuniform is
+// set (the block was zeroed before the launch) as soon as one mass differs from m_0, and it reduces the bounding box
+// of the particles into ctl (order-preserving unsigned images of the floats, atomicMax) for grav_plan.
+// No host read-back: every kernel variant is launched and the ones that do not apply return at once.
+__device__ __forceinline__ unsigned int ford(float x) {   // monotone map float -> unsigned (finite inputs)
+    const unsigned int b = __float_as_uint(x);
+    return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__device__ __forceinline__ float ford_inv(unsigned int o) {
+    return __uint_as_float((o & 0x80000000u) ? (o & 0x7fffffffu) : ~o);
+}
 __global__ void __launch_bounds__(256) grav_pack_sources(const float4* __restrict__ posm, int n, int n_pad,
-                                                         float4* __restrict__ pk, unsigned int* nonuniform) {
+                                                         float4* __restrict__ pk, GravCtl* ctl) {
     int q = blockIdx.x * blockDim.x + threadIdx.x;
-    if (2 * q >= n_pad) return;
+    const bool live = 2 * q < n_pad;
     const float m0 = posm[0].w;
     float4 a = make_float4(kPadCoord, kPadCoord, kPadCoord, 0.f), b = a;
     bool differs = false;
-    if (2 * q < n) {
+    unsigned int lo[3] = {0xffffffffu, 0xffffffffu, 0xffffffffu}, hi[3] = {0u, 0u, 0u};
+    if (live && 2 * q < n) {
         a = posm[2 * q];
         differs = a.w != m0;
+        lo[0] = hi[0] = ford(a.x);
+        lo[1] = hi[1] = ford(a.y);
+        lo[2] = hi[2] = ford(a.z);
     }
-    if (2 * q + 1 < n) {
+    if (live && 2 * q + 1 < n) {
         b = posm[2 * q + 1];
         differs = differs || b.w != m0;
+        lo[0] = min(lo[0], ford(b.x)), hi[0] = max(hi[0], ford(b.x));
+        lo[1] = min(lo[1], ford(b.y)), hi[1] = max(hi[1], ford(b.y));
+        lo[2] = min(lo[2], ford(b.z)), hi[2] = max(hi[2], ford(b.z));
     }
-    pk[2 * q] = make_float4(a.x, b.x, a.y, b.y);
-    pk[2 * q + 1] = make_float4(a.z, b.z, a.w, b.w);
-    const unsigned active = __activemask();
-    const unsigned any = __ballot_sync(active, differs);
-    if (any != 0u && (threadIdx.x & 31) == (unsigned)(__ffs((int)any) - 1)) atomicOr(nonuniform, 1u);   // one per warp
+    if (live) {
+        pk[2 * q] = make_float4(a.x, b.x, a.y, b.y);
+        pk[2 * q + 1] = make_float4(a.z, b.z, a.w, b.w);
+    }
+    // block reduction: nonuniform flag and bounding box, then 7 atomics per block at most
+    __shared__ unsigned int s_lo[3][8], s_hi[3][8], s_diff;
+    if (threadIdx.x == 0) s_diff = 0u;
+    __syncthreads();
+    const unsigned int any = __ballot_sync(0xffffffffu, differs);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        lo[d] = __reduce_min_sync(0xffffffffu, lo[d]);
+        hi[d] = __reduce_max_sync(0xffffffffu, hi[d]);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (any != 0u) s_diff = 1u;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) s_lo[d][threadIdx.x >> 5] = lo[d], s_hi[d][threadIdx.x >> 5] = hi[d];
+    }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        const int d = threadIdx.x;
+        unsigned int l = s_lo[d][0], h = s_hi[d][0];
+        for (int w = 1; w < 8; ++w) l = min(l, s_lo[d][w]), h = max(h, s_hi[d][w]);
+        if (h != 0u) {   // the block held at least one real particle
+            atomicMax(&ctl->bmin_c[d], ~l);
+            atomicMax(&ctl->bmax[d], h);
+        }
+    } else if (threadIdx.x == 3 && s_diff != 0u) {
+        atomicOr(&ctl->nonuniform, 1u);
+    }
+}
+
+// Decides, on the device, whether the pair-symmetric kernel (gravity_sym.cu) takes this evaluation and with which
+// fixed-point scale.  Largest possible |sum_j d w| is n_pad * max_r r/(r^2+delta^2)^(3/2) = 0.385 n_pad/delta^2;
+// 2^k times twice that must stay below 2^62.  The path is taken when the masses are uniform and the resolution
+// 2^-k is finer than 2^-26 of n/R^2, R = diagonal of the bounding box (the natural size of a particle's sum).
+__global__ void grav_plan(GravCtl* ctl, int n, int n_pad, float eps2) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    double R2 = 0.0;
+    for (int d = 0; d < 3; ++d) {
+        const double e = (double)ford_inv(ctl->bmax[d]) - (double)ford_inv(~ctl->bmin_c[d]);
+        R2 += e * e;
+    }
+    const double bound = 2.0 * 0.385 * (double)n_pad / (double)eps2;
+    int k = 62 - (int)ceil(log2(bound));
+    if (k > 100) k = 100;      // 2^k and products with FP32 partials stay far inside the FP32 range
+    if (k < -100) k = -100;
+    const double res = ldexp(1.0, -k);
+    const bool fine = res * R2 <= ldexp((double)n, -26) || R2 == 0.0;
+    ctl->scale = (float)ldexp(1.0, k);
+    ctl->inv_scale = res;
+    ctl->sym = (ctl->nonuniform == 0u && fine) ? 1u : 0u;
 }
 
 constexpr int kTilePairs = kGravTileSrc / 2;           // 1024 source pairs = 32 KB per stage
@@ -119,15 +127,19 @@ constexpr int kStages = 2;
 template <int I, int THREADS, int MINB, bool ZERO_SOFT, int UNROLL = 2, bool UNIFORM = false>
 __global__ void __launch_bounds__(THREADS, MINB)
     grav_pp_kernel(const float4* __restrict__ posm /*targets*/, const float4* __restrict__ pk, int n, int tiles_total,
-                   int tiles_per_chunk, float eps2, float4* __restrict__ part,
-                   const unsigned int* __restrict__ nonuniform) {
+                   int tiles_per_chunk, int diag_tiles, float eps2, float4* __restrict__ part,
+                   const GravCtl* __restrict__ ctl) {
     extern __shared__ __align__(128) float4 tiles[];   // [kStages][2 * kTilePairs]
     __shared__ __align__(8) uint64_t full_bar[kStages];
-    if ((*nonuniform == 0u) != UNIFORM) return;        // uniform over the grid
+    // uniform over the grid: this variant runs iff the masses are (not) uniform and, diag_tiles > 0 (the diagonal
+    // blocks that the pair-symmetric kernel leaves out), iff that kernel takes the rest of the evaluation
+    if ((ctl->nonuniform == 0u) != UNIFORM || (ctl->sym != 0u) != (diag_tiles > 0)) return;
 
     const int tid = threadIdx.x;
-    const int tile0 = blockIdx.y * tiles_per_chunk;
-    const int ntiles = min(tiles_per_chunk, tiles_total - tile0);
+    // diag_tiles > 0: the sources are the column block of `diag_tiles` tiles that holds this CTA's targets
+    const int tile0 = diag_tiles > 0 ? (int)((blockIdx.x * (THREADS * I)) / (diag_tiles * kGravTileSrc)) * diag_tiles
+                                     : blockIdx.y * tiles_per_chunk;
+    const int ntiles = min(diag_tiles > 0 ? diag_tiles : tiles_per_chunk, tiles_total - tile0);
     if (ntiles <= 0) return;   // uniform per CTA
 
     if (tid == 0) {
@@ -224,20 +236,30 @@ __global__ void __launch_bounds__(THREADS, MINB)
     }
 }
 
-// acc[i] = G * sum_s part[s][i]  in fixed order s = 0..S-1 (dx was r_j - r_i, so the sign of Eq. 4 is in).
+// acc[i] = G [m_0] * sum, in a fixed order (dx was r_j - r_i, so the sign of Eq. 4 is in).  One-sided path: the S chunk
+// partials s = 0..S-1.  Pair-symmetric path (ctl->sym): the fixed-point sums of gravity_sym.cu, exact integers
+// whatever the order they were added in, plus the diagonal-block partial in part[0].
 __global__ void __launch_bounds__(256) grav_reduce(const float4* __restrict__ part, int i0, int n, int S, float G,
                                                    float4* __restrict__ acc, const float4* __restrict__ posm,
-                                                   const unsigned int* __restrict__ nonuniform) {
+                                                   const long long* __restrict__ acc64,
+                                                   const GravCtl* __restrict__ ctl) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;   // slice-local target
     if (i >= n) return;
     float4 a = part[i];
-    for (int s = 1; s < S; ++s) {
-        float4 b = part[(size_t)s * n + i];
-        a.x += b.x;
-        a.y += b.y;
-        a.z += b.z;
+    if (ctl->sym != 0u) {
+        const double inv = ctl->inv_scale;
+        a.x = (float)((double)acc64[3 * (size_t)i + 0] * inv + (double)a.x);
+        a.y = (float)((double)acc64[3 * (size_t)i + 1] * inv + (double)a.y);
+        a.z = (float)((double)acc64[3 * (size_t)i + 2] * inv + (double)a.z);
+    } else {
+        for (int s = 1; s < S; ++s) {
+            float4 b = part[(size_t)s * n + i];
+            a.x += b.x;
+            a.y += b.y;
+            a.z += b.z;
+        }
     }
-    const float scale = (*nonuniform == 0u) ? G * posm[0].w : G;   // uniform masses: m_0 was left out of the loop
+    const float scale = (ctl->nonuniform == 0u) ? G * posm[0].w : G;   // uniform masses: m_0 was left out of the loop
     acc[i0 + i] = make_float4(scale * a.x, scale * a.y, scale * a.z, 0.f);
 }
 
@@ -277,27 +299,30 @@ int grav_splits(int64_t n_total) {
 }
 
 template <int I, int THREADS, int MINB, bool ZERO_SOFT, int UNROLL, bool UNIFORM>
-static int launch_one(dim3 grid, const float4* targets, const float4* pk, int n, int tiles, int tpc, float eps2,
-                      float4* part, const unsigned int* nonuniform, cudaStream_t st) {
+static int launch_one(dim3 grid, const float4* targets, const float4* pk, int n, int tiles, int tpc, int diag_tiles,
+                      float eps2, float4* part, const GravCtl* ctl, cudaStream_t st) {
     const size_t smem = (size_t)kStages * kTileBytes;
     auto kfn = grav_pp_kernel<I, THREADS, MINB, ZERO_SOFT, UNROLL, UNIFORM>;
     SPHB_CUDA(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kfn<<<grid, THREADS, smem, st>>>(targets, pk, n, tiles, tpc, eps2, part, nonuniform);
+    kfn<<<grid, THREADS, smem, st>>>(targets, pk, n, tiles, tpc, diag_tiles, eps2, part, ctl);
     SPHB_LAUNCHED();
     return SPH_OK;
 }
 
-// both mass variants, back to back; exactly one of them does the work (decided on the device)
+// both mass variants, back to back; at most one of them does the work (decided on the device).  diag_tiles > 0:
+// only the diagonal column blocks, for the pair-symmetric path (uniform masses only).
 template <int I, int THREADS, int MINB, int UNROLL>
-static int launch_grav(const float4* targets, const float4* pk, int n, int tiles, int tpc, int S, float eps2,
-                       bool zero_soft, float4* part, const unsigned int* nonuniform, cudaStream_t st) {
+static int launch_grav(const float4* targets, const float4* pk, int n, int tiles, int tpc, int S, int diag_tiles, float eps2,
+                       bool zero_soft, float4* part, const GravCtl* ctl, cudaStream_t st) {
     dim3 grid((unsigned)cdiv(n, (int64_t)I * THREADS), (unsigned)S);
     if (zero_soft) {
-        SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, true>(grid, targets, pk, n, tiles, tpc, eps2, part, nonuniform, st)));
-        SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, false>(grid, targets, pk, n, tiles, tpc, eps2, part, nonuniform, st)));
+        SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, true>(grid, targets, pk, n, tiles, tpc, diag_tiles, eps2, part, ctl, st)));
+        if (diag_tiles == 0)
+            SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, false>(grid, targets, pk, n, tiles, tpc, 0, eps2, part, ctl, st)));
     } else {
-        SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, true>(grid, targets, pk, n, tiles, tpc, eps2, part, nonuniform, st)));
-        SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, false>(grid, targets, pk, n, tiles, tpc, eps2, part, nonuniform, st)));
+        SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, true>(grid, targets, pk, n, tiles, tpc, diag_tiles, eps2, part, ctl, st)));
+        if (diag_tiles == 0)
+            SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, false>(grid, targets, pk, n, tiles, tpc, 0, eps2, part, ctl, st)));
     }
     return SPH_OK;
 }
@@ -307,7 +332,7 @@ static int launch_grav(const float4* targets, const float4* pk, int n, int tiles
 // The partial buffer holds grav_splits(n_total) * n_total float4; a slice may use more, shorter j-chunks (to keep
 // the grid many waves deep) as long as S * (i1 - i0) fits in it.
 int gravity(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, float G, float delta, float4* acc_grav,
-            float4* src_pk, float4* grav_part, unsigned int* grav_flag, cudaStream_t st) {
+            float4* src_pk, float4* grav_part, long long* grav_acc64, unsigned int* grav_flag, cudaStream_t st) {
     if (n_total <= 0 || i1 <= i0) return SPH_OK;
     const int nt = (int)(i1 - i0);
     if (G == 0.0f) {   // no self-gravity (BASELINE config 4, "SPH-only"): Eq. 4 is identically 0
@@ -323,17 +348,28 @@ int gravity(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, float G
     const int tiles = n_pad / kGravTileSrc;
     const int tpc = (int)cdiv(tiles, S);
     S = (int)cdiv(tiles, tpc);
-
-    SPHB_CUDA(cudaMemsetAsync(grav_flag, 0, sizeof(unsigned int), st));
-    grav_pack_sources<<<(unsigned)cdiv(n_pad / 2, 256), 256, 0, st>>>(posm, n, n_pad, src_pk, grav_flag);
-    SPHB_LAUNCHED();
     const float eps2 = delta * delta;
     const bool zero_soft = !(eps2 > 0.f);
+    // The pair-symmetric path (gravity_sym.cu) is offered for a whole evaluation with softening at N >= kSymMinN;
+    // whether it is TAKEN (uniform masses, fixed-point range) is decided on the device by grav_plan.
+    const bool offer_sym = (i0 == 0 && i1 == n_total && !zero_soft && n_total >= kSymMinN && I == 8);
+    GravCtl* ctl = reinterpret_cast<GravCtl*>(grav_flag);
+
+    SPHB_CUDA(cudaMemsetAsync(ctl, 0, sizeof(GravCtl), st));
+    grav_pack_sources<<<(unsigned)cdiv(n_pad / 2, 256), 256, 0, st>>>(posm, n, n_pad, src_pk, ctl);
+    SPHB_LAUNCHED();
+    if (offer_sym) {
+        SPHB_CUDA(cudaMemsetAsync(grav_acc64, 0, (size_t)n_pad * 3 * sizeof(long long), st));
+        grav_plan<<<1, 32, 0, st>>>(ctl, n, n_pad, eps2);
+        SPHB_LAUNCHED();
+        SPHB_TRY(gravity_sym_launch(posm, src_pk, n_pad, eps2, grav_acc64, ctl, st));
+        SPHB_TRY((launch_grav<8, 128, 2, 1>(posm, src_pk, nt, tiles, tpc, 1, kSymL / kGravTileSrc, eps2, false, grav_part, ctl, st)));
+    }
     if (I == 8)
-        SPHB_TRY((launch_grav<8, 128, 2, 1>(posm + i0, src_pk, nt, tiles, tpc, S, eps2, zero_soft, grav_part, grav_flag, st)));
+        SPHB_TRY((launch_grav<8, 128, 2, 1>(posm + i0, src_pk, nt, tiles, tpc, S, 0, eps2, zero_soft, grav_part, ctl, st)));
     else
-        SPHB_TRY((launch_grav<1, 128, 4, 2>(posm + i0, src_pk, nt, tiles, tpc, S, eps2, zero_soft, grav_part, grav_flag, st)));
-    grav_reduce<<<(unsigned)cdiv(nt, 256), 256, 0, st>>>(grav_part, (int)i0, nt, S, G, acc_grav, posm, grav_flag);
+        SPHB_TRY((launch_grav<1, 128, 4, 2>(posm + i0, src_pk, nt, tiles, tpc, S, 0, eps2, zero_soft, grav_part, ctl, st)));
+    grav_reduce<<<(unsigned)cdiv(nt, 256), 256, 0, st>>>(grav_part, (int)i0, nt, S, G, acc_grav, posm, grav_acc64, ctl);
     SPHB_LAUNCHED();
     return SPH_OK;
 }

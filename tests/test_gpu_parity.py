@@ -561,17 +561,21 @@ def test_gravity_slices_equal_full(cuda_lib):
             before = acc.clone()
             b.nbody_pp_gravity_slice(d, n, i0, i1, w.G, w.delta, acc, ws)
             assert torch.equal(acc[:i0], before[:i0]) and torch.equal(acc[i1:], before[i1:])   # rows outside untouched
-        # a slice may use more, shorter j-chunks: same sums in another (fixed) order
+        # a slice runs the one-sided kernel (possibly with more, shorter j-chunks), the full call the pair-symmetric
+        # one: the same sums in FP32 in another (fixed) order; each is held to the oracle separately below
         err = (acc[:, :3] - full[:, :3]).norm(dim=1) / full[:, :3].norm(dim=1).clamp_min(1e-3)
-        assert err.max().item() < 2e-6
+        print("slices vs full, world", world, "max", err.max().item(), "median", err.median().item())
+        assert err.max().item() < 2e-5 and err.median().item() < 1e-6
     tg = np.arange(0, n, 97)
-    check_values(acc.cpu().numpy()[tg, :3], oracle.gravity(w.posm, w.G, w.delta, targets=tg), "a_grav 8 slices")
+    ref = oracle.gravity(w.posm, w.G, w.delta, targets=tg)
+    check_values(acc.cpu().numpy()[tg, :3], ref, "a_grav 8 slices")
+    check_values(full.cpu().numpy()[tg, :3], ref, "a_grav full (pair-symmetric)")
     # ragged and degenerate slices
     b.nbody_pp_gravity_slice(d, n, 5, 5, w.G, w.delta, acc, ws)
     one = torch.zeros((n, 4), device="cuda")
     b.nbody_pp_gravity_slice(d, n, 12345, 12346, w.G, w.delta, one, ws)
     assert torch.count_nonzero(one[:12345]).item() == 0 and torch.count_nonzero(one[12346:]).item() == 0
-    assert (one[12345, :3] - full[12345, :3]).norm().item() < 2e-6 * full[12345, :3].norm().item()
+    assert (one[12345, :3] - full[12345, :3]).norm().item() < 2e-5 * full[12345, :3].norm().item()
     with pytest.raises(b.SphError):
         b.nbody_pp_gravity_slice(d, n, 10, n + 1, w.G, w.delta, acc, ws)
 
