@@ -248,6 +248,15 @@ int sph_correct(float* vele, const float* hsml /*or NULL*/, int64_t n_gas, int64
 int sph_set_profiling(int on);
 int sph_get_stage_ms(float out_ms[5] /*HOST*/);
 
+/* Diagnostic: which variant of the gravity kernel the LAST evaluation enqueued with workspace `ws` (sized for n_gas,
+ * n_total and g, as in that call) took.  The choice is made on the device, so this reads the
+ * 32-byte control block back and SYNCHRONISES `stream`.  *path_host = SPH_GRAV_ONE_SIDED (unequal masses),
+ * SPH_GRAV_ONE_SIDED_UNIFORM (equal masses: m_j leaves the loop) or SPH_GRAV_PAIR_SYMMETRIC (equal masses, every
+ * unordered pair evaluated once, fixed-point accumulation).  Eq. 4.                              */
+enum { SPH_GRAV_ONE_SIDED = 0, SPH_GRAV_ONE_SIDED_UNIFORM = 1, SPH_GRAV_PAIR_SYMMETRIC = 2 };
+int sph_gravity_path(const void* ws /*DEVICE*/, size_t ws_bytes, int64_t n_gas, int64_t n_total,
+                     const sph_grid* g /*HOST, may be NULL if n_gas == 0*/, int* path_host /*HOST*/, void* stream);
+
 /* Number of kernel launches this library has enqueued in the calling process since load. */
 int64_t sph_launch_count(void);
 

@@ -26,7 +26,7 @@ EXPORTS = (
     "sph_host_ctx_create", "sph_host_ctx_step", "sph_host_ctx_destroy", "sph_neighbour_lists",
     "sph_set_profiling", "sph_get_stage_ms", "sph_launch_count", "sph_cfl_dt",
     "nbody_pp_gravity_slice", "sph_position_slice", "sph_predict", "sph_correct",
-    "sph_smoothing_lengths", "sph_density_h", "sph_forces_h", "sph_evaluate_h", "sph_step_h", "sph_neighbour_lists_h",
+    "sph_gravity_path", "sph_smoothing_lengths", "sph_density_h", "sph_forces_h", "sph_evaluate_h", "sph_step_h", "sph_neighbour_lists_h",
 )
 
 
@@ -92,6 +92,7 @@ def load():
     L.sph_density.argtypes = [vp, i64, pp, gp, vp, vp, vp, vp, sz, vp]
     L.sph_forces.argtypes = [vp, vp, vp, i64, pp, gp, vp, vp, vp, vp, sz, vp]
     L.nbody_pp_gravity.argtypes = [vp, i64, f32, f32, vp, vp, sz, vp]
+    L.sph_gravity_path.argtypes = [vp, sz, i64, i64, gp, C.POINTER(C.c_int), vp]
     L.sph_cfl_dt.argtypes = [vp, vp, vp, vp, vp, i64, pp, gp, vp, vp, f32, vp, vp, vp, sz, vp]
     L.sph_step.argtypes = [vp, vp, i64, i64, pp, gp, f32, C.c_int, vp, vp, vp, vp, sz, vp]
     L.sph_evaluate.argtypes = [vp, vp, i64, i64, pp, gp, vp, vp, vp, vp, sz, vp]
@@ -345,6 +346,18 @@ def sph_get_stage_ms() -> dict:
     out = (C.c_float * 5)()
     _chk("sph_get_stage_ms", load().sph_get_stage_ms(out))
     return dict(zip(STAGES, [float(x) for x in out]))
+
+
+GRAV_PATHS = ("one_sided", "one_sided_uniform", "pair_symmetric")
+
+
+def sph_gravity_path(ws, n_gas, n_total, grid=None) -> str:
+    """Which gravity kernel variant the last evaluation with workspace `ws` took (chosen on the device)."""
+    p, nb = _ws(ws)
+    out = C.c_int(-1)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_gravity_path", load().sph_gravity_path(p, nb, int(n_gas), int(n_total), g, C.byref(out), _stream()))
+    return GRAV_PATHS[out.value]
 
 
 def sph_launch_count() -> int:

@@ -244,6 +244,19 @@ int nbody_pp_gravity_slice(const float* posm, int64_t n_total, int64_t i0, int64
                    w.src_pk, w.grav_part, w.grav_acc64, w.grav_flag, st);
 }
 
+int sph_gravity_path(const void* ws, size_t ws_bytes, int64_t n_gas, int64_t n_total, const sph_grid* g, int* path_host,
+                     void* stream) {
+    if (!ws || !path_host || bad_count(n_total) || bad_count(n_gas) || (n_gas > 0 && !g)) return SPH_ERR_ARG;
+    Workspace w = carve(const_cast<void*>(ws), n_gas, n_total, g);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    unsigned int ctl[2] = {0u, 0u};   // GravCtl: nonuniform, sym
+    cudaStream_t st = (cudaStream_t)stream;
+    SPHB_CUDA(cudaMemcpyAsync(ctl, w.grav_flag, sizeof(ctl), cudaMemcpyDeviceToHost, st));
+    SPHB_CUDA(cudaStreamSynchronize(st));
+    *path_host = ctl[0] != 0u ? SPH_GRAV_ONE_SIDED : (ctl[1] != 0u ? SPH_GRAV_PAIR_SYMMETRIC : SPH_GRAV_ONE_SIDED_UNIFORM);
+    return SPH_OK;
+}
+
 int nbody_pp_gravity(const float* posm, int64_t n_total, float G, float delta, float* acc_grav, void* ws,
                      size_t ws_bytes, void* stream) {
     return nbody_pp_gravity_slice(posm, n_total, 0, n_total, G, delta, acc_grav, ws, ws_bytes, stream);

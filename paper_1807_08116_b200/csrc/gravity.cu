@@ -352,7 +352,7 @@ int gravity(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, float G
     const bool zero_soft = !(eps2 > 0.f);
     // The pair-symmetric path (gravity_sym.cu) is offered for a whole evaluation with softening at N >= kSymMinN;
     // whether it is TAKEN (uniform masses, fixed-point range) is decided on the device by grav_plan.
-    const bool offer_sym = (i0 == 0 && i1 == n_total && !zero_soft && n_total >= kSymMinN && I == 8);
+    const bool offer_sym = (i0 == 0 && i1 == n_total && !zero_soft && n_total >= kSymMinN);
     GravCtl* ctl = reinterpret_cast<GravCtl*>(grav_flag);
 
     SPHB_CUDA(cudaMemsetAsync(ctl, 0, sizeof(GravCtl), st));

@@ -657,3 +657,68 @@ def test_gravity_mass_variants_large_shape(cuda_lib, masses):
     got0 = acc.cpu().numpy()
     check_values(got0[tg, :3], oracle.gravity(posm, w.G, 0.0, targets=tg), f"a_grav delta=0 masses={masses}",
                  max_tol=5e-4, med_tol=2e-5)
+
+
+# ---------------------------------------------------------------- (a10) pair-symmetric gravity path
+def _grav(b, posm, G, delta):
+    n = posm.shape[0]
+    d = _t(posm)
+    acc = torch.full((n, 4), 7.0, device="cuda")
+    ws = b.alloc_workspace(0, n)
+    b.nbody_pp_gravity(d, n, G, delta, acc, ws)
+    return acc, b.sph_gravity_path(ws, 0, n)
+
+
+@pytest.mark.parametrize("n", [32768, 45001, 2 ** 17])
+def test_gravity_pair_symmetric_path(cuda_lib, n):
+    """Eq. 4 (L47) with every unordered pair evaluated once (gravity_sym.cu): whole column blocks and a ragged
+    tail (45000 = 21 blocks of 2048 + 1992 real sources in the padded last block), the smallest N that takes the
+    path, and config 1's N.  Against the oracle on a seeded subset; momentum; bitwise repeatable although the
+    work items are handed out dynamically (the sums are integers)."""
+    b = cuda_lib
+    w = wl.make_workload(1, scale=n / 2 ** 17)
+    n = w.n_total                                  # the generator keeps the four components equal: 45001 -> 45000
+    assert n % 2048 != 0 or n in (32768, 2 ** 17)
+    acc, path = _grav(b, w.posm, w.G, w.delta)
+    assert path == "pair_symmetric"
+    got = acc.cpu().numpy()
+    assert np.all(np.isfinite(got)) and np.all(got[:, 3] == 0)
+    tg = np.unique(np.concatenate([np.arange(0, n, max(1, n // 1500)), [0, 1, 2047, 2048, 2049, n - 2, n - 1],
+                                   np.arange((n - 1) // 2048 * 2048 - 3, min(n, (n - 1) // 2048 * 2048 + 3))]))
+    check_values(got[tg, :3], oracle.gravity(w.posm, w.G, w.delta, targets=tg), f"a_grav pair-symmetric n={n}")
+    # P5: sum_i m_i a_i = 0.  The off-diagonal pairs cancel EXACTLY in the integer sums; what is left is the
+    # FP32 rounding of the per-particle results and of the one-sided diagonal blocks.
+    m = w.posm[:, 3].astype(np.float64)
+    a = got[:, :3].astype(np.float64)
+    assert np.linalg.norm((m[:, None] * a).sum(0)) < 2e-7 * (m * np.linalg.norm(a, axis=1)).sum()
+    for _ in range(2):
+        again, path2 = _grav(b, w.posm, w.G, w.delta)
+        assert path2 == "pair_symmetric" and torch.equal(acc, again)
+
+
+def test_gravity_path_selection(cuda_lib):
+    """The variant is chosen on the device (grav_plan): unequal masses, a fixed-point range that would be too
+    coarse (bounding box / delta too large), delta = 0 and small N all stay on the one-sided kernel, and every
+    choice matches the oracle."""
+    b = cuda_lib
+    n = 40000
+    w = wl.make_workload(1, scale=n / 2 ** 17)
+    tg = np.concatenate([np.arange(0, n, 53), [0, 5, n - 1]])
+
+    def check(posm, delta, want, what, **tol):
+        acc, path = _grav(b, posm, w.G, delta)
+        assert path == want, (what, path)
+        check_values(acc.cpu().numpy()[tg, :3], oracle.gravity(posm, w.G, delta, targets=tg), what, **tol)
+
+    check(w.posm, w.delta, "pair_symmetric", "equal masses")
+    p = w.posm.copy()
+    p[n - 1, 3] *= 2.0
+    check(p, w.delta, "one_sided", "one mass differs")
+    p = w.posm.copy()
+    p[5, :3] = (3.0e4, 0.0, 0.0)                 # box diagonal / delta = 6e6: 2^-k would be > 2^-26 of n / R^2
+    check(p, w.delta, "one_sided_uniform", "far-away particle")
+    check(w.posm, 1.0e-6, "one_sided_uniform", "tiny delta", max_tol=5e-4, med_tol=2e-5)
+    check(w.posm, 0.0, "one_sided_uniform", "delta = 0", max_tol=5e-4, med_tol=2e-5)
+    w0 = wl.make_workload(0)
+    acc, path = _grav(b, w0.posm, w0.G, w0.delta)
+    assert path == "one_sided_uniform"           # N = 8192 < 32768
