@@ -311,14 +311,25 @@ def run_ours(args, w):
     roofline = None
     if w.G != 0.0 and grav_ms > 0:
         achieved = FLOPS_PER_INTERACTION * float(n_slice) * float(n) / (grav_ms * 1e-3) / 1e12   # per GPU (rank 0's slice)
-        tr = ncu_traffic("grav_pp_kernel")
+        path = b.sph_gravity_path(sim.ws, ng, n, sim.grid)           # chosen on the device
+        # FP32 lane-operations the variant really executes per INTERACTION (an FMA counted once) and its dominant kernel
+        kernel, ops = {"pair_symmetric": ("grav_sym_kernel", 7.0), "one_sided_uniform": ("grav_pp_kernel", 11.0),
+                       "one_sided": ("grav_pp_kernel", 12.0)}[path]
+        tr = ncu_traffic(kernel)
         traffic = tr["bytes"] if tr and tr["n_total"] == n else None   # the capture is of this workload only
-        roofline = {"kernel": "grav_pp_kernel", "bound": "alu", "achieved": achieved, "peak": alu_peak_tflops,
+        lane_peak = 128 * SM_COUNT_B200 * sm_max * 1e6                 # FP32 lane-operations per second
+        roofline = {"kernel": kernel, "bound": "alu", "achieved": achieved, "peak": alu_peak_tflops,
                     "unit": "TFLOP/s", "frac": achieved / alu_peak_tflops, "traffic": traffic,
                     "traffic_note": "DRAM bytes per launch (ncu --set full, profiles/traffic_r01.csv); irrelevant to an ALU-bound kernel",
                     "peak_source": f"2*128*148*sm_max_mhz ({peak_src} sm_max_mhz={sm_max:.0f}); 20 flops/interaction",
-                    "kernel_ms": grav_ms, "launches_per_step": 1,
-                    "note": "gravity stage = pack + grav_pp_kernel + reduce; the two O(N) kernels are <0.1% of it"}
+                    "kernel_ms": grav_ms, "launches_per_step": 1, "gravity_path": path,
+                    "executed_lane_ops_per_interaction": ops,
+                    "fp32_pipe_util": ops * float(n_slice) * float(n) / (grav_ms * 1e-3) / lane_peak,
+                    "note": "achieved = ALGORITHMIC flops (BASELINE.json convention: 20 per ordered interaction, N^2 of them) / "
+                            "gravity stage time (pack + kernel + reduce; the O(N) kernels are <0.1%).  The pair-symmetric "
+                            "kernel evaluates each UNORDERED pair once (14 FP32 lane-ops + 1 MUFU per pair = 7 + 0.5 per "
+                            "interaction), so frac can exceed the 20-flop instruction-mix ceiling and even 1; "
+                            "fp32_pipe_util is the share of FP32 issue capacity (128 lanes/clk/SM) the executed operations take"}
     hbm = float(peaks.get("hbm_gbs", 6650.0))
     sort_bytes = ng * 92 + M * 16
     # gas: predictor 64 B read + 48 B written, corrector 64 + 16; halo particles never touch acc_sph: 48 + 48, 48 + 16
