@@ -232,6 +232,35 @@ int nbody_pp_gravity_slice(const float* posm, int64_t n_total, int64_t i0, int64
 int sph_position_slice(const float* posm, float* hsml /*or NULL*/, float sigma, int64_t n_gas, int64_t n_halo,
                        int64_t i0, int64_t i1, const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/,
                        float* rho, float* acc_grav, void* ws, size_t ws_bytes, void* stream);
+
+/* One GPU's SHARE of the position-only stage (NEXT-4: k GPUs, N/k particles each): SP and DC in full
+ * (O(N), replicated), and rank `rank` of `world`'s part of the Eq. 4 evaluation (L47).  Which gravity kernel runs is
+ * decided on the device, so the share has two forms and the caller exchanges BOTH before calling the finish:
+ *   - one-sided path: targets [i0, i1) against all sources -> acc_grav rows [i0, i1) (other rows untouched);
+ *     exchange = all-gather of the row slices;
+ *   - pair-symmetric path (equal masses, delta > 0, N >= 32768, fixed-point range fits): the work items
+ *     rank, rank + world, ... of the unordered-pair decomposition -> 64-bit fixed-point sums in the workspace region
+ *     sph_workspace_gravity_sums() reports (zeroed by this call; acc_grav not written);
+ *     exchange = integer SUM all-reduce of that region (exact: the result is bit for bit the same for every world size).
+ * nbody_pp_gravity_finish then writes acc_grav rows [0, n) from the summed region if the pair-symmetric path was taken
+ * and does nothing otherwise.  world = 1, [i0, i1) = [0, n): share + finish is sph_position_slice on the full range.
+ * Errors: SPH_ERR_ARG (world < 1, rank outside [0, world), bad slice, null / misaligned pointers), SPH_ERR_GRID,
+ * SPH_ERR_WORKSPACE, SPH_ERR_UNSUPPORTED (delta < 0), SPH_ERR_CUDA.  Asynchronous on `stream`.                        */
+int sph_position_share(const float* posm, float* hsml /*or NULL*/, float sigma, int64_t n_gas, int64_t n_halo, int rank,
+                       int world, int64_t i0, int64_t i1, const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/,
+                       float* rho, float* acc_grav, void* ws, size_t ws_bytes, void* stream);
+/* The gravity part alone (workspace sized for n_gas = 0). */
+int nbody_pp_gravity_share(const float* posm, int64_t n_total, int rank, int world, int64_t i0, int64_t i1, float G,
+                           float delta, float* acc_grav, void* ws, size_t ws_bytes, void* stream);
+/* After the exchange.  (n_gas, n_halo, g) only locate the regions in `ws`: the values the share call was given
+ * (n_gas = 0, g = NULL after nbody_pp_gravity_share). */
+int nbody_pp_gravity_finish(const float* posm, int64_t n_gas, int64_t n_halo, const sph_grid* g /*HOST or NULL*/, float G,
+                            float* acc_grav, void* ws, size_t ws_bytes, void* stream);
+/* Byte offset and size, inside a workspace of sph_workspace_bytes(n_gas, n_total, g), of the int64 sums
+ * [padded N][3] of the pair-symmetric path.  Host-only, no CUDA call. */
+int sph_workspace_gravity_sums(int64_t n_gas, int64_t n_total, const sph_grid* g /*HOST or NULL*/,
+                               size_t* offset_host, size_t* bytes_host);
+
 int sph_predict(float* posm, float* vele, const float* hsml /*or NULL*/, int64_t n_gas, int64_t n_halo,
                 const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/, float dt,
                 const float* rho, float* acc_sph, const float* acc_grav, void* ws, size_t ws_bytes, void* stream);

@@ -26,7 +26,8 @@ EXPORTS = (
     "sph_host_ctx_create", "sph_host_ctx_step", "sph_host_ctx_destroy", "sph_neighbour_lists",
     "sph_set_profiling", "sph_get_stage_ms", "sph_launch_count", "sph_cfl_dt",
     "nbody_pp_gravity_slice", "sph_position_slice", "sph_predict", "sph_correct",
-    "sph_gravity_path", "sph_smoothing_lengths", "sph_density_h", "sph_forces_h", "sph_evaluate_h", "sph_step_h", "sph_neighbour_lists_h",
+    "sph_gravity_path", "sph_position_share", "nbody_pp_gravity_share", "nbody_pp_gravity_finish",
+    "sph_workspace_gravity_sums", "sph_smoothing_lengths", "sph_density_h", "sph_forces_h", "sph_evaluate_h", "sph_step_h", "sph_neighbour_lists_h",
 )
 
 
@@ -92,6 +93,10 @@ def load():
     L.sph_density.argtypes = [vp, i64, pp, gp, vp, vp, vp, vp, sz, vp]
     L.sph_forces.argtypes = [vp, vp, vp, i64, pp, gp, vp, vp, vp, vp, sz, vp]
     L.nbody_pp_gravity.argtypes = [vp, i64, f32, f32, vp, vp, sz, vp]
+    L.sph_position_share.argtypes = [vp, vp, f32, i64, i64, C.c_int, C.c_int, i64, i64, pp, gp, vp, vp, vp, sz, vp]
+    L.nbody_pp_gravity_share.argtypes = [vp, i64, C.c_int, C.c_int, i64, i64, f32, f32, vp, vp, sz, vp]
+    L.nbody_pp_gravity_finish.argtypes = [vp, i64, i64, gp, f32, vp, vp, sz, vp]
+    L.sph_workspace_gravity_sums.argtypes = [i64, i64, gp, C.POINTER(sz), C.POINTER(sz)]
     L.sph_gravity_path.argtypes = [vp, sz, i64, i64, gp, C.POINTER(C.c_int), vp]
     L.sph_cfl_dt.argtypes = [vp, vp, vp, vp, vp, i64, pp, gp, vp, vp, f32, vp, vp, vp, sz, vp]
     L.sph_step.argtypes = [vp, vp, i64, i64, pp, gp, f32, C.c_int, vp, vp, vp, vp, sz, vp]
@@ -218,6 +223,37 @@ def nbody_pp_gravity_slice(posm, n_total, i0, i1, G, delta, acc_grav, ws):
     p, nb = _ws(ws)
     _chk("nbody_pp_gravity_slice", load().nbody_pp_gravity_slice(_ptr(posm), int(n_total), int(i0), int(i1), float(G),
                                                                  float(delta), _ptr(acc_grav), p, nb, _stream()))
+
+
+def sph_position_share(posm, hsml, sigma, n_gas, n_halo, rank, world, i0, i1, params, grid, rho, acc_grav, ws):
+    p, nb = _ws(ws)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_position_share", load().sph_position_share(_ptr(posm), _ptr(hsml), float(sigma), int(n_gas), int(n_halo),
+                                                         int(rank), int(world), int(i0), int(i1), C.byref(params), g,
+                                                         _ptr(rho), _ptr(acc_grav), p, nb, _stream()))
+
+
+def nbody_pp_gravity_share(posm, n_total, rank, world, i0, i1, G, delta, acc_grav, ws):
+    p, nb = _ws(ws)
+    _chk("nbody_pp_gravity_share", load().nbody_pp_gravity_share(_ptr(posm), int(n_total), int(rank), int(world), int(i0),
+                                                                 int(i1), float(G), float(delta), _ptr(acc_grav), p, nb,
+                                                                 _stream()))
+
+
+def nbody_pp_gravity_finish(posm, n_gas, n_halo, grid, G, acc_grav, ws):
+    p, nb = _ws(ws)
+    g = C.byref(grid) if grid is not None else None
+    _chk("nbody_pp_gravity_finish", load().nbody_pp_gravity_finish(_ptr(posm), int(n_gas), int(n_halo), g, float(G),
+                                                                   _ptr(acc_grav), p, nb, _stream()))
+
+
+def gravity_sums_view(ws, n_gas, n_total, grid=None) -> torch.Tensor:
+    """int64 view of the workspace region that holds the pair-symmetric path's fixed-point sums (for the all-reduce)."""
+    off, nbytes = C.c_size_t(0), C.c_size_t(0)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_workspace_gravity_sums", load().sph_workspace_gravity_sums(int(n_gas), int(n_total), g, C.byref(off),
+                                                                         C.byref(nbytes)))
+    return ws[off.value:off.value + nbytes.value].view(torch.int64)
 
 
 def sph_position_slice(posm, hsml, sigma, n_gas, n_halo, i0, i1, params, grid, rho, acc_grav, ws):

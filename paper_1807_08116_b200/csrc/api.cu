@@ -46,9 +46,11 @@ int check_params(const sph_params* p, bool need_h) {
 // SP + DC + GFC at the current positions: everything that depends on r only (L123, A11).
 // hsml != NULL (NEXT-2): per-particle smoothing lengths; with sigma > 0 they are renewed from the refined density
 // right after DC, h_i = min(sigma (m_i/rho_i)^(1/3), p->h) (L82, readings A25/A26), and re-gathered into cell order.
+// world == 0: a one-GPU call (targets [i0, i1), complete on return).  world >= 1: rank's SHARE of the gravity evaluation
+// (gravity_share); the caller exchanges and then calls nbody_pp_gravity_finish.
 int position_only(const float4* posm, float* hsml, float sigma, int64_t n_gas, int64_t n_total, int64_t i0, int64_t i1,
                   const sph_params* p, const sph_grid* g, float* rho, float4* acc_grav, const Workspace& w,
-                  cudaStream_t st) {
+                  cudaStream_t st, int rank = 0, int world = 0) {
     if (n_gas > 0) {
         {
             Span sp(ST_SORT, st);
@@ -67,7 +69,11 @@ int position_only(const float4* posm, float* hsml, float sigma, int64_t n_gas, i
     }
     {
         Span sp(ST_GRAVITY, st);
-        SPHB_TRY(gravity(posm, n_total, i0, i1, p->G, p->delta, acc_grav, w.src_pk, w.grav_part, w.grav_acc64, w.grav_flag, st));   // GFC
+        if (world == 0)
+            SPHB_TRY(gravity(posm, n_total, i0, i1, p->G, p->delta, acc_grav, w.src_pk, w.grav_part, w.grav_acc64, w.grav_flag, st));   // GFC
+        else
+            SPHB_TRY(gravity_share(posm, n_total, i0, i1, rank, world, true, p->G, p->delta, acc_grav, w.src_pk, w.grav_part,
+                                   w.grav_acc64, w.grav_flag, st));
     }
     return SPH_OK;
 }
@@ -300,6 +306,62 @@ int sph_position_slice(const float* posm, float* hsml, float sigma, int64_t n_ga
     if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
     return position_only(reinterpret_cast<const float4*>(posm), n_gas > 0 ? hsml : nullptr, sigma, n_gas, n, i0, i1, p, g,
                          rho, reinterpret_cast<float4*>(acc_grav), w, (cudaStream_t)stream);
+}
+
+int sph_position_share(const float* posm, float* hsml, float sigma, int64_t n_gas, int64_t n_halo, int rank, int world,
+                       int64_t i0, int64_t i1, const sph_params* p, const sph_grid* g, float* rho, float* acc_grav,
+                       void* ws, size_t ws_bytes, void* stream) {
+    if (bad_count(n_gas) || bad_count(n_halo) || bad_count(n_gas + n_halo)) return SPH_ERR_ARG;
+    const int64_t n = n_gas + n_halo;
+    if (world < 1 || rank < 0 || rank >= world || i0 < 0 || i1 < i0 || i1 > n || sigma < 0.f) return SPH_ERR_ARG;
+    SPHB_TRY(check_params(p, n_gas > 0));
+    if (n == 0) return SPH_OK;
+    if (!posm || !acc_grav || !aligned16(posm) || !aligned16(acc_grav) || (n_gas > 0 && !rho)) return SPH_ERR_ARG;
+    if (n_gas > 0) SPHB_TRY(check_grid(g, p->h));
+    if (!ws || (reinterpret_cast<uintptr_t>(ws) & 255u)) return SPH_ERR_ARG;
+    Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    return position_only(reinterpret_cast<const float4*>(posm), n_gas > 0 ? hsml : nullptr, sigma, n_gas, n, i0, i1, p, g,
+                         rho, reinterpret_cast<float4*>(acc_grav), w, (cudaStream_t)stream, rank, world);
+}
+
+int nbody_pp_gravity_share(const float* posm, int64_t n_total, int rank, int world, int64_t i0, int64_t i1, float G,
+                           float delta, float* acc_grav, void* ws, size_t ws_bytes, void* stream) {
+    if (bad_count(n_total) || world < 1 || rank < 0 || rank >= world || i0 < 0 || i1 < i0 || i1 > n_total) return SPH_ERR_ARG;
+    if (delta < 0.f) return SPH_ERR_UNSUPPORTED;
+    if (n_total == 0) return SPH_OK;
+    if (!posm || !acc_grav || !ws || !aligned16(posm) || !aligned16(acc_grav) || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return SPH_ERR_ARG;
+    Workspace w = carve(ws, 0, n_total, nullptr);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    Span sp(ST_GRAVITY, st);
+    return gravity_share(reinterpret_cast<const float4*>(posm), n_total, i0, i1, rank, world, true, G, delta,
+                         reinterpret_cast<float4*>(acc_grav), w.src_pk, w.grav_part, w.grav_acc64, w.grav_flag, st);
+}
+
+int nbody_pp_gravity_finish(const float* posm, int64_t n_gas, int64_t n_halo, const sph_grid* g, float G, float* acc_grav,
+                            void* ws, size_t ws_bytes, void* stream) {
+    if (bad_count(n_gas) || bad_count(n_halo) || bad_count(n_gas + n_halo) || (n_gas > 0 && !g)) return SPH_ERR_ARG;
+    const int64_t n = n_gas + n_halo;
+    if (n == 0) return SPH_OK;
+    if (!posm || !acc_grav || !ws || !aligned16(posm) || !aligned16(acc_grav) || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return SPH_ERR_ARG;
+    Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    Span sp(ST_GRAVITY, st);
+    return gravity_finish(reinterpret_cast<const float4*>(posm), n, G, reinterpret_cast<float4*>(acc_grav), w.grav_acc64,
+                          w.grav_flag, st);
+}
+
+int sph_workspace_gravity_sums(int64_t n_gas, int64_t n_total, const sph_grid* g, size_t* offset_host, size_t* bytes_host) {
+    if (!offset_host || !bytes_host || bad_count(n_gas) || bad_count(n_total) || n_gas > n_total || (n_gas > 0 && !g))
+        return SPH_ERR_ARG;
+    Workspace w = carve(nullptr, n_gas, n_total, n_gas > 0 ? g : nullptr);
+    *offset_host = w.grav_acc64_off;
+    *bytes_host = (size_t)grav_padded(n_total) * 3 * sizeof(long long);
+    return SPH_OK;
 }
 
 int sph_predict(float* posm, float* vele, const float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p,

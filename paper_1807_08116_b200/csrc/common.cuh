@@ -70,6 +70,7 @@ struct Workspace {
     float4* src_pk;        // [n_pad] packed source pairs
     float4* grav_part;     // [S][n_total] partial accelerations
     long long* grav_acc64;     // [n_pad][3] fixed-point accumulators of the pair-symmetric gravity kernel
+    size_t grav_acc64_off;     // its byte offset in the workspace (sph_workspace_gravity_sums)
     unsigned int* grav_flag;   // 256-byte device control block of one gravity evaluation (GravCtl, grav_dev.cuh)
     // integrator
     float4* vele0;         // [n_total] v(t), e(t) saved by the predictor
@@ -102,6 +103,11 @@ int gather_sorted_h(const float* hsml, const uint32_t* perm, int64_t n_gas, floa
 int cfl_sorted(const float4* posm_s, const float4* vele, const float* rho, const float4* acc_sph, const float4* acc_grav,
                const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
                float c_cfl, float4* velr_s, float2* pc_s, float* dt_out, float* dt_particle, cudaStream_t st);
+int gravity_share(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, int rank, int world, bool offer_sym,
+                  float G, float delta, float4* acc_grav, float4* src_pk, float4* grav_part, long long* grav_acc64,
+                  unsigned int* grav_flag, cudaStream_t st);   // one GPU's share of an evaluation (gravity.cu)
+int gravity_finish(const float4* posm, int64_t n_total, float G, float4* acc_grav, const long long* grav_acc64,
+                   const unsigned int* grav_flag, cudaStream_t st);   // after the exchange: sums -> acc_grav, if pair-symmetric
 int gravity(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, float G, float delta, float4* acc_grav,
             float4* src_pk, float4* grav_part, long long* grav_acc64, unsigned int* grav_flag, cudaStream_t st);   // targets [i0, i1) against all sources
 int update_predictor(float4* posm, float4* vele, float4* vele0, const float4* acc_sph, const float4* acc_grav,

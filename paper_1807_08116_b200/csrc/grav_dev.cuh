@@ -91,7 +91,7 @@ constexpr float kPadCoord = 1.0e18f;   // padded sources: mass 0 far away, contr
 constexpr int kSymL = 2048;            // sources (columns) per work item of the pair-symmetric kernel
 constexpr int kSymMinN = 32768;        // below this the one-sided kernel is used
 
-int gravity_sym_launch(const float4* posm, const float4* src_pk, int n_pad, float eps2, long long* acc64,
-                       GravCtl* ctl, cudaStream_t st);
+int gravity_sym_launch(const float4* posm, const float4* src_pk, int n_pad, int share_rank, int share_world, float eps2,
+                       long long* acc64, GravCtl* ctl, cudaStream_t st);
 
 }  // namespace sphb

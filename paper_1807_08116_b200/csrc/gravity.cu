@@ -124,11 +124,19 @@ constexpr int kStages = 2;
 // UNIFORM: all masses are equal (*nonuniform == 0): the factor m_j leaves the loop (11 instead of 12 packed FP32
 // operations per interaction pair) and is applied once, with G, in grav_reduce.  Each variant returns immediately
 // when the flag says the other one applies, so launching both costs one empty grid (~20 us) and no synchronisation.
+// Diagonal mode (dg.tiles > 0): the part of the pair-symmetric path that kernel leaves out — each CTA's sources are the
+// column block of dg.tiles tiles that holds its targets; only the blocks c with c % dg.world == dg.rank are done (one
+// GPU's share, NEXT-4), and the FP32 sums are added, in fixed point, to the accumulators dg.acc64 of gravity_sym.cu.
+struct GravDiag {
+    int tiles, rank, world;
+    long long* acc64;
+};
 template <int I, int THREADS, int MINB, bool ZERO_SOFT, int UNROLL = 2, bool UNIFORM = false>
 __global__ void __launch_bounds__(THREADS, MINB)
     grav_pp_kernel(const float4* __restrict__ posm /*targets*/, const float4* __restrict__ pk, int n, int tiles_total,
-                   int tiles_per_chunk, int diag_tiles, float eps2, float4* __restrict__ part,
+                   int tiles_per_chunk, const GravDiag dg, float eps2, float4* __restrict__ part,
                    const GravCtl* __restrict__ ctl) {
+    const int diag_tiles = dg.tiles;
     extern __shared__ __align__(128) float4 tiles[];   // [kStages][2 * kTilePairs]
     __shared__ __align__(8) uint64_t full_bar[kStages];
     // uniform over the grid: this variant runs iff the masses are (not) uniform and, diag_tiles > 0 (the diagonal
@@ -141,6 +149,7 @@ __global__ void __launch_bounds__(THREADS, MINB)
                                      : blockIdx.y * tiles_per_chunk;
     const int ntiles = min(diag_tiles > 0 ? diag_tiles : tiles_per_chunk, tiles_total - tile0);
     if (ntiles <= 0) return;   // uniform per CTA
+    if (diag_tiles > 0 && (tile0 / diag_tiles) % dg.world != dg.rank) return;   // another GPU's column block
 
     if (tid == 0) {
 #pragma unroll
@@ -228,6 +237,20 @@ __global__ void __launch_bounds__(THREADS, MINB)
         }
     }
 
+    if (diag_tiles > 0) {
+        const float scale = ctl->scale;
+        u64* const out64 = reinterpret_cast<u64*>(dg.acc64);
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            int i = ibase + k * THREADS + tid;
+            if (i < n) {
+                atomicAdd(out64 + 3 * (size_t)i + 0, (u64)__float2ll_rn(ox[k] * scale));
+                atomicAdd(out64 + 3 * (size_t)i + 1, (u64)__float2ll_rn(oy[k] * scale));
+                atomicAdd(out64 + 3 * (size_t)i + 2, (u64)__float2ll_rn(oz[k] * scale));
+            }
+        }
+        return;
+    }
     float4* __restrict__ out = part + (size_t)blockIdx.y * n;
 #pragma unroll
     for (int k = 0; k < I; ++k) {
@@ -236,22 +259,26 @@ __global__ void __launch_bounds__(THREADS, MINB)
     }
 }
 
-// acc[i] = G [m_0] * sum, in a fixed order (dx was r_j - r_i, so the sign of Eq. 4 is in).  One-sided path: the S chunk
-// partials s = 0..S-1.  Pair-symmetric path (ctl->sym): the fixed-point sums of gravity_sym.cu, exact integers
-// whatever the order they were added in, plus the diagonal-block partial in part[0].
+// acc[i] = G [m_0] * sum (dx was r_j - r_i, so the sign of Eq. 4 is in).  Two modes, each a no-op when the device chose the
+// other path.  SYM = false, one-sided path: the S chunk partials of the slice's targets, s = 0..S-1 in fixed order.
+// SYM = true, pair-symmetric path: the fixed-point sums acc64 — exact integers whatever the order, and whichever GPUs,
+// they were added by — for ALL n targets.
+template <bool SYM>
 __global__ void __launch_bounds__(256) grav_reduce(const float4* __restrict__ part, int i0, int n, int S, float G,
                                                    float4* __restrict__ acc, const float4* __restrict__ posm,
                                                    const long long* __restrict__ acc64,
                                                    const GravCtl* __restrict__ ctl) {
+    if ((ctl->sym != 0u) != SYM) return;
     int i = blockIdx.x * blockDim.x + threadIdx.x;   // slice-local target
     if (i >= n) return;
-    float4 a = part[i];
-    if (ctl->sym != 0u) {
+    float4 a;
+    if (SYM) {
         const double inv = ctl->inv_scale;
-        a.x = (float)((double)acc64[3 * (size_t)i + 0] * inv + (double)a.x);
-        a.y = (float)((double)acc64[3 * (size_t)i + 1] * inv + (double)a.y);
-        a.z = (float)((double)acc64[3 * (size_t)i + 2] * inv + (double)a.z);
+        a.x = (float)((double)acc64[3 * (size_t)i + 0] * inv);
+        a.y = (float)((double)acc64[3 * (size_t)i + 1] * inv);
+        a.z = (float)((double)acc64[3 * (size_t)i + 2] * inv);
     } else {
+        a = part[i];
         for (int s = 1; s < S; ++s) {
             float4 b = part[(size_t)s * n + i];
             a.x += b.x;
@@ -299,61 +326,63 @@ int grav_splits(int64_t n_total) {
 }
 
 template <int I, int THREADS, int MINB, bool ZERO_SOFT, int UNROLL, bool UNIFORM>
-static int launch_one(dim3 grid, const float4* targets, const float4* pk, int n, int tiles, int tpc, int diag_tiles,
+static int launch_one(dim3 grid, const float4* targets, const float4* pk, int n, int tiles, int tpc, const GravDiag& dg,
                       float eps2, float4* part, const GravCtl* ctl, cudaStream_t st) {
     const size_t smem = (size_t)kStages * kTileBytes;
     auto kfn = grav_pp_kernel<I, THREADS, MINB, ZERO_SOFT, UNROLL, UNIFORM>;
     SPHB_CUDA(cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kfn<<<grid, THREADS, smem, st>>>(targets, pk, n, tiles, tpc, diag_tiles, eps2, part, ctl);
+    kfn<<<grid, THREADS, smem, st>>>(targets, pk, n, tiles, tpc, dg, eps2, part, ctl);
     SPHB_LAUNCHED();
     return SPH_OK;
 }
 
-// both mass variants, back to back; at most one of them does the work (decided on the device).  diag_tiles > 0:
+// both mass variants, back to back; at most one of them does the work (decided on the device).  dg.tiles > 0:
 // only the diagonal column blocks, for the pair-symmetric path (uniform masses only).
 template <int I, int THREADS, int MINB, int UNROLL>
-static int launch_grav(const float4* targets, const float4* pk, int n, int tiles, int tpc, int S, int diag_tiles, float eps2,
-                       bool zero_soft, float4* part, const GravCtl* ctl, cudaStream_t st) {
+static int launch_grav(const float4* targets, const float4* pk, int n, int tiles, int tpc, int S, const GravDiag& dg,
+                       float eps2, bool zero_soft, float4* part, const GravCtl* ctl, cudaStream_t st) {
     dim3 grid((unsigned)cdiv(n, (int64_t)I * THREADS), (unsigned)S);
     if (zero_soft) {
-        SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, true>(grid, targets, pk, n, tiles, tpc, diag_tiles, eps2, part, ctl, st)));
-        if (diag_tiles == 0)
-            SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, false>(grid, targets, pk, n, tiles, tpc, 0, eps2, part, ctl, st)));
+        SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, true>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
+        if (dg.tiles == 0)
+            SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, false>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
     } else {
-        SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, true>(grid, targets, pk, n, tiles, tpc, diag_tiles, eps2, part, ctl, st)));
-        if (diag_tiles == 0)
-            SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, false>(grid, targets, pk, n, tiles, tpc, 0, eps2, part, ctl, st)));
+        SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, true>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
+        if (dg.tiles == 0)
+            SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, false>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
     }
     return SPH_OK;
 }
 
-// Targets [i0, i1) against all n_total sources (i0 = 0, i1 = n_total: the whole evaluation; a proper sub-range:
-// one GPU's share in the paper's N/k-per-GPU decomposition, L139).  Rows outside [i0, i1) of acc_grav are untouched.
-// The partial buffer holds grav_splits(n_total) * n_total float4; a slice may use more, shorter j-chunks (to keep
-// the grid many waves deep) as long as S * (i1 - i0) fits in it.
-int gravity(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, float G, float delta, float4* acc_grav,
-            float4* src_pk, float4* grav_part, long long* grav_acc64, unsigned int* grav_flag, cudaStream_t st) {
-    if (n_total <= 0 || i1 <= i0) return SPH_OK;
-    const int nt = (int)(i1 - i0);
+// One GPU's SHARE of an evaluation (rank of world; world = 1: all of it).  Whichever path the device chooses, the
+// share is complete after this call:
+//  * one-sided path: targets [i0, i1) against all n_total sources -> acc_grav rows [i0, i1), other rows untouched
+//    (i0 = 0, i1 = n_total: the whole evaluation; a proper sub-range: the paper's N/k-per-GPU decomposition, L139).
+//    The partial buffer holds grav_splits(n_total) * n_total float4; a slice may use more, shorter j-chunks (to keep
+//    the grid many waves deep) as long as S * (i1 - i0) fits in it.
+//  * pair-symmetric path (offered when `offer_sym`): work items rank, rank + world, ... and the diagonal blocks
+//    c = rank (mod world) -> fixed-point sums in grav_acc64 (zeroed here); acc_grav is not written.  The shares of the
+//    world's GPUs add up (an integer all-reduce) to the sums of the whole evaluation, bit for bit whatever the world size.
+// gravity_finish then turns the (all-reduced) sums into acc_grav rows [0, n_total) if that path was taken.
+int gravity_share(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, int rank, int world, bool offer_sym,
+                  float G, float delta, float4* acc_grav, float4* src_pk, float4* grav_part, long long* grav_acc64,
+                  unsigned int* grav_flag, cudaStream_t st) {
+    if (n_total <= 0) return SPH_OK;
+    const int nt = (int)(i1 > i0 ? i1 - i0 : 0);
+    GravCtl* ctl = reinterpret_cast<GravCtl*>(grav_flag);
     if (G == 0.0f) {   // no self-gravity (BASELINE config 4, "SPH-only"): Eq. 4 is identically 0
-        SPHB_CUDA(cudaMemsetAsync(acc_grav + i0, 0, (size_t)nt * sizeof(float4), st));
+        SPHB_CUDA(cudaMemsetAsync(ctl, 0, sizeof(GravCtl), st));   // path: one-sided, nothing for gravity_finish to do
+        if (nt > 0) SPHB_CUDA(cudaMemsetAsync(acc_grav + i0, 0, (size_t)nt * sizeof(float4), st));
         return SPH_OK;
     }
     const int n = (int)n_total;
     const int n_pad = (int)grav_padded(n_total);
-    int I, threads, S;
-    grav_shape(nt, n_total, I, threads, S);
-    const int64_t cap = (int64_t)grav_splits(n_total) * n_total / nt;   // chunks the partial buffer can hold
-    if (S > cap) S = (int)cap;
     const int tiles = n_pad / kGravTileSrc;
-    const int tpc = (int)cdiv(tiles, S);
-    S = (int)cdiv(tiles, tpc);
     const float eps2 = delta * delta;
     const bool zero_soft = !(eps2 > 0.f);
-    // The pair-symmetric path (gravity_sym.cu) is offered for a whole evaluation with softening at N >= kSymMinN;
-    // whether it is TAKEN (uniform masses, fixed-point range) is decided on the device by grav_plan.
-    const bool offer_sym = (i0 == 0 && i1 == n_total && !zero_soft && n_total >= kSymMinN);
-    GravCtl* ctl = reinterpret_cast<GravCtl*>(grav_flag);
+    // The pair-symmetric path (gravity_sym.cu) needs softening and N >= kSymMinN; whether it is TAKEN (uniform
+    // masses, fixed-point range) is decided on the device by grav_plan.
+    offer_sym = offer_sym && !zero_soft && n_total >= kSymMinN;
 
     SPHB_CUDA(cudaMemsetAsync(ctl, 0, sizeof(GravCtl), st));
     grav_pack_sources<<<(unsigned)cdiv(n_pad / 2, 256), 256, 0, st>>>(posm, n, n_pad, src_pk, ctl);
@@ -362,15 +391,43 @@ int gravity(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, float G
         SPHB_CUDA(cudaMemsetAsync(grav_acc64, 0, (size_t)n_pad * 3 * sizeof(long long), st));
         grav_plan<<<1, 32, 0, st>>>(ctl, n, n_pad, eps2);
         SPHB_LAUNCHED();
-        SPHB_TRY(gravity_sym_launch(posm, src_pk, n_pad, eps2, grav_acc64, ctl, st));
-        SPHB_TRY((launch_grav<8, 128, 2, 1>(posm, src_pk, nt, tiles, tpc, 1, kSymL / kGravTileSrc, eps2, false, grav_part, ctl, st)));
+        SPHB_TRY(gravity_sym_launch(posm, src_pk, n_pad, rank, world, eps2, grav_acc64, ctl, st));
+        const GravDiag dg = {kSymL / kGravTileSrc, rank, world, grav_acc64};
+        SPHB_TRY((launch_grav<8, 128, 2, 1>(posm, src_pk, n, tiles, tiles, 1, dg, eps2, false, grav_part, ctl, st)));
     }
+    if (nt == 0) return SPH_OK;
+    int I, threads, S;
+    grav_shape(nt, n_total, I, threads, S);
+    const int64_t cap = (int64_t)grav_splits(n_total) * n_total / nt;   // chunks the partial buffer can hold
+    if (S > cap) S = (int)cap;
+    const int tpc = (int)cdiv(tiles, S);
+    S = (int)cdiv(tiles, tpc);
+    const GravDiag none = {0, 0, 1, nullptr};
     if (I == 8)
-        SPHB_TRY((launch_grav<8, 128, 2, 1>(posm + i0, src_pk, nt, tiles, tpc, S, 0, eps2, zero_soft, grav_part, ctl, st)));
+        SPHB_TRY((launch_grav<8, 128, 2, 1>(posm + i0, src_pk, nt, tiles, tpc, S, none, eps2, zero_soft, grav_part, ctl, st)));
     else
-        SPHB_TRY((launch_grav<1, 128, 4, 2>(posm + i0, src_pk, nt, tiles, tpc, S, 0, eps2, zero_soft, grav_part, ctl, st)));
-    grav_reduce<<<(unsigned)cdiv(nt, 256), 256, 0, st>>>(grav_part, (int)i0, nt, S, G, acc_grav, posm, grav_acc64, ctl);
+        SPHB_TRY((launch_grav<1, 128, 4, 2>(posm + i0, src_pk, nt, tiles, tpc, S, none, eps2, zero_soft, grav_part, ctl, st)));
+    grav_reduce<false><<<(unsigned)cdiv(nt, 256), 256, 0, st>>>(grav_part, (int)i0, nt, S, G, acc_grav, posm, grav_acc64, ctl);
     SPHB_LAUNCHED();
+    return SPH_OK;
+}
+
+int gravity_finish(const float4* posm, int64_t n_total, float G, float4* acc_grav, const long long* grav_acc64,
+                   const unsigned int* grav_flag, cudaStream_t st) {
+    if (n_total <= 0 || G == 0.0f) return SPH_OK;
+    const GravCtl* ctl = reinterpret_cast<const GravCtl*>(grav_flag);
+    grav_reduce<true><<<(unsigned)cdiv(n_total, 256), 256, 0, st>>>(nullptr, 0, (int)n_total, 0, G, acc_grav, posm, grav_acc64, ctl);
+    SPHB_LAUNCHED();
+    return SPH_OK;
+}
+
+// The whole of a one-GPU call: targets [i0, i1); the pair-symmetric path is offered for a whole evaluation only.
+int gravity(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, float G, float delta, float4* acc_grav,
+            float4* src_pk, float4* grav_part, long long* grav_acc64, unsigned int* grav_flag, cudaStream_t st) {
+    if (n_total <= 0 || i1 <= i0) return SPH_OK;
+    const bool whole = (i0 == 0 && i1 == n_total);
+    SPHB_TRY(gravity_share(posm, n_total, i0, i1, 0, 1, whole, G, delta, acc_grav, src_pk, grav_part, grav_acc64, grav_flag, st));
+    if (whole) SPHB_TRY(gravity_finish(posm, n_total, G, acc_grav, grav_acc64, grav_flag, st));
     return SPH_OK;
 }
 

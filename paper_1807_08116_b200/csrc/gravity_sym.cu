@@ -19,7 +19,8 @@
 // Work decomposition.  Particles are cut into column blocks of L = 2048 (the packed source layout of
 // grav_pack_sources, one TMA bulk copy per block).  The pairs (i, j) with i < c L <= j < (c+1) L, i.e. block c
 // against ALL EARLIER particles, are cut into work items of at most `rows_per_item` rows; the diagonal blocks
-// (i, j in the same column block) go to the one-sided kernel (N x L interactions, 0.2 % at N = 2^20).  One CTA of
+// (i, j in the same column block) go to the one-sided kernel (N x L interactions, 0.2 % at N = 2^20), which adds its
+// FP32 sums into the same fixed-point accumulators.  One CTA of
 // 4 warps takes an item: all warps hold the SAME 32 I rows and each owns a quarter of the column block, so a source
 // belongs to exactly one warp (its sums live in that warp's shared-memory slots, no inter-warp traffic), and the
 // target sums of the 4 warps are added through shared memory once per row tile.  Items are handed out by an atomic
@@ -68,7 +69,8 @@ constexpr size_t kSymSmem = (size_t)kSymL * 16 + (size_t)kSymL * 12 + 4 * kSymRo
 
 __global__ void __launch_bounds__(kSymThreads, 2)
     grav_sym_kernel(const float4* __restrict__ posm, const float4* __restrict__ pk, int n_pad, int rows_per_item,
-                    int n_items, float eps2, long long* __restrict__ acc64, GravCtl* __restrict__ ctl) {
+                    int n_items, int share_rank, int share_world, float eps2, long long* __restrict__ acc64,
+                    GravCtl* __restrict__ ctl) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float4* spk = reinterpret_cast<float4*>(smem_raw);
     u64* sacc = reinterpret_cast<u64*>(smem_raw + (size_t)kSymL * 16);
@@ -91,8 +93,9 @@ __global__ void __launch_bounds__(kSymThreads, 2)
     for (;;) {
         if (tid == 0) s_item = atomicAdd(&ctl->counter, 1u);
         __syncthreads();
-        const unsigned int item = s_item;
-        if (item >= (unsigned int)n_items) break;
+        // one GPU's share of the evaluation (NEXT-4): items rank, rank + world, ... ; all of them if world == 1
+        const unsigned int item = s_item * (unsigned int)share_world + (unsigned int)share_rank;
+        if (s_item >= (unsigned int)n_items || item >= (unsigned int)n_items) break;
         // item -> (column block c >= 1, run): block c has ceil(c L / rows_per_item) runs of rows below c L
         int c = 1, run = (int)item;
         for (;; ++c) {
@@ -195,8 +198,8 @@ static int sym_rows_per_item(int64_t ncols, int slots) {
     return rpi;
 }
 
-int gravity_sym_launch(const float4* posm, const float4* src_pk, int n_pad, float eps2, long long* acc64,
-                       GravCtl* ctl, cudaStream_t st) {
+int gravity_sym_launch(const float4* posm, const float4* src_pk, int n_pad, int share_rank, int share_world, float eps2,
+                       long long* acc64, GravCtl* ctl, cudaStream_t st) {
     static int occ = 0;
     if (occ == 0) {
         SPHB_CUDA(cudaFuncSetAttribute(grav_sym_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSymSmem));
@@ -208,9 +211,11 @@ int gravity_sym_launch(const float4* posm, const float4* src_pk, int n_pad, floa
     const int rpi = sym_rows_per_item(ncols, slots);
     int64_t items = 0;
     for (int64_t c = 1; c < ncols; ++c) items += cdiv(c * kSymL, rpi);
-    if (items <= 0) return SPH_OK;
-    const unsigned grid = (unsigned)(items < slots ? items : slots);
-    grav_sym_kernel<<<grid, kSymThreads, kSymSmem, st>>>(posm, src_pk, n_pad, rpi, (int)items, eps2, acc64, ctl);
+    const int64_t mine = items > share_rank ? cdiv(items - share_rank, share_world) : 0;   // this rank's items
+    if (mine <= 0) return SPH_OK;
+    const unsigned grid = (unsigned)(mine < slots ? mine : slots);
+    grav_sym_kernel<<<grid, kSymThreads, kSymSmem, st>>>(posm, src_pk, n_pad, rpi, (int)items, share_rank, share_world, eps2,
+                                                         acc64, ctl);
     SPHB_LAUNCHED();
     return SPH_OK;
 }

@@ -42,6 +42,7 @@ Workspace carve(void* base, int64_t n_gas, int64_t n_total, const sph_grid* g) {
     w.h_s = (float*)take(ng * 4);
     w.src_pk = (float4*)take((size_t)grav_padded(n_total) * 16);
     w.grav_part = (float4*)take((size_t)grav_splits(n_total) * nt * 16);
+    w.grav_acc64_off = off;
     w.grav_acc64 = (long long*)take((size_t)grav_padded(n_total) * 3 * sizeof(long long));
     w.grav_flag = (unsigned int*)take(256);
     w.vele0 = (float4*)take(nt * 16);

@@ -1,12 +1,17 @@
 """N/k-per-GPU decomposition of the step, one process per GPU.
 
 The paper gives each of k GPUs N/k particles and, before the gravity kernel, copies the other GPUs' particles
-over GPU-Direct (L139).  Here every rank keeps the whole state (64 B per particle: nothing at 180 GB per GPU),
-computes the O(N^2) gravity stage only for its own TARGET slice against all N sources
-(`sph_position_slice`), and the ranks exchange the acceleration slices with ONE all-gather per force
-evaluation (16 B x N/k per rank over NCCL / NVLink: 16 MiB in total at N = 2^20 against ~0.4 s / k of gravity,
-so there is nothing to gain from fusing it into the kernel).  The O(N) and SPH stages (0.1 % of the step) run
-redundantly on every rank; they are deterministic, so the replicas stay bitwise identical and no other
+over GPU-Direct (L139).  Here every rank keeps the whole state (64 B per particle: nothing at 180 GB per GPU) and
+computes its SHARE of the O(N^2) gravity stage (`sph_position_share`).  Which gravity kernel runs is decided on the
+device, so a share has two forms and both exchanges are issued every evaluation (41 MiB in total at N = 2^20 against
+~0.26 s / k of gravity, so there is nothing to gain from fusing them into the kernel):
+  * pair-symmetric path (equal masses — every BASELINE.json config): the rank's work items of the unordered-pair
+    decomposition, accumulated as 64-bit fixed-point integers; ONE integer SUM all-reduce of that region.  Integer
+    addition is exact, so every world size gives the same bits as one GPU.
+  * one-sided path (unequal masses, delta = 0, ...): the rank's TARGET slice against all N sources; ONE all-gather of
+    the acceleration slices.
+`nbody_pp_gravity_finish` then writes the accelerations from whichever applies.  The O(N) and SPH stages (0.2 % of
+the step) run redundantly on every rank; they are deterministic, so the replicas stay bitwise identical and no other
 exchange is needed.
 
 This module holds no arithmetic of the method: slice bookkeeping, buffers and the collective.
@@ -30,6 +35,14 @@ def slice_bounds(n: int, rank: int, world: int, align: int = SLICE_ALIGN):
     i0 = min(rank * chunk, n)
     i1 = min(i0 + chunk, n)
     return i0, i1, chunk
+
+
+def allreduce_sums(sums: torch.Tensor, world: int, group=None) -> None:
+    """Integer SUM all-reduce of the fixed-point sums (int64; NCCL on the GPUs, gloo in the CPU tests)."""
+    if world == 1 and not dist.is_initialized():
+        return
+    assert sums.dtype == torch.int64 and sums.is_contiguous()
+    dist.all_reduce(sums, op=dist.ReduceOp.SUM, group=group)
 
 
 def allgather_rows(full: torch.Tensor, rank: int, world: int, chunk: int, group=None) -> None:
@@ -60,6 +73,7 @@ class ShardedSimulation:
         self.acc_grav = torch.zeros(world * self.chunk, 4, dtype=torch.float32, device="cuda")
         self.grid = b.sph_grid_from_bbox(self.posm, self.n_gas, w.h) if self.n_gas > 0 else None
         self.ws = b.alloc_workspace(self.n_gas, self.n, self.grid)
+        self.sums = b.gravity_sums_view(self.ws, self.n_gas, self.n, self.grid)   # int64 view, all-reduced each evaluation
         self.sigma = sigma
         self.hsml = None
         if sigma is not None and self.n_gas > 0:
@@ -67,9 +81,12 @@ class ShardedSimulation:
         self.first = True
 
     def _position(self, sigma):
-        self.b.sph_position_slice(self.posm, self.hsml, sigma, self.n_gas, self.n_halo, self.i0, self.i1, self.params,
-                                  self.grid, self.rho, self.acc_grav, self.ws)
-        allgather_rows(self.acc_grav, self.rank, self.world, self.chunk, self.group)
+        b = self.b
+        b.sph_position_share(self.posm, self.hsml, sigma, self.n_gas, self.n_halo, self.rank, self.world, self.i0, self.i1,
+                             self.params, self.grid, self.rho, self.acc_grav, self.ws)
+        allreduce_sums(self.sums, self.world, self.group)                       # pair-symmetric path
+        allgather_rows(self.acc_grav, self.rank, self.world, self.chunk, self.group)   # one-sided path
+        b.nbody_pp_gravity_finish(self.posm, self.n_gas, self.n_halo, self.grid, self.params.G, self.acc_grav, self.ws)
 
     def step(self, dt=None):
         dt = self.w.dt if dt is None else dt

@@ -104,3 +104,32 @@ def test_allgather_rows_gloo_world2():
     rows = np.arange(2500, dtype=np.float32)
     expect = np.stack([rows, 2 * rows, 3 * rows, np.zeros_like(rows)], 1)
     assert np.array_equal(out[0], expect) and np.array_equal(out[1], expect)     # every rank holds every row
+
+
+def _reduce_worker(rank, world, port, out):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    from paper_1807_08116_b200.sharded import allreduce_sums
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        # "my share of the fixed-point sums": values near +-2^62 so that a float detour would lose bits, and
+        # wrap-around (two's complement) must behave like the device's unsigned adds
+        base = torch.arange(3 * 2048, dtype=torch.int64)
+        mine = (base * 1315423911 + (2 ** 61 + 12345) * (1 if rank == 0 else -1)) * (rank + 1)
+        allreduce_sums(mine, world)
+        out[rank] = mine.clone().numpy()
+    finally:
+        dist.destroy_process_group()
+
+
+def test_allreduce_sums_gloo_world2():
+    """The exchange of the pair-symmetric path: an exact int64 SUM, identical on every rank."""
+    import numpy as np
+    world, port = 2, _free_port()
+    mgr = mp.Manager()
+    out = mgr.dict()
+    mp.spawn(_reduce_worker, args=(world, port, out), nprocs=world, join=True)
+    base = np.arange(3 * 2048, dtype=np.int64)
+    with np.errstate(over="ignore"):
+        expect = (base * 1315423911 + (2 ** 61 + 12345)) * 1 + (base * 1315423911 - (2 ** 61 + 12345)) * 2
+    assert np.array_equal(out[0], expect) and np.array_equal(out[1], expect)

@@ -580,33 +580,46 @@ def test_gravity_slices_equal_full(cuda_lib):
         b.nbody_pp_gravity_slice(d, n, 10, n + 1, w.G, w.delta, acc, ws)
 
 
-def test_staged_step_two_slices_sequential(cuda_lib):
-    """Two replicas of the state, each doing the gravity of its own slice, exchanging acc_grav by a plain copy
-    between the stages (what the all-gather does), run one after the other on this one GPU: both replicas must
-    stay bitwise identical and match the single-GPU step."""
+def _exchange(reps):
+    """What the two collectives of sharded.py do, by plain copies on one GPU: integer SUM of the fixed-point sums
+    (all-reduce) and every replica receiving every acceleration slice (all-gather)."""
+    total = sum(s.sums.clone() for s in reps)
+    for s in reps:
+        s.sums.copy_(total)
+    for s in reps:
+        for o in reps:
+            if o is not s:
+                s.acc_grav[o.i0:o.i1] = o.acc_grav[o.i0:o.i1]
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_staged_step_shares_sequential(cuda_lib, world):
+    """`world` replicas of the state, each doing its own SHARE of the gravity evaluation, run one after the other on
+    this one GPU with the exchange done by copies: the replicas must stay bitwise identical and — the pair-symmetric
+    path accumulates integers — reproduce the single-GPU step BIT FOR BIT."""
     b = cuda_lib
-    from paper_1807_08116_b200.sharded import ShardedSimulation, slice_bounds
+    from paper_1807_08116_b200.sharded import ShardedSimulation
     w = wl.make_workload(1, scale=0.75)
     n, ng, nh = w.n_total, w.n_gas, w.n_halo
     ref = b.Simulation(w)
     ref.step()
     ref.step()
+    assert b.sph_gravity_path(ref.ws, ng, n, ref.grid) == "pair_symmetric"
     # world = 1 through the class (same calls, no collective): bit for bit the plain step
     one = ShardedSimulation(w, 0, 1)
     one.step()
     one.step()
     for x, y in ((one.posm, ref.posm), (one.vele, ref.vele), (one.rho, ref.rho), (one.acc_grav[:n], ref.acc_grav)):
         assert torch.equal(x, y)
-    world = 2
     reps = [ShardedSimulation(w, r, world) for r in range(world)]
 
     def position(sigma):
         for s in reps:
-            b.sph_position_slice(s.posm, s.hsml, sigma, ng, nh, s.i0, s.i1, s.params, s.grid, s.rho, s.acc_grav, s.ws)
-        for s in reps:                                    # the exchange: every replica receives every slice
-            for o in reps:
-                if o is not s:
-                    s.acc_grav[o.i0:o.i1] = o.acc_grav[o.i0:o.i1]
+            b.sph_position_share(s.posm, s.hsml, sigma, ng, nh, s.rank, world, s.i0, s.i1, s.params, s.grid, s.rho,
+                                 s.acc_grav, s.ws)
+        _exchange(reps)
+        for s in reps:
+            b.nbody_pp_gravity_finish(s.posm, ng, nh, s.grid, s.params.G, s.acc_grav, s.ws)
 
     position(0.0)
     for _ in range(2):
@@ -615,12 +628,57 @@ def test_staged_step_two_slices_sequential(cuda_lib):
         position(0.0)
         for s in reps:
             b.sph_correct(s.vele, s.hsml, ng, nh, s.params, s.grid, w.dt, s.rho, s.acc_sph, s.acc_grav, s.ws)
-    a, c = reps
-    for x, y in ((a.posm, c.posm), (a.vele, c.vele), (a.rho, c.rho), (a.acc_sph, c.acc_sph), (a.acc_grav, c.acc_grav)):
-        assert torch.equal(x, y)
-    assert (a.posm - ref.posm).abs().max().item() < 1e-6
-    check_values(a.vele.cpu().numpy()[:, :3], ref.vele.cpu().numpy()[:, :3].astype(np.float64), "v sliced vs single",
-                 max_tol=2e-6, med_tol=2e-7)
+    for c in reps:
+        for x, y in ((c.posm, ref.posm), (c.vele, ref.vele), (c.rho, ref.rho), (c.acc_sph, ref.acc_sph),
+                     (c.acc_grav[:n], ref.acc_grav)):
+            assert torch.equal(x, y)
+
+
+@pytest.mark.parametrize("masses", ["equal", "random"])
+def test_gravity_shares_add_up(cuda_lib, masses):
+    """nbody_pp_gravity_share over 3 ranks + the exchange + nbody_pp_gravity_finish against the one-call evaluation:
+    equal masses (pair-symmetric path, integer sums) bit for bit; unequal masses (one-sided slices) to rounding;
+    a rank's share call must not touch acceleration rows outside its slice."""
+    b = cuda_lib
+    from paper_1807_08116_b200.sharded import slice_bounds
+    w = wl.make_workload(1, scale=45001 / 2 ** 17)
+    n = w.n_total
+    posm = w.posm.copy()
+    if masses == "random":
+        rng = np.random.Generator(np.random.Philox(key=[5, 9]))
+        posm[:, 3] = ((0.2 + rng.random(n)) / n).astype(np.float32)
+    d = _t(posm)
+    ws = b.alloc_workspace(0, n)
+    full = torch.zeros((n, 4), device="cuda")
+    b.nbody_pp_gravity(d, n, w.G, w.delta, full, ws)
+    path = b.sph_gravity_path(ws, 0, n)
+    assert path == ("pair_symmetric" if masses == "equal" else "one_sided")
+    world = 3
+    sums_view = b.gravity_sums_view(ws, 0, n)
+    acc = torch.full((n, 4), 7.0, device="cuda")
+    total = torch.zeros_like(sums_view)
+    for r in range(world):
+        i0, i1, _ = slice_bounds(n, r, world)
+        before = acc.clone()
+        b.nbody_pp_gravity_share(d, n, r, world, i0, i1, w.G, w.delta, acc, ws)
+        assert b.sph_gravity_path(ws, 0, n) == path
+        assert torch.equal(acc[:i0], before[:i0]) and torch.equal(acc[i1:], before[i1:])
+        if masses == "equal":
+            assert torch.equal(acc, before)               # the pair-symmetric share writes only the sums
+            total += sums_view
+    if masses == "equal":
+        assert 0 < torch.count_nonzero(sums_view).item()
+        sums_view.copy_(total)
+    b.nbody_pp_gravity_finish(d, 0, n, None, w.G, acc, ws)
+    if masses == "equal":
+        assert torch.equal(acc, full)
+    else:
+        err = (acc[:, :3] - full[:, :3]).norm(dim=1) / full[:, :3].norm(dim=1).clamp_min(1e-3)
+        assert err.max().item() < 2e-5
+    tg = np.arange(0, n, 89)
+    check_values(acc.cpu().numpy()[tg, :3], oracle.gravity(posm, w.G, w.delta, targets=tg), f"a_grav 3 shares {masses}")
+    with pytest.raises(b.SphError):
+        b.nbody_pp_gravity_share(d, n, 3, 3, 0, n, w.G, w.delta, acc, ws)      # rank outside [0, world)
 
 
 @pytest.mark.parametrize("masses", ["equal", "one_differs_last", "one_differs_first", "random", "equal_zero"])
