@@ -313,7 +313,8 @@ def run_ours(args, w):
         achieved = FLOPS_PER_INTERACTION * float(n_slice) * float(n) / (grav_ms * 1e-3) / 1e12   # per GPU (rank 0's slice)
         path = b.sph_gravity_path(sim.ws, ng, n, sim.grid)           # chosen on the device
         # FP32 lane-operations the variant really executes per INTERACTION (an FMA counted once) and its dominant kernel
-        kernel, ops = {"pair_symmetric": ("grav_sym_kernel", 7.0), "one_sided_uniform": ("grav_pp_kernel", 11.0),
+        kernel, ops = {"pair_symmetric": ("grav_sym_kernel", 7.0), "pair_symmetric_general": ("grav_sym_kernel", 8.0),
+                       "one_sided_uniform": ("grav_pp_kernel", 11.0),
                        "one_sided": ("grav_pp_kernel", 12.0)}[path]
         tr = ncu_traffic(kernel)
         traffic = tr["bytes"] if tr and tr["n_total"] == n else None   # the capture is of this workload only

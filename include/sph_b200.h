@@ -238,7 +238,7 @@ int sph_position_slice(const float* posm, float* hsml /*or NULL*/, float sigma, 
  * decided on the device, so the share has two forms and the caller exchanges BOTH before calling the finish:
  *   - one-sided path: targets [i0, i1) against all sources -> acc_grav rows [i0, i1) (other rows untouched);
  *     exchange = all-gather of the row slices;
- *   - pair-symmetric path (equal masses, delta > 0, N >= 32768, fixed-point range fits): the work items
+ *   - pair-symmetric path (delta > 0, N >= 32768, positive masses, fixed-point range fits): the work items
  *     rank, rank + world, ... of the unordered-pair decomposition -> 64-bit fixed-point sums in the workspace region
  *     sph_workspace_gravity_sums() reports (zeroed by this call; acc_grav not written);
  *     exchange = integer SUM all-reduce of that region (exact: the result is bit for bit the same for every world size).
@@ -279,10 +279,12 @@ int sph_get_stage_ms(float out_ms[5] /*HOST*/);
 
 /* Diagnostic: which variant of the gravity kernel the LAST evaluation enqueued with workspace `ws` (sized for n_gas,
  * n_total and g, as in that call) took.  The choice is made on the device, so this reads the
- * 32-byte control block back and SYNCHRONISES `stream`.  *path_host = SPH_GRAV_ONE_SIDED (unequal masses),
- * SPH_GRAV_ONE_SIDED_UNIFORM (equal masses: m_j leaves the loop) or SPH_GRAV_PAIR_SYMMETRIC (equal masses, every
- * unordered pair evaluated once, fixed-point accumulation).  Eq. 4.                              */
-enum { SPH_GRAV_ONE_SIDED = 0, SPH_GRAV_ONE_SIDED_UNIFORM = 1, SPH_GRAV_PAIR_SYMMETRIC = 2 };
+ * control block back and SYNCHRONISES `stream`.  One-sided: every ordered interaction evaluated (target slices,
+ * delta = 0, N < 32768, non-positive masses, or a fixed-point range that would be too coarse); pair-symmetric: every
+ * unordered pair evaluated once with fixed-point accumulation.  _UNIFORM / plain PAIR_SYMMETRIC: all masses equal
+ * (m_j leaves the loop).  Eq. 4.                                                                   */
+enum { SPH_GRAV_ONE_SIDED = 0, SPH_GRAV_ONE_SIDED_UNIFORM = 1, SPH_GRAV_PAIR_SYMMETRIC = 2,
+       SPH_GRAV_PAIR_SYMMETRIC_GENERAL = 3 };
 int sph_gravity_path(const void* ws /*DEVICE*/, size_t ws_bytes, int64_t n_gas, int64_t n_total,
                      const sph_grid* g /*HOST, may be NULL if n_gas == 0*/, int* path_host /*HOST*/, void* stream);
 

@@ -384,7 +384,7 @@ def sph_get_stage_ms() -> dict:
     return dict(zip(STAGES, [float(x) for x in out]))
 
 
-GRAV_PATHS = ("one_sided", "one_sided_uniform", "pair_symmetric")
+GRAV_PATHS = ("one_sided", "one_sided_uniform", "pair_symmetric", "pair_symmetric_general")
 
 
 def sph_gravity_path(ws, n_gas, n_total, grid=None) -> str:

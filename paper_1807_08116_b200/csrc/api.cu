@@ -259,7 +259,8 @@ int sph_gravity_path(const void* ws, size_t ws_bytes, int64_t n_gas, int64_t n_t
     cudaStream_t st = (cudaStream_t)stream;
     SPHB_CUDA(cudaMemcpyAsync(ctl, w.grav_flag, sizeof(ctl), cudaMemcpyDeviceToHost, st));
     SPHB_CUDA(cudaStreamSynchronize(st));
-    *path_host = ctl[0] != 0u ? SPH_GRAV_ONE_SIDED : (ctl[1] != 0u ? SPH_GRAV_PAIR_SYMMETRIC : SPH_GRAV_ONE_SIDED_UNIFORM);
+    *path_host = ctl[1] != 0u ? (ctl[0] != 0u ? SPH_GRAV_PAIR_SYMMETRIC_GENERAL : SPH_GRAV_PAIR_SYMMETRIC)
+                              : (ctl[0] != 0u ? SPH_GRAV_ONE_SIDED : SPH_GRAV_ONE_SIDED_UNIFORM);
     return SPH_OK;
 }
 

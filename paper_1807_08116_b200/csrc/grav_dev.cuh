@@ -78,12 +78,13 @@ __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, u
 // block selects.  No host read-back anywhere.
 struct GravCtl {
     unsigned int nonuniform;   // != 0: the masses are not all equal to m_0
-    unsigned int sym;          // != 0: the pair-symmetric path applies (uniform masses, fixed-point range fits)
+    unsigned int sym;          // != 0: the pair-symmetric path applies (delta > 0, positive masses, fixed-point range fits)
     unsigned int counter;      // work-item counter of the persistent pair-symmetric kernel
     float scale;               // fixed-point scale 2^k of the int64 accumulators
     double inv_scale;          // 2^-k
     unsigned int bmin_c[3];    // bounding box of all particles: max over particles of ~ord(x) (so 0 = empty)
     unsigned int bmax[3];      // max over particles of ord(x); ord() maps floats to order-preserving unsigned
+    unsigned int mmin_c, mmax; // the same for the masses: max of ~ord(m), max of ord(m)
 };
 static_assert(sizeof(GravCtl) <= 256, "GravCtl must fit the workspace slot");
 

@@ -46,13 +46,14 @@ __global__ void __launch_bounds__(256) grav_pack_sources(const float4* __restric
     const float m0 = posm[0].w;
     float4 a = make_float4(kPadCoord, kPadCoord, kPadCoord, 0.f), b = a;
     bool differs = false;
-    unsigned int lo[3] = {0xffffffffu, 0xffffffffu, 0xffffffffu}, hi[3] = {0u, 0u, 0u};
+    unsigned int lo[4] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu}, hi[4] = {0u, 0u, 0u, 0u};   // x, y, z, m
     if (live && 2 * q < n) {
         a = posm[2 * q];
         differs = a.w != m0;
         lo[0] = hi[0] = ford(a.x);
         lo[1] = hi[1] = ford(a.y);
         lo[2] = hi[2] = ford(a.z);
+        lo[3] = hi[3] = ford(a.w);
     }
     if (live && 2 * q + 1 < n) {
         b = posm[2 * q + 1];
@@ -60,44 +61,47 @@ __global__ void __launch_bounds__(256) grav_pack_sources(const float4* __restric
         lo[0] = min(lo[0], ford(b.x)), hi[0] = max(hi[0], ford(b.x));
         lo[1] = min(lo[1], ford(b.y)), hi[1] = max(hi[1], ford(b.y));
         lo[2] = min(lo[2], ford(b.z)), hi[2] = max(hi[2], ford(b.z));
+        lo[3] = min(lo[3], ford(b.w)), hi[3] = max(hi[3], ford(b.w));
     }
     if (live) {
         pk[2 * q] = make_float4(a.x, b.x, a.y, b.y);
         pk[2 * q + 1] = make_float4(a.z, b.z, a.w, b.w);
     }
-    // block reduction: nonuniform flag and bounding box, then 7 atomics per block at most
-    __shared__ unsigned int s_lo[3][8], s_hi[3][8], s_diff;
+    // block reduction: nonuniform flag, bounding box and mass range, then 9 atomics per block at most
+    __shared__ unsigned int s_lo[4][8], s_hi[4][8], s_diff;
     if (threadIdx.x == 0) s_diff = 0u;
     __syncthreads();
     const unsigned int any = __ballot_sync(0xffffffffu, differs);
 #pragma unroll
-    for (int d = 0; d < 3; ++d) {
+    for (int d = 0; d < 4; ++d) {
         lo[d] = __reduce_min_sync(0xffffffffu, lo[d]);
         hi[d] = __reduce_max_sync(0xffffffffu, hi[d]);
     }
     if ((threadIdx.x & 31) == 0) {
         if (any != 0u) s_diff = 1u;
 #pragma unroll
-        for (int d = 0; d < 3; ++d) s_lo[d][threadIdx.x >> 5] = lo[d], s_hi[d][threadIdx.x >> 5] = hi[d];
+        for (int d = 0; d < 4; ++d) s_lo[d][threadIdx.x >> 5] = lo[d], s_hi[d][threadIdx.x >> 5] = hi[d];
     }
     __syncthreads();
-    if (threadIdx.x < 3) {
+    if (threadIdx.x < 4) {
         const int d = threadIdx.x;
         unsigned int l = s_lo[d][0], h = s_hi[d][0];
         for (int w = 1; w < 8; ++w) l = min(l, s_lo[d][w]), h = max(h, s_hi[d][w]);
         if (h != 0u) {   // the block held at least one real particle
-            atomicMax(&ctl->bmin_c[d], ~l);
-            atomicMax(&ctl->bmax[d], h);
+            atomicMax(d < 3 ? &ctl->bmin_c[d] : &ctl->mmin_c, ~l);
+            atomicMax(d < 3 ? &ctl->bmax[d] : &ctl->mmax, h);
         }
-    } else if (threadIdx.x == 3 && s_diff != 0u) {
+    } else if (threadIdx.x == 4 && s_diff != 0u) {
         atomicOr(&ctl->nonuniform, 1u);
     }
 }
 
 // Decides, on the device, whether the pair-symmetric kernel (gravity_sym.cu) takes this evaluation and with which
-// fixed-point scale.  Largest possible |sum_j d w| is n_pad * max_r r/(r^2+delta^2)^(3/2) = 0.385 n_pad/delta^2;
-// 2^k times twice that must stay below 2^62.  The path is taken when the masses are uniform and the resolution
-// 2^-k is finer than 2^-26 of n/R^2, R = diagonal of the bounding box (the natural size of a particle's sum).
+// fixed-point scale.  The kernels sum w d (equal masses: m_0 is applied afterwards) or m w d; the largest possible
+// |sum| is n_pad * m_max * max_r r/(r^2+delta^2)^(3/2) = 0.385 n_pad m_max/delta^2 (m_max := 1 for equal masses), and
+// 2^k times twice that must stay below 2^62.  The path is taken when the masses are positive and the resolution 2^-k
+// is finer than 2^-26 of n m_min/R^2, R = diagonal of the bounding box (the natural size of a particle's sum; m_min
+// makes the rule conservative when the masses differ widely).
 __global__ void grav_plan(GravCtl* ctl, int n, int n_pad, float eps2) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     double R2 = 0.0;
@@ -105,15 +109,19 @@ __global__ void grav_plan(GravCtl* ctl, int n, int n_pad, float eps2) {
         const double e = (double)ford_inv(ctl->bmax[d]) - (double)ford_inv(~ctl->bmin_c[d]);
         R2 += e * e;
     }
-    const double bound = 2.0 * 0.385 * (double)n_pad / (double)eps2;
+    const bool uniform = ctl->nonuniform == 0u;
+    const double mmax = uniform ? 1.0 : (double)ford_inv(ctl->mmax);
+    const double mmin = uniform ? 1.0 : (double)ford_inv(~ctl->mmin_c);
+    const bool masses_ok = uniform || (mmin > 0.0 && mmax < 1.0e30);
+    const double bound = 2.0 * 0.385 * (double)n_pad * (masses_ok ? mmax : 1.0) / (double)eps2;
     int k = 62 - (int)ceil(log2(bound));
     if (k > 100) k = 100;      // 2^k and products with FP32 partials stay far inside the FP32 range
     if (k < -100) k = -100;
     const double res = ldexp(1.0, -k);
-    const bool fine = res * R2 <= ldexp((double)n, -26) || R2 == 0.0;
+    const bool fine = res * R2 <= ldexp((double)n * mmin, -26) || R2 == 0.0;
     ctl->scale = (float)ldexp(1.0, k);
     ctl->inv_scale = res;
-    ctl->sym = (ctl->nonuniform == 0u && fine) ? 1u : 0u;
+    ctl->sym = (masses_ok && fine) ? 1u : 0u;
 }
 
 constexpr int kTilePairs = kGravTileSrc / 2;           // 1024 source pairs = 32 KB per stage
@@ -337,19 +345,17 @@ static int launch_one(dim3 grid, const float4* targets, const float4* pk, int n,
 }
 
 // both mass variants, back to back; at most one of them does the work (decided on the device).  dg.tiles > 0:
-// only the diagonal column blocks, for the pair-symmetric path (uniform masses only).
+// only the diagonal column blocks, for the pair-symmetric path.
 template <int I, int THREADS, int MINB, int UNROLL>
 static int launch_grav(const float4* targets, const float4* pk, int n, int tiles, int tpc, int S, const GravDiag& dg,
                        float eps2, bool zero_soft, float4* part, const GravCtl* ctl, cudaStream_t st) {
     dim3 grid((unsigned)cdiv(n, (int64_t)I * THREADS), (unsigned)S);
     if (zero_soft) {
         SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, true>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
-        if (dg.tiles == 0)
-            SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, false>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
+        SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, false>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
     } else {
         SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, true>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
-        if (dg.tiles == 0)
-            SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, false>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
+        SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, false>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
     }
     return SPH_OK;
 }

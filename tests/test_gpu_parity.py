@@ -634,25 +634,29 @@ def test_staged_step_shares_sequential(cuda_lib, world):
             assert torch.equal(x, y)
 
 
-@pytest.mark.parametrize("masses", ["equal", "random"])
+@pytest.mark.parametrize("masses", ["equal", "random", "zero_mass"])
 def test_gravity_shares_add_up(cuda_lib, masses):
     """nbody_pp_gravity_share over 3 ranks + the exchange + nbody_pp_gravity_finish against the one-call evaluation:
-    equal masses (pair-symmetric path, integer sums) bit for bit; unequal masses (one-sided slices) to rounding;
-    a rank's share call must not touch acceleration rows outside its slice."""
+    equal and unequal positive masses (pair-symmetric path, integer sums) bit for bit; a massless particle among
+    unequal masses (one-sided slices) to rounding; a rank's share call must not touch acceleration rows outside its
+    slice."""
     b = cuda_lib
     from paper_1807_08116_b200.sharded import slice_bounds
     w = wl.make_workload(1, scale=45001 / 2 ** 17)
     n = w.n_total
     posm = w.posm.copy()
-    if masses == "random":
+    if masses != "equal":
         rng = np.random.Generator(np.random.Philox(key=[5, 9]))
         posm[:, 3] = ((0.2 + rng.random(n)) / n).astype(np.float32)
+    if masses == "zero_mass":
+        posm[n // 2, 3] = 0.0
     d = _t(posm)
+    sym = masses != "zero_mass"
     ws = b.alloc_workspace(0, n)
     full = torch.zeros((n, 4), device="cuda")
     b.nbody_pp_gravity(d, n, w.G, w.delta, full, ws)
     path = b.sph_gravity_path(ws, 0, n)
-    assert path == ("pair_symmetric" if masses == "equal" else "one_sided")
+    assert path == ("pair_symmetric" if masses == "equal" else "pair_symmetric_general" if masses == "random" else "one_sided")
     world = 3
     sums_view = b.gravity_sums_view(ws, 0, n)
     acc = torch.full((n, 4), 7.0, device="cuda")
@@ -663,14 +667,14 @@ def test_gravity_shares_add_up(cuda_lib, masses):
         b.nbody_pp_gravity_share(d, n, r, world, i0, i1, w.G, w.delta, acc, ws)
         assert b.sph_gravity_path(ws, 0, n) == path
         assert torch.equal(acc[:i0], before[:i0]) and torch.equal(acc[i1:], before[i1:])
-        if masses == "equal":
+        if sym:
             assert torch.equal(acc, before)               # the pair-symmetric share writes only the sums
             total += sums_view
-    if masses == "equal":
+    if sym:
         assert 0 < torch.count_nonzero(sums_view).item()
         sums_view.copy_(total)
     b.nbody_pp_gravity_finish(d, 0, n, None, w.G, acc, ws)
-    if masses == "equal":
+    if sym:
         assert torch.equal(acc, full)
     else:
         err = (acc[:, :3] - full[:, :3]).norm(dim=1) / full[:, :3].norm(dim=1).clamp_min(1e-3)
@@ -771,7 +775,17 @@ def test_gravity_path_selection(cuda_lib):
     check(w.posm, w.delta, "pair_symmetric", "equal masses")
     p = w.posm.copy()
     p[n - 1, 3] *= 2.0
-    check(p, w.delta, "one_sided", "one mass differs")
+    check(p, w.delta, "pair_symmetric_general", "one mass differs")
+    rng = np.random.Generator(np.random.Philox(key=[33, 1]))
+    p = w.posm.copy()
+    p[:, 3] = ((0.2 + rng.random(n)) / n).astype(np.float32)
+    check(p, w.delta, "pair_symmetric_general", "random masses")
+    check(p, 0.0, "one_sided", "random masses, delta = 0", max_tol=5e-4, med_tol=2e-5)
+    p[17, 3] = 0.0                               # a massless particle: m_min = 0, no scale for the fixed-point range
+    check(p, w.delta, "one_sided", "a zero mass")
+    p = w.posm.copy()
+    p[::2, 3] *= 1.0e9                           # masses differing by 10^9: 2^-k against n m_min / R^2 too coarse
+    check(p, w.delta, "one_sided", "mass ratio 1e9")
     p = w.posm.copy()
     p[5, :3] = (3.0e4, 0.0, 0.0)                 # box diagonal / delta = 6e6: 2^-k would be > 2^-26 of n / R^2
     check(p, w.delta, "one_sided_uniform", "far-away particle")
