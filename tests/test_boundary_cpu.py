@@ -56,3 +56,19 @@ def test_sass_is_blackwell_native():
     assert "sm_100a" in sass
     for mnem in ("FFMA2", "FADD2", "FMUL2", "MUFU.RSQ", "UBLKCP"):
         assert mnem in sass, mnem
+
+
+def test_gravity_sums_region_without_gpu():
+    """sph_workspace_gravity_sums (host-only): the int64 region of the pair-symmetric path lies inside the workspace,
+    256-byte aligned, 24 bytes per source padded to whole 2048-source blocks."""
+    lib = binding.load()
+    off, nb = ctypes.c_size_t(0), ctypes.c_size_t(0)
+    g = binding.sph_grid.make((0, 0, 0), 0.4, 2.5, (48, 48, 49))
+    for n_gas, n, grid in ((0, 100000, None), (4096, 8192, g), (0, 1, None), (0, 2048, None), (0, 2049, None)):
+        gp = ctypes.byref(grid) if grid is not None else None
+        assert lib.sph_workspace_gravity_sums(n_gas, n, gp, ctypes.byref(off), ctypes.byref(nb)) == 0
+        assert nb.value == 24 * ((n + 2047) // 2048 * 2048) and off.value % 256 == 0
+        assert off.value + nb.value <= lib.sph_workspace_bytes(n_gas, n, gp)
+    assert lib.sph_workspace_gravity_sums(5, 3, None, ctypes.byref(off), ctypes.byref(nb)) == binding.SPH_ERR_ARG
+    assert lib.sph_workspace_gravity_sums(5, 8, None, ctypes.byref(off), ctypes.byref(nb)) == binding.SPH_ERR_ARG   # gas needs a grid
+    assert lib.sph_workspace_gravity_sums(0, 8, None, None, ctypes.byref(nb)) == binding.SPH_ERR_ARG

@@ -436,6 +436,28 @@ def test_error_codes(cuda_lib):
     assert e.value.rc == b.SPH_ERR_GRID
     # n = 0 is legal everywhere
     b.nbody_pp_gravity(d, 0, 1.0, 0.1, acc, ws)
+    # shares (NEXT-4): world >= 1, 0 <= rank < world, slice inside [0, n]
+    n = w.n_total
+    for rank, world, i0, i1 in ((0, 0, 0, n), (-1, 2, 0, n), (2, 2, 0, n), (0, 2, 5, 4), (0, 2, 0, n + 1)):
+        with pytest.raises(b.SphError) as e:
+            b.nbody_pp_gravity_share(d, n, rank, world, i0, i1, 1.0, 0.1, acc, ws)
+        assert e.value.rc == b.SPH_ERR_ARG
+    with pytest.raises(b.SphError) as e:
+        b.nbody_pp_gravity_share(d, n, 0, 2, 0, n, 1.0, -0.1, acc, ws)
+    assert e.value.rc == b.SPH_ERR_UNSUPPORTED
+    with pytest.raises(b.SphError) as e:
+        b.nbody_pp_gravity_finish(d, 0, n, None, 1.0, acc, small)
+    assert e.value.rc == b.SPH_ERR_WORKSPACE
+    with pytest.raises(b.SphError) as e:
+        b.sph_gravity_path(small, 0, n)
+    assert e.value.rc == b.SPH_ERR_WORKSPACE
+    # a rank with an EMPTY target slice still does its share; G = 0 leaves a defined (one-sided) path and zeros
+    b.nbody_pp_gravity_share(d, n, 1, 2, n, n, 1.0, 0.1, acc, ws)
+    b.nbody_pp_gravity_share(d, n, 0, 1, 0, n, 0.0, 0.1, acc, ws)
+    b.nbody_pp_gravity_finish(d, 0, n, None, 0.0, acc, ws)
+    assert torch.count_nonzero(acc).item() == 0 and b.sph_gravity_path(ws, 0, n) == "one_sided_uniform"
+    sums = b.gravity_sums_view(ws, 0, n)
+    assert sums.dtype == torch.int64 and sums.numel() == 3 * ((n + 2047) // 2048 * 2048)
     assert b.sph_launch_count() > 0
 
 
