@@ -1,6 +1,12 @@
 // gravity.cu — (a10) direct Particle-Particle softened gravity, Eq. 4 under
 // reading A1:  a_i = -G sum_j m_j (r_i - r_j) / (|r_i - r_j|^2 + delta^2)^(3/2).
 //
+// This file: source packing, the device-side choice of the kernel variant (grav_plan), the ONE-SIDED kernel
+// (every ordered interaction evaluated: explicit target slices, delta = 0, small N, non-positive masses, a fixed-point
+// range that would be too coarse, and the diagonal blocks of the pair-symmetric path), the final reduction, and the
+// host-side orchestration gravity_share / gravity_finish / gravity.  The pair-symmetric kernel — every unordered pair
+// once, the default for a whole evaluation — is in gravity_sym.cu.
+//
 // Design for sm_100a.  The kernel is bound by the FP32 FMA pipe
 // (128 lanes/clk/SM), not by memory.  One interaction is 12 FP32 operations + 1 MUFU.RSQ:
 //   3 sub (dx,dy,dz)  3 fma (r2 = dx^2+dy^2+dz^2+delta^2)  1 rsqrt
