@@ -343,6 +343,11 @@ def run_ours(args, w):
         "sort_hbm_gbs": (sort_bytes / (sort_ms * 1e-3) / 1e9) if ng and sort_ms > 0 else None,
         "sort_hbm_frac": (sort_bytes / (sort_ms * 1e-3) / 1e9 / hbm) if ng and sort_ms > 0 else None,
         "update_hbm_frac": (upd_bytes / (upd_ms * 1e-3) / 1e9 / hbm) if upd_ms > 0 else None,
+        # the neighbour passes are latency- / ALU-bound, not HBM-bound: their COMPULSORY bytes (density
+        # 16 r + 4 w per gas particle; one forces pass 16+16+8 r + 16 w + the EOS gather 24 r + 24 w) against the HBM peak,
+        # reported because BASELINE.json asks for the fraction — it measures how far from memory-bound they are
+        "density_hbm_frac": (ng * 20 / (dens_ms * 1e-3) / 1e9 / hbm) if ng and dens_ms > 0 else None,
+        "forces_hbm_frac": (2 * ng * 104 / (forc_ms * 1e-3) / 1e9 / hbm) if ng and forc_ms > 0 else None,
         "hbm_peak_gbs": hbm, "peak_source": peak_src,
     }
 
