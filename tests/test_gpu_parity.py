@@ -816,3 +816,36 @@ def test_gravity_path_selection(cuda_lib):
     w0 = wl.make_workload(0)
     acc, path = _grav(b, w0.posm, w0.G, w0.delta)
     assert path == "one_sided_uniform"           # N = 8192 < 32768
+
+
+# ---------------------------------------------------------------- the step as a CUDA graph
+@pytest.mark.parametrize("cfg,scale", [(0, 1.0), (1, 0.5)])
+def test_step_captures_into_cuda_graph(cuda_lib, cfg, scale):
+    """sph_step enqueues on the caller's stream and never synchronises or reads back (the kernel variants are chosen
+    on the device), so a whole step can be captured into a CUDA graph and replayed: bit for bit the eager steps.
+    Config 0 (one-sided gravity) and config 1 at N = 65536 (pair-symmetric gravity: persistent grid, work counter
+    and fixed-point sums re-initialised inside the captured step)."""
+    b = cuda_lib
+    w = wl.make_workload(cfg, scale=scale)
+    ref = b.Simulation(w)
+    for _ in range(4):
+        ref.step()
+    sim = b.Simulation(w)
+    sim.step()                                   # the seeding step (first = 1) stays eager
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        sim.step()                               # warm-up on the capture stream (lazy function attributes)
+        n0 = b.sph_launch_count()
+        with torch.cuda.graph(graph, stream=side):
+            sim.step()
+        launches = b.sph_launch_count() - n0
+    torch.cuda.current_stream().wait_stream(side)
+    assert launches >= 15                        # the step kernels went into the graph (capture does not run them)
+    graph.replay()
+    graph.replay()
+    torch.cuda.synchronize()
+    for x, y in ((sim.posm, ref.posm), (sim.vele, ref.vele), (sim.rho, ref.rho), (sim.acc_sph, ref.acc_sph),
+                 (sim.acc_grav, ref.acc_grav)):
+        assert torch.equal(x, y)
