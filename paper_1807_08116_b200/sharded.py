@@ -5,10 +5,10 @@ over GPU-Direct (L139).  Here every rank keeps the whole state (64 B per particl
 computes its SHARE of the O(N^2) gravity stage (`sph_position_share`).  Which gravity kernel runs is decided on the
 device, so a share has two forms and both exchanges are issued every evaluation (41 MiB in total at N = 2^20 against
 ~0.26 s / k of gravity, so there is nothing to gain from fusing them into the kernel):
-  * pair-symmetric path (equal masses — every BASELINE.json config): the rank's work items of the unordered-pair
+  * pair-symmetric path (positive masses, delta > 0 — every BASELINE.json config): the rank's work items of the unordered-pair
     decomposition, accumulated as 64-bit fixed-point integers; ONE integer SUM all-reduce of that region.  Integer
     addition is exact, so every world size gives the same bits as one GPU.
-  * one-sided path (unequal masses, delta = 0, ...): the rank's TARGET slice against all N sources; ONE all-gather of
+  * one-sided path (delta = 0, a zero mass, ...): the rank's TARGET slice against all N sources; ONE all-gather of
     the acceleration slices.
 `nbody_pp_gravity_finish` then writes the accelerations from whichever applies.  The O(N) and SPH stages (0.2 % of
 the step) run redundantly on every rank; they are deterministic, so the replicas stay bitwise identical and no other
