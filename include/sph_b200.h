@@ -111,7 +111,11 @@ int sph_forces(const float* posm, const float* vele, const float* rho, int64_t n
 
 /* (a10) Direct Particle-Particle gravity, Eq. 4 (L47) with Plummer softening (A1):
  *   acc_grav[i] = -G sum_{j=1..N} m_j (r_i - r_j) / (|r_i - r_j|^2 + delta^2)^(3/2), w = 0.
- * delta >= 0; with delta = 0 coincident pairs contribute 0.                                   */
+ * delta >= 0; with delta = 0 coincident pairs contribute 0.  Two kernels compute it: for
+ * n_total >= 32768, delta > 0 and positive masses every UNORDERED pair is evaluated once and the sums are kept as
+ * 64-bit fixed-point integers (bitwise reproducible; taken when the range rule of DESIGN.md 5.1.1 holds), otherwise
+ * every ordered interaction is evaluated; the choice is made on the device and sph_gravity_path() reports it.
+ * Both are held to the same tolerance against the oracle (2e-4 of the per-particle value, 1e-5 median).          */
 int nbody_pp_gravity(const float* posm, int64_t n_total, float G, float delta,
                      float* acc_grav /*[n_total][4]*/, void* ws, size_t ws_bytes, void* stream);
 
