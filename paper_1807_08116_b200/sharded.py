@@ -58,26 +58,30 @@ def allgather_rows(full: torch.Tensor, rank: int, world: int, chunk: int, group=
 class ShardedSimulation:
     """The Simulation of binding.py with the gravity stage split over the ranks of `group`."""
 
-    def __init__(self, workload, rank: int, world: int, group=None, sigma=None):
-        from . import binding as b
+    def __init__(self, workload, rank: int, world: int, group=None, sigma=None, binding=None, device="cuda"):
+        """binding / device: the C-ABI face and the device of the buffers; the CPU tests of the exchange pass a
+        recording stand-in and "cpu" (the product path never does: without the CUDA library binding.load() raises)."""
+        if binding is None:
+            from . import binding
+        b = binding
         self.b, self.w, self.rank, self.world, self.group = b, workload, rank, world, group
         w = workload
         self.n_gas, self.n_halo, self.n = w.n_gas, w.n_halo, w.n_total
         self.i0, self.i1, self.chunk = slice_bounds(self.n, rank, world)
         self.params = b.sph_params.from_workload(w)
-        self.posm = torch.from_numpy(np.ascontiguousarray(w.posm)).cuda()
-        self.vele = torch.from_numpy(np.ascontiguousarray(w.vele)).cuda()
-        self.rho = torch.zeros(max(self.n_gas, 1), dtype=torch.float32, device="cuda")
-        self.acc_sph = torch.zeros(max(self.n_gas, 1), 4, dtype=torch.float32, device="cuda")
+        self.posm = torch.from_numpy(np.ascontiguousarray(w.posm)).to(device)
+        self.vele = torch.from_numpy(np.ascontiguousarray(w.vele)).to(device)
+        self.rho = torch.zeros(max(self.n_gas, 1), dtype=torch.float32, device=device)
+        self.acc_sph = torch.zeros(max(self.n_gas, 1), 4, dtype=torch.float32, device=device)
         # world * chunk rows so that the all-gather slots are equal; the library only sees the first n
-        self.acc_grav = torch.zeros(world * self.chunk, 4, dtype=torch.float32, device="cuda")
+        self.acc_grav = torch.zeros(world * self.chunk, 4, dtype=torch.float32, device=device)
         self.grid = b.sph_grid_from_bbox(self.posm, self.n_gas, w.h) if self.n_gas > 0 else None
         self.ws = b.alloc_workspace(self.n_gas, self.n, self.grid)
         self.sums = b.gravity_sums_view(self.ws, self.n_gas, self.n, self.grid)   # int64 view, all-reduced each evaluation
         self.sigma = sigma
         self.hsml = None
         if sigma is not None and self.n_gas > 0:
-            self.hsml = torch.full((self.n_gas,), float(np.float32(w.h)), dtype=torch.float32, device="cuda")
+            self.hsml = torch.full((self.n_gas,), float(np.float32(w.h)), dtype=torch.float32, device=device)
         self.first = True
 
     def _position(self, sigma):

@@ -133,3 +133,94 @@ def test_allreduce_sums_gloo_world2():
     with np.errstate(over="ignore"):
         expect = (base * 1315423911 + (2 ** 61 + 12345)) * 1 + (base * 1315423911 - (2 ** 61 + 12345)) * 2
     assert np.array_equal(out[0], expect) and np.array_equal(out[1], expect)
+
+
+class _StubBinding:
+    """Stands in for the C-ABI face in the world-2 test of ShardedSimulation's exchange: no arithmetic of the method —
+    each share call writes rank-tagged values where the library would (the fixed-point sums, the rank's acceleration
+    rows), the finish call records what it was handed."""
+
+    class sph_params:                                   # noqa: N801 (mirrors binding.sph_params)
+        G = 1.0
+
+        @classmethod
+        def from_workload(cls, w):
+            return cls()
+
+    def __init__(self, pair_symmetric):
+        self.pair_symmetric, self.calls, self.seen = pair_symmetric, [], None
+
+    def sph_grid_from_bbox(self, posm, n_gas, h):
+        return "grid"
+
+    def alloc_workspace(self, n_gas, n, grid):
+        return torch.zeros(64 + 24 * 4096, dtype=torch.uint8)
+
+    def gravity_sums_view(self, ws, n_gas, n, grid):
+        return ws[64:].view(torch.int64)
+
+    def sph_position_share(self, posm, hsml, sigma, n_gas, n_halo, rank, world, i0, i1, params, grid, rho, acc_grav, ws):
+        self.calls.append("share")
+        sums = ws[64:].view(torch.int64)
+        sums.zero_()
+        if self.pair_symmetric:                         # this rank's part of the integer sums
+            sums += (rank + 1) * (torch.arange(sums.numel(), dtype=torch.int64) - 2 ** 40)
+        else:                                           # this rank's acceleration rows
+            acc_grav[i0:i1] = float(rank + 1)
+
+    def nbody_pp_gravity_finish(self, posm, n_gas, n_halo, grid, G, acc_grav, ws):
+        self.calls.append("finish")
+        self.seen = (ws[64:].view(torch.int64).clone(), acc_grav.clone())
+
+    def sph_predict(self, *a):
+        self.calls.append("predict")
+
+    def sph_correct(self, *a):
+        self.calls.append("correct")
+
+
+def _sharded_worker(rank, world, port, out):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import numpy as np
+    from types import SimpleNamespace
+    from paper_1807_08116_b200.sharded import ShardedSimulation
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        n = 2500
+        w = SimpleNamespace(n_gas=1000, n_halo=1500, n_total=n, h=0.1, dt=1e-3, posm=np.zeros((n, 4), np.float32),
+                            vele=np.zeros((n, 4), np.float32))
+        res = {}
+        for sym in (True, False):
+            stub = _StubBinding(sym)
+            sim = ShardedSimulation(w, rank, world, binding=stub, device="cpu")
+            sim.step()
+            sums, acc = stub.seen
+            res[sym] = (stub.calls, sums.numpy(), acc[:n].numpy(), (sim.i0, sim.i1))
+        out[rank] = res
+    finally:
+        dist.destroy_process_group()
+
+
+def test_sharded_step_exchange_gloo_world2():
+    """The N > 1 step on CPU (gloo, world 2) with a stand-in for the library: per force evaluation every rank calls
+    share -> integer all-reduce -> all-gather -> finish, in that order, twice in the first step (seeding + the step);
+    what finish sees is the SUM of the ranks' fixed-point parts and ALL ranks' acceleration rows."""
+    import numpy as np
+    world, port = 2, _free_port()
+    mgr = mp.Manager()
+    out = mgr.dict()
+    mp.spawn(_sharded_worker, args=(world, port, out), nprocs=world, join=True)
+    k = np.arange(3 * 4096, dtype=np.int64) - 2 ** 40
+    for rank in range(world):
+        for sym in (True, False):
+            calls, sums, acc, (i0, i1) = out[rank][sym]
+            assert calls == ["share", "finish", "predict", "share", "finish", "correct"]
+            if sym:
+                assert np.array_equal(sums, 3 * k)                           # (1 + 2) * k: both ranks' parts, exact
+            else:
+                b0 = out[0][sym][3]
+                b1 = out[1][sym][3]
+                assert b0[0] == 0 and b0[1] == b1[0] and b1[1] == 2500       # the slices tile [0, n)
+                assert np.all(acc[b0[0]:b0[1]] == 1.0) and np.all(acc[b1[0]:b1[1]] == 2.0)
+    assert np.array_equal(out[0][True][1], out[1][True][1]) and np.array_equal(out[0][False][2], out[1][False][2])
