@@ -5,6 +5,7 @@ IEEE operation; no -march=native so the library runs on any x86-64 host; no -ffa
 """
 from __future__ import annotations
 
+import fcntl
 import os
 import subprocess
 
@@ -13,13 +14,30 @@ SRC = os.path.join(HERE, "sph_oracle.c")
 LIB = os.path.join(HERE, "libsph_oracle.so")
 
 
+def _fresh() -> bool:
+    return os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC)
+
+
 def build(force: bool = False) -> str:
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
+    """Compile if stale; concurrent callers serialise on a lock file and each compiles into its own temporary name."""
+    if not force and _fresh():
         return LIB
-    cmd = ["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC",
-           "-o", LIB + ".tmp", SRC, "-lm"]
-    subprocess.run(cmd, check=True)
-    os.replace(LIB + ".tmp", LIB)
+    with open(LIB + ".lock", "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if not force and _fresh():
+                return LIB
+            tmp = f"{LIB}.{os.getpid()}.tmp"
+            cmd = ["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC",
+                   "-o", tmp, SRC, "-lm"]
+            try:
+                subprocess.run(cmd, check=True)
+                os.replace(tmp, LIB)
+            finally:
+                if os.path.exists(tmp):
+                    os.unlink(tmp)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
     return LIB
 
 

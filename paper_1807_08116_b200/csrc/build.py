@@ -5,6 +5,7 @@ cutoff code paths are bit-exact FP32 sequences).  Cross-compiles without a GPU.
 """
 from __future__ import annotations
 
+import fcntl
 import os
 import subprocess
 
@@ -23,16 +24,31 @@ def _stale() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile if stale.  Safe when several processes call it at once (torchrun ranks on a fresh checkout): one holds an
+    exclusive lock on libsph_b200.so.lock and compiles into its OWN temporary name before the atomic rename; the others
+    wait on the lock and then find the library fresh."""
     if not force and not _stale():
         return LIB
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-           "-Xcompiler", "-fPIC", "-shared", "-o", LIB + ".tmp"]
-    if verbose:
-        cmd += ["-Xptxas", "-v"]
-    cmd += [os.path.join(HERE, s) for s in SOURCES]
-    subprocess.run(cmd, check=True)
-    os.replace(LIB + ".tmp", LIB)
+    with open(LIB + ".lock", "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if not force and not _stale():          # another process built it while this one waited
+                return LIB
+            nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+            tmp = f"{LIB}.{os.getpid()}.tmp"
+            cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+                   "-Xcompiler", "-fPIC", "-shared", "-o", tmp]
+            if verbose:
+                cmd += ["-Xptxas", "-v"]
+            cmd += [os.path.join(HERE, s) for s in SOURCES]
+            try:
+                subprocess.run(cmd, check=True)
+                os.replace(tmp, LIB)
+            finally:
+                if os.path.exists(tmp):
+                    os.unlink(tmp)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
     return LIB
 
 

@@ -3,6 +3,7 @@
 // with the oracle.
 #pragma once
 #include <cuda_runtime.h>
+#include <atomic>
 #include <stdint.h>
 #include <stddef.h>
 #include "../../include/sph_b200.h"
@@ -11,7 +12,7 @@ namespace sphb {
 
 // ---- error plumbing ---------------------------------------------------------------------
 extern thread_local int g_last_cuda_error;
-extern long long g_launch_count;   // kernels enqueued by this library (sph_launch_count)
+extern std::atomic<long long> g_launch_count;   // kernels enqueued by this library (sph_launch_count)
 
 inline int cuda_fail(cudaError_t e) {
     g_last_cuda_error = (int)e;

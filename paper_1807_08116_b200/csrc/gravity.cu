@@ -220,7 +220,12 @@ __global__ void __launch_bounds__(THREADS, MINB)
                 float r2a, r2b;
                 upk2(r2, r2a, r2b);
                 float ua = rsqrt_approx(r2a), ub = rsqrt_approx(r2b);
-                if (ZERO_SOFT) {   // delta = 0: coincident pair contributes 0 (Eq. 4 numerator is 0)
+                if (ZERO_SOFT) {
+                    // delta = 0: nothing bounds 1/r^3 from above, so a particle's sum can be one or two huge terms and the
+                    // 2^-22.9 of rsqrt.approx (cubed: 3.5e-7) is no longer averaged down over N sources — one Newton step
+                    // (this instance is not the hot one); a coincident pair contributes 0 (Eq. 4's numerator is 0)
+                    ua = ua * fmaf(-0.5f * r2a * ua, ua, 1.5f);
+                    ub = ub * fmaf(-0.5f * r2b * ub, ub, 1.5f);
                     ua = (r2a > 0.f) ? ua : 0.f;
                     ub = (r2b > 0.f) ? ub : 0.f;
                 }

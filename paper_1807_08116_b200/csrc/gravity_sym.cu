@@ -214,15 +214,21 @@ static int sym_rows_per_item(int64_t ncols, int slots) {
 
 int gravity_sym_launch(const float4* posm, const float4* src_pk, int n_pad, int share_rank, int share_world, float eps2,
                        long long* acc64, GravCtl* ctl, cudaStream_t st) {
-    static int occ = 0;
+    // the opt-in for > 48 KB of dynamic shared memory is per device (context): set it on every launch, as gravity.cu's
+    // launch_one does, and cache the occupancy per device, so that a process driving several GPUs gets it right on each
+    static int occ_dev[64] = {0};
+    int dev = 0;
+    SPHB_CUDA(cudaGetDevice(&dev));
+    SPHB_CUDA(cudaFuncSetAttribute(grav_sym_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSymSmem));
+    SPHB_CUDA(cudaFuncSetAttribute(grav_sym_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSymSmem));
+    int occ = (dev >= 0 && dev < 64) ? occ_dev[dev] : 0;
     if (occ == 0) {
-        SPHB_CUDA(cudaFuncSetAttribute(grav_sym_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSymSmem));
-        SPHB_CUDA(cudaFuncSetAttribute(grav_sym_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSymSmem));
         int o1 = 0, o2 = 0;
         SPHB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o1, grav_sym_kernel<true>, kSymThreads, kSymSmem));
         SPHB_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o2, grav_sym_kernel<false>, kSymThreads, kSymSmem));
         occ = o1 < o2 ? o1 : o2;
         if (occ < 1) occ = 1;
+        if (dev >= 0 && dev < 64) occ_dev[dev] = occ;
     }
     const int64_t ncols = cdiv(n_pad, kSymL);
     const int slots = num_sms() * occ;

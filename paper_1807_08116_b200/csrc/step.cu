@@ -5,16 +5,18 @@
 namespace sphb {
 
 thread_local int g_last_cuda_error = 0;
-long long g_launch_count = 0;
+std::atomic<long long> g_launch_count{0};
 
-int num_sms() {
-    static int n = 0;
-    if (n == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
-            n = 148;
+int num_sms() {   // of the CURRENT device (a process may drive several)
+    static int n_dev[64] = {0};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+    if (n_dev[dev] == 0) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+        n_dev[dev] = n;
     }
-    return n;
+    return n_dev[dev];
 }
 
 // ---------------------------------------------------------------- workspace

@@ -1,4 +1,4 @@
-"""Error measures used by the GPU parity tests (DESIGN.md reading A17).
+"""Error measures used by the GPU parity tests (DESIGN.md §8, reading A17).
 
 north_star: density to a relative 1e-5; accelerations and de/dt to 2e-4 of the per-particle
 value (1e-5 median).  The per-particle value can be exactly 0 (a gas particle without
@@ -8,8 +8,17 @@ with |.| the 2-norm for vectors, and exact zeros of the reference must be matche
 For the SPH sums the terms of one particle can cancel by a factor of 1000 or more (measured:
 config 0, particle 2480, four terms of size ~0.2 summing to de/dt = -4e-4); no FP32 evaluation
 can then hold 2e-4 of the net value (per-term rounding ~1e-7 x cancellation), so where the oracle
-supplies the gross sum S_i = sum_j |term_ij| the floor is max(floor, 1e-3 * S_i): the
-"per-particle value" is never taken smaller than a thousandth of what was actually summed.
+supplies the gross sum S_i = sum_j |term_ij| (pinned by test_A17_gross_sums_by_hand) the floor is
+max(floor, 1e-3 * S_i): the "per-particle value" is never taken smaller than a thousandth of what
+was actually summed.
+
+Neither floor is taken on trust: every call records how many values each floor touched and by how
+much it loosened the bar for the worst of them (denominator / |ref|), the numbers are printed in
+the terminal summary of the test run (tests/conftest.py), and both are held under the ceilings
+below.  Measured with the oracle alone (no GPU involved): config 0 — median floor 25 (a_sph) / 34 (de/dt)
+of 2339 non-zero values, gross floor 0 / 1 (x2.9); uniform random gas of 20000 — median floor 0 / 11,
+gross floor 0 / 22 (x38: de/dt cancelled to 3e-5 of what was summed); config 4 at 1/512 — median floor
+120 / 155 of 10835, gross floor 0 / 1 (x3.3); gravity — neither floor touches anything.
 """
 import numpy as np
 
@@ -17,39 +26,79 @@ RHO_TOL = 1e-5
 VAL_TOL = 2e-4
 MED_TOL = 1e-5
 
+# ceilings on the reach of the floors (fractions of the non-zero reference values, and the largest loosening)
+MEDIAN_FLOOR_MAX_FRACTION = 0.02     # values below 1e-3 of the array's median magnitude
+GROSS_FLOOR_MAX_FRACTION = 0.01      # values below 1e-3 of their own gross sum
+GROSS_FLOOR_MAX_LOOSENING = 100.0    # i.e. a net value cancelled below 1e-5 of what was summed fails the test
+
+REPORT = []          # one dict per check_values call, printed by conftest.pytest_terminal_summary
+
 
 def rel_err(got, ref, gross=None):
+    """|got - ref| and the denominator max(|ref|, floors) per value, plus the reach of the two floors.
+    Returns (num, denom, info, zero_mask)."""
     got = np.asarray(got, dtype=np.float64)
     ref = np.asarray(ref, dtype=np.float64)
     if got.ndim == 1:
         num, mag = np.abs(got - ref), np.abs(ref)
     else:
         num, mag = np.linalg.norm(got - ref, axis=1), np.linalg.norm(ref, axis=1)
-    nz = mag[mag > 0]
-    floor = 1e-3 * np.median(nz) if len(nz) else 1.0
+    nzm = mag > 0
+    nz = mag[nzm]
+    fmed = 1e-3 * np.median(nz) if len(nz) else 1.0
+    denom = np.maximum(mag, fmed)
+    med_touched = nzm & (mag < fmed)
+    gross_touched = np.zeros_like(nzm)
     if gross is not None:
-        floor = np.maximum(floor, 1e-3 * np.asarray(gross, dtype=np.float64))
-    err = num / np.maximum(mag, floor)
-    touched = int(np.count_nonzero((mag < floor) & (mag > 0)))
-    return err, touched, mag == 0
+        fg = 1e-3 * np.asarray(gross, dtype=np.float64)
+        gross_touched = nzm & (fg > denom)
+        denom = np.maximum(denom, fg)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        loosen = np.where(nzm, denom / mag, 1.0)
+    info = {
+        "n": int(nzm.sum()),
+        "median_floor_touched": int(med_touched.sum()),
+        "median_floor_loosening": float(loosen[med_touched].max()) if med_touched.any() else 1.0,
+        "gross_floor_touched": int(gross_touched.sum()),
+        "gross_floor_loosening": float(loosen[gross_touched].max()) if gross_touched.any() else 1.0,
+    }
+    return num, denom, info, ~nzm
 
 
-def check_values(got, ref, what, max_tol=VAL_TOL, med_tol=MED_TOL, gross=None):
-    err, touched, zero = rel_err(got, ref, gross)
+def check_values(got, ref, what, max_tol=VAL_TOL, med_tol=MED_TOL, gross=None, extra_abs=None):
+    """Assert the north-star bar and the ceilings on the floors' reach; returns (max, median) of err.
+    extra_abs: an additional ABSOLUTE allowance per value (same shape as the magnitudes), used by the tests whose two
+    sides take different inputs by a known, bounded amount (own-density forces test)."""
+    num, denom, info, zero = rel_err(got, ref, gross)
     got = np.asarray(got, dtype=np.float64)
     gz = got[zero]
     assert np.all(gz == 0), f"{what}: reference zeros not matched exactly"
-    nz = err[~zero]
+    if extra_abs is not None:
+        num = np.maximum(num - np.asarray(extra_abs, dtype=np.float64), 0.0)
+    nz = (num / denom)[~zero]
+    rec = dict(what=what, max_tol=max_tol, **info, max_err=0.0, median_err=0.0)
+    REPORT.append(rec)
     if len(nz) == 0:
         return 0.0, 0.0
     mx, med = float(nz.max()), float(np.median(nz))
-    assert mx <= max_tol, f"{what}: max rel err {mx:.3e} > {max_tol} (floor touched {touched})"
+    rec.update(max_err=mx, median_err=med)
+    print(f"[parity] {what}: max {mx:.2e} median {med:.2e} over {info['n']} values; median floor touched "
+          f"{info['median_floor_touched']} (x{info['median_floor_loosening']:.1f}), gross floor touched "
+          f"{info['gross_floor_touched']} (x{info['gross_floor_loosening']:.1f})")
+    assert mx <= max_tol, f"{what}: max rel err {mx:.3e} > {max_tol} ({info})"
     assert med <= med_tol, f"{what}: median rel err {med:.3e} > {med_tol}"
+    n = max(info["n"], 1)
+    assert info["median_floor_touched"] <= max(2, MEDIAN_FLOOR_MAX_FRACTION * n), f"{what}: median floor reach {info}"
+    assert info["gross_floor_touched"] <= max(2, GROSS_FLOOR_MAX_FRACTION * n), f"{what}: gross floor reach {info}"
+    assert info["gross_floor_loosening"] <= GROSS_FLOOR_MAX_LOOSENING, f"{what}: gross floor loosening {info}"
     return mx, med
 
 
 def check_density(got, ref, what="rho"):
     got = np.asarray(got, dtype=np.float64)
     err = np.abs(got - ref) / ref
+    REPORT.append(dict(what=what, max_tol=RHO_TOL, n=int(err.size), median_floor_touched=0, median_floor_loosening=1.0,
+                       gross_floor_touched=0, gross_floor_loosening=1.0, max_err=float(err.max()),
+                       median_err=float(np.median(err))))
     assert err.max() <= RHO_TOL, f"{what}: max rel err {err.max():.3e} > {RHO_TOL}"
     return float(err.max())

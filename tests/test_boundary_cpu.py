@@ -72,3 +72,18 @@ def test_gravity_sums_region_without_gpu():
     assert lib.sph_workspace_gravity_sums(5, 3, None, ctypes.byref(off), ctypes.byref(nb)) == binding.SPH_ERR_ARG
     assert lib.sph_workspace_gravity_sums(5, 8, None, ctypes.byref(off), ctypes.byref(nb)) == binding.SPH_ERR_ARG   # gas needs a grid
     assert lib.sph_workspace_gravity_sums(0, 8, None, None, ctypes.byref(nb)) == binding.SPH_ERR_ARG
+
+
+def test_concurrent_builds_do_not_corrupt_the_library():
+    """torchrun ranks on a fresh checkout all call build() at once: each must compile into its own
+    temporary and serialise on the lock, so that the library every one of them ends up loading is whole.  Exercised
+    on the oracle's build (same pattern as csrc/build.py, seconds instead of half a minute)."""
+    import subprocess
+    import sys
+    code = ("import sys; sys.path.insert(0, %r); from oracle.build import build; import ctypes; "
+            "p = build(force=True); L = ctypes.CDLL(p); L.orc_rc2.restype = ctypes.c_float; "
+            "L.orc_rc2.argtypes = [ctypes.c_float]; assert L.orc_rc2(1.0) == 4.0" % ROOT)
+    procs = [subprocess.Popen([sys.executable, "-c", code]) for _ in range(4)]
+    assert [p.wait(timeout=300) for p in procs] == [0, 0, 0, 0]
+    left = [f for f in os.listdir(os.path.join(ROOT, "oracle")) if f.endswith(".tmp")]
+    assert left == []

@@ -46,14 +46,15 @@ def _check_structures(b, sim, w):
     return og, okey, ocount, ostart, operm
 
 
-def _check_sph_subset(w, posm, vele, rho_gpu, acc_sph_gpu, g_idx, og, sort):
+def _check_sph_subset(w, posm, vele, rho_gpu, acc_sph_gpu, g_idx, og, sort, density=True):
     """density for the subset, forces for the subset with the GPU's verified rho as input."""
     off, idx = oracle.neighbours(posm, w.n_gas, w.h, targets=g_idx, method="grid", grid=og, sort=sort)
-    orho = oracle.density(posm, w.h, off, idx, targets=g_idx)
-    check_density(rho_gpu[g_idx], orho, "rho subset")
+    if density:
+        orho = oracle.density(posm, w.h, off, idx, targets=g_idx)
+        check_density(rho_gpu[g_idx], orho, "rho subset")
     # every neighbour's density is also checked (two-hop closure): a wrong rho_j would otherwise hide
     closure = np.unique(idx.astype(np.int64))
-    if len(closure):
+    if density and len(closure):
         off2, idx2 = oracle.neighbours(posm, w.n_gas, w.h, targets=closure, method="grid", grid=og, sort=sort)
         check_density(rho_gpu[closure], oracle.density(posm, w.h, off2, idx2, targets=closure), "rho closure")
     of, gross = oracle.forces(posm, vele, rho_gpu.astype(np.float64), w.h, off, idx, targets=g_idx, gamma=w.gamma,
@@ -63,8 +64,72 @@ def _check_sph_subset(w, posm, vele, rho_gpu, acc_sph_gpu, g_idx, og, sort):
     return np.diff(off)
 
 
+def _staged_step_checked(b, sim, w, og, g_idx, h_idx, check_sort):
+    """One step of sph_step_h, issued as the three stage calls it is composed of (sph_predict, sph_position_slice,
+    sph_correct: the same code path, bit for bit), with every stage checked TEACHER-FORCED (SURVEY §8(c) large-N
+    protocol): the oracle's input at each stage is the GPU's verified output of the stage before, so it never advances
+    10^6 particles by O(N^2) itself.  O(N) update formulas on ALL particles, sums on the seeded subset."""
+    ng, n, nh, dt = w.n_gas, w.n_total, w.n_halo, w.dt
+    tg = np.concatenate([g_idx, h_idx])
+    p0 = sim.posm.cpu().numpy()
+    v0f = sim.vele.cpu().numpy()
+    rho0 = sim.rho.cpu().numpy()
+    ag0 = sim.acc_grav.cpu().numpy().astype(np.float64)
+    # ---- HFC(predictor) + SU(predictor)
+    b.sph_predict(sim.posm, sim.vele, None, ng, nh, sim.params, sim.grid, dt, sim.rho, sim.acc_sph, sim.acc_grav, sim.ws)
+    as0 = sim.acc_sph.cpu().numpy()
+    key0 = oracle.cell_keys(p0, ng, og)
+    _, start0, perm0 = oracle.counting_sort(key0, og.M)
+    _check_sph_subset(w, p0, v0f, rho0, as0, g_idx, og, (key0, start0, perm0), density=False)
+    p1 = sim.posm.cpu().numpy()
+    vt_g = sim.vele.cpu().numpy()
+    Q0 = ag0[:, :3].copy()
+    Q0[:ng] += as0[:, :3]
+    v0 = v0f[:, :3].astype(np.float64)
+    e0 = v0f[:ng, 3].astype(np.float64)
+    vt = v0 + dt * Q0                                                # Eq. 12
+    et = e0 + dt * as0[:, 3].astype(np.float64)                      # Eq. 13
+    r1 = p0[:, :3].astype(np.float64) + 0.5 * dt * (vt + v0)         # Eq. 14
+    check_values(vt_g[:, :3], vt, "v~ (Eq. 12) all", max_tol=2e-6, med_tol=2e-7)
+    check_values(vt_g[:ng, 3], et, "e~ (Eq. 13) all", max_tol=2e-6, med_tol=2e-7)
+    assert np.abs(p1[:, :3] - r1).max() <= 2e-7 * max(1.0, np.abs(r1).max())       # Eq. 14: one FP32 rounding of r
+    assert np.array_equal(p1[:, 3], p0[:, 3])
+    # ---- SP, DC, GFC at r(t+dt)
+    b.sph_position_slice(sim.posm, None, 0.0, ng, nh, 0, n, sim.params, sim.grid, sim.rho, sim.acc_grav, sim.ws)
+    ag1 = sim.acc_grav.cpu().numpy().astype(np.float64)
+    check_values(ag1[tg, :3], oracle.gravity(p1, w.G, w.delta, targets=tg), "a_grav(t+dt) subset")
+    assert np.all(ag1[:, 3] == 0)
+    key1 = oracle.cell_keys(p1, ng, og)
+    _, start1, perm1 = oracle.counting_sort(key1, og.M)
+    if check_sort:                                                   # the grid the library carries, ALL particles
+        key = torch.zeros(ng, dtype=torch.int32, device="cuda")
+        perm = torch.zeros(ng, dtype=torch.int32, device="cuda")
+        count = torch.zeros(og.M, dtype=torch.int32, device="cuda")
+        start = torch.zeros(og.M + 1, dtype=torch.int32, device="cuda")
+        ws2 = b.alloc_workspace(ng, ng, sim.grid)
+        b.sph_build_grid(sim.posm, ng, sim.grid, key, perm, count, start, ws2)
+        assert np.array_equal(key.cpu().numpy().view(np.uint32), key1)
+        assert np.array_equal(start.cpu().numpy().view(np.uint32), start1)
+        assert np.array_equal(perm.cpu().numpy().view(np.uint32), perm1)
+        del key, perm, count, start, ws2
+    rho1 = sim.rho.cpu().numpy()
+    # ---- HFC(corrector) + SU(corrector)
+    b.sph_correct(sim.vele, None, ng, nh, sim.params, sim.grid, dt, sim.rho, sim.acc_sph, sim.acc_grav, sim.ws)
+    as1 = sim.acc_sph.cpu().numpy()
+    _check_sph_subset(w, p1, vt_g, rho1, as1, g_idx, og, (key1, start1, perm1))
+    v1 = sim.vele.cpu().numpy()
+    Q1 = ag1[:, :3].copy()
+    Q1[:ng] += as1[:, :3]
+    vt64 = vt_g[:, :3].astype(np.float64)
+    check_values(v1[:, :3], 0.5 * (v0 + vt64) + 0.5 * dt * Q1, "v(t+dt) (Eq. 15) all", max_tol=2e-6, med_tol=2e-7)
+    check_values(v1[:ng, 3], 0.5 * (e0 + vt_g[:ng, 3]) + 0.5 * dt * as1[:, 3], "e(t+dt) (Eq. 16) all", max_tol=2e-6,
+                 med_tol=2e-7)
+
+
 @pytest.mark.parametrize("cfg", [2, 3])
 def test_full_size_collision(cuda_lib, cfg):
+    """BASELINE.json configs 2 and 3 at their stated size AND step count (10 and 5 steps), every stage of every step
+    against the oracle, teacher-forced."""
     b = cuda_lib
     w = wl.make_workload(cfg)
     ng, n = w.n_gas, w.n_total
@@ -72,7 +137,7 @@ def test_full_size_collision(cuda_lib, cfg):
     og, okey, ocount, ostart, operm = _check_structures(b, sim, w)
     g_idx, h_idx = _subset(w, okey, ocount)
     tg = np.concatenate([g_idx, h_idx])
-    # ---- force evaluation at t = 0
+    # ---- force evaluation at t = 0 (seeds the carried state)
     sim.evaluate()
     rho0 = sim.rho.cpu().numpy()
     as0 = sim.acc_sph.cpu().numpy()
@@ -81,36 +146,17 @@ def test_full_size_collision(cuda_lib, cfg):
     assert np.all(ag0[:, 3] == 0)
     nn = _check_sph_subset(w, w.posm, w.vele, rho0, as0, g_idx, og, (okey, ostart, operm))
     assert nn.max() > 10
-    if cfg == 3:
-        return                      # one evaluation at N = 2^22 is enough for the suite's time budget
-    # ---- one step; O(N) update formulas on ALL particles from the GPU's own stage outputs (FP64 restatement)
-    sim.step()
-    p1 = sim.posm.cpu().numpy()
-    v1 = sim.vele.cpu().numpy()
-    ag1 = sim.acc_grav.cpu().numpy().astype(np.float64)
-    as1 = sim.acc_sph.cpu().numpy().astype(np.float64)
-    dt = w.dt
-    Q0 = ag0[:, :3].astype(np.float64)
-    Q0[:ng] += as0[:, :3]
-    v0 = w.vele[:, :3].astype(np.float64)
-    e0 = w.vele[:ng, 3].astype(np.float64)
-    vt = v0 + dt * Q0                                                # Eq. 12
-    et = e0 + dt * as0[:, 3].astype(np.float64)                      # Eq. 13
-    r1 = w.posm[:, :3].astype(np.float64) + 0.5 * dt * (vt + v0)     # Eq. 14
-    assert np.abs(p1[:, :3] - r1).max() <= 2e-6 * max(1.0, np.abs(r1).max())
-    assert np.array_equal(p1[:, 3], w.posm[:, 3])
-    Q1 = ag1[:, :3].copy()
-    Q1[:ng] += as1[:, :3]
-    check_values(v1[:, :3], 0.5 * (v0 + vt) + 0.5 * dt * Q1, "v(t+dt) all", max_tol=2e-6, med_tol=2e-7)     # Eq. 15
-    check_values(v1[:ng, 3], 0.5 * (e0 + et) + 0.5 * dt * as1[:, 3], "e(t+dt) all", max_tol=2e-6, med_tol=2e-7)  # Eq. 16
-    # ---- the position-only quantities and the corrector's hydro terms at r(t+dt), subset
-    check_values(ag1[tg, :3], oracle.gravity(p1, w.G, w.delta, targets=tg), "a_grav(t+dt) subset")
-    key1 = oracle.cell_keys(p1, ng, og)
-    _, start1, perm1 = oracle.counting_sort(key1, og.M)
-    vele_t = np.zeros((n, 4))
-    vele_t[:, :3] = vt
-    vele_t[:ng, 3] = et
-    _check_sph_subset(w, p1, vele_t, sim.rho.cpu().numpy(), sim.acc_sph.cpu().numpy(), g_idx, og, (key1, start1, perm1))
+    # ---- the config's steps, staged.  At config 2 a plain sph_step replica runs beside them and must stay bit-identical
+    # (at config 3 that would double 20 s of gravity; the identity is also tested at N = 98304).
+    ref = b.Simulation(w, grid=sim.grid) if cfg == 2 else None
+    for k in range(w.steps):
+        _staged_step_checked(b, sim, w, og, g_idx, h_idx, check_sort=(cfg == 2 or k == w.steps - 1))
+        if ref is not None:
+            ref.step()
+    if ref is not None:
+        for x, y in ((sim.posm, ref.posm), (sim.vele, ref.vele), (sim.rho, ref.rho), (sim.acc_sph, ref.acc_sph),
+                     (sim.acc_grav, ref.acc_grav)):
+            assert torch.equal(x, y)
 
 
 def test_full_size_sph_only_config4(cuda_lib):

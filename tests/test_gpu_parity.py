@@ -242,6 +242,34 @@ def test_density_and_forces_parity(cuda_lib, case):
     assert torch.equal(acc, acc2)
 
 
+@pytest.mark.parametrize("case", ["galaxy", "dense"])
+def test_forces_parity_oracle_own_density(cuda_lib, case):
+    """The same comparison as above WITHOUT teacher forcing: the oracle's forces use the oracle's own FP64 density,
+    the GPU's forces its own FP32 density.  Bound: every term of Eqs. 10-11 depends on the densities
+    through Pi_ij = (gamma-1)(e_i/rho_i + e_j/rho_j) + nu_ij, nu_ij = mu (beta mu - alpha c_ij)/rho_ij with mu <= 0: three
+    NON-NEGATIVE parts, each proportional to one 1/rho, so relative density differences <= eps move Pi_ij, and with it the
+    term, by at most eps/(1-eps) of its magnitude, and a particle's sum by at most that times S_i, the gross sum of its
+    term magnitudes.  With eps the MEASURED largest relative difference between the two densities (itself held to
+    RHO_TOL first):  |got - ref| <= VAL_TOL * max(|ref|, floors) + 2 eps S_i."""
+    b = cuda_lib
+    w, og = _grid_case(case)
+    n = w.n_gas
+    d, g, perm, start, ws = _build(b, w, og)
+    prm = b.sph_params.from_workload(w)
+    rho = torch.zeros(n, device="cuda")
+    b.sph_density(d, n, prm, g, perm, start, rho, ws)
+    acc = torch.zeros((n, 4), device="cuda")
+    b.sph_forces(d, _t(w.vele), rho, n, prm, g, perm, start, acc, ws)
+    ooff, oidx = oracle.neighbours(w.posm, n, w.h, method="grid")
+    orho = oracle.density(w.posm, w.h, ooff, oidx)
+    eps = check_density(rho.cpu().numpy(), orho, f"rho {case} (own-density test)")
+    of, gross = oracle.forces(w.posm, w.vele, orho, w.h, ooff, oidx, gamma=w.gamma, alpha=w.alpha, beta=w.beta, eta=w.eta,
+                              with_gross=True)
+    got = acc.cpu().numpy()
+    check_values(got[:, :3], of[:, :3], f"a_sph {case}, oracle's own rho", gross=gross[:, 0], extra_abs=2 * eps * gross[:, 0])
+    check_values(got[:, 3], of[:, 3], f"de/dt {case}, oracle's own rho", gross=gross[:, 1], extra_abs=2 * eps * gross[:, 1])
+
+
 @pytest.mark.parametrize("case", ["galaxy", "dense", "clumps"])
 def test_cfl_step_parity(cuda_lib, case):
     """NEXT-1, Eq. 17 (L125-129): per-particle bracket and the global minimum against the oracle.  Both sides
@@ -316,9 +344,11 @@ def test_evaluate_config0(cuda_lib):
     check_values(a[:, 3], hy[:, 3], "de/dt", gross=gross[:, 1])
 
 
-@pytest.mark.parametrize("cfg,scale,steps", [(0, 1.0, 1), (0, 1.0, 3), (1, 1 / 16, 4)])
+@pytest.mark.parametrize("cfg,scale,steps", [(0, 1.0, 1), (0, 1.0, 3), (0, 1.0, 10), (1, 1 / 16, 4), (1, 1.0, 10)])
 def test_step_parity_free_running(cuda_lib, cfg, scale, steps):
-    """Free-running multi-step trajectories: GPU FP32 state against the oracle's FP64 state."""
+    """Free-running multi-step trajectories: GPU FP32 state against the oracle's FP64 state (configs 0-1
+    end to end).  (1, 1.0, 10) is BASELINE.json config 1 at its stated size and step count: N = 2^17, 10 steps —
+    11 oracle gravity evaluations of 1.7e10 FP64 interactions."""
     b = cuda_lib
     w = wl.make_workload(cfg, scale=scale)
     sim = b.Simulation(w)
@@ -332,13 +362,25 @@ def test_step_parity_free_running(cuda_lib, cfg, scale, steps):
     pos = sim.posm.cpu().numpy()
     vel = sim.vele.cpu().numpy()
     ng = w.n_gas
-    # positions: absolute, a few FP32 ulps of the coordinate scale per step
-    assert np.abs(pos[:, :3] - st.posm[:, :3]).max() < 4e-6 * steps * max(1.0, np.abs(st.posm[:, :3]).max())
+    # positions: absolute; one FP32 rounding of r per step (<= 6e-8 |r|) plus dt times the velocity difference
+    assert np.abs(pos[:, :3] - st.posm[:, :3]).max() < 2e-7 * steps * max(1.0, np.abs(st.posm[:, :3]).max())
     assert np.array_equal(pos[:, 3], w.posm[:, 3])
     check_values(vel[:, :3], st.vele[:, :3], "v(t+dt)", max_tol=2e-5, med_tol=2e-6)
     check_values(vel[:ng, 3], st.vele[:ng, 3], "e(t+dt)", max_tol=2e-5, med_tol=2e-6)
-    check_density(sim.rho.cpu().numpy()[:ng], st.rho, "rho(t+dt)") if steps == 1 else None
-    check_values(sim.acc_grav.cpu().numpy()[:, :3], st.acc_grav, "a_grav(t+dt)", max_tol=1e-3 if steps > 1 else 2e-4)
+    if steps == 1:
+        check_density(sim.rho.cpu().numpy()[:ng], st.rho, "rho(t+dt)")
+        check_values(sim.acc_grav.cpu().numpy()[:, :3], st.acc_grav, "a_grav(t+dt)")
+    else:
+        # After several steps the two trajectories differ by FP32 rounding of the positions (~1e-6), and a_grav and rho
+        # are not Lipschitz in r at the north-star tolerances (a neighbour at distance ~delta moves its term by
+        # 3 * 1e-6 / delta ~ 6e-4).  So the carried position-only quantities are held to the north-star bars against
+        # the oracle evaluated AT THE GPU'S OWN final positions; the free-running comparison above covers the state.
+        tg = np.arange(0, w.n_total, max(1, w.n_total // 4096))
+        check_values(sim.acc_grav.cpu().numpy()[tg, :3], oracle.gravity(pos, w.G, w.delta, targets=tg),
+                     "a_grav at the GPU's r(t+dt)")
+        g_t = tg[tg < ng]
+        off, idx = oracle.neighbours(pos, ng, w.h, targets=g_t, method="grid")
+        check_density(sim.rho.cpu().numpy()[g_t], oracle.density(pos, w.h, off, idx, targets=g_t), "rho at the GPU's r(t+dt)")
 
 
 def test_step_collisionless_and_gas_only(cuda_lib):

@@ -200,6 +200,66 @@ def test_P10_single_pair_by_hand():
     assert np.allclose(f2[0, :3], -m2 * Pi0 * gradWp, rtol=1e-14)
 
 
+def _golden_frac(name):
+    import os
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "closed_forms.txt")):
+        f = line.split()
+        if f and f[0] == name:
+            return float(Fraction(f[1]))
+    raise KeyError(name)
+
+
+def test_A17_gross_sums_by_hand():
+    """The second output of oracle.forces, S_i = (sum_j |m_j Pi_ij grad W_p|, sum_j |1/2 m_j Pi_ij dv.grad W_p|), sets the
+    floor of the parity tolerance (reading A17, tests/parity_util.py), so it is pinned like a value:
+    (1) one pair (the P10 configuration): a single term, so S equals the magnitude of the value itself;
+    (2) three collinear particles worked by hand (tests/golden/closed_forms.txt: gross_collinear_*): the two terms of
+        the middle particle cancel exactly — value 0, S = twice one term — which is the situation S exists for;
+    (3) the same with unequal neighbour masses: value = difference, S = sum of the two magnitudes."""
+    # (1) P10's pair, viscosity on (approaching)
+    h, gamma = 0.5, 1.4
+    posm = np.array([[0, 0, 0, 0.3], [0.6, 0, 0, 0.7]], dtype=np.float64)
+    vele = np.array([[0.4, 0.1, 0, 1.2], [-0.2, 0.0, 0, 0.8]], dtype=np.float64)
+    off, idx = oracle.neighbours(posm, 2, h)
+    rho = oracle.density(posm, h, off, idx)
+    f, g = oracle.forces(posm, vele, rho, h, off, idx, gamma=gamma, with_gross=True)
+    assert g.shape == (2, 2)
+    assert np.allclose(g[:, 0], np.linalg.norm(f[:, :3], axis=1), rtol=1e-14)
+    assert np.allclose(g[:, 1], np.abs(f[:, 3]), rtol=1e-14)
+    assert np.all(g > 0)
+    # (2) three collinear particles; rho is an INPUT of the force sums, so round values are given
+    h = 1.0
+    posm = np.array([[0, 0, 0, 1.0], [1, 0, 0, 2.0], [-1, 0, 0, 2.0]], dtype=np.float64)
+    vele = np.array([[0, 0, 0, 1.5], [0.5, 0, 0, 1.5], [0.5, 0, 0, 1.5]], dtype=np.float64)
+    rho = np.array([1.0, 2.0, 2.0])
+    off, idx = oracle.neighbours(posm, 3, h)
+    assert np.diff(off).tolist() == [2, 1, 1]                   # the outer two are exactly 2h apart: not a pair (A8)
+    kw = dict(gamma=5.0 / 3.0, alpha=0.0, beta=0.0, eta=0.1)
+    f, g = oracle.forces(posm, vele, rho, h, off, idx, with_gross=True, **kw)
+    assert np.all(np.abs(f[0]) < 1e-16)                         # exact cancellation
+    assert np.isclose(g[0, 0] * PI, _golden_frac("gross_collinear_a_times_pi"), rtol=1e-14)
+    assert np.isclose(g[0, 1] * PI, _golden_frac("gross_collinear_e_times_pi"), rtol=1e-14)
+    # the outer particles have one term each: S = |value| again, half of the middle particle's S per unit mass
+    assert np.allclose(g[1:, 0], np.linalg.norm(f[1:, :3], axis=1), rtol=1e-14)
+    assert np.allclose(g[1:, 1], np.abs(f[1:, 3]), rtol=1e-14)
+    assert np.isclose(g[1, 0] * 2 * posm[1, 3] / posm[0, 3], g[0, 0], rtol=1e-14)   # term m_0 Pi |grad| vs 2 terms m_1 Pi |grad|
+    # (3) unequal neighbour masses: net and gross differ
+    posm[2, 3] = 1.0
+    f, g = oracle.forces(posm, vele, rho, h, off, idx, with_gross=True, **kw)
+    assert np.isclose(f[0, 0] * PI, _golden_frac("gross_unequal_net_times_pi"), rtol=1e-14)
+    assert np.isclose(g[0, 0] * PI, _golden_frac("gross_unequal_a_times_pi"), rtol=1e-14)
+    assert f[0, 1] == 0 and f[0, 2] == 0
+    # S never falls below the value it bounds, on a dense random gas (triangle inequality), and is invariant under
+    # relabelling of the neighbours (a sum of magnitudes has no order)
+    posm, vele, h = _dense_gas()
+    n = len(posm)
+    off, idx = oracle.neighbours(posm, n, h)
+    rho = oracle.density(posm, h, off, idx)
+    f, g = oracle.forces(posm, vele, rho, h, off, idx, with_gross=True)
+    assert np.all(g[:, 0] >= np.linalg.norm(f[:, :3], axis=1) * (1 - 1e-12))
+    assert np.all(g[:, 1] >= np.abs(f[:, 3]) * (1 - 1e-12))
+
+
 def test_A9_coincident_pair_contributes_density_only():
     h = 0.5
     posm = np.array([[1, 1, 1, 0.2], [1, 1, 1, 0.3], [1.3, 1, 1, 0.1]], dtype=np.float32)
