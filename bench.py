@@ -4,15 +4,22 @@
     python bench.py --gpus N --steps K --warmup W [--config C] [--impl reference]
 
 One "step" = one sph_step (all §8(a) rows: HFC x2, SU x2, grid sort, density, PP gravity).
-Prints ONE JSON line (see DESIGN.md §7 for every key).  --gpus N (under torchrun, one rank per GPU) splits
-the O(N^2) gravity stage by target slices (the paper's N/k-per-GPU decomposition, L139) with one NCCL
-all-gather of the acceleration slices per force evaluation; total work is fixed ("scaling": "strong").
+Prints ONE JSON line (see DESIGN.md §7 for every key).
+
+--gpus N > 1: one rank per GPU.  Started plainly (`python bench.py --gpus N`) the script re-launches itself under
+`python -m torch.distributed.run --nproc-per-node N` (and fails loudly if the box has fewer than N devices); started
+by torchrun it takes RANK / LOCAL_RANK / WORLD_SIZE from the environment.  Every rank keeps the whole state and does
+its SHARE of the O(N^2) gravity stage (the paper's N/k-per-GPU decomposition, L139): on the
+pair-symmetric path (every BASELINE config from config 1 up) the work items rank, rank + N, ... with one int64 SUM
+all-reduce of the fixed-point sums per evaluation; on the one-sided path target slices with one all-gather of the
+acceleration rows.  Total work is fixed ("scaling": "strong").
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
 import subprocess
 import sys
 import tempfile
@@ -35,13 +42,48 @@ def _peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
-def workload_config(args, w, grid_dims=None, cells=None, world=1):
+def parallelism_text(world, path=None):
+    """What the N > 1 run does per force evaluation, from the gravity path the device chose (sph_gravity_path)."""
+    if world <= 1:
+        return "single GPU"
+    if path is None:
+        how = "gravity shared over the GPUs, one collective per evaluation (int64 all-reduce or all-gather, by the path the device chooses)"
+    elif path.startswith("pair_symmetric"):
+        how = (f"gravity: unordered-pair work items rank, rank+{world}, ... per GPU + 1 int64 SUM all-reduce of the "
+               f"fixed-point sums (24 B x N) per evaluation")
+    elif path == "none":
+        how = "no gravity (G = 0): no collective"
+    else:
+        how = f"gravity: target slices of N/{world} per GPU + 1 all-gather of the acceleration rows (16 B x N/{world} per GPU) per evaluation"
+    return how + "; O(N) and SPH stages replicated"
+
+
+def workload_config(args, w, grid_dims=None, cells=None, world=1, path=None):
     """The `config` object of the JSON line: identical for both arms (ours / reference)."""
     src = f"BASELINE.json configs[{args.config}]" if args.config <= 4 else "SURVEY.md 8(f) NEXT-3 (collisionless, not a BASELINE config)"
     return {"workload": f"{src} ({w.name}): N={w.n_total}, N_g={w.n_gas}, h={w.h:g}, delta={w.delta:g}, dt={w.dt:g}",
-            "grid_dims": grid_dims, "cells": cells, "parallelism": (f"gravity targets sliced N/{world} per GPU + 1 all-gather of acc_grav per evaluation; O(N) and SPH stages replicated"
-                            if world > 1 else "single GPU"),
+            "grid_dims": grid_dims, "cells": cells, "parallelism": parallelism_text(world, path),
             "l2": "no flush: one step streams >300 MB (cell arrays, gravity partials, particle arrays) > 126 MB L2"}
+
+
+def free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def launch_ranks(n: int, script: str, argv, check_devices: bool = True) -> int:
+    """Start `script argv` as n ranks on this node, the way the driver does for N > 1:
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node n --master-addr 127.0.0.1 --master-port P script argv.
+    Returns the launcher's exit code.  check_devices: refuse (loudly) when the box has fewer than n CUDA devices."""
+    if check_devices:
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < n:
+            raise SystemExit(f"bench.py: --gpus {n} needs {n} CUDA devices, this box has {have}")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr",
+           "127.0.0.1", "--master-port", str(free_port()), script, *argv]
+    return subprocess.call(cmd)
 
 
 def reduce_max_ms(ms: float, world: int, device: str = "cuda") -> float:
@@ -212,6 +254,9 @@ def run_ours(args, w):
     rank, local_rank, world = _env_rank()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device — the product path has no CPU fallback")
+    if local_rank >= torch.cuda.device_count():
+        raise SystemExit(f"bench.py: rank {rank} needs CUDA device {local_rank}; --gpus {world} needs {world} devices, "
+                         f"this box has {torch.cuda.device_count()}")
     torch.cuda.set_device(local_rank)
     # under torchrun (any world size, also 1) the sharded path runs, collective included; plain `python bench.py` is
     # the single-GPU sph_step path
@@ -227,7 +272,7 @@ def run_ours(args, w):
         sim = ShardedSimulation(w, rank, world, sigma=args.sigma)
     else:
         sim = b.Simulation(w, sigma=args.sigma)
-    n_slice = (sim.i1 - sim.i0) if use_dist else n           # this rank's gravity targets
+    share = 1.0 / world                                       # this rank's part of the N^2 interactions (work items or target slice)
     M = sim.grid.M if ng else 0
 
     def barrier():
@@ -239,6 +284,9 @@ def run_ours(args, w):
     for _ in range(max(args.warmup, 3)):
         sim.step()
     barrier()
+    sim_steps = args.steps
+    if use_dist:
+        sim.exchanged_bytes = 0
     sampler = ClockSampler(local_rank) if rank == 0 else None
     launches0 = b.sph_launch_count()
     b.sph_set_profiling(True)
@@ -310,7 +358,7 @@ def run_ours(args, w):
     alu_peak_tflops = 2 * 128 * SM_COUNT_B200 * sm_max * 1e6 / 1e12
     roofline = None
     if w.G != 0.0 and grav_ms > 0:
-        achieved = FLOPS_PER_INTERACTION * float(n_slice) * float(n) / (grav_ms * 1e-3) / 1e12   # per GPU (rank 0's slice)
+        achieved = FLOPS_PER_INTERACTION * share * float(n) * float(n) / (grav_ms * 1e-3) / 1e12   # per GPU (rank 0's share)
         path = b.sph_gravity_path(sim.ws, ng, n, sim.grid)           # chosen on the device
         # FP32 lane-operations the variant really executes per INTERACTION (an FMA counted once) and its dominant kernel
         kernel, ops = {"pair_symmetric": ("grav_sym_kernel", 7.0), "pair_symmetric_general": ("grav_sym_kernel", 8.0),
@@ -325,7 +373,7 @@ def run_ours(args, w):
                     "peak_source": f"2*128*148*sm_max_mhz ({peak_src} sm_max_mhz={sm_max:.0f}); 20 flops/interaction",
                     "kernel_ms": grav_ms, "launches_per_step": 1, "gravity_path": path,
                     "executed_lane_ops_per_interaction": ops,
-                    "fp32_pipe_util": ops * float(n_slice) * float(n) / (grav_ms * 1e-3) / lane_peak,
+                    "fp32_pipe_util": ops * share * float(n) * float(n) / (grav_ms * 1e-3) / lane_peak,
                     "note": "achieved = ALGORITHMIC flops (BASELINE.json convention: 20 per ordered interaction, N^2 of them) / "
                             "gravity stage time (pack + kernel + reduce; the O(N) kernels are <0.1%).  The pair-symmetric "
                             "kernel evaluates each UNORDERED pair once (14 FP32 lane-ops + 1 MUFU per pair = 7 + 0.5 per "
@@ -363,10 +411,13 @@ def run_ours(args, w):
         "metric": "step_ms", "value": ms_step, "unit": "ms", "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_step, "higher_is_better": False, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "config": dict(workload_config(args, w, list(sim.grid.dims) if ng else None, M, world),
+        "config": dict(workload_config(args, w, list(sim.grid.dims) if ng else None, M, world,
+                                       getattr(sim, "path", None) if use_dist else None),
                        **({"smoothing_lengths": f"per particle, sigma={args.sigma:g}, cap h"} if args.sigma is not None else {})),
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "stages": stages,
+        "exchange": ({"gravity_path": sim.path, "payload_bytes_per_rank_per_step": sim.exchanged_bytes // max(sim_steps, 1),
+                      "collectives_per_evaluation": 0 if sim.path == "none" else 1} if use_dist else None),
         "context": "paper Table 1 (K40, N=2^20, units inferred as s): t_SPH=7.87, t_GFC=53.62 — other hardware, not a target",
     }
     print(json.dumps(line), flush=True)
@@ -390,6 +441,14 @@ def main():
     ap.add_argument("--cpu-targets", type=int, default=32768)
     ap.add_argument("--ref-targets", type=int, default=8192)
     args = ap.parse_args()
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+    under_launcher = "RANK" in os.environ and "WORLD_SIZE" in os.environ
+    if under_launcher and int(os.environ["WORLD_SIZE"]) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but the launcher started WORLD_SIZE={os.environ['WORLD_SIZE']} ranks")
+    if args.gpus > 1 and not under_launcher and args.impl == "ours":
+        # started plainly: become N ranks (one per GPU) ourselves; rank 0 of the children prints the JSON line
+        raise SystemExit(launch_ranks(args.gpus, os.path.abspath(__file__), sys.argv[1:]))
     from paper_1807_08116_b200 import workloads as wl
     w = wl.make_workload(args.config, scale=args.scale)
     if args.impl == "reference":

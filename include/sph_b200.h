@@ -215,12 +215,16 @@ int sph_neighbour_lists_h(const float* posm, const float* hsml, int64_t n_gas, f
                           uint64_t* nbr_offset, uint32_t* nbr_index, uint64_t nbr_capacity,
                           void* ws, size_t ws_bytes, void* stream);
 
-/* ---- the stages of a step, and target slices, for the N/k-per-GPU decomposition (L133-139) ----
+/* ---- the stages of a step, target slices and shares, for the N/k-per-GPU decomposition (L133-139) ----
  * The paper gives each of k GPUs N/k particles and copies the other GPUs' particles over before GFC (L139).  Here every
- * GPU keeps the whole (replicated) state and computes the O(N^2) stage — gravity, 99.9 % of the step — only for its own
- * TARGET slice [i0, i1) against all N sources; the caller then exchanges the acc_grav slices (one all-gather of
- * 16 B x N/k per GPU; paper_1807_08116_b200/binding.py ShardedSimulation does it with torch.distributed / NCCL) and all
- * GPUs run the O(N) and SPH stages redundantly — they are deterministic, so the replicas stay bitwise identical.
+ * GPU keeps the whole (replicated) state and computes only its part of the O(N^2) stage — gravity, 99.8 % of the step.
+ * The part has two forms, by the gravity kernel the device chooses: on the pair-symmetric path a
+ * SHARE of the unordered-pair work items, whose 64-bit fixed-point sums the caller adds over the GPUs (one integer SUM
+ * all-reduce, 24 B x N); on the one-sided path a TARGET SLICE [i0, i1) against all N sources, whose acceleration rows the
+ * caller gathers (one all-gather, 16 B x N/k per GPU).  See sph_position_share below;
+ * paper_1807_08116_b200/sharded.py (ShardedSimulation) drives it with torch.distributed / NCCL and issues the one
+ * collective the chosen path needs.  All GPUs run the O(N) and SPH stages redundantly — they are deterministic, so the
+ * replicas stay bitwise identical.
  *
  * nbody_pp_gravity_slice: Eq. 4 for targets [i0, i1) only; rows outside the slice of acc_grav are not touched.
  * sph_position_slice:     SP, DC (+ renewal of hsml if sigma > 0, as in sph_step_h), GFC for targets [i0, i1):

@@ -3,16 +3,19 @@
 The paper gives each of k GPUs N/k particles and, before the gravity kernel, copies the other GPUs' particles
 over GPU-Direct (L139).  Here every rank keeps the whole state (64 B per particle: nothing at 180 GB per GPU) and
 computes its SHARE of the O(N^2) gravity stage (`sph_position_share`).  Which gravity kernel runs is decided on the
-device, so a share has two forms and both exchanges are issued every evaluation (41 MiB in total at N = 2^20 against
-~0.26 s / k of gravity, so there is nothing to gain from fusing them into the kernel):
-  * pair-symmetric path (positive masses, delta > 0 — every BASELINE.json config): the rank's work items of the unordered-pair
-    decomposition, accumulated as 64-bit fixed-point integers; ONE integer SUM all-reduce of that region.  Integer
-    addition is exact, so every world size gives the same bits as one GPU.
-  * one-sided path (delta = 0, a zero mass, ...): the rank's TARGET slice against all N sources; ONE all-gather of
-    the acceleration slices.
-`nbody_pp_gravity_finish` then writes the accelerations from whichever applies.  The O(N) and SPH stages (0.2 % of
-the step) run redundantly on every rank; they are deterministic, so the replicas stay bitwise identical and no other
-exchange is needed.
+device, identically on every rank (the replicas hold the same bits), so after the share each rank reads the choice back
+(`sph_gravity_path`, one 8-byte read) and issues the ONE collective that path needs:
+  * pair-symmetric path (positive masses, delta > 0, N >= 32768 — every BASELINE.json config from config 1 up): the
+    rank's work items of the unordered-pair decomposition, accumulated as 64-bit fixed-point integers; one integer SUM
+    all-reduce of that region (24 B x N: 25 MiB at N = 2^20).  Integer addition is exact, so every world size gives the
+    same bits as one GPU.
+  * one-sided path (delta = 0, a zero mass, small N, ...): the rank's TARGET slice against all N sources; one
+    all-gather of the acceleration slices (16 B x N/k per rank).
+  * G = 0 (config 4): Eq. 4 is identically zero — no collective at all.
+`nbody_pp_gravity_finish` then writes the accelerations from the summed integers if that path was taken.  The exchange is
+~25 MiB against ~0.26 s / k of gravity at N = 2^20, so there is nothing to gain from fusing it into the kernel.  The O(N)
+and SPH stages (0.2 % of the step) run redundantly on every rank; they are deterministic, so the replicas stay bitwise
+identical and no other exchange is needed.
 
 This module holds no arithmetic of the method: slice bookkeeping, buffers and the collective.
 """
@@ -45,13 +48,17 @@ def allreduce_sums(sums: torch.Tensor, world: int, group=None) -> None:
     dist.all_reduce(sums, op=dist.ReduceOp.SUM, group=group)
 
 
-def allgather_rows(full: torch.Tensor, rank: int, world: int, chunk: int, group=None) -> None:
+def allgather_rows(full: torch.Tensor, rank: int, world: int, chunk: int, group=None, send: torch.Tensor = None) -> None:
     """`full` has world * chunk rows; rank r has written rows [r * chunk, (r+1) * chunk).  After the call every
-    rank holds all rows.  Works for any backend (NCCL on the GPUs, gloo in the CPU tests)."""
+    rank holds all rows.  Works for any backend (NCCL on the GPUs, gloo in the CPU tests).  `send`: a persistent
+    [chunk, ...] staging buffer (the input of an all-gather must not alias its output); allocated if not given."""
     if world == 1 and not dist.is_initialized():
         return                                   # no process group: plain single-GPU use of the staged calls
     assert full.shape[0] == world * chunk and full.is_contiguous()
-    send = full[rank * chunk:(rank + 1) * chunk].clone()
+    mine = full[rank * chunk:(rank + 1) * chunk]
+    if send is None:
+        send = torch.empty_like(mine)
+    send.copy_(mine)
     dist.all_gather_into_tensor(full, send, group=group)
 
 
@@ -83,13 +90,27 @@ class ShardedSimulation:
         if sigma is not None and self.n_gas > 0:
             self.hsml = torch.full((self.n_gas,), float(np.float32(w.h)), dtype=torch.float32, device=device)
         self.first = True
+        self._send = None                        # staging buffer of the all-gather, made on first use
+        self.path = None                         # gravity path of the last evaluation (sph_gravity_path)
+        self.exchanged_bytes = 0                 # payload this rank handed to collectives so far (bench.py reports it)
 
     def _position(self, sigma):
         b = self.b
         b.sph_position_share(self.posm, self.hsml, sigma, self.n_gas, self.n_halo, self.rank, self.world, self.i0, self.i1,
                              self.params, self.grid, self.rho, self.acc_grav, self.ws)
-        allreduce_sums(self.sums, self.world, self.group)                       # pair-symmetric path
-        allgather_rows(self.acc_grav, self.rank, self.world, self.chunk, self.group)   # one-sided path
+        if self.params.G == 0.0 or self.n == 0:
+            self.path = "none"                   # Eq. 4 is identically 0: the share zeroed its rows, nothing to exchange
+            return
+        # the device's choice — the same on every rank, because every rank holds the same bits
+        self.path = b.sph_gravity_path(self.ws, self.n_gas, self.n, self.grid)
+        if self.path.startswith("pair_symmetric"):
+            allreduce_sums(self.sums, self.world, self.group)
+            self.exchanged_bytes += self.sums.numel() * 8
+        else:
+            if self._send is None:
+                self._send = torch.empty_like(self.acc_grav[:self.chunk])
+            allgather_rows(self.acc_grav, self.rank, self.world, self.chunk, self.group, self._send)
+            self.exchanged_bytes += self.chunk * 16
         b.nbody_pp_gravity_finish(self.posm, self.n_gas, self.n_halo, self.grid, self.params.G, self.acc_grav, self.ws)
 
     def step(self, dt=None):

@@ -29,7 +29,11 @@ MED_TOL = 1e-5
 # ceilings on the reach of the floors (fractions of the non-zero reference values, and the largest loosening)
 MEDIAN_FLOOR_MAX_FRACTION = 0.02     # values below 1e-3 of the array's median magnitude
 GROSS_FLOOR_MAX_FRACTION = 0.01      # values below 1e-3 of their own gross sum
-GROSS_FLOOR_MAX_LOOSENING = 100.0    # i.e. a net value cancelled below 1e-5 of what was summed fails the test
+# The ratio |net| / S of a cancelling sum has a finite density at 0, so among the touched values the loosening L is
+# distributed like P(> L) = 1/L: a ceiling of 100 fired on a legitimate value at config 3 (1 of ~30 touched values over
+# the 11 evaluations, x160).  The count ceiling above is what guards against a wrong (too large) S; this one only stops
+# a value that is numerically nothing (< 1e-7 of what was summed) from being compared at all.
+GROSS_FLOOR_MAX_LOOSENING = 1.0e4
 
 REPORT = []          # one dict per check_values call, printed by conftest.pytest_terminal_summary
 

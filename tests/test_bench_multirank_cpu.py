@@ -56,7 +56,13 @@ def test_config_is_shared_by_both_arms():
     c1 = bench.workload_config(a, w, [3, 4, 5], 60, 1)
     c2 = bench.workload_config(a, w, [3, 4, 5], 60, 2)
     assert c1["workload"] == c2["workload"] and "configs[0]" in c1["workload"]
-    assert c1["parallelism"] == "single GPU" and "N/2 per GPU" in c2["parallelism"]
+    assert c1["parallelism"] == "single GPU" and "one collective per evaluation" in c2["parallelism"]
+    # the text follows the path the device chose: work items + int64 all-reduce, or target slices + all-gather
+    sym = bench.workload_config(a, w, [3, 4, 5], 60, 2, "pair_symmetric")["parallelism"]
+    one = bench.workload_config(a, w, [3, 4, 5], 60, 2, "one_sided_uniform")["parallelism"]
+    assert "int64 SUM all-reduce" in sym and "all-gather" not in sym
+    assert "all-gather" in one and "all-reduce" not in one and "N/2 per GPU" in one
+    assert "no collective" in bench.workload_config(a, w, [3, 4, 5], 60, 2, "none")["parallelism"]
 
 
 # ---------------------------------------------------------------- NEXT-4: slices and the exchange (host logic)
@@ -153,6 +159,10 @@ class _StubBinding:
     def sph_grid_from_bbox(self, posm, n_gas, h):
         return "grid"
 
+    def sph_gravity_path(self, ws, n_gas, n, grid):
+        self.calls.append("path")
+        return "pair_symmetric" if self.pair_symmetric else "one_sided"
+
     def alloc_workspace(self, n_gas, n, grid):
         return torch.zeros(64 + 24 * 4096, dtype=torch.uint8)
 
@@ -204,8 +214,9 @@ def _sharded_worker(rank, world, port, out):
 
 def test_sharded_step_exchange_gloo_world2():
     """The N > 1 step on CPU (gloo, world 2) with a stand-in for the library: per force evaluation every rank calls
-    share -> integer all-reduce -> all-gather -> finish, in that order, twice in the first step (seeding + the step);
-    what finish sees is the SUM of the ranks' fixed-point parts and ALL ranks' acceleration rows."""
+    share -> path read-back -> the ONE collective that path needs -> finish, in that order, twice in the first step
+    (seeding + the step); what finish sees is the SUM of the ranks' fixed-point parts (pair-symmetric path) or ALL
+    ranks' acceleration rows (one-sided path), and the other buffer is NOT exchanged."""
     import numpy as np
     world, port = 2, _free_port()
     mgr = mp.Manager()
@@ -215,12 +226,53 @@ def test_sharded_step_exchange_gloo_world2():
     for rank in range(world):
         for sym in (True, False):
             calls, sums, acc, (i0, i1) = out[rank][sym]
-            assert calls == ["share", "finish", "predict", "share", "finish", "correct"]
+            assert calls == ["share", "path", "finish", "predict", "share", "path", "finish", "correct"]
             if sym:
                 assert np.array_equal(sums, 3 * k)                           # (1 + 2) * k: both ranks' parts, exact
+                assert np.all(acc == 0)                                      # no all-gather on this path
             else:
+                assert np.all(sums == 0)                                     # no all-reduce on this path
                 b0 = out[0][sym][3]
                 b1 = out[1][sym][3]
                 assert b0[0] == 0 and b0[1] == b1[0] and b1[1] == 2500       # the slices tile [0, n)
                 assert np.all(acc[b0[0]:b0[1]] == 1.0) and np.all(acc[b1[0]:b1[1]] == 2.0)
     assert np.array_equal(out[0][True][1], out[1][True][1]) and np.array_equal(out[0][False][2], out[1][False][2])
+
+
+# ---------------------------------------------------------------- `python bench.py --gpus N` starts its own ranks
+def test_bench_gpus_without_devices_fails_loudly():
+    """On a box with fewer than N CUDA devices `python bench.py --gpus N` must refuse, not measure one GPU silently."""
+    import subprocess
+    if torch.cuda.is_available() and torch.cuda.device_count() >= 2:
+        pytest.skip("box has 2 GPUs")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--config", "0"],
+                       capture_output=True, text=True, timeout=300)
+    assert r.returncode != 0 and "needs 2 CUDA devices" in (r.stderr + r.stdout)
+    # a launcher that started another number of ranks than --gpus says is refused as well
+    env = dict(os.environ, RANK="0", WORLD_SIZE="4", LOCAL_RANK="0", MASTER_ADDR="127.0.0.1", MASTER_PORT="29999")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--config", "0"],
+                       capture_output=True, text=True, timeout=300, env=env)
+    assert r.returncode != 0 and "WORLD_SIZE=4" in (r.stderr + r.stdout)
+
+
+def test_bench_launch_ranks_world2_gloo(tmp_path):
+    """bench.launch_ranks — the code path `python bench.py --gpus 2` takes — started for 2 ranks on CPU: the probe
+    script below is what bench.py's ranks do with the GPU parts replaced (gloo instead of NCCL, the recording stand-in
+    instead of the library): rendezvous from the launcher's environment, ShardedSimulation steps with their collective,
+    barrier, max over ranks, ONE JSON line from rank 0."""
+    import json
+    import subprocess
+    sys.path.insert(0, ROOT)
+    import bench
+    out = tmp_path / "line.json"
+    probe = os.path.join(ROOT, "tests", "spawn_probe.py")
+    code = (f"import sys; sys.path.insert(0, {ROOT!r}); import bench; "
+            f"sys.exit(bench.launch_ranks(2, {probe!r}, ['--out', {str(out)!r}], check_devices=False))")
+    r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in open(out).read().splitlines() if ln.strip()]
+    assert len(lines) == 1                                   # rank 0 alone reports
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["ranks_seen"] == [0, 1] and d["value"] == 15.0      # max over ranks of 10, 15
+    assert d["calls"] == ["share", "path", "finish", "predict", "share", "path", "finish", "correct"]
+    assert d["parallelism"] == bench.parallelism_text(2, "pair_symmetric")

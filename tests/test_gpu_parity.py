@@ -83,7 +83,7 @@ def test_gravity_zero_softening_and_duplicates(cuda_lib):
     b.nbody_pp_gravity(d, n, 1.0, 0.0, acc, ws)
     got = acc.cpu().numpy()
     assert np.all(np.isfinite(got))
-    check_values(got[:, :3], oracle.gravity(posm, 1.0, 0.0), "a_grav delta=0", max_tol=5e-4, med_tol=2e-5)
+    check_values(got[:, :3], oracle.gravity(posm, 1.0, 0.0), "a_grav delta=0")
 
 
 def test_gravity_medium_subset(cuda_lib):
@@ -781,8 +781,7 @@ def test_gravity_mass_variants_large_shape(cuda_lib, masses):
     # delta = 0 goes through the same two variants
     b.nbody_pp_gravity(d, n, w.G, 0.0, acc, ws)
     got0 = acc.cpu().numpy()
-    check_values(got0[tg, :3], oracle.gravity(posm, w.G, 0.0, targets=tg), f"a_grav delta=0 masses={masses}",
-                 max_tol=5e-4, med_tol=2e-5)
+    check_values(got0[tg, :3], oracle.gravity(posm, w.G, 0.0, targets=tg), f"a_grav delta=0 masses={masses}")
 
 
 # ---------------------------------------------------------------- (a10) pair-symmetric gravity path
@@ -844,7 +843,7 @@ def test_gravity_path_selection(cuda_lib):
     p = w.posm.copy()
     p[:, 3] = ((0.2 + rng.random(n)) / n).astype(np.float32)
     check(p, w.delta, "pair_symmetric_general", "random masses")
-    check(p, 0.0, "one_sided", "random masses, delta = 0", max_tol=5e-4, med_tol=2e-5)
+    check(p, 0.0, "one_sided", "random masses, delta = 0")
     p[17, 3] = 0.0                               # a massless particle: m_min = 0, no scale for the fixed-point range
     check(p, w.delta, "one_sided", "a zero mass")
     p = w.posm.copy()
@@ -853,8 +852,8 @@ def test_gravity_path_selection(cuda_lib):
     p = w.posm.copy()
     p[5, :3] = (3.0e4, 0.0, 0.0)                 # box diagonal / delta = 6e6: 2^-k would be > 2^-26 of n / R^2
     check(p, w.delta, "one_sided_uniform", "far-away particle")
-    check(w.posm, 1.0e-6, "one_sided_uniform", "tiny delta", max_tol=5e-4, med_tol=2e-5)
-    check(w.posm, 0.0, "one_sided_uniform", "delta = 0", max_tol=5e-4, med_tol=2e-5)
+    check(w.posm, 1.0e-6, "one_sided_uniform", "tiny delta")
+    check(w.posm, 0.0, "one_sided_uniform", "delta = 0")
     w0 = wl.make_workload(0)
     acc, path = _grav(b, w0.posm, w0.G, w0.delta)
     assert path == "one_sided_uniform"           # N = 8192 < 32768
