@@ -296,6 +296,14 @@ enum { SPH_GRAV_ONE_SIDED = 0, SPH_GRAV_ONE_SIDED_UNIFORM = 1, SPH_GRAV_PAIR_SYM
 int sph_gravity_path(const void* ws /*DEVICE*/, size_t ws_bytes, int64_t n_gas, int64_t n_total,
                      const sph_grid* g /*HOST, may be NULL if n_gas == 0*/, int* path_host /*HOST*/, void* stream);
 
+/* Diagnostic: how many work items the LAST density / forces / grid-building call enqueued with workspace `ws` (sized for
+ * n_gas, n_total and g, as in that call) handed to the dense-cell walk of the neighbour passes (DESIGN.md section 5.3:
+ * cells holding at least 32 particles, 128 targets per item; the DC / HFC sums of PAPER.md L143-145, L207 over the cell
+ * lists).  0 means every particle was walked by the thread-per-slot kernels.  Reads the counter back and SYNCHRONISES
+ * `stream`.                                                                                                        */
+int sph_dense_items(const void* ws /*DEVICE*/, size_t ws_bytes, int64_t n_gas, int64_t n_total,
+                    const sph_grid* g /*HOST*/, uint32_t* items_host /*HOST*/, void* stream);
+
 /* Number of kernel launches this library has enqueued in the calling process since load. */
 int64_t sph_launch_count(void);
 

@@ -26,7 +26,7 @@ EXPORTS = (
     "sph_host_ctx_create", "sph_host_ctx_step", "sph_host_ctx_destroy", "sph_neighbour_lists",
     "sph_set_profiling", "sph_get_stage_ms", "sph_launch_count", "sph_cfl_dt",
     "nbody_pp_gravity_slice", "sph_position_slice", "sph_predict", "sph_correct",
-    "sph_gravity_path", "sph_position_share", "nbody_pp_gravity_share", "nbody_pp_gravity_finish",
+    "sph_gravity_path", "sph_dense_items", "sph_position_share", "nbody_pp_gravity_share", "nbody_pp_gravity_finish",
     "sph_workspace_gravity_sums", "sph_smoothing_lengths", "sph_density_h", "sph_forces_h", "sph_evaluate_h", "sph_step_h", "sph_neighbour_lists_h",
 )
 
@@ -98,6 +98,7 @@ def load():
     L.nbody_pp_gravity_finish.argtypes = [vp, i64, i64, gp, f32, vp, vp, sz, vp]
     L.sph_workspace_gravity_sums.argtypes = [i64, i64, gp, C.POINTER(sz), C.POINTER(sz)]
     L.sph_gravity_path.argtypes = [vp, sz, i64, i64, gp, C.POINTER(C.c_int), vp]
+    L.sph_dense_items.argtypes = [vp, sz, i64, i64, gp, C.POINTER(C.c_uint32), vp]
     L.sph_cfl_dt.argtypes = [vp, vp, vp, vp, vp, i64, pp, gp, vp, vp, f32, vp, vp, vp, sz, vp]
     L.sph_step.argtypes = [vp, vp, i64, i64, pp, gp, f32, C.c_int, vp, vp, vp, vp, sz, vp]
     L.sph_evaluate.argtypes = [vp, vp, i64, i64, pp, gp, vp, vp, vp, vp, sz, vp]
@@ -394,6 +395,14 @@ def sph_gravity_path(ws, n_gas, n_total, grid=None) -> str:
     g = C.byref(grid) if grid is not None else None
     _chk("sph_gravity_path", load().sph_gravity_path(p, nb, int(n_gas), int(n_total), g, C.byref(out), _stream()))
     return GRAV_PATHS[out.value]
+
+
+def sph_dense_items(ws, n_gas, n_total, grid) -> int:
+    """Work items the last density / forces / grid-building call with `ws` gave to the dense-cell walk (0: none)."""
+    p, nb = _ws(ws)
+    out = C.c_uint32(0)
+    _chk("sph_dense_items", load().sph_dense_items(p, nb, int(n_gas), int(n_total), C.byref(grid), C.byref(out), _stream()))
+    return int(out.value)
 
 
 def sph_launch_count() -> int:

@@ -55,7 +55,7 @@ int position_only(const float4* posm, float* hsml, float sigma, int64_t n_gas, i
         {
             Span sp(ST_SORT, st);
             SPHB_TRY(grid_build(posm, n_gas, g, w.key, w.perm, w.cell_count, w.cell_start, w.rank_u, w.tmp, w.tile_sums,
-                                w.posm_s, st));
+                                w.posm_s, &w.dense, st));
             if (hsml) SPHB_TRY(gather_sorted_h(hsml, w.perm, n_gas, w.h_s, st));
         }
         {
@@ -82,8 +82,8 @@ int hydro(const float4* vele, const float* rho, bool varh, int64_t n_gas, const 
           float4* acc_sph, const Workspace& w, cudaStream_t st) {
     if (n_gas <= 0) return SPH_OK;
     Span sp(ST_FORCES, st);
-    return forces_sorted(w.posm_s, vele, rho, varh ? w.h_s : nullptr, w.perm, w.cell_start, n_gas, p, g, w.velr_s, w.pc_s,
-                         acc_sph, st);
+    return forces_sorted(w.posm_s, vele, rho, varh ? w.h_s : nullptr, w.perm, w.cell_start, n_gas, p, g, &w.dense, w.velr_s,
+                         w.pc_s, acc_sph, st);
 }
 
 int check_state_args(const void* posm, const void* vele, int64_t n_gas, int64_t n_halo, const sph_params* p,
@@ -176,7 +176,7 @@ int sph_build_grid(const float* posm, int64_t n_gas, const sph_grid* g, uint32_t
     cudaStream_t st = (cudaStream_t)stream;
     Span sp(ST_SORT, st);
     return grid_build(reinterpret_cast<const float4*>(posm), n_gas, g, key, perm, cell_count, cell_start, w.rank_u, w.tmp,
-                      w.tile_sums, nullptr, st);
+                      w.tile_sums, nullptr, &w.dense, st);
 }
 
 int sph_density(const float* posm, int64_t n_gas, const sph_params* p, const sph_grid* g, const uint32_t* perm,
@@ -209,9 +209,10 @@ int sph_forces(const float* posm, const float* vele, const float* rho, int64_t n
     if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
+    SPHB_TRY(dense_list_from_start(cell_start, g, w.dense, st));
     Span sp(ST_FORCES, st);
-    return forces_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, nullptr, perm, cell_start, n_gas, p, g, w.velr_s,
-                         w.pc_s, reinterpret_cast<float4*>(acc_sph), st);
+    return forces_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, nullptr, perm, cell_start, n_gas, p, g, &w.dense,
+                         w.velr_s, w.pc_s, reinterpret_cast<float4*>(acc_sph), st);
 }
 
 int sph_cfl_dt(const float* posm, const float* vele, const float* rho, const float* acc_sph, const float* acc_grav,
@@ -261,6 +262,17 @@ int sph_gravity_path(const void* ws, size_t ws_bytes, int64_t n_gas, int64_t n_t
     SPHB_CUDA(cudaStreamSynchronize(st));
     *path_host = ctl[1] != 0u ? (ctl[0] != 0u ? SPH_GRAV_PAIR_SYMMETRIC_GENERAL : SPH_GRAV_PAIR_SYMMETRIC)
                               : (ctl[0] != 0u ? SPH_GRAV_ONE_SIDED : SPH_GRAV_ONE_SIDED_UNIFORM);
+    return SPH_OK;
+}
+
+int sph_dense_items(const void* ws, size_t ws_bytes, int64_t n_gas, int64_t n_total, const sph_grid* g, uint32_t* items_host,
+                    void* stream) {
+    if (!ws || !items_host || bad_count(n_total) || bad_count(n_gas) || n_gas <= 0 || !g) return SPH_ERR_ARG;
+    Workspace w = carve(const_cast<void*>(ws), n_gas, n_total, g);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    SPHB_CUDA(cudaMemcpyAsync(items_host, w.dense.ctl, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    SPHB_CUDA(cudaStreamSynchronize(st));
     return SPH_OK;
 }
 
@@ -457,7 +469,7 @@ int sph_forces_h(const float* posm, const float* vele, const float* rho, const f
     SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
     SPHB_TRY(gather_sorted_h(hsml, perm, n_gas, w.h_s, st));
     Span sp(ST_FORCES, st);
-    return forces_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, w.h_s, perm, cell_start, n_gas, p, g,
+    return forces_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, w.h_s, perm, cell_start, n_gas, p, g, nullptr,
                          w.velr_s, w.pc_s, reinterpret_cast<float4*>(acc_sph), st);
 }
 

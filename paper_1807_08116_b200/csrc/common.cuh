@@ -52,6 +52,22 @@ inline int64_t grid_cells(const sph_grid* g) { return (int64_t)g->dims[0] * g->d
 int check_grid(const sph_grid* g, float h);          // SPH_OK or SPH_ERR_GRID
 GridDev to_dev(const sph_grid* g);
 
+// ---- dense-cell work list (sph_dense.cu) ----------------------------------------------------
+// A cell holding at least kDenseMin particles is walked by the dense kernels, kDenseTT targets per work item; the
+// thread-per-slot kernels skip its slots.  The list is written by the grid build (k_scan_apply has every cell's
+// count in registers) or, for the stand-alone calls that get cell_start from the caller, by dense_list_from_start.
+constexpr int kDenseMin = 32;
+constexpr int kDenseTT = 128;
+struct DenseItem {
+    uint32_t key;     // cell number
+    uint32_t chunk;   // targets [start[key] + chunk kDenseTT, ... + kDenseTT) of that cell
+};
+struct DenseList {
+    unsigned int* ctl;   // device: ctl[0] = number of items
+    DenseItem* items;    // device: [dense_capacity(n_gas)]
+};
+inline size_t dense_capacity(int64_t n_gas) { return (size_t)(n_gas / kDenseMin + n_gas / kDenseTT + 16); }
+
 // ---- workspace layout (device scratch carved from the caller's ws) -------------------------
 struct Workspace {
     // grid sort
@@ -67,6 +83,7 @@ struct Workspace {
     float4* velr_s;        // [n_gas] (vx,vy,vz,rho)
     float2* pc_s;          // [n_gas] (p/rho^2, c)
     float* h_s;            // [n_gas] per-particle smoothing lengths in cell order (NEXT-2)
+    DenseList dense;       // work list of the densely populated cells
     // gravity
     float4* src_pk;        // [n_pad] packed source pairs
     float4* grav_part;     // [S][n_total] partial accelerations
@@ -90,14 +107,17 @@ int64_t grav_padded(int64_t n_total);              // sources padded to a whole 
 // ---- internal stage entry points (all enqueue on `st`, no synchronisation) -----------------
 int grid_build(const float4* posm, int64_t n_gas, const sph_grid* g, uint32_t* key, uint32_t* perm,
                uint32_t* cell_count, uint32_t* cell_start, uint32_t* rank_u, uint32_t* tmp, uint32_t* tile_sums,
-               float4* posm_s /*may be NULL*/, cudaStream_t st);
+               float4* posm_s /*may be NULL*/, const DenseList* dense /*may be NULL*/, cudaStream_t st);
+int dense_list_from_start(const uint32_t* cell_start, const sph_grid* g, const DenseList& dl, cudaStream_t st);
 int gather_sorted_pos(const float4* posm, const uint32_t* perm, int64_t n_gas, float4* posm_s, cudaStream_t st);
 // h_s: per-particle smoothing lengths in cell order (NEXT-2), or NULL for the one global p->h
 int density_sorted(const float4* posm_s, const float* h_s, const uint32_t* perm, const uint32_t* cell_start,
                    int64_t n_gas, const sph_params* p, const sph_grid* g, float* rho, cudaStream_t st);
+// dense: the work list of the densely populated cells, matching cell_start (global h only; NULL: every slot is walked
+// by the thread-per-slot kernel)
 int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const float* h_s, const uint32_t* perm,
                   const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
-                  float4* velr_s, float2* pc_s, float4* acc_sph, cudaStream_t st);
+                  const DenseList* dense, float4* velr_s, float2* pc_s, float4* acc_sph, cudaStream_t st);
 int smoothing_lengths(const float4* posm, const float* rho, int64_t n_gas, float sigma, float h_max, float* hsml,
                       cudaStream_t st);
 int gather_sorted_h(const float* hsml, const uint32_t* perm, int64_t n_gas, float* h_s, cudaStream_t st);

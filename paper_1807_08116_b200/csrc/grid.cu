@@ -19,7 +19,7 @@
 //               cell-ordered copy posm_s.
 // All results are deterministic (integer atomics commute; the fix-up removes the only order
 // the atomics decide).
-#include "common.cuh"
+#include "sph_dev.cuh"
 
 namespace sphb {
 
@@ -165,8 +165,10 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_tile_sums(const uint32_t*
 // slice [t*per, (t+1)*per): local sum, one block scan over the 1024 slice sums, local rescan —
 // a single pass whatever n_tiles is (the chunked version needed n_tiles/256 dependent block scans).
 constexpr int kOffThreads = 1024;
-__global__ void __launch_bounds__(kOffThreads) k_scan_tile_offsets(uint32_t* tile_sums, int n_tiles) {
+__global__ void __launch_bounds__(kOffThreads) k_scan_tile_offsets(uint32_t* tile_sums, int n_tiles,
+                                                                  unsigned int* dense_ctl) {
     __shared__ uint32_t ws[32];
+    if (dense_ctl && threadIdx.x == 0) *dense_ctl = 0u;   // the work list k_scan_apply is about to write
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int per = (n_tiles + kOffThreads - 1) / kOffThreads;
     const int lo = min(threadIdx.x * per, n_tiles), hi = min(lo + per, n_tiles);
@@ -200,7 +202,8 @@ __global__ void __launch_bounds__(kOffThreads) k_scan_tile_offsets(uint32_t* til
 
 __global__ void __launch_bounds__(kScanThreads) k_scan_apply(const uint32_t* __restrict__ count, int64_t M,
                                                              const uint32_t* __restrict__ tile_offsets,
-                                                             uint32_t* __restrict__ start, uint32_t n_gas) {
+                                                             uint32_t* __restrict__ start, uint32_t n_gas,
+                                                             unsigned int* dense_ctl, DenseItem* dense_items) {
     __shared__ uint32_t ws[kScanThreads / 32];
     uint32_t c[kScanItems];
     const int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
@@ -226,6 +229,12 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_apply(const uint32_t* __r
             if (base + q < M) start[base + q] = out[q];
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) start[M] = n_gas;   // A13: start[M] = N_g
+    // the densely populated cells go on the work list of sph_dense.cu (the counts are in registers here)
+    if (dense_ctl && s >= (uint32_t)kDenseMin) {
+#pragma unroll
+        for (int q = 0; q < kScanItems; ++q)
+            if (c[q] >= (uint32_t)kDenseMin) dense_append((uint32_t)(base + q), c[q], dense_ctl, dense_items);
+    }
 }
 
 // ---------------------------------------------------------------- (a4) scatter and stable fix-up
@@ -299,7 +308,7 @@ GridDev to_dev(const sph_grid* g) {
 
 int grid_build(const float4* posm, int64_t n_gas, const sph_grid* g, uint32_t* key, uint32_t* perm,
                uint32_t* cell_count, uint32_t* cell_start, uint32_t* rank_u, uint32_t* tmp, uint32_t* tile_sums,
-               float4* posm_s, cudaStream_t st) {
+               float4* posm_s, const DenseList* dense, cudaStream_t st) {
     const int64_t M = grid_cells(g);
     const int n = (int)n_gas;
     SPHB_CUDA(cudaMemsetAsync(cell_count, 0, (size_t)M * sizeof(uint32_t), st));          // K0
@@ -310,9 +319,10 @@ int grid_build(const float4* posm, int64_t n_gas, const sph_grid* g, uint32_t* k
     const int n_tiles = (int)cdiv(M, kScanTile);
     k_scan_tile_sums<<<n_tiles, kScanThreads, 0, st>>>(cell_count, M, tile_sums);          // K2 (in-block)
     SPHB_LAUNCHED();
-    k_scan_tile_offsets<<<1, kOffThreads, 0, st>>>(tile_sums, n_tiles);                   // K2 (across blocks)
+    k_scan_tile_offsets<<<1, kOffThreads, 0, st>>>(tile_sums, n_tiles, dense ? dense->ctl : nullptr);   // K2 (across blocks)
     SPHB_LAUNCHED();
-    k_scan_apply<<<n_tiles, kScanThreads, 0, st>>>(cell_count, M, tile_sums, cell_start, (uint32_t)n);   // K3
+    k_scan_apply<<<n_tiles, kScanThreads, 0, st>>>(cell_count, M, tile_sums, cell_start, (uint32_t)n,
+                                                   dense ? dense->ctl : nullptr, dense ? dense->items : nullptr);   // K3
     SPHB_LAUNCHED();
     if (n > 0) {
         k_scatter<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(key, rank_u, cell_start, n, tmp);                 // K4

@@ -10,27 +10,9 @@
 //
 // Cutoff predicate (A8), identical op sequence to the oracle:
 //   dx = x_i (-) x_j ...  d2 = fma(dz,dz, fma(dy,dy, dx*dx))  neighbour iff d2 < fl(fl(2h)^2).
-#include "common.cuh"
+#include "sph_dev.cuh"
 
 namespace sphb {
-
-struct RunCtx {
-    int mx, my, mz;
-};
-
-__device__ __forceinline__ float dist2_f32(const float4 a, const float4 b, float& dx, float& dy, float& dz) {
-    dx = __fsub_rn(a.x, b.x);
-    dy = __fsub_rn(a.y, b.y);
-    dz = __fsub_rn(a.z, b.z);
-    return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-}
-
-// cell coordinates of a particle (reading A7, same FP32 op sequence as the key kernel); no div / mod needed
-__device__ __forceinline__ void cell_of(const float4 p, const GridDev g, int& ix, int& iy, int& iz) {
-    ix = (int)fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.x, g.ox), g.inv_cell)), 0.0f), g.fx);
-    iy = (int)fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.y, g.oy), g.inv_cell)), 0.0f), g.fy);
-    iz = (int)fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.z, g.oz), g.inv_cell)), 0.0f), g.fz);
-}
 
 // 9 x-runs of the stencil of the cell (ix,iy,iz): run r -> [lo, hi) sorted slots, (0,0) outside the grid
 __device__ __forceinline__ void stencil_run(const uint32_t* __restrict__ start, const GridDev g, int ix, int iy, int iz,
@@ -44,15 +26,15 @@ __device__ __forceinline__ void stencil_run(const uint32_t* __restrict__ start, 
     }
 }
 
-// ---------------------------------------------------------------- (a7) density, Eq. 7-8
-// W(xi,h) = 1/(pi h^3) { 1 - 3/2 xi^2 + 3/4 xi^3 (xi<=1) ; 1/4 (2-xi)^3 (1<=xi<=2) ; 0 }   (L79)
-__device__ __forceinline__ float w_spline_unnorm(float xi) {
-    float t = 2.0f - xi;
-    float outer = 0.25f * t * t * t;
-    float inner = fmaf(xi * xi, fmaf(0.75f, xi, -1.5f), 1.0f);
-    return xi <= 1.0f ? inner : fmaxf(outer, 0.0f);
+// dense_min > 0: the cells holding at least that many particles belong to the dense walk (sph_dense.cu)
+__device__ __forceinline__ bool own_cell_is_dense(const uint32_t* __restrict__ start, const GridDev g, int ix, int iy,
+                                                  int iz, uint32_t dense_min) {
+    if (dense_min == 0u) return false;
+    const uint32_t k = (uint32_t)ix + (uint32_t)g.mx * ((uint32_t)iy + (uint32_t)g.my * (uint32_t)iz);
+    return start[k + 1u] - start[k] >= dense_min;
 }
 
+// ---------------------------------------------------------------- (a7) density, Eq. 7-8
 // VARH: per-particle smoothing lengths h_s[] in cell order; the pair length is
 // h_ij = (h_i + h_j)/2, the pair is a neighbour pair iff d2 < fl(fl(h_i + h_j)^2) (reading A24, FP32 like A8),
 // and W(|dr|/h_ij, h_ij) carries its own 1/(pi h_ij^3).  VARH = false is the global-h kernel, unchanged.
@@ -120,6 +102,10 @@ int gather_sorted_h(const float* hsml, const uint32_t* perm, int64_t n_gas, floa
     return SPH_OK;
 }
 
+int forces_dense(const float4* posm_s, const float4* velr_s, const float2* pc_s, const uint32_t* perm,
+                 const uint32_t* cell_start, const sph_grid* g, float rc2, const ViscDev& q, const DenseList& dl,
+                 float4* acc_sph, cudaStream_t st);   // sph_dense.cu
+
 int density_sorted(const float4* posm_s, const float* h_s /*cell order, or NULL: global h*/, const uint32_t* perm,
                    const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g, float* rho,
                    cudaStream_t st) {
@@ -157,13 +143,6 @@ __global__ void __launch_bounds__(256) k_eos_gather(const float4* __restrict__ v
 }
 
 // ---------------------------------------------------------------- (a9) hydro force, Eqs. 10-11
-struct ViscDev {
-    float h, alpha, beta, eta_h2, gw;   // gw = -45 / (64 pi h^4): grad W_p = gw (2-xi)^2 dr/|dr|
-    float inv_h2;                       // 1 / h^2
-    double rc2_64;                      // 4 h^2 in FP64 (h as given, widened)
-    float eta, gw_unit;                 // VARH: eta and -45 / (64 pi); the h powers are applied per pair
-};
-
 // Compensated (Kahan) accumulation.  The hydro terms of one particle routinely cancel by 10^2-10^3
 // and dense cells sum hundreds of them; a plain FP32 running sum loses ~sqrt(n) ulps of the GROSS
 // sum, which is what broke the 2e-4 parity bar on the clumpy configs.  Cost: 3 extra FADD per add.
@@ -182,16 +161,17 @@ template <bool VARH>
 __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_s, const float4* __restrict__ velr_s,
                                                 const float2* __restrict__ pc_s, const float* __restrict__ h_s,
                                                 const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start,
-                                                int n, GridDev g, float rc2, ViscDev q, float4* __restrict__ acc) {
+                                                int n, GridDev g, float rc2, ViscDev q, uint32_t dense_min,
+                                                float4* __restrict__ acc) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
     const float4 pi = posm_s[s];
+    int ix, iy, iz;
+    cell_of(pi, g, ix, iy, iz);
+    if (own_cell_is_dense(start, g, ix, iy, iz, dense_min)) return;   // sph_dense.cu walks that cell
     const float4 vi = velr_s[s];
     const float2 ci = pc_s[s];
     const float h_i = VARH ? h_s[s] : 0.f;
-    int ix, iy, iz;
-    cell_of(pi, g, ix, iy, iz);
-    const float inv_h_glob = 1.0f / q.h;
     KSum ax, ay, az, de;
 #pragma unroll 1
     for (int r = 0; r < 9; ++r) {
@@ -201,9 +181,7 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
             const float4 pj = posm_s[t];
             float dx, dy, dz;
             const float d2 = dist2_f32(pi, pj, dx, dy, dz);
-            // pair constants: global h, or the pair length h_ij
-            float rc2p = rc2, hh = q.h, eta_h2 = q.eta_h2;
-            float hsum = 0.f;
+            float rc2p = rc2, hsum = 0.f;
             if (VARH) {
                 hsum = __fadd_rn(h_i, h_s[t]);                     // 2 h_ij
                 rc2p = __fmul_rn(hsum, hsum);
@@ -211,36 +189,31 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
             if (d2 < rc2p && d2 > 0.f) {   // d2 == 0: self, or a coincident pair (A9) — no contribution
                 const float4 vj = velr_s[t];
                 const float2 cj = pc_s[t];
-                float rinv = rsqrtf(d2);
-                rinv = rinv * fmaf(-0.5f * d2 * rinv, rinv, 1.5f);   // one Newton step: ~1 ulp
-                const float rr = d2 * rinv;                        // |dr|
-                // 2 - xi = (4h^2 - |dr|^2) / (h^2 (2 + xi)).  Formed as 2 - rr/h in FP32 it loses a factor
-                // xi/(2-xi) of relative accuracy near the kernel edge (every term of a sparsely surrounded
-                // particle sits there), so the numerator alone is taken in FP64: 3 cvt + 3 DFMA per pair.
-                // grad W_p = dWp/dxi * dr/|dr| / h,  dWp/dxi = -45/(64 pi h^3) (2-xi)^2   (L95, Eq. 9, A3)
-                float gmag;                                        // grad W_p = gmag * dr
+                float f, rv;
                 if (VARH) {
+                    float rinv = rsqrtf(d2);
+                    rinv = rinv * fmaf(-0.5f * d2 * rinv, rinv, 1.5f);   // one Newton step: ~1 ulp
+                    const float rr = d2 * rinv;                        // |dr|
                     // the pair factor goes like h_ij^-8: with a per-pair h its roundings no longer cancel as a
                     // common factor of the particle's sum, so it is formed in FP64 and rounded once
                     const double hd = 0.5 * (double)hsum, ihd = 1.0 / hd, ih2 = ihd * ihd;
                     const double num = fma(-(double)dz, (double)dz, fma(-(double)dy, (double)dy, fma(-(double)dx, (double)dx, (double)hsum * (double)hsum)));
                     const double tqd = fmax(num, 0.0) * ih2 / (2.0 + (double)rr * ihd);       // 2 - xi
-                    gmag = (float)((double)q.gw_unit * ih2 * ih2 * tqd * tqd) * rinv;
-                    hh = 0.5f * hsum;
-                    eta_h2 = q.eta * hh * hh;
+                    const float gmag = (float)((double)q.gw_unit * ih2 * ih2 * tqd * tqd) * rinv;   // grad W_p = gmag * dr
+                    const float hh = 0.5f * hsum;
+                    const float eta_h2 = q.eta * hh * hh;
+                    const float dvx = vi.x - vj.x, dvy = vi.y - vj.y, dvz = vi.z - vj.z;
+                    rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
+                    // mu_ij = h dr.dv / (|dr|^2 + eta h^2) if dr.dv < 0   (L97)
+                    const float mu = rv < 0.f ? (hh * rv) / (d2 + eta_h2) : 0.f;       // IEEE division
+                    const float rho_ij = 0.5f * (vi.w + vj.w), c_ij = 0.5f * (ci.y + cj.y);
+                    const float nu = (mu * (q.beta * mu - q.alpha * c_ij)) / rho_ij;
+                    const float Pi = ci.x + cj.x + nu;                 // p_i/rho_i^2 + p_j/rho_j^2 + nu  (L95, A2)
+                    f = pj.w * Pi * gmag;                              // m_j Pi |grad Wp| / |dr|
                 } else {
-                    const double num = fma(-(double)dz, (double)dz, fma(-(double)dy, (double)dy, fma(-(double)dx, (double)dx, q.rc2_64)));
-                    const float tq = fmaxf((float)num, 0.0f) * q.inv_h2 / (2.0f + rr * inv_h_glob);   // 2 - xi
-                    gmag = q.gw * tq * tq * rinv;
+                    float mu, c_ij;
+                    f = hydro_pair<false>(vi, ci, pj.w, vj, cj, dx, dy, dz, d2, q, rv, mu, c_ij);
                 }
-                const float dvx = vi.x - vj.x, dvy = vi.y - vj.y, dvz = vi.z - vj.z;
-                const float rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
-                // mu_ij = h dr.dv / (|dr|^2 + eta h^2) if dr.dv < 0   (L97)
-                const float mu = rv < 0.f ? (hh * rv) / (d2 + eta_h2) : 0.f;       // IEEE division
-                const float rho_ij = 0.5f * (vi.w + vj.w), c_ij = 0.5f * (ci.y + cj.y);
-                const float nu = (mu * (q.beta * mu - q.alpha * c_ij)) / rho_ij;
-                const float Pi = ci.x + cj.x + nu;                 // p_i/rho_i^2 + p_j/rho_j^2 + nu  (L95, A2)
-                const float f = pj.w * Pi * gmag;                  // m_j Pi |grad Wp| / |dr|
                 ax.add(-f * dx);
                 ay.add(-f * dy);
                 az.add(-f * dz);
@@ -253,7 +226,7 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
 
 int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const float* h_s /*or NULL*/,
                   const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
-                  float4* velr_s, float2* pc_s, float4* acc_sph, cudaStream_t st) {
+                  const DenseList* dense, float4* velr_s, float2* pc_s, float4* acc_sph, cudaStream_t st) {
     if (n_gas <= 0) return SPH_OK;
     const int n = (int)n_gas;
     k_eos_gather<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(vele, rho, perm, n, p->gamma, velr_s, pc_s);
@@ -270,13 +243,19 @@ int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, co
     q.rc2_64 = 4.0 * h * h;
     q.eta = p->eta;
     q.gw_unit = (float)(-45.0 / (64.0 * 3.14159265358979323846));
-    if (h_s)
+    q.inv_h = 1.0f / p->h;
+    q.rc2 = two_h * two_h;
+    if (h_s) {
         k_forces<true><<<(unsigned)cdiv(n, 128), 128, 0, st>>>(posm_s, velr_s, pc_s, h_s, perm, cell_start, n, to_dev(g),
-                                                               two_h * two_h, q, acc_sph);
-    else
+                                                               two_h * two_h, q, 0u, acc_sph);
+        SPHB_LAUNCHED();
+    } else {
         k_forces<false><<<(unsigned)cdiv(n, 128), 128, 0, st>>>(posm_s, velr_s, pc_s, nullptr, perm, cell_start, n,
-                                                                to_dev(g), two_h * two_h, q, acc_sph);
-    SPHB_LAUNCHED();
+                                                                to_dev(g), two_h * two_h, q,
+                                                                dense ? (uint32_t)kDenseMin : 0u, acc_sph);
+        SPHB_LAUNCHED();
+        if (dense) SPHB_TRY(forces_dense(posm_s, velr_s, pc_s, perm, cell_start, g, two_h * two_h, q, *dense, acc_sph, st));
+    }
     return SPH_OK;
 }
 

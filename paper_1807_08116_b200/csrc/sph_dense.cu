@@ -1,0 +1,411 @@
+// sph_dense.cu — (a9) hydro force / energy rate for DENSELY populated cells (>= kDenseMin particles per cell).
+//
+// The thread-per-slot walk of sph.cu suits the sparse galaxy grids (a handful of neighbours, latency bound).  In a
+// clump (config 4: up to ~570 particles per cell, ~2000 neighbours, one candidate in five to six accepted) its
+// ~100-instruction pair term runs at 14 active lanes per instruction and waits on global gathers.  Here, per work item
+// (one cell, <= kDenseTT targets):
+//   * the candidates of each of the 9 stencil rows — ONE contiguous slot range per row, which is what the x-fastest cell
+//     order buys (L160, L203, L207) — are staged in shared memory by TMA bulk copies (cp.async.bulk + mbarrier), in
+//     chunks of kDenseK slots, once for all the item's targets; the copy of the next chunk runs under the work on this one;
+//   * the CTA re-orders each staged chunk in shared memory by SUB-CELL (a stable counting sort over 24 bins: the
+//     three cells of the row x 2x2x2 octants, x fastest), so that the candidates a target can reach are a few contiguous
+//     ranges: a 2h sphere meets ~84 octants of h^3 against the 27 x 8 = 216 of the whole stencil — 2.6 candidates per
+//     neighbour instead of 6.  The order is internal to this kernel: the exported keys / perm (A7, A16) are untouched;
+//   * a WARP takes a target: lane b finds out whether the sphere reaches bin b (distance to the octant's box, pulled out
+//     by eps and open-ended on the outside of boundary cells, where clamped particles sit); the reachable bins, in bin
+//     order, are the target's candidate list, addressed by a flat position through at most four slot ranges, so the 32
+//     lanes test 32 candidates per step with every lane busy whatever the bins' sizes;
+//   * accepted candidates are compacted by ballot + popc into a per-warp ring queue and the pair term (sph_dev.cuh:
+//     hydro_pair) runs on full warps, its operands read from the staged tile;
+//   * a lane's partial sum over one chunk (<= kDenseK/32 candidates) is plain FP32; the 32 partials are added across the
+//     warp in FP64 (one butterfly for the four sums) and accumulated per target in FP64 shared memory, so a target's sum
+//     has a fixed order (bitwise reproducible) and is at least as accurate as the compensated FP32 sum of the sparse walk.
+// Work items come from the list the grid build writes (grid.cu: k_scan_apply) — or k_dense_list for the stand-alone
+// calls — and are taken round-robin by a persistent grid (kDenseCtasPerSm CTAs per SM).
+// The density pass (a7) stays on the thread-per-slot walk everywhere: its pair term is ~15 instructions, so nothing is
+// won by compacting the accepted pairs, and the staged, binned walk measured slower (46 against 31 ms at config 4).
+#include "sph_dev.cuh"
+#include "tma_dev.cuh"
+
+namespace sphb {
+
+namespace {
+
+constexpr int kDenseThreads = 256;
+constexpr int kDenseWarps = kDenseThreads / 32;
+constexpr int kDenseCtasPerSm = 3;
+constexpr int kDenseK = 736;              // candidate slots per staged chunk
+constexpr int kDenseKS = kDenseK + 2;     // + the even-slot alignment of the float2 array at either end
+constexpr int kRounds = (kDenseK + kDenseThreads - 1) / kDenseThreads;
+constexpr int kBins = 24;                 // (sz, sy) sub-row x (cell of the row, sx): bin = (2 sz + sy) 6 + 2 c + sx
+constexpr int kQueue = 64;                // ring queue entries per warp
+
+struct DenseLayout {
+    // byte offsets inside the dynamic shared memory block (all multiples of 16)
+    static constexpr int raw_pos = 0;                                   // float4 [KS]   landing zone of the bulk copies
+    static constexpr int raw_vel = raw_pos + kDenseKS * 16;             // float4 [KS]
+    static constexpr int raw_pc = raw_vel + kDenseKS * 16;              // float2 [KS]
+    static constexpr int pos = raw_pc + kDenseKS * 8;                   // float4 [K]    the chunk in bin order: (x, y, z, m)
+    static constexpr int vel = pos + kDenseK * 16;                      // float4 [K]    (v, rho)
+    static constexpr int pc = vel + kDenseK * 16;                       // float2 [K]    (p/rho^2, c)
+    static constexpr int tpos = pc + kDenseK * 8;                       // float4 [TT]   the item's targets
+    static constexpr int tvel = tpos + kDenseTT * 16;                   // float4 [TT]
+    static constexpr int tpc = tvel + kDenseTT * 16;                    // float2 [TT]
+    static constexpr int acc = tpc + kDenseTT * 8;                      // double [TT][4]
+    static constexpr int runs = acc + kDenseTT * 8 * 4;                 // uint32 [9][4]
+    static constexpr int hist = runs + 9 * 4 * 4;                       // uint32 [rounds][warps][bins]
+    static constexpr int bstart = hist + kRounds * kDenseWarps * kBins * 4;   // uint32 [32]: start of bin b in the sorted chunk
+    static constexpr int box = bstart + 32 * 4;                         // float [bins][8]: xl, xh, yl, yh, zl, zh, -, -
+    static constexpr int tab = box + kBins * 8 * 4;                     // uint2 [warps][4]: a target's candidate groups
+    static constexpr int queue = tab + kDenseWarps * 4 * 8;             // uint32 [warps][kQueue]
+    static constexpr int bar = queue + kDenseWarps * kQueue * 4;        // uint64
+    static constexpr int bytes = bar + 16;
+};
+static_assert((DenseLayout::bytes + 1024) * kDenseCtasPerSm <= 227 * 1024, "shared memory per SM");
+
+__global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
+    k_dense_forces(const float4* __restrict__ posm_s, const float4* __restrict__ velr_s, const float2* __restrict__ pc_s,
+            const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start, GridDev g, float cell, float rc2,
+            ViscDev q, const unsigned int* __restrict__ ctl, const DenseItem* __restrict__ items,
+            float4* __restrict__ acc_out) {
+    using L = DenseLayout;
+    extern __shared__ __align__(128) unsigned char smem[];
+    float4* r_pos = reinterpret_cast<float4*>(smem + L::raw_pos);
+    float4* r_vel = reinterpret_cast<float4*>(smem + L::raw_vel);
+    float2* r_pc = reinterpret_cast<float2*>(smem + L::raw_pc);
+    float4* c_pos = reinterpret_cast<float4*>(smem + L::pos);
+    float4* c_vel = reinterpret_cast<float4*>(smem + L::vel);
+    float2* c_pc = reinterpret_cast<float2*>(smem + L::pc);
+    float4* t_pos = reinterpret_cast<float4*>(smem + L::tpos);
+    float4* t_vel = reinterpret_cast<float4*>(smem + L::tvel);
+    float2* t_pc = reinterpret_cast<float2*>(smem + L::tpc);
+    double* s_acc = reinterpret_cast<double*>(smem + L::acc);
+    uint32_t* s_runs = reinterpret_cast<uint32_t*>(smem + L::runs);
+    uint32_t* s_hist = reinterpret_cast<uint32_t*>(smem + L::hist);
+    uint32_t* s_bstart = reinterpret_cast<uint32_t*>(smem + L::bstart);
+    float4* s_box = reinterpret_cast<float4*>(smem + L::box);
+    uint64_t* s_bar = reinterpret_cast<uint64_t*>(smem + L::bar);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    const uint32_t sbase = smem_u32(smem);
+    const uint32_t a_pos = sbase + L::pos, a_vel = sbase + L::vel, a_pc = sbase + L::pc;
+    const uint32_t a_tpos = sbase + L::tpos, a_tvel = sbase + L::tvel, a_tpc = sbase + L::tpc;
+    const uint32_t a_tab = sbase + L::tab + 32u * (uint32_t)warp, a_q = sbase + L::queue + 4u * kQueue * (uint32_t)warp;
+    const uint32_t n_items = ctl[0];
+    if (blockIdx.x >= n_items) return;   // uniform per CTA
+
+    if (tid == 0) {
+        mbar_init(s_bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    uint32_t n_staged = 0;   // chunks this CTA has waited for so far: the barrier's phase parity
+
+    // stage the slots [cs, ce) of a stencil row: bulk copies need 16-byte alignment, the float2 array gives it on even
+    // slots only, so every array is staged from the even slot at or below cs (raw index = slot - (cs & ~1))
+    auto issue = [&](uint32_t cs, uint32_t ce) {
+        const uint32_t base = cs & ~1u;
+        const uint32_t cnt = (ce - base + 1u) & ~1u;   // <= kDenseKS, even
+        mbar_expect_tx(s_bar, cnt * 40u);
+        bulk_g2s(r_pos, posm_s + base, cnt * 16u, s_bar);
+        bulk_g2s(r_vel, velr_s + base, cnt * 16u, s_bar);
+        bulk_g2s(r_pc, pc_s + base, cnt * 8u, s_bar);
+    };
+    // chunk sequence of an item: rows 0..8 in order, each row [b0, b3) cut into pieces of kDenseK slots
+    auto skip_empty = [&](int& r, uint32_t& cs) {
+        while (r < 9 && s_runs[4 * r] >= s_runs[4 * r + 3]) ++r;
+        if (r < 9) cs = s_runs[4 * r];
+    };
+    auto next_chunk = [&](int& r, uint32_t& cs) {
+        cs += kDenseK;
+        if (cs >= s_runs[4 * r + 3]) {
+            ++r;
+            skip_empty(r, cs);
+        }
+    };
+
+    const float eps = cell * 0.00390625f;   // 2^-8 of a cell: covers the rounding of the cell assignment (A7) and of the faces
+    const float half = 0.5f * cell;
+    const float big = 3.0e38f;
+
+    for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const DenseItem it = items[item];
+        const uint32_t mx = (uint32_t)g.mx, my = (uint32_t)g.my;
+        const int ix = (int)(it.key % mx), iy = (int)((it.key / mx) % my), iz = (int)(it.key / (mx * my));
+        const uint32_t ts = start[it.key] + it.chunk * kDenseTT;
+        const uint32_t nt = min(start[it.key + 1u] - ts, (uint32_t)kDenseTT);
+        __syncthreads();   // the previous item's shared memory is no longer read
+        if (tid < 9) {
+            // row r: the cells (ix-1, ix, ix+1) at (iy + r%3 - 1, iz + r/3 - 1); boundaries b0 <= b1 <= b2 <= b3
+            const int cy = iy + (tid % 3) - 1, cz = iz + (tid / 3) - 1;
+            uint32_t b0 = 0, b1 = 0, b2 = 0, b3 = 0;
+            if (cy >= 0 && cy < g.my && cz >= 0 && cz < g.mz) {
+                const uint32_t row = mx * ((uint32_t)cy + my * (uint32_t)cz);
+                b1 = start[row + (uint32_t)ix];
+                b2 = start[row + (uint32_t)ix + 1u];
+                b0 = ix > 0 ? start[row + (uint32_t)ix - 1u] : b1;
+                b3 = ix + 1 < g.mx ? start[row + (uint32_t)ix + 2u] : b2;
+            }
+            s_runs[4 * tid] = b0;
+            s_runs[4 * tid + 1] = b1;
+            s_runs[4 * tid + 2] = b2;
+            s_runs[4 * tid + 3] = b3;
+        }
+        for (uint32_t t = tid; t < nt; t += kDenseThreads) {
+            t_pos[t] = posm_s[ts + t];
+            t_vel[t] = velr_s[ts + t];
+            t_pc[t] = pc_s[ts + t];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) s_acc[4 * t + c] = 0.0;
+        }
+        __syncthreads();
+
+        int r = 0;
+        uint32_t cs = 0;
+        skip_empty(r, cs);
+        if (tid == 0 && r < 9) issue(cs, min(cs + kDenseK, s_runs[4 * r + 3]));
+        while (r < 9) {
+            const uint32_t ce = min(cs + kDenseK, s_runs[4 * r + 3]);
+            const uint32_t ncand = ce - cs, roff = cs & 1u;   // candidates of this chunk; raw index of slot cs
+            const uint32_t b1 = s_runs[4 * r + 1], b2 = s_runs[4 * r + 2];
+            const int cy = iy + (r % 3) - 1, cz = iz + (r / 3) - 1;
+            // mid-planes of the three cells of the row, and of the row itself
+            const float xm0 = fmaf((float)(ix - 1) + 0.5f, cell, g.ox), xm1 = xm0 + cell, xm2 = xm1 + cell;
+            const float ym = fmaf((float)cy + 0.5f, cell, g.oy), zm = fmaf((float)cz + 0.5f, cell, g.oz);
+
+            // ---- counting sort of the chunk by bin, stable (slot order inside a bin): raw -> sorted ----
+            for (int i = tid; i < kRounds * kDenseWarps * kBins; i += kDenseThreads) s_hist[i] = 0u;
+            mbar_wait(s_bar, n_staged & 1u);
+            ++n_staged;
+            __syncthreads();   // histogram zeroed; every warp is past the previous chunk's candidates
+            uint32_t my_bin[kRounds], my_rank[kRounds];
+#pragma unroll
+            for (int rd = 0; rd < kRounds; ++rd) {
+                const uint32_t i = (uint32_t)(rd * kDenseThreads + tid);
+                uint32_t bin = 31u;   // past the end of the chunk
+                if (i < ncand) {
+                    const float4 p = r_pos[roff + i];
+                    const uint32_t slot = cs + i;
+                    const uint32_t c = (slot >= b1 ? 1u : 0u) + (slot >= b2 ? 1u : 0u);
+                    const float xm = c == 0u ? xm0 : (c == 1u ? xm1 : xm2);
+                    bin = ((p.z >= zm ? 2u : 0u) + (p.y >= ym ? 1u : 0u)) * 6u + 2u * c + (p.x >= xm ? 1u : 0u);
+                }
+                const unsigned peers = __match_any_sync(0xffffffffu, bin);
+                my_bin[rd] = bin;
+                my_rank[rd] = __popc(peers & lt_mask);
+                if (bin < (uint32_t)kBins && my_rank[rd] == 0u) s_hist[(rd * kDenseWarps + warp) * kBins + bin] = __popc(peers);
+            }
+            __syncthreads();
+            if (tid < 32) {
+                // lane b: exclusive prefix of bin b over (round, warp), then the bins' starts
+                uint32_t run = 0u;
+                if (lane < kBins) {
+                    for (int j = 0; j < kRounds * kDenseWarps; ++j) {
+                        const uint32_t v = s_hist[j * kBins + lane];
+                        s_hist[j * kBins + lane] = run;
+                        run += v;
+                    }
+                }
+                uint32_t inc = run;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += v;
+                }
+                s_bstart[lane] = inc - run;   // lanes >= kBins: ncand
+            }
+            if (tid >= 32 && tid < 32 + kBins) {
+                // (warp 1, after the barrier above: no warp still reads the previous chunk's boxes)
+                // box of bin b: the octant, pulled out by eps; open-ended on the outside of a boundary cell, where the
+                // particles clamped into the grid sit (A7)
+                const int bb = tid - 32, k = bb % 6, sr = bb / 6, c = k >> 1, sx = k & 1, sy = sr & 1, sz = sr >> 1;
+                const int cx = ix - 1 + c;
+                const float xm = c == 0 ? xm0 : (c == 1 ? xm1 : xm2);
+                float xl = (sx ? xm : xm - half) - eps, xh = (sx ? xm + half : xm) + eps;
+                float yl = (sy ? ym : ym - half) - eps, yh = (sy ? ym + half : ym) + eps;
+                float zl = (sz ? zm : zm - half) - eps, zh = (sz ? zm + half : zm) + eps;
+                if (cx == 0 && !sx) xl = -big;
+                if (cx == g.mx - 1 && sx) xh = big;
+                if (cx < 0 || cx >= g.mx) xl = big;   // no such cell (the row ends here): out of reach, like the lanes >= kBins
+                if (cy <= 0 && !sy) yl = -big;
+                if (cy >= g.my - 1 && sy) yh = big;
+                if (cz <= 0 && !sz) zl = -big;
+                if (cz >= g.mz - 1 && sz) zh = big;
+                s_box[2 * bb] = make_float4(xl, xh, yl, yh);
+                s_box[2 * bb + 1] = make_float4(zl, zh, 0.f, 0.f);
+            }
+            __syncthreads();
+#pragma unroll
+            for (int rd = 0; rd < kRounds; ++rd) {
+                const uint32_t i = (uint32_t)(rd * kDenseThreads + tid);
+                if (i < ncand) {
+                    const uint32_t dst = s_bstart[my_bin[rd]] + s_hist[(rd * kDenseWarps + warp) * kBins + my_bin[rd]] + my_rank[rd];
+                    c_pos[dst] = r_pos[roff + i];
+                    c_vel[dst] = r_vel[roff + i];
+                    c_pc[dst] = r_pc[roff + i];
+                }
+            }
+            __syncthreads();   // the sorted chunk is complete, the landing zone is free
+
+            int rn = r;
+            uint32_t csn = cs;
+            next_chunk(rn, csn);
+            if (tid == 0 && rn < 9) issue(csn, min(csn + kDenseK, s_runs[4 * rn + 3]));
+
+            // ---- the item's targets against the chunk ----
+            // (shared memory by 32-bit address from here on: byte offsets in registers, no generic-address arithmetic)
+            const float4 bx0 = lane < kBins ? s_box[2 * lane] : make_float4(big, big, big, big);
+            const float4 bx1 = lane < kBins ? s_box[2 * lane + 1] : make_float4(big, big, 0.f, 0.f);
+            const uint32_t bs0 = s_bstart[lane];                                   // lane b: slots [bs0, bs0 + blen) of the
+            const uint32_t blen = lane < kBins ? s_bstart[lane + 1] - bs0 : 0u;    // sorted chunk hold bin b
+            for (uint32_t t = warp; t < nt; t += kDenseWarps) {
+                const float4 pi = lds_f4(a_tpos + 16u * t);
+                // lane b: does the 2h sphere of the target reach the box of bin b?  (a lower bound of the distance)
+                const float ex = fmaxf(fmaxf(bx0.x - pi.x, pi.x - bx0.y), 0.f);
+                const float ey = fmaxf(fmaxf(bx0.z - pi.y, pi.y - bx0.w), 0.f);
+                const float ez = fmaxf(fmaxf(bx1.x - pi.z, pi.z - bx1.y), 0.f);
+                const bool reach_b = fmaf(ez, ez, fmaf(ey, ey, ex * ex)) < rc2;   // lanes >= kBins: their box is out of reach
+                const unsigned reach = __ballot_sync(0xffffffffu, reach_b);
+                // The reachable bins, in bin order, are the target's candidate list: flat position v = 0 .. T-1.  Consecutive
+                // reachable bins are one slot range (a "group").  Along a (sz, sy) sub-row the distance to the 6 x-slabs
+                // falls and rises once, so the reachable bins of a sub-row are consecutive: at most 4 groups.  Each is
+                // described by the flat position where it ends and the offset from a flat position to a slot — both
+                // kept in BYTES of the float4 array (x16), so a candidate's address is one add.
+                uint32_t incl = reach_b ? blen : 0u;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+                    if (lane >= o) incl += v;
+                }
+                uint32_t T = __shfl_sync(0xffffffffu, incl, 31);
+                if (T == 0u) continue;
+                const unsigned gstart = reach & ~(reach << 1);                           // first bin of every group
+                const int ng = __popc(gstart);
+                const int e = lane + __ffs(~(reach >> lane)) - 1;                        // (for a first bin) one past the group's last bin
+                const uint32_t gend = __shfl_sync(0xffffffffu, incl, (e - 1) & 31);
+                if (lane < 4 && lane >= ng) sts_u2(a_tab + 8u * lane, 0xffffffffu, 0u);   // no such group
+                if (((gstart >> lane) & 1u) && ng <= 4)
+                    sts_u2(a_tab + 8u * __popc(gstart & lt_mask), 16u * gend, 16u * (bs0 - (incl - blen)));
+                __syncwarp();
+                uint2 g0 = lds_u2(a_tab);
+                const uint2 g1 = lds_u2(a_tab + 8u), g2 = lds_u2(a_tab + 16u), g3 = lds_u2(a_tab + 24u);
+                if (ng > 4) {   // cannot happen for boxes in a row (see above); if it ever does, every slot of the chunk is a candidate
+                    T = ncand;
+                    g0 = make_uint2(0xffffffffu, 0u);
+                }
+
+                const float4 vi = lds_f4(a_tvel + 16u * t);
+                const float2 ci = lds_f2(a_tpc + 8u * t);
+                float ax = 0.f, ay = 0.f, az = 0.f, de = 0.f;
+                uint32_t qh = 0, qt = 0;   // ring queue of accepted candidates (byte offsets in the float4 arrays): head, tail x4
+                auto pair_term = [&](uint32_t rel) {
+                    const float4 pj = lds_f4(a_pos + rel);
+                    const float4 vj = lds_f4(a_vel + rel);
+                    const float2 cj = lds_f2(a_pc + (rel >> 1));
+                    float dx, dy, dz, rv, mu, c_ij;
+                    const float d2 = dist2_f32(pi, pj, dx, dy, dz);
+                    const float f = hydro_pair<true>(vi, ci, pj.w, vj, cj, dx, dy, dz, d2, q, rv, mu, c_ij);
+                    ax = fmaf(-f, dx, ax);
+                    ay = fmaf(-f, dy, ay);
+                    az = fmaf(-f, dz, az);
+                    de = fmaf(0.5f * f, rv, de);   // 1/2 m_j Pi dv . grad W_p   (Eq. 11)
+                };
+                // one step: 32 flat positions, one per lane; `in` is false only for the lanes past the end in the last step
+                auto step = [&](uint32_t v16, bool in) {
+                    uint32_t rel = v16 + g3.y;
+                    rel = v16 < g2.x ? v16 + g2.y : rel;
+                    rel = v16 < g1.x ? v16 + g1.y : rel;
+                    rel = v16 < g0.x ? v16 + g0.y : rel;
+                    rel = in ? rel : 0u;
+                    float dx, dy, dz;
+                    const float d2 = dist2_f32(pi, lds_f4(a_pos + rel), dx, dy, dz);
+                    // d2 == 0: self, or a coincident pair (A9) — no contribution
+                    const bool ok = in && d2 < rc2 && d2 > 0.f;
+                    const unsigned m = __ballot_sync(0xffffffffu, ok);
+                    if (ok) sts_u32(a_q + ((qt + 4u * __popc(m & lt_mask)) & (4u * kQueue - 4u)), rel);
+                    qt += 4u * __popc(m);
+                    if (qt - qh >= 128u) {
+                        __syncwarp();
+                        pair_term(lds_u32(a_q + ((qh + 4u * (uint32_t)lane) & (4u * kQueue - 4u))));
+                        qh += 128u;
+                    }
+                };
+                const uint32_t T16 = 16u * T, full16 = T16 & ~511u;
+                uint32_t v16 = 16u * (uint32_t)lane;
+                for (; v16 < full16; v16 += 512u) step(v16, true);     // v16 - 16 lane < full16 for every lane: uniform
+                if (full16 != T16) step(v16, v16 < T16);
+                if (qt != qh) {
+                    __syncwarp();
+                    if (4u * (uint32_t)lane < qt - qh) pair_term(lds_u32(a_q + ((qh + 4u * (uint32_t)lane) & (4u * kQueue - 4u))));
+                }
+                __syncwarp();   // the queue and the table are rewritten for the next target
+                if (qt != 0u) {
+                    // the four sums over the 32 lanes in FP64, as one butterfly: after the exchange over lane bit 4 a
+                    // lane holds two of them, after bit 3 one; lanes 0, 8, 16, 24 end with a_x, a_y, a_z, de/dt
+                    const bool hi16 = (lane & 16) != 0, hi8 = (lane & 8) != 0;
+                    const double dxs = (double)ax, dys = (double)ay, dzs = (double)az, des = (double)de;
+                    double k0 = hi16 ? dzs : dxs, k1 = hi16 ? des : dys;
+                    const double s0 = hi16 ? dxs : dzs, s1 = hi16 ? dys : des;
+                    k0 += __shfl_xor_sync(0xffffffffu, s0, 16);
+                    k1 += __shfl_xor_sync(0xffffffffu, s1, 16);
+                    double k = hi8 ? k1 : k0;
+                    k += __shfl_xor_sync(0xffffffffu, hi8 ? k0 : k1, 8);
+                    k += __shfl_xor_sync(0xffffffffu, k, 4);
+                    k += __shfl_xor_sync(0xffffffffu, k, 2);
+                    k += __shfl_xor_sync(0xffffffffu, k, 1);
+                    if ((lane & 7) == 0) s_acc[4 * t + (lane >> 3)] += k;
+                }
+            }
+            r = rn;
+            cs = csn;
+            // the __syncthreads() after the wait at the top of the next chunk (or the one before the write-out below)
+            // separates this chunk's reads of the sorted tile from the next re-ordering
+        }
+        __syncthreads();
+
+        for (uint32_t t = tid; t < nt; t += kDenseThreads) {
+            acc_out[perm[ts + t]] = make_float4((float)s_acc[4 * t], (float)s_acc[4 * t + 1], (float)s_acc[4 * t + 2],
+                                                (float)s_acc[4 * t + 3]);
+        }
+    }
+}
+
+// the work list from a caller's cell_start (stand-alone calls): one thread per cell
+__global__ void __launch_bounds__(256) k_dense_list(const uint32_t* __restrict__ start, int64_t M, unsigned int* ctl,
+                                                    DenseItem* items) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= M) return;
+    const uint32_t c = start[k + 1] - start[k];
+    if (c >= (uint32_t)kDenseMin) dense_append((uint32_t)k, c, ctl, items);
+}
+
+}  // namespace
+
+int dense_list_from_start(const uint32_t* cell_start, const sph_grid* g, const DenseList& dl, cudaStream_t st) {
+    const int64_t M = grid_cells(g);
+    SPHB_CUDA(cudaMemsetAsync(dl.ctl, 0, sizeof(unsigned int), st));
+    k_dense_list<<<(unsigned)cdiv(M, 256), 256, 0, st>>>(cell_start, M, dl.ctl, dl.items);
+    SPHB_LAUNCHED();
+    return SPH_OK;
+}
+
+int forces_dense(const float4* posm_s, const float4* velr_s, const float2* pc_s, const uint32_t* perm,
+                 const uint32_t* cell_start, const sph_grid* g, float rc2, const ViscDev& q, const DenseList& dl,
+                 float4* acc_sph, cudaStream_t st) {
+    int dev = 0;
+    SPHB_CUDA(cudaGetDevice(&dev));
+    static std::atomic<bool> opted[64];   // per device: the dynamic shared-memory opt-in
+    if (dev < 0 || dev >= 64) return SPH_ERR_UNSUPPORTED;
+    if (!opted[dev].load(std::memory_order_acquire)) {
+        SPHB_CUDA(cudaFuncSetAttribute(k_dense_forces, cudaFuncAttributeMaxDynamicSharedMemorySize, DenseLayout::bytes));
+        opted[dev].store(true, std::memory_order_release);
+    }
+    // the faces of the cells follow the rule the keys are made with (A7: c = (x - origin) * inv_cell), so the cell
+    // edge is taken from inv_cell, not from g->cell
+    k_dense_forces<<<kDenseCtasPerSm * num_sms(), kDenseThreads, DenseLayout::bytes, st>>>(
+        posm_s, velr_s, pc_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, rc2, q, dl.ctl, dl.items, acc_sph);
+    SPHB_LAUNCHED();
+    return SPH_OK;
+}
+
+}  // namespace sphb

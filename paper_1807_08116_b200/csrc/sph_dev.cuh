@@ -1,0 +1,98 @@
+// sph_dev.cuh — device functions shared by the two SPH walks (sph.cu: thread per sorted slot, the sparse galaxy
+// grids; sph_dense.cu: CTA per populated cell, shared-memory staged, warp per target).  Both walks evaluate a pair
+// with exactly these operation sequences, so a pair's term is the same bits whichever walk reaches it; only the
+// order of a particle's sum differs.  Internal to libsph_b200; nothing here is shared with the oracle.
+#pragma once
+#include "common.cuh"
+
+namespace sphb {
+
+// Cutoff predicate (A8), identical op sequence to the oracle:
+//   dx = x_i (-) x_j ...  d2 = fma(dz,dz, fma(dy,dy, dx*dx))  neighbour iff d2 < fl(fl(2h)^2).
+__device__ __forceinline__ float dist2_f32(const float4 a, const float4 b, float& dx, float& dy, float& dz) {
+    dx = __fsub_rn(a.x, b.x);
+    dy = __fsub_rn(a.y, b.y);
+    dz = __fsub_rn(a.z, b.z);
+    return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+}
+
+// cell coordinates of a particle (reading A7, same FP32 op sequence as the key kernel); no div / mod needed
+__device__ __forceinline__ void cell_of(const float4 p, const GridDev g, int& ix, int& iy, int& iz) {
+    ix = (int)fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.x, g.ox), g.inv_cell)), 0.0f), g.fx);
+    iy = (int)fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.y, g.oy), g.inv_cell)), 0.0f), g.fy);
+    iz = (int)fminf(fmaxf(floorf(__fmul_rn(__fsub_rn(p.z, g.oz), g.inv_cell)), 0.0f), g.fz);
+}
+
+// W(xi,h) = 1/(pi h^3) { 1 - 3/2 xi^2 + 3/4 xi^3 (xi<=1) ; 1/4 (2-xi)^3 (1<=xi<=2) ; 0 }   (Eq. 8)
+__device__ __forceinline__ float w_spline_unnorm(float xi) {
+    float t = 2.0f - xi;
+    float outer = 0.25f * t * t * t;
+    float inner = fmaf(xi * xi, fmaf(0.75f, xi, -1.5f), 1.0f);
+    return xi <= 1.0f ? inner : fmaxf(outer, 0.0f);
+}
+
+struct ViscDev {
+    float h, alpha, beta, eta_h2, gw;   // gw = -45 / (64 pi h^4): grad W_p = gw (2-xi)^2 dr/|dr|
+    float inv_h2;                       // 1 / h^2
+    double rc2_64;                      // 4 h^2 in FP64 (h as given, widened)
+    float eta, gw_unit;                 // VARH: eta and -45 / (64 pi); the h powers are applied per pair
+    float inv_h;                        // 1 / h (IEEE division on the host side of the launch)
+    float rc2;                          // fl(fl(2h)^2), the FP32 cutoff of A8
+};
+
+// One accepted pair (d2 < 4h^2, d2 > 0) of Eqs. 10-11 with the one global h: returns f = m_j Pi_ij |grad W_p| / |dr| and
+// rv = dr . dv, so that a_i -= f dr and de_i/dt += f rv / 2; mu_ij (L97, <= 0) and c_ij = (c_i + c_j)/2 come out for the
+// step criterion of Eq. 17.
+//   2 - xi = (4h^2 - |dr|^2) / (h^2 (2 + xi)).  Formed as 2 - |dr|/h in FP32 it loses a factor xi/(2-xi) of relative
+//   accuracy near the kernel edge (every term of a sparsely surrounded particle sits there), so the numerator alone is
+//   taken in FP64: 3 cvt + 3 DFMA per pair.
+//   grad W_p = dWp/dxi * dr/|dr| / h,  dWp/dxi = -45/(64 pi h^3) (2-xi)^2   (L95, Eq. 9, A3)
+// a / b for b > 0 in the normal range: reciprocal by MUFU.RCP and one Newton step (~1 ulp), 4 instructions against the
+// ~17 of the IEEE division with its range check
+__device__ __forceinline__ float div_newton(float a, float b) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(b));
+    r = fmaf(r, fmaf(-b, r, 1.0f), r);
+    return a * r;
+}
+// FAST (the dense walk, where a particle's sum has tens to thousands of terms spread over the whole kernel support):
+// the three divisions by div_newton, MUFU.RSQ without its Newton step (2^-22 of pseudo-random error per term), and the
+// numerator 4h^2 - |dr|^2 in FP32 — its absolute error, <= 2 ulp of 4h^2, is that of any FP32 term; only the RELATIVE
+// error of a term at the kernel edge grows, which matters where ALL of a particle's few terms sit at the edge, i.e. in
+// the sparse walk, which keeps the FP64 numerator, the refined rsqrt and the IEEE divisions.
+template <bool FAST>
+__device__ __forceinline__ float hydro_pair(const float4 vi /*v, rho*/, const float2 ci /*p/rho^2, c*/, const float m_j,
+                                            const float4 vj, const float2 cj, const float dx, const float dy,
+                                            const float dz, const float d2, const ViscDev& q, float& rv, float& mu,
+                                            float& c_ij) {
+    float rinv = rsqrtf(d2);
+    if (!FAST) rinv = rinv * fmaf(-0.5f * d2 * rinv, rinv, 1.5f);   // one Newton step: ~1 ulp
+    const float rr = d2 * rinv;                          // |dr|
+    float num;
+    if (FAST)
+        num = q.rc2 - d2;
+    else
+        num = (float)fma(-(double)dz, (double)dz, fma(-(double)dy, (double)dy, fma(-(double)dx, (double)dx, q.rc2_64)));
+    const float tqn = fmaxf(num, 0.0f) * q.inv_h2, tqd = 2.0f + rr * q.inv_h;
+    const float tq = FAST ? div_newton(tqn, tqd) : tqn / tqd;   // 2 - xi
+    const float gmag = q.gw * tq * tq * rinv;            // grad W_p = gmag * dr
+    const float dvx = vi.x - vj.x, dvy = vi.y - vj.y, dvz = vi.z - vj.z;
+    rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
+    // mu_ij = h dr.dv / (|dr|^2 + eta h^2) if dr.dv < 0   (L97)
+    const float mun = q.h * rv, mud = d2 + q.eta_h2;
+    mu = rv < 0.f ? (FAST ? div_newton(mun, mud) : mun / mud) : 0.f;
+    const float rho_ij = 0.5f * (vi.w + vj.w);
+    c_ij = 0.5f * (ci.y + cj.y);
+    const float nun = mu * (q.beta * mu - q.alpha * c_ij);
+    const float nu = FAST ? div_newton(nun, rho_ij) : nun / rho_ij;
+    const float Pi = ci.x + cj.x + nu;                   // p_i/rho_i^2 + p_j/rho_j^2 + nu  (L95, A2)
+    return m_j * Pi * gmag;                              // m_j Pi |grad Wp| / |dr|
+}
+
+// ---- dense-cell work list (common.cuh: DenseItem, DenseList) ------------------------------------------------------
+__device__ __forceinline__ void dense_append(uint32_t key, uint32_t count, unsigned int* ctl, DenseItem* items) {
+    const uint32_t nchunk = (count + kDenseTT - 1) / kDenseTT;
+    const uint32_t at = atomicAdd(ctl, nchunk);
+    for (uint32_t c = 0; c < nchunk; ++c) items[at + c] = DenseItem{key, c};
+}
+}  // namespace sphb

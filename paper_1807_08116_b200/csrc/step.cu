@@ -42,6 +42,8 @@ Workspace carve(void* base, int64_t n_gas, int64_t n_total, const sph_grid* g) {
     w.velr_s = (float4*)take(ng * 16);
     w.pc_s = (float2*)take(ng * 8);
     w.h_s = (float*)take(ng * 4);
+    w.dense.ctl = (unsigned int*)take(256);
+    w.dense.items = (DenseItem*)take(dense_capacity((int64_t)ng) * sizeof(DenseItem));
     w.src_pk = (float4*)take((size_t)grav_padded(n_total) * 16);
     w.grav_part = (float4*)take((size_t)grav_splits(n_total) * nt * 16);
     w.grav_acc64_off = off;

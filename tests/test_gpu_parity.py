@@ -121,7 +121,35 @@ def _grid_case(case):
     if case == "ragged_M":
         w = _dense(4099, 6, 0.031)
         return w, None
+    # ---- cases for the dense-cell walk (sph_dense.cu: cells of >= 32 particles) ----
+    if case == "packed":          # 4^3 cells of ~310: several target chunks per cell, stencil rows longer than one staged chunk
+        return _dense(20000, 7, 0.15), None
+    if case == "tight_clumps":    # sparse background (thread-per-slot walk) + clumps half a cell wide (dense walk), side by side
+        rng = np.random.Generator(np.random.Philox(key=[11, 0]))
+        n_u, n_c = 12000, 12000
+        uni = 2.0 * rng.random((n_u, 3)) - 1.0
+        centres = 1.6 * rng.random((24, 3)) - 0.8
+        clump = centres[rng.integers(0, 24, size=n_c)] + 0.02 * rng.standard_normal((n_c, 3))
+        n = n_u + n_c
+        posm = np.zeros((n, 4), np.float32)
+        vele = np.zeros((n, 4), np.float32)
+        posm[:, :3] = np.concatenate([uni, clump])
+        posm[:, 3] = 1.0 / n
+        vele[:, :3] = 0.1 * rng.standard_normal((n, 3))
+        vele[:, 3] = 0.5 + 0.5 * rng.random(n)
+        return wl.Workload("tight_clumps", posm, vele, n, 0, 0.03, 0.01, 0.0, 1e-3, 1, 11), None
+    if case == "one_cell_sph":    # every particle in the one cell of a 1x1x1 grid
+        w = _dense(1500, 4, 0.03)
+        w.h = 3.0
+        return w, None
+    if case == "clamped_dense":   # a 3^3 grid inside the box: the outside particles are clamped into its boundary cells
+        w = _dense(12000, 8, 0.08)
+        g = oracle.grid_from_bbox(w.posm, w.n_gas, w.h)
+        return w, oracle.Grid((0.3, 0.3, 0.3), g.cell, g.inv_cell, (3, 3, 3))
     raise KeyError(case)
+
+
+DENSE_CASES = ("packed", "tight_clumps", "one_cell_sph", "clamped_dense")
 
 
 @pytest.mark.parametrize("case", ["galaxy", "dense", "clumps", "clamped", "one_cell", "ragged_M"])
@@ -205,7 +233,7 @@ def test_neighbour_sets_bit_exact(cuda_lib, case):
     assert np.array_equal(idx.cpu().numpy().view(np.uint32), oidx)
 
 
-@pytest.mark.parametrize("case", ["galaxy", "dense", "clumps", "clamped"])
+@pytest.mark.parametrize("case", ["galaxy", "dense", "clumps", "clamped"] + list(DENSE_CASES))
 def test_density_and_forces_parity(cuda_lib, case):
     b = cuda_lib
     w, og = _grid_case(case)
@@ -214,6 +242,8 @@ def test_density_and_forces_parity(cuda_lib, case):
     prm = b.sph_params.from_workload(w)
     rho = torch.zeros(n, device="cuda")
     b.sph_density(d, n, prm, g, perm, start, rho, ws)
+    if case in DENSE_CASES:      # these cases are there for the dense-cell walk: make sure it ran
+        assert b.sph_dense_items(ws, n, n, g) > 0
     ooff, oidx = oracle.neighbours(w.posm, n, w.h, method="grid")
     orho = oracle.density(w.posm, w.h, ooff, oidx)
     check_density(rho.cpu().numpy(), orho, f"rho {case}")
