@@ -245,6 +245,45 @@ def run_reference(args, w):
     print(json.dumps(line), flush=True)
 
 
+def sph_pair_counts(b, sim, w):
+    """Diagnostics for the SPH throughput figures (quote candidate-pairs/s and accepted-pairs/s, with the
+    neighbour and occupancy histograms beside them).  Outside every timed region.  Candidate pairs are the ALGORITHMIC
+    ones of the paper's cell-list search (every particle against the 27 cells of its stencil, L207), counted from the
+    library's own histogram; accepted pairs are the neighbour counts of the library's sph_neighbour_lists (count pass
+    only: capacity 0).  torch is used here for sums over those device arrays — it is not on the path."""
+    import torch
+    ng = w.n_gas
+    g = sim.grid
+    key = torch.zeros(ng, dtype=torch.int32, device="cuda")
+    perm = torch.zeros(ng, dtype=torch.int32, device="cuda")
+    count = torch.zeros(g.M, dtype=torch.int32, device="cuda")
+    start = torch.zeros(g.M + 1, dtype=torch.int32, device="cuda")
+    b.sph_build_grid(sim.posm, ng, g, key, perm, count, start, sim.ws)
+    mx, my, mz = (int(d) for d in g.dims)
+    c = count.view(1, 1, mz, my, mx).to(torch.float32)
+    c27 = torch.nn.functional.conv3d(c, torch.ones(1, 1, 3, 3, 3, device="cuda"), padding=1)
+    candidates = float((c.double() * c27.double()).sum().item())
+    cnt = torch.zeros(max(ng, 1), dtype=torch.int32, device="cuda")
+    off = torch.zeros(ng + 1, dtype=torch.int64, device="cuda")
+    L = b.load()
+    p, nb = b._ws(sim.ws)
+    rc = L.sph_neighbour_lists(b._ptr(sim.posm), ng, float(w.h), b.C.byref(g), b._ptr(perm), b._ptr(start), b._ptr(cnt),
+                               b._ptr(off), None, 0, p, nb, b._stream())
+    if rc not in (b.SPH_OK, b.SPH_ERR_WORKSPACE):
+        raise b.SphError("sph_neighbour_lists", rc)
+    accepted = float(off[ng].item())
+    occ = count[count > 0].to(torch.float32)
+    nb_f = cnt[:ng].to(torch.float32)
+    q = torch.tensor([0.5, 0.9, 0.99], device="cuda")
+    return {
+        "candidate_pairs": candidates, "accepted_pairs": accepted,
+        "neighbours_mean": accepted / ng, "neighbours_p50_p90_p99_max": [float(x) for x in torch.quantile(nb_f[:: max(1, ng // 1000000)], q)] + [float(nb_f.max())],
+        "occupied_cells": int(occ.numel()), "cells": int(g.M),
+        "occupancy_p50_p90_p99_max": [float(x) for x in torch.quantile(occ[:: max(1, occ.numel() // 1000000)], q)] + [float(occ.max())],
+        "dense_walk_items": b.sph_dense_items(sim.ws, ng, w.n_total, g),
+    }
+
+
 # ------------------------------------------------------------------------------------------------
 def run_ours(args, w):
     import torch
@@ -380,6 +419,7 @@ def run_ours(args, w):
                             "interaction), so frac can exceed the 20-flop instruction-mix ceiling and even 1; "
                             "fp32_pipe_util is the share of FP32 issue capacity (128 lanes/clk/SM) the executed operations take"}
     hbm = float(peaks.get("hbm_gbs", 6650.0))
+    pairs = sph_pair_counts(b, sim, w) if (ng and world == 1) else None
     sort_bytes = ng * 92 + M * 16
     # gas: predictor 64 B read + 48 B written, corrector 64 + 16; halo particles never touch acc_sph: 48 + 48, 48 + 16
     upd_bytes = ng * (112 + 80) + (n - ng) * (96 + 64)
@@ -398,6 +438,20 @@ def run_ours(args, w):
         "forces_hbm_frac": (2 * ng * 104 / (forc_ms * 1e-3) / 1e9 / hbm) if ng and forc_ms > 0 else None,
         "hbm_peak_gbs": hbm, "peak_source": peak_src,
     }
+    if pairs and dens_ms > 0 and forc_ms > 0:
+        # SURVEY 8(d) op counts: a candidate test is ~7 FP32 lane-operations, an accepted density pair ~12 more, an
+        # accepted force pair ~60 more; one density pass and two forces passes per step
+        cand, acc = pairs["candidate_pairs"], pairs["accepted_pairs"]
+        lane_ops = (cand * 7 + acc * 12) + 2 * (cand * 7 + acc * 60)
+        stages.update({
+            "sph_pairs": pairs,
+            "sph_candidate_pairs_per_s": 3 * cand / ((dens_ms + forc_ms) * 1e-3),
+            "sph_accepted_pairs_per_s": 3 * acc / ((dens_ms + forc_ms) * 1e-3),
+            "sph_fp32_frac": lane_ops / ((dens_ms + forc_ms) * 1e-3) / (128 * SM_COUNT_B200 * sm_max * 1e6),
+            "sph_fp32_note": "ALGORITHMIC lane-operations (27-cell candidates x 7 + accepted pairs x 12 (density) or x 60 "
+                             "(forces); 3 passes per step) / (density + forces time) / (128 lanes x 148 SMs x sm_max); the "
+                             "dense-cell walk tests fewer candidates than the 27-cell count (octant binning)",
+        })
 
     # ---- the oracle on this box's host cores, bounded sample (rank 0, N = 1 only) ----------------
     cpu = None

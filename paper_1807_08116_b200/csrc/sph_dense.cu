@@ -21,7 +21,7 @@
 //     warp in FP64 (one butterfly for the four sums) and accumulated per target in FP64 shared memory, so a target's sum
 //     has a fixed order (bitwise reproducible) and is at least as accurate as the compensated FP32 sum of the sparse walk.
 // Work items come from the list the grid build writes (grid.cu: k_scan_apply) — or k_dense_list for the stand-alone
-// calls — and are taken round-robin by a persistent grid (kDenseCtasPerSm CTAs per SM).
+// calls — and are drawn from a counter by a persistent grid (kDenseCtasPerSm CTAs per SM).
 // The density pass (a7) stays on the thread-per-slot walk everywhere: its pair term is ~15 instructions, so nothing is
 // won by compacting the accepted pairs, and the staged, binned walk measured slower (46 against 31 ms at config 4).
 #include "sph_dev.cuh"
@@ -31,10 +31,10 @@ namespace sphb {
 
 namespace {
 
-constexpr int kDenseThreads = 256;
+constexpr int kDenseThreads = 384;
 constexpr int kDenseWarps = kDenseThreads / 32;
-constexpr int kDenseCtasPerSm = 3;
-constexpr int kDenseK = 736;              // candidate slots per staged chunk
+constexpr int kDenseCtasPerSm = 2;
+constexpr int kDenseK = 1152;             // candidate slots per staged chunk
 constexpr int kDenseKS = kDenseK + 2;     // + the even-slot alignment of the float2 array at either end
 constexpr int kRounds = (kDenseK + kDenseThreads - 1) / kDenseThreads;
 constexpr int kBins = 24;                 // (sz, sy) sub-row x (cell of the row, sx): bin = (2 sz + sy) 6 + 2 c + sx
@@ -59,6 +59,7 @@ struct DenseLayout {
     static constexpr int tab = box + kBins * 8 * 4;                     // uint2 [warps][4]: a target's candidate groups
     static constexpr int queue = tab + kDenseWarps * 4 * 8;             // uint32 [warps][kQueue]
     static constexpr int bar = queue + kDenseWarps * kQueue * 4;        // uint64
+    static constexpr int item = bar + 8;                                // uint32: the work item the CTA has drawn
     static constexpr int bytes = bar + 16;
 };
 static_assert((DenseLayout::bytes + 1024) * kDenseCtasPerSm <= 227 * 1024, "shared memory per SM");
@@ -66,7 +67,7 @@ static_assert((DenseLayout::bytes + 1024) * kDenseCtasPerSm <= 227 * 1024, "shar
 __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
     k_dense_forces(const float4* __restrict__ posm_s, const float4* __restrict__ velr_s, const float2* __restrict__ pc_s,
             const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start, GridDev g, float cell, float rc2,
-            ViscDev q, const unsigned int* __restrict__ ctl, const DenseItem* __restrict__ items,
+            ViscDev q, unsigned int* __restrict__ ctl, const DenseItem* __restrict__ items,
             float4* __restrict__ acc_out) {
     using L = DenseLayout;
     extern __shared__ __align__(128) unsigned char smem[];
@@ -85,6 +86,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
     uint32_t* s_bstart = reinterpret_cast<uint32_t*>(smem + L::bstart);
     float4* s_box = reinterpret_cast<float4*>(smem + L::box);
     uint64_t* s_bar = reinterpret_cast<uint64_t*>(smem + L::bar);
+    uint32_t* s_item = reinterpret_cast<uint32_t*>(smem + L::item);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned lt_mask = (1u << lane) - 1u;
@@ -128,13 +130,19 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
     const float half = 0.5f * cell;
     const float big = 3.0e38f;
 
-    for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+    for (;;) {
+        // items are handed out by a counter (ctl[1], zeroed before the launch): they differ by 100x in work, and a
+        // target's sum does not depend on which CTA takes its item
+        __syncthreads();   // the previous item's shared memory is no longer read
+        if (tid == 0) *s_item = atomicAdd(ctl + 1, 1u);
+        __syncthreads();
+        const uint32_t item = *s_item;
+        if (item >= n_items) break;
         const DenseItem it = items[item];
         const uint32_t mx = (uint32_t)g.mx, my = (uint32_t)g.my;
         const int ix = (int)(it.key % mx), iy = (int)((it.key / mx) % my), iz = (int)(it.key / (mx * my));
         const uint32_t ts = start[it.key] + it.chunk * kDenseTT;
         const uint32_t nt = min(start[it.key + 1u] - ts, (uint32_t)kDenseTT);
-        __syncthreads();   // the previous item's shared memory is no longer read
         if (tid < 9) {
             // row r: the cells (ix-1, ix, ix+1) at (iy + r%3 - 1, iz + r/3 - 1); boundaries b0 <= b1 <= b2 <= b3
             const int cy = iy + (tid % 3) - 1, cz = iz + (tid / 3) - 1;
@@ -402,6 +410,7 @@ int forces_dense(const float4* posm_s, const float4* velr_s, const float2* pc_s,
     }
     // the faces of the cells follow the rule the keys are made with (A7: c = (x - origin) * inv_cell), so the cell
     // edge is taken from inv_cell, not from g->cell
+    SPHB_CUDA(cudaMemsetAsync(dl.ctl + 1, 0, sizeof(unsigned int), st));   // the item counter
     k_dense_forces<<<kDenseCtasPerSm * num_sms(), kDenseThreads, DenseLayout::bytes, st>>>(
         posm_s, velr_s, pc_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, rc2, q, dl.ctl, dl.items, acc_sph);
     SPHB_LAUNCHED();

@@ -65,8 +65,13 @@ __device__ __forceinline__ float hydro_pair(const float4 vi /*v, rho*/, const fl
                                             const float4 vj, const float2 cj, const float dx, const float dy,
                                             const float dz, const float d2, const ViscDev& q, float& rv, float& mu,
                                             float& c_ij) {
-    float rinv = rsqrtf(d2);
-    if (!FAST) rinv = rinv * fmaf(-0.5f * d2 * rinv, rinv, 1.5f);   // one Newton step: ~1 ulp
+    float rinv;
+    if (FAST) {
+        asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(d2));   // d2 > 0 and far from the denormals (d2 ~ h^2)
+    } else {
+        rinv = rsqrtf(d2);
+        rinv = rinv * fmaf(-0.5f * d2 * rinv, rinv, 1.5f);   // one Newton step: ~1 ulp
+    }
     const float rr = d2 * rinv;                          // |dr|
     float num;
     if (FAST)
