@@ -78,7 +78,7 @@ def lib():
         L.orc_neighbours_grid.restype = None
         L.orc_density.argtypes = [dp, C.c_double, dp, ip, C.c_int64, ip, up, dp]
         L.orc_density.restype = None
-        L.orc_cfl_terms.argtypes = [dp, dp, dp, C.POINTER(_Params), ip, C.c_int64, ip, up, dp]
+        L.orc_cfl_terms.argtypes = [dp, dp, dp, C.POINTER(_Params), dp, ip, C.c_int64, ip, up, dp]
         L.orc_cfl_terms.restype = None
         L.orc_forces.argtypes = [dp, dp, dp, C.POINTER(_Params), dp, ip, C.c_int64, ip, up, dp, dp]
         L.orc_forces.restype = None
@@ -268,11 +268,13 @@ def forces(posm, vele, rho_all, h, offsets, index, targets=None, gamma=5.0 / 3.0
 
 
 def cfl_dt(posm, vele, rho_all, acc_sph, acc_grav, h, offsets, index, c_cfl, targets=None, gamma=5.0 / 3.0, alpha=0.5,
-           beta=1.0, eta=0.1):
+           beta=1.0, eta=0.1, hs=None):
     """Eq. 17 (L125-129): returns (dt, bracket[nt]) with dt = C_CFL min_i bracket_i,
     bracket_i = s_i / (c_i^max (1 + 1.2 alpha) + 1.2 beta mu_i^max + sqrt(s_i (|Q_i| + |E_i|))).
     acc_sph[nt,4] = (a_sph, de/dt) and acc_grav[nt,>=3] are given FOR THE TARGETS (Q_i = a_sph + a_grav is the
-    right-hand side of Eq. 10, E_i of Eq. 11); rho_all is indexed by gas index."""
+    right-hand side of Eq. 10, E_i of Eq. 11); rho_all is indexed by gas index.
+    hs: per-particle smoothing lengths (L82): mu_ij then uses h_ij = (h_i + h_j)/2 and a particle without a neighbour
+    takes s = 2 h_i (reading A22)."""
     posm, vele, rho_all = _f64(posm), _f64(vele), _f64(rho_all)
     tg = _tg(targets)
     nt = len(offsets) - 1
@@ -284,8 +286,9 @@ def cfl_dt(posm, vele, rho_all, acc_sph, acc_grav, h, offsets, index, c_cfl, tar
     prm = _Params(float(h), float(gamma), float(alpha), float(beta), float(eta))
     if nt == 0:
         return np.inf, np.zeros(0)
+    hs = _hs64(hs)
     lib().orc_cfl_terms(_p(posm, C.c_double), _p(vele, C.c_double), _p(rho_all, C.c_double), C.byref(prm),
-                        _p(tg, C.c_int64), nt, _p(off, C.c_int64), _p(idx, C.c_uint32), _p(terms, C.c_double))
+                        _p(hs, C.c_double), _p(tg, C.c_int64), nt, _p(off, C.c_int64), _p(idx, C.c_uint32), _p(terms, C.c_double))
     a_s = np.asarray(acc_sph, dtype=np.float64)
     a_g = np.asarray(acc_grav, dtype=np.float64)
     Q = np.linalg.norm(a_s[:, :3] + a_g[:, :3], axis=1)
@@ -330,7 +333,7 @@ def hydro(state: State, h, nbr, hs=None, **visc):
     return forces(state.posm, state.vele, state.rho, h, off, idx, hs=hs, **visc)
 
 
-def step(state: State, dt, h, G, delta, nbr=None, method="grid", hs=None, sigma=0.0, **visc):
+def step(state: State, dt, h, G, delta, nbr=None, method="grid", hs=None, sigma=0.0, c_cfl=None, **visc):
     """One predictor-corrector step, Eqs. 12-16 (L103-121), sequence of DESIGN.md A11:
     HFC(pred) -> SU(pred) -> SP, DC, GFC at r(t+dt) -> HFC(corr) -> SU(corr).
     `state` must carry rho and acc_grav at the current r (call position_only first);
@@ -339,7 +342,11 @@ def step(state: State, dt, h, G, delta, nbr=None, method="grid", hs=None, sigma=
     Per-particle smoothing lengths (L82, reading A26): with `hs` the pair length is h_ij = (h_i + h_j)/2 and h is the
     cap h_max; with sigma > 0 the lengths are renewed from the refined density, h_i = min(sigma (m_i/rho_i)^(1/3), h_max),
     right after DC at r(t+dt) — the density itself was summed with the old lengths — and used by the corrector and by
-    the next step (diag["hs"])."""
+    the next step (diag["hs"]).
+    Step size (Eq. 17): with c_cfl the step taken is min(dt, C_CFL min_i [...]) (diag["dt"]), the bracket
+    evaluated over the gas particles at the time layer t the step starts from — s^min, c^max, mu^max come out of the
+    same neighbour walk as HFC(predictor), Q_i and E_i are that walk's results — so `dt` is then the largest step
+    allowed (and the step of a run without gas, which Eq. 17 does not bound)."""
     ng = state.n_gas
     if nbr is None:
         nbr = _nbr(state.posm, ng, h, method, hs)
@@ -347,6 +354,11 @@ def step(state: State, dt, h, G, delta, nbr=None, method="grid", hs=None, sigma=
     hy = hydro(state, h, nbr, hs=hs, **visc)                   # HFC(predictor) at (r, v, e, rho)(t)
     Q[:ng] += hy[:, :3]
     E = hy[:, 3] if ng else np.zeros(0)
+    bracket = None
+    if c_cfl is not None and ng:
+        dt_cfl, bracket = cfl_dt(state.posm, state.vele, state.rho, hy, state.acc_grav[:ng], h, nbr[0], nbr[1], c_cfl, hs=hs,
+                                 **visc)
+        dt = min(float(dt), dt_cfl)
     v0 = state.vele[:, :3].copy()
     e0 = state.vele[:ng, 3].copy()
     v_t = v0 + dt * Q                                          # Eq. 12
@@ -366,7 +378,7 @@ def step(state: State, dt, h, G, delta, nbr=None, method="grid", hs=None, sigma=
     E1 = hy1[:, 3] if ng else np.zeros(0)
     new.vele[:, :3] = 0.5 * (v0 + v_t) + 0.5 * dt * Q1         # Eq. 15
     new.vele[:ng, 3] = 0.5 * (e0 + e_t) + 0.5 * dt * E1        # Eq. 16
-    diag = dict(hydro_pred=hy, hydro_corr=hy1, v_pred=v_t, e_pred=e_t, hs=hs1)
+    diag = dict(hydro_pred=hy, hydro_corr=hy1, v_pred=v_t, e_pred=e_t, hs=hs1, dt=float(dt), cfl_bracket=bracket)
     return new, nbr1, diag
 
 

@@ -426,9 +426,10 @@ void orc_forces(const double* posm, const double* vele, const double* rho_all, c
  * be 0); A9 pairs at zero separation are skipped; A22 a particle with no neighbour gets s = 2h,
  * c^max = c_i, mu^max = 0.  out[t] = (s_i, c_i^max, mu_i^max).                                     */
 void orc_cfl_terms(const double* posm, const double* vele, const double* rho_all, const orc_sph_params* p,
+                   const double* hs /*[n_gas] or NULL: h_ij = (h_i + h_j)/2 in mu_ij (L82, L97); no neighbour: s = 2 h_i*/,
                    const int64_t* targets, int64_t nt,
                    const int64_t* nbr_offset, const uint32_t* nbr_index, double* out) {
-    const double h = p->h, gm1 = p->gamma - 1.0;
+    const double gm1 = p->gamma - 1.0;
 #pragma omp parallel for schedule(dynamic, 64)
     for (int64_t t = 0; t < nt; ++t) {
         int64_t i = targets ? targets[t] : t;
@@ -442,6 +443,7 @@ void orc_cfl_terms(const double* posm, const double* vele, const double* rho_all
             double r = sqrt(r2);
             double rv = dx * (vele[4 * i] - vele[4 * j]) + dy * (vele[4 * i + 1] - vele[4 * j + 1]) +
                         dz * (vele[4 * i + 2] - vele[4 * j + 2]);
+            double h = hs ? 0.5 * (hs[i] + hs[j]) : p->h;
             double mu = (rv < 0.0) ? h * rv / (r2 + p->eta * h * h) : 0.0;
             double cj = sqrt(p->gamma * (gm1 * rho_all[j] * vele[4 * j + 3]) / rho_all[j]);
             double cij = 0.5 * (ci + cj);
@@ -449,7 +451,7 @@ void orc_cfl_terms(const double* posm, const double* vele, const double* rho_all
             if (cij > cmax) cmax = cij;
             if (fabs(mu) > mumax) mumax = fabs(mu);
         }
-        out[3 * t + 0] = smin < 0.0 ? 2.0 * h : smin;
+        out[3 * t + 0] = smin < 0.0 ? 2.0 * (hs ? hs[i] : p->h) : smin;
         out[3 * t + 1] = cmax;
         out[3 * t + 2] = mumax;
     }

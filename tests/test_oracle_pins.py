@@ -561,6 +561,59 @@ def test_CFL_isolated_particle_and_monotonicity():
     assert np.isclose(br2[0], 2 * h / (1.6 + math.sqrt(2 * h * 10.0)), rtol=1e-14)
 
 
+def test_CFL_pair_lengths_by_hand():
+    """Eq. 17 with per-particle smoothing lengths (L82): mu_ij takes h_ij = (h_1 + h_2)/2.  The hand-worked pair of
+    cfl_two_particles with h_1 = 0.75, h_2 = 1.25 (h_ij = 1) gives the same bracket as the global h = 1; with h_1 = h_2 = 2
+    |mu| = 2/(1 + 0.4) = 10/7: bracket 1/(1.6 + 1.2*10/7 + 2).  A particle without a neighbour takes s = 2 h_i (A22)."""
+    posm = np.array([[0, 0, 0, 1.0], [1, 0, 0, 1.0], [50, 0, 0, 1.0]], dtype=np.float64)
+    vele = np.array([[0.5, 0, 0, 0.9], [-0.5, 0, 0, 0.9], [0, 0, 0, 0.9]], dtype=np.float64)
+    acc_sph = np.array([[3.0, 0, 0, 1.0], [0, 2.0, 0, -1.0], [0, 0, 0, 0.0]])
+    acc_grav = np.array([[0.0, 0, 0, 0], [0, 1.0, 0, 0], [0, 0, 0, 0]])
+    num, den = _golden("cfl_two_particles").split("/")
+    expect = float(Fraction(num) / Fraction(den)) / 0.5                          # the bracket itself
+    for hs, want in (([0.75, 1.25, 0.25], expect), ([2.0, 2.0, 0.25], 1.0 / (1.6 + 12.0 / 7.0 + 2.0))):   # exact in FP32
+        hs = np.array(hs)
+        off, idx = oracle.neighbours(posm, 3, 2.0, hs=hs)
+        assert np.diff(off).tolist() == [1, 1, 0]
+        rho = oracle.density(posm, 2.0, off, idx, hs=hs)
+        dt, br = oracle.cfl_dt(posm, vele, rho, acc_sph, acc_grav, 2.0, off, idx, 1.0, hs=hs)
+        assert np.allclose(br[:2], want, rtol=1e-14, atol=0)
+        assert np.isclose(br[2], 2 * 0.25 / 1.6, rtol=1e-14, atol=0)             # isolated: s = 2 h_i, c = 1, alpha = 0.5
+        assert np.isclose(dt, br.min())
+    # equal lengths reduce to the global-h result
+    off, idx = oracle.neighbours(posm, 3, 1.0)
+    rho = oracle.density(posm, 1.0, off, idx)
+    _, br_g = oracle.cfl_dt(posm, vele, rho, acc_sph, acc_grav, 1.0, off, idx, 1.0)
+    _, br_h = oracle.cfl_dt(posm, vele, rho, acc_sph, acc_grav, 1.0, off, idx, 1.0, hs=np.ones(3))
+    assert np.array_equal(br_g, br_h)
+
+
+def test_CFL_adaptive_step():
+    """oracle.step(c_cfl=): the step taken is min(dt, C_CFL min_i bracket_i) with the bracket of Eq. 17 at the time layer
+    the step starts from.  (1) a large ceiling: the step equals C_CFL times the minimum of cfl_dt called by hand on the
+    same state; (2) a ceiling below the CFL value: bit for bit the fixed-step result; (3) energy (pin P7): 10 adaptive
+    steps at config 0, C_CFL = 0.5, stay inside the drift bound of the fixed-step run over the same time."""
+    w = wl.make_workload(0, scale=0.25)
+    st0 = oracle.State(w.posm.astype(np.float64), w.vele.astype(np.float64), w.n_gas)
+    nbr = oracle.position_only(st0, w.h, w.G, w.delta)
+    hy = oracle.hydro(st0, w.h, nbr)
+    dt_hand, br = oracle.cfl_dt(st0.posm, st0.vele, st0.rho, hy, st0.acc_grav[: w.n_gas], w.h, nbr[0], nbr[1], 0.5)
+    s1, _, d1 = oracle.step(st0, 1.0, w.h, w.G, w.delta, nbr=nbr, c_cfl=0.5)
+    assert d1["dt"] == dt_hand and dt_hand == 0.5 * br.min() and 0 < dt_hand < 1.0
+    tiny = 0.1 * dt_hand
+    s2, _, d2 = oracle.step(st0, tiny, w.h, w.G, w.delta, nbr=nbr, c_cfl=0.5)
+    s3, _, _ = oracle.step(st0, tiny, w.h, w.G, w.delta, nbr=nbr)
+    assert d2["dt"] == tiny and np.array_equal(s2.posm, s3.posm) and np.array_equal(s2.vele, s3.vele)
+    # energy over 10 adaptive steps
+    e0 = oracle.total_energy(st0, w.G, w.delta)
+    st, nb, t = st0, nbr, 0.0
+    for _ in range(10):
+        st, nb, d = oracle.step(st, 1.0, w.h, w.G, w.delta, nbr=nb, c_cfl=0.5)
+        t += d["dt"]
+    drift = abs(oracle.total_energy(st, w.G, w.delta) - e0) / abs(e0)
+    assert t > 0 and drift < 1e-7 * max(1.0, t / 0.01), (drift, t)
+
+
 # ---------------------------------------------------------------- NEXT-2: per-particle smoothing lengths (L82)
 def _varh_case(n=1500, seed=11, h_max=0.08):
     rng = np.random.Generator(np.random.Philox(key=[seed, 0]))
