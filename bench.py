@@ -217,6 +217,26 @@ def oracle_sample_step(w, n_targets=1024, seed=123):
     return step_s * 1e3, sample_s, desc, t
 
 
+def oracle_full_steps():
+    """configs 0 and 1 are small enough to time the oracle's WHOLE step (no extrapolation), config 0
+    also on one thread.  The carried state (grid, density, gravity at the current positions) is seeded untimed,
+    as for the CUDA path."""
+    import oracle
+    from paper_1807_08116_b200 import workloads as wl
+    out = {}
+    cores = oracle.num_threads()
+    for cfg, threads in ((0, cores), (0, 1), (1, cores)):
+        w = wl.make_workload(cfg)
+        oracle.set_num_threads(threads)
+        st = oracle.State(w.posm.astype(np.float64), w.vele.astype(np.float64), w.n_gas)
+        nbr = oracle.position_only(st, w.h, w.G, w.delta)
+        t0 = time.perf_counter()
+        oracle.step(st, w.dt, w.h, w.G, w.delta, nbr=nbr)
+        out[f"config{cfg}_step_ms_{threads}_threads"] = (time.perf_counter() - t0) * 1e3
+    oracle.set_num_threads(cores)
+    return out
+
+
 def run_reference(args, w):
     import oracle
     rank, _, _ = _env_rank()
@@ -224,7 +244,7 @@ def run_reference(args, w):
         return
     vals = []
     for i in range(args.warmup + args.steps):
-        ms, _, desc, _ = oracle_sample_step(w, n_targets=args.ref_targets, seed=100 + i)
+        ms, _, desc, _ = oracle_sample_step(w, n_targets=args.ref_targets)
         if i >= args.warmup:
             vals.append(ms)
     v = float(np.mean(vals))
@@ -420,7 +440,7 @@ def run_ours(args, w):
                             "fp32_pipe_util is the share of FP32 issue capacity (128 lanes/clk/SM) the executed operations take"}
     hbm = float(peaks.get("hbm_gbs", 6650.0))
     pairs = sph_pair_counts(b, sim, w) if (ng and world == 1) else None
-    sort_bytes = ng * 92 + M * 16
+    sort_bytes = ng * 92 + M * 12          # 92 B per gas particle, 12 B per cell (zero 4, scan read 4 + write 4)
     # gas: predictor 64 B read + 48 B written, corrector 64 + 16; halo particles never touch acc_sph: 48 + 48, 48 + 16
     upd_bytes = ng * (112 + 80) + (n - ng) * (96 + 64)
     stages = {
@@ -459,7 +479,8 @@ def run_ours(args, w):
         import oracle
         ms, sample_s, desc, _ = oracle_sample_step(w, n_targets=args.cpu_targets)
         cpu = {"value": ms, "unit": "ms", "cores": oracle.num_threads(), "kind": "oracle",
-               "sample": desc + f" ({sample_s:.1f} s of CPU wall time)", "extrapolated": True}
+               "sample": desc + f" ({sample_s:.1f} s of CPU wall time)", "extrapolated": True,
+               "full_steps_timed": oracle_full_steps()}
 
     line = {
         "metric": "step_ms", "value": ms_step, "unit": "ms", "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
@@ -492,8 +513,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    # one sample size for the cpu_baseline leg and the reference arm: the two estimate the same quantity
     ap.add_argument("--cpu-targets", type=int, default=32768)
-    ap.add_argument("--ref-targets", type=int, default=8192)
+    ap.add_argument("--ref-targets", type=int, default=32768)
     args = ap.parse_args()
     if args.gpus < 1:
         raise SystemExit("bench.py: --gpus must be >= 1")

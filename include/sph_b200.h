@@ -148,7 +148,9 @@ int sph_evaluate(const float* posm, const float* vele, int64_t n_gas, int64_t n_
  * acc_grav are the arrays the last sph_evaluate / sph_step left behind; perm / cell_start the grid
  * of the same positions.  dt_out: DEVICE, one float (+inf if n_gas = 0).  dt_particle: DEVICE
  * [n_gas], the bracket of Eq. 17 per particle WITHOUT C_CFL, or NULL.  The minimum is taken with
- * integer atomics on the float bit pattern: exact and order-independent.                       */
+ * integer atomics on the float bit pattern: exact and order-independent.  The terms s, c^max, mu^max are
+ * gathered "inside the HFC neighbour loop": this call runs the forces walk (the same kernels as sph_forces, in their
+ * CFL instantiation) and discards its sums; sph_step_cfl below gets them from the step's own HFC(predictor).  */
 int sph_cfl_dt(const float* posm, const float* vele, const float* rho, const float* acc_sph, const float* acc_grav,
                int64_t n_gas, const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/,
                const uint32_t* perm, const uint32_t* cell_start, float c_cfl,
@@ -188,8 +190,9 @@ int sph_neighbour_lists(const float* posm, int64_t n_gas, float h, const sph_gri
  * in grad W_p (L95) and in mu_ij (L97); (i, j) is a neighbour pair iff d2 < fl(fl(h_i + h_j)^2), FP32 like the
  * global cutoff (reading A24; equal to it when h_i = h_j = h).  In these calls p->h is the CAP h_max of the
  * lengths: the grid needs cell >= 2 h_max for the 3x3x3 stencil (that is what the paper's per-cell hmaxCell
- * array, L164, provides for a finer grid), and every hsml[i] must be <= p->h — not checked (it would need a
- * device reduction and a synchronisation); a larger value silently loses neighbours.
+ * array, L164, provides for a finer grid), and every hsml[i] must be <= p->h.  A larger value (or a NaN) would lose
+ * neighbours; the kernel that brings the lengths into cell order raises SPH_STATUS_HSML_ABOVE_CAP in the workspace's
+ * status word, which sph_workspace_status() reads back (no synchronisation on the step path itself).
  *
  * sph_smoothing_lengths: hsml[i] = min(sigma (m_i / rho_i)^(1/3), h_max)        (L82; reading A25)
  * sph_density_h / sph_forces_h / sph_evaluate_h / sph_neighbour_lists_h: as the calls without _h.
@@ -210,6 +213,18 @@ int sph_evaluate_h(const float* posm, const float* vele, const float* hsml, int6
 int sph_step_h(float* posm, float* vele, float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p /*HOST*/,
                const sph_grid* g /*HOST*/, float sigma, float dt, int first, float* rho, float* acc_sph,
                float* acc_grav, void* ws, size_t ws_bytes, void* stream);
+/* One predictor-corrector step whose size comes from Eq. 17 (L125-129): as sph_step_h, but the step taken is
+ *   dt = min(dt_max, C_CFL min_i [ s_i / (c_i^max (1 + 1.2 alpha) + 1.2 beta mu_i^max + sqrt(s_i (|Q_i| + |E_i|))) ])
+ * with the bracket evaluated over the gas particles at the time layer the step starts from: s_i, c_i^max, mu_i^max are
+ * reduced by HFC(predictor) itself over its accepted pairs, Q_i and E_i are its results (+ the carried a_grav).  The
+ * minimum is taken on the device and read by the update kernels from device memory: no host read-back, the call stays
+ * asynchronous and graph-capturable.  dt_used: DEVICE, one float, the step taken.  hsml may be NULL (one global h);
+ * with hsml, mu_ij uses h_ij and a particle without a neighbour takes s = 2 h_i.  Without gas the step is dt_max.
+ * c_cfl > 0 (the paper: 0.5 <~ C_CFL < 1), dt_max > 0.                                                             */
+int sph_step_cfl(float* posm, float* vele, float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p /*HOST*/,
+                 const sph_grid* g /*HOST*/, float sigma, float c_cfl, float dt_max, int first, float* rho,
+                 float* acc_sph, float* acc_grav, float* dt_used /*DEVICE [1]*/, void* ws, size_t ws_bytes, void* stream);
+
 int sph_neighbour_lists_h(const float* posm, const float* hsml, int64_t n_gas, float h_max, const sph_grid* g /*HOST*/,
                           const uint32_t* perm, const uint32_t* cell_start, uint32_t* nbr_count,
                           uint64_t* nbr_offset, uint32_t* nbr_index, uint64_t nbr_capacity,
@@ -296,7 +311,16 @@ enum { SPH_GRAV_ONE_SIDED = 0, SPH_GRAV_ONE_SIDED_UNIFORM = 1, SPH_GRAV_PAIR_SYM
 int sph_gravity_path(const void* ws /*DEVICE*/, size_t ws_bytes, int64_t n_gas, int64_t n_total,
                      const sph_grid* g /*HOST, may be NULL if n_gas == 0*/, int* path_host /*HOST*/, void* stream);
 
-/* Diagnostic: how many work items the LAST density / forces / grid-building call enqueued with workspace `ws` (sized for
+/* Status word of a workspace: bits raised on the device by the calls that ran with `ws` (sized for n_gas, n_total and g,
+ * as in those calls) since the word was last read.  Reads it back, clears it and SYNCHRONISES `stream`.
+ * SPH_STATUS_HSML_ABOVE_CAP: a per-particle smoothing length (L82) exceeded the cap p->h that sized the cells (or was NaN):
+ * the neighbour sets of the calls since the last read are incomplete.  The word lives in the first 256 bytes of the
+ * workspace: zero those once in a new workspace for it to start clear (nothing else in a workspace needs initialising). */
+enum { SPH_STATUS_HSML_ABOVE_CAP = 1 };
+int sph_workspace_status(void* ws /*DEVICE*/, size_t ws_bytes, int64_t n_gas, int64_t n_total,
+                         const sph_grid* g /*HOST, may be NULL if n_gas == 0*/, uint32_t* status_host /*HOST*/, void* stream);
+
+/* Diagnostic: how many work items the LAST forces / grid-building call enqueued with workspace `ws` (sized for
  * n_gas, n_total and g, as in that call) handed to the dense-cell walk of the neighbour passes (DESIGN.md section 5.3:
  * cells holding at least 32 particles, 128 targets per item; the DC / HFC sums of PAPER.md L143-145, L207 over the cell
  * lists).  0 means every particle was walked by the thread-per-slot kernels.  Reads the counter back and SYNCHRONISES

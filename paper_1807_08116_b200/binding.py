@@ -26,8 +26,8 @@ EXPORTS = (
     "sph_host_ctx_create", "sph_host_ctx_step", "sph_host_ctx_destroy", "sph_neighbour_lists",
     "sph_set_profiling", "sph_get_stage_ms", "sph_launch_count", "sph_cfl_dt",
     "nbody_pp_gravity_slice", "sph_position_slice", "sph_predict", "sph_correct",
-    "sph_gravity_path", "sph_dense_items", "sph_position_share", "nbody_pp_gravity_share", "nbody_pp_gravity_finish",
-    "sph_workspace_gravity_sums", "sph_smoothing_lengths", "sph_density_h", "sph_forces_h", "sph_evaluate_h", "sph_step_h", "sph_neighbour_lists_h",
+    "sph_gravity_path", "sph_dense_items", "sph_workspace_status", "sph_position_share", "nbody_pp_gravity_share", "nbody_pp_gravity_finish",
+    "sph_workspace_gravity_sums", "sph_smoothing_lengths", "sph_density_h", "sph_forces_h", "sph_evaluate_h", "sph_step_h", "sph_neighbour_lists_h", "sph_step_cfl",
 )
 
 
@@ -99,6 +99,7 @@ def load():
     L.sph_workspace_gravity_sums.argtypes = [i64, i64, gp, C.POINTER(sz), C.POINTER(sz)]
     L.sph_gravity_path.argtypes = [vp, sz, i64, i64, gp, C.POINTER(C.c_int), vp]
     L.sph_dense_items.argtypes = [vp, sz, i64, i64, gp, C.POINTER(C.c_uint32), vp]
+    L.sph_workspace_status.argtypes = [vp, sz, i64, i64, gp, C.POINTER(C.c_uint32), vp]
     L.sph_cfl_dt.argtypes = [vp, vp, vp, vp, vp, i64, pp, gp, vp, vp, f32, vp, vp, vp, sz, vp]
     L.sph_step.argtypes = [vp, vp, i64, i64, pp, gp, f32, C.c_int, vp, vp, vp, vp, sz, vp]
     L.sph_evaluate.argtypes = [vp, vp, i64, i64, pp, gp, vp, vp, vp, vp, sz, vp]
@@ -117,6 +118,7 @@ def load():
     L.sph_forces_h.argtypes = [vp, vp, vp, vp, i64, pp, gp, vp, vp, vp, vp, sz, vp]
     L.sph_evaluate_h.argtypes = [vp, vp, vp, i64, i64, pp, gp, vp, vp, vp, vp, sz, vp]
     L.sph_step_h.argtypes = [vp, vp, vp, i64, i64, pp, gp, f32, f32, C.c_int, vp, vp, vp, vp, sz, vp]
+    L.sph_step_cfl.argtypes = [vp, vp, vp, i64, i64, pp, gp, f32, f32, f32, C.c_int, vp, vp, vp, vp, vp, sz, vp]
     _lib = L
     return L
 
@@ -148,7 +150,9 @@ def _ws(ws):
 
 def alloc_workspace(n_gas, n_total, grid=None) -> torch.Tensor:
     nbytes = sph_workspace_bytes(n_gas, n_total, grid)
-    return torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    ws[:256].zero_()          # the status word (sph_workspace_status) starts clear
+    return ws
 
 
 # ------------------------------------------------------------------ the boundary, one function per entry point
@@ -313,6 +317,15 @@ def sph_step_h(posm, vele, hsml, n_gas, n_halo, params, grid, sigma, dt, first, 
                                          _ptr(acc_grav), p, nb, _stream()))
 
 
+def sph_step_cfl(posm, vele, hsml, n_gas, n_halo, params, grid, sigma, c_cfl, dt_max, first, rho, acc_sph, acc_grav, dt_used,
+                 ws):
+    p, nb = _ws(ws)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_step_cfl", load().sph_step_cfl(_ptr(posm), _ptr(vele), _ptr(hsml), int(n_gas), int(n_halo), C.byref(params), g,
+                                             float(sigma), float(c_cfl), float(dt_max), int(bool(first)), _ptr(rho),
+                                             _ptr(acc_sph), _ptr(acc_grav), _ptr(dt_used), p, nb, _stream()))
+
+
 def _hp(a):
     if a is None:
         return None
@@ -397,6 +410,18 @@ def sph_gravity_path(ws, n_gas, n_total, grid=None) -> str:
     return GRAV_PATHS[out.value]
 
 
+SPH_STATUS_HSML_ABOVE_CAP = 1
+
+
+def sph_workspace_status(ws, n_gas, n_total, grid=None) -> int:
+    """Status bits the device raised in `ws` since the last read (read back and cleared; synchronises)."""
+    p, nb = _ws(ws)
+    out = C.c_uint32(0)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_workspace_status", load().sph_workspace_status(p, nb, int(n_gas), int(n_total), g, C.byref(out), _stream()))
+    return int(out.value)
+
+
 def sph_dense_items(ws, n_gas, n_total, grid) -> int:
     """Work items the last density / forces / grid-building call with `ws` gave to the dense-cell walk (0: none)."""
     p, nb = _ws(ws)
@@ -439,8 +464,17 @@ class Simulation:
                        self.acc_sph, self.acc_grav, self.ws)
         self.first = False
 
-    def step(self, dt=None):
-        sph_step_h(self.posm, self.vele, self.hsml, self.n_gas, self.n_halo, self.params, self.grid,
-                   self.sigma or 0.0, self.w.dt if dt is None else dt, self.first, self.rho, self.acc_sph, self.acc_grav,
-                   self.ws)
+    def step(self, dt=None, c_cfl=None):
+        """c_cfl: the step is min(dt, C_CFL min_i [...]) of Eq. 17, chosen on the device; self.dt_used (a device float)
+        holds it afterwards."""
+        dt = self.w.dt if dt is None else dt
+        if c_cfl is None:
+            sph_step_h(self.posm, self.vele, self.hsml, self.n_gas, self.n_halo, self.params, self.grid,
+                       self.sigma or 0.0, dt, self.first, self.rho, self.acc_sph, self.acc_grav, self.ws)
+        else:
+            if getattr(self, "dt_used", None) is None:
+                self.dt_used = torch.zeros(1, dtype=torch.float32, device="cuda")
+            sph_step_cfl(self.posm, self.vele, self.hsml, self.n_gas, self.n_halo, self.params, self.grid,
+                         self.sigma or 0.0, c_cfl, dt, self.first, self.rho, self.acc_sph, self.acc_grav, self.dt_used,
+                         self.ws)
         self.first = False

@@ -56,14 +56,14 @@ int position_only(const float4* posm, float* hsml, float sigma, int64_t n_gas, i
             Span sp(ST_SORT, st);
             SPHB_TRY(grid_build(posm, n_gas, g, w.key, w.perm, w.cell_count, w.cell_start, w.rank_u, w.tmp, w.tile_sums,
                                 w.posm_s, &w.dense, st));
-            if (hsml) SPHB_TRY(gather_sorted_h(hsml, w.perm, n_gas, w.h_s, st));
+            if (hsml) SPHB_TRY(gather_sorted_h(hsml, w.perm, n_gas, p->h, w.status, w.h_s, st));
         }
         {
             Span sp(ST_DENSITY, st);
             SPHB_TRY(density_sorted(w.posm_s, hsml ? w.h_s : nullptr, w.perm, w.cell_start, n_gas, p, g, rho, st));
             if (hsml && sigma > 0.f) {
                 SPHB_TRY(smoothing_lengths(posm, rho, n_gas, sigma, p->h, hsml, st));
-                SPHB_TRY(gather_sorted_h(hsml, w.perm, n_gas, w.h_s, st));
+                SPHB_TRY(gather_sorted_h(hsml, w.perm, n_gas, p->h, w.status, w.h_s, st));
             }
         }
     }
@@ -79,11 +79,11 @@ int position_only(const float4* posm, float* hsml, float sigma, int64_t n_gas, i
 }
 
 int hydro(const float4* vele, const float* rho, bool varh, int64_t n_gas, const sph_params* p, const sph_grid* g,
-          float4* acc_sph, const Workspace& w, cudaStream_t st) {
+          float4* acc_sph, const Workspace& w, cudaStream_t st, const CflArgs* cfl = nullptr) {
     if (n_gas <= 0) return SPH_OK;
     Span sp(ST_FORCES, st);
-    return forces_sorted(w.posm_s, vele, rho, varh ? w.h_s : nullptr, w.perm, w.cell_start, n_gas, p, g, &w.dense, w.velr_s,
-                         w.pc_s, acc_sph, st);
+    return forces_sorted(w.posm_s, vele, rho, varh ? w.h_s : nullptr, w.perm, w.cell_start, n_gas, p, g, &w.dense, cfl,
+                         w.velr_s, w.pc_s, acc_sph, st);
 }
 
 int check_state_args(const void* posm, const void* vele, int64_t n_gas, int64_t n_halo, const sph_params* p,
@@ -138,9 +138,9 @@ size_t sph_workspace_bytes(int64_t n_gas, int64_t n_total, const sph_grid* g) {
 int sph_grid_from_bbox(const float* posm, int64_t n_gas, float h, sph_grid* out, void* ws, size_t ws_bytes,
                        void* stream) {
     if (!posm || !out || !ws || n_gas <= 0 || bad_count(n_gas) || !(h > 0.f) || !aligned16(posm)) return SPH_ERR_ARG;
-    if (ws_bytes < 8 * sizeof(float)) return SPH_ERR_WORKSPACE;
+    if (ws_bytes < 256 + 8 * sizeof(float)) return SPH_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
-    float* bb = static_cast<float*>(ws);
+    float* bb = reinterpret_cast<float*>(static_cast<char*>(ws) + 256);   // behind the status block (Workspace::bbox)
     SPHB_TRY(bbox_gas(reinterpret_cast<const float4*>(posm), n_gas, bb, st));
     float host[6];
     SPHB_CUDA(cudaMemcpyAsync(host, bb, sizeof(host), cudaMemcpyDeviceToHost, st));
@@ -212,7 +212,7 @@ int sph_forces(const float* posm, const float* vele, const float* rho, int64_t n
     SPHB_TRY(dense_list_from_start(cell_start, g, w.dense, st));
     Span sp(ST_FORCES, st);
     return forces_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, nullptr, perm, cell_start, n_gas, p, g, &w.dense,
-                         w.velr_s, w.pc_s, reinterpret_cast<float4*>(acc_sph), st);
+                         nullptr, w.velr_s, w.pc_s, reinterpret_cast<float4*>(acc_sph), st);
 }
 
 int sph_cfl_dt(const float* posm, const float* vele, const float* rho, const float* acc_sph, const float* acc_grav,
@@ -221,9 +221,8 @@ int sph_cfl_dt(const float* posm, const float* vele, const float* rho, const flo
     if (bad_count(n_gas) || !dt_out || !(c_cfl > 0.f)) return SPH_ERR_ARG;
     SPHB_TRY(check_params(p, n_gas > 0));
     cudaStream_t st = (cudaStream_t)stream;
-    if (n_gas == 0)
-        return cfl_sorted(nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, 0, p, g, c_cfl, nullptr, nullptr,
-                          dt_out, dt_particle, st);
+    SPHB_TRY(cfl_init(dt_out, __builtin_inff(), st));
+    if (n_gas == 0) return SPH_OK;
     if (!posm || !vele || !rho || !acc_sph || !acc_grav || !perm || !cell_start || !ws || !aligned16(posm) ||
         !aligned16(vele) || !aligned16(acc_sph) || !aligned16(acc_grav) || (reinterpret_cast<uintptr_t>(ws) & 255u))
         return SPH_ERR_ARG;
@@ -231,9 +230,12 @@ int sph_cfl_dt(const float* posm, const float* vele, const float* rho, const flo
     Workspace w = carve(ws, n_gas, n_gas, g);
     if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
     SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
-    return cfl_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, reinterpret_cast<const float4*>(acc_sph),
-                      reinterpret_cast<const float4*>(acc_grav), perm, cell_start, n_gas, p, g, c_cfl, w.velr_s, w.pc_s,
-                      dt_out, dt_particle, st);
+    SPHB_TRY(dense_list_from_start(cell_start, g, w.dense, st));
+    // the forces walk in its CFL mode, its own sums discarded: |Q_i| and |E_i| come from the caller's arrays
+    const CflArgs cfl{c_cfl, reinterpret_cast<const float4*>(acc_sph), reinterpret_cast<const float4*>(acc_grav), dt_particle,
+                      reinterpret_cast<unsigned int*>(dt_out)};
+    return forces_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, nullptr, perm, cell_start, n_gas, p, g, &w.dense,
+                         &cfl, w.velr_s, w.pc_s, nullptr, st);
 }
 
 int nbody_pp_gravity_slice(const float* posm, int64_t n_total, int64_t i0, int64_t i1, float G, float delta,
@@ -262,6 +264,18 @@ int sph_gravity_path(const void* ws, size_t ws_bytes, int64_t n_gas, int64_t n_t
     SPHB_CUDA(cudaStreamSynchronize(st));
     *path_host = ctl[1] != 0u ? (ctl[0] != 0u ? SPH_GRAV_PAIR_SYMMETRIC_GENERAL : SPH_GRAV_PAIR_SYMMETRIC)
                               : (ctl[0] != 0u ? SPH_GRAV_ONE_SIDED : SPH_GRAV_ONE_SIDED_UNIFORM);
+    return SPH_OK;
+}
+
+int sph_workspace_status(void* ws, size_t ws_bytes, int64_t n_gas, int64_t n_total, const sph_grid* g, uint32_t* status_host,
+                         void* stream) {
+    if (!ws || !status_host || bad_count(n_total) || bad_count(n_gas) || n_gas > n_total || (n_gas > 0 && !g)) return SPH_ERR_ARG;
+    Workspace w = carve(ws, n_gas, n_total, n_gas > 0 ? g : nullptr);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    SPHB_CUDA(cudaMemcpyAsync(status_host, w.status, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+    SPHB_CUDA(cudaMemsetAsync(w.status, 0, sizeof(uint32_t), st));
+    SPHB_CUDA(cudaStreamSynchronize(st));
     return SPH_OK;
 }
 
@@ -377,24 +391,36 @@ int sph_workspace_gravity_sums(int64_t n_gas, int64_t n_total, const sph_grid* g
     return SPH_OK;
 }
 
-int sph_predict(float* posm, float* vele, const float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p,
-                const sph_grid* g, float dt, const float* rho, float* acc_sph, const float* acc_grav, void* ws,
-                size_t ws_bytes, void* stream) {
+}  // extern "C"
+
+namespace {
+// HFC(predictor) + SU(predictor).  c_cfl > 0: the step is min(dt, C_CFL min_i [...]) of Eq. 17, reduced by the forces
+// walk itself into *dt_dev (device), which the update kernels then read — no host read-back.
+int predict(float* posm, float* vele, const float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p,
+            const sph_grid* g, float dt, float c_cfl, float* dt_dev, const float* rho, float* acc_sph, const float* acc_grav,
+            void* ws, size_t ws_bytes, void* stream) {
     SPHB_TRY(check_state_args(posm, vele, n_gas, n_halo, p, g, rho, acc_sph, acc_grav, ws, ws_bytes));
     const int64_t n = n_gas + n_halo;
     if (n == 0) return SPH_OK;
     Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
     cudaStream_t st = (cudaStream_t)stream;
     float4* as4 = reinterpret_cast<float4*>(acc_sph);
-    SPHB_TRY(hydro(reinterpret_cast<const float4*>(vele), rho, hsml != nullptr && n_gas > 0, n_gas, p, g, as4, w, st));
+    const bool varh = hsml != nullptr && n_gas > 0;
+    if (dt_dev) {
+        SPHB_TRY(cfl_init(dt_dev, dt, st));
+        const CflArgs cfl{c_cfl, nullptr, reinterpret_cast<const float4*>(acc_grav), nullptr, reinterpret_cast<unsigned int*>(dt_dev)};
+        SPHB_TRY(hydro(reinterpret_cast<const float4*>(vele), rho, varh, n_gas, p, g, as4, w, st, &cfl));
+    } else {
+        SPHB_TRY(hydro(reinterpret_cast<const float4*>(vele), rho, varh, n_gas, p, g, as4, w, st));
+    }
     Span sp(ST_UPDATE, st);
     return update_predictor(reinterpret_cast<float4*>(posm), reinterpret_cast<float4*>(vele), w.vele0, as4,
-                            reinterpret_cast<const float4*>(acc_grav), n_gas, n, dt, st);   // Eqs. 12-14
+                            reinterpret_cast<const float4*>(acc_grav), n_gas, n, dt, dt_dev, st);   // Eqs. 12-14
 }
 
-int sph_correct(float* vele, const float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p, const sph_grid* g,
-                float dt, const float* rho, float* acc_sph, const float* acc_grav, void* ws, size_t ws_bytes,
-                void* stream) {
+int correct(float* vele, const float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p, const sph_grid* g, float dt,
+            const float* dt_dev, const float* rho, float* acc_sph, const float* acc_grav, void* ws, size_t ws_bytes,
+            void* stream) {
     SPHB_TRY(check_state_args(vele, vele, n_gas, n_halo, p, g, rho, acc_sph, acc_grav, ws, ws_bytes));
     const int64_t n = n_gas + n_halo;
     if (n == 0) return SPH_OK;
@@ -404,7 +430,36 @@ int sph_correct(float* vele, const float* hsml, int64_t n_gas, int64_t n_halo, c
     SPHB_TRY(hydro(reinterpret_cast<const float4*>(vele), rho, hsml != nullptr && n_gas > 0, n_gas, p, g, as4, w, st));
     Span sp(ST_UPDATE, st);
     return update_corrector(reinterpret_cast<float4*>(vele), w.vele0, as4, reinterpret_cast<const float4*>(acc_grav),
-                            n_gas, n, dt, st);                                               // Eqs. 15-16
+                            n_gas, n, dt, dt_dev, st);                                       // Eqs. 15-16
+}
+}  // namespace
+
+extern "C" {
+
+int sph_predict(float* posm, float* vele, const float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p,
+                const sph_grid* g, float dt, const float* rho, float* acc_sph, const float* acc_grav, void* ws,
+                size_t ws_bytes, void* stream) {
+    return predict(posm, vele, hsml, n_gas, n_halo, p, g, dt, 0.f, nullptr, rho, acc_sph, acc_grav, ws, ws_bytes, stream);
+}
+
+int sph_correct(float* vele, const float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p, const sph_grid* g,
+                float dt, const float* rho, float* acc_sph, const float* acc_grav, void* ws, size_t ws_bytes,
+                void* stream) {
+    return correct(vele, hsml, n_gas, n_halo, p, g, dt, nullptr, rho, acc_sph, acc_grav, ws, ws_bytes, stream);
+}
+
+int sph_step_cfl(float* posm, float* vele, float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p,
+                 const sph_grid* g, float sigma, float c_cfl, float dt_max, int first, float* rho, float* acc_sph,
+                 float* acc_grav, float* dt_used, void* ws, size_t ws_bytes, void* stream) {
+    SPHB_TRY(check_state_args(posm, vele, n_gas, n_halo, p, g, rho, acc_sph, acc_grav, ws, ws_bytes));
+    if (sigma < 0.f || !(c_cfl > 0.f) || !(dt_max > 0.f) || !dt_used) return SPH_ERR_ARG;
+    const int64_t n = n_gas + n_halo;
+    if (n == 0) return SPH_OK;
+    if (first)   // seed the carried state: SP, DC, GFC at the current positions
+        SPHB_TRY(sph_position_slice(posm, hsml, 0.f, n_gas, n_halo, 0, n, p, g, rho, acc_grav, ws, ws_bytes, stream));
+    SPHB_TRY(predict(posm, vele, hsml, n_gas, n_halo, p, g, dt_max, c_cfl, dt_used, rho, acc_sph, acc_grav, ws, ws_bytes, stream));
+    SPHB_TRY(sph_position_slice(posm, hsml, sigma, n_gas, n_halo, 0, n, p, g, rho, acc_grav, ws, ws_bytes, stream));
+    return correct(vele, hsml, n_gas, n_halo, p, g, dt_max, dt_used, rho, acc_sph, acc_grav, ws, ws_bytes, stream);
 }
 
 int sph_step_h(float* posm, float* vele, float* hsml, int64_t n_gas, int64_t n_halo, const sph_params* p,
@@ -448,7 +503,7 @@ int sph_density_h(const float* posm, const float* hsml, int64_t n_gas, const sph
     if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
-    SPHB_TRY(gather_sorted_h(hsml, perm, n_gas, w.h_s, st));
+    SPHB_TRY(gather_sorted_h(hsml, perm, n_gas, p->h, w.status, w.h_s, st));
     Span sp(ST_DENSITY, st);
     return density_sorted(w.posm_s, w.h_s, perm, cell_start, n_gas, p, g, rho, st);
 }
@@ -467,10 +522,10 @@ int sph_forces_h(const float* posm, const float* vele, const float* rho, const f
     if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
-    SPHB_TRY(gather_sorted_h(hsml, perm, n_gas, w.h_s, st));
+    SPHB_TRY(gather_sorted_h(hsml, perm, n_gas, p->h, w.status, w.h_s, st));
     Span sp(ST_FORCES, st);
     return forces_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, w.h_s, perm, cell_start, n_gas, p, g, nullptr,
-                         w.velr_s, w.pc_s, reinterpret_cast<float4*>(acc_sph), st);
+                         nullptr, w.velr_s, w.pc_s, reinterpret_cast<float4*>(acc_sph), st);
 }
 
 }  // extern "C"

@@ -68,6 +68,17 @@ struct DenseList {
 };
 inline size_t dense_capacity(int64_t n_gas) { return (size_t)(n_gas / kDenseMin + n_gas / kDenseTT + 16); }
 
+// ---- Eq. 17 gathered inside the HFC neighbour walk (L125-129) ---------------------------------
+// With a CflArgs the forces kernels also reduce, per gas particle, s^min, c^max and mu^max over the accepted pairs, form
+// the bracket of Eq. 17 and take its minimum (x c_cfl) into *dt_bits by integer atomicMin on the float's bit pattern.
+struct CflArgs {
+    float c_cfl;
+    const float4* q_sph;      // (a_sph, de/dt) by original index for |Q_i|, |E_i|, or NULL: the sums this very walk computes
+    const float4* acc_grav;   // a_grav by original index
+    float* dt_particle;       // [n_gas] bracket per particle (without c_cfl), or NULL
+    unsigned int* dt_bits;    // the running minimum (float bits; positive floats order like unsigned integers)
+};
+
 // ---- workspace layout (device scratch carved from the caller's ws) -------------------------
 struct Workspace {
     // grid sort
@@ -84,6 +95,7 @@ struct Workspace {
     float2* pc_s;          // [n_gas] (p/rho^2, c)
     float* h_s;            // [n_gas] per-particle smoothing lengths in cell order (NEXT-2)
     DenseList dense;       // work list of the densely populated cells
+    unsigned int* status;  // 256-byte block; word 0: SPH_STATUS_* bits raised by kernels (sph_workspace_status)
     // gravity
     float4* src_pk;        // [n_pad] packed source pairs
     float4* grav_part;     // [S][n_total] partial accelerations
@@ -117,13 +129,13 @@ int density_sorted(const float4* posm_s, const float* h_s, const uint32_t* perm,
 // by the thread-per-slot kernel)
 int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const float* h_s, const uint32_t* perm,
                   const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
-                  const DenseList* dense, float4* velr_s, float2* pc_s, float4* acc_sph, cudaStream_t st);
+                  const DenseList* dense, const CflArgs* cfl /*or NULL*/, float4* velr_s, float2* pc_s,
+                  float4* acc_sph /*or NULL with cfl: only the step criterion is wanted*/, cudaStream_t st);
+int cfl_init(float* dt_dev, float dt_max, cudaStream_t st);   // *dt_dev = dt_max (+inf: no ceiling)
 int smoothing_lengths(const float4* posm, const float* rho, int64_t n_gas, float sigma, float h_max, float* hsml,
                       cudaStream_t st);
-int gather_sorted_h(const float* hsml, const uint32_t* perm, int64_t n_gas, float* h_s, cudaStream_t st);
-int cfl_sorted(const float4* posm_s, const float4* vele, const float* rho, const float4* acc_sph, const float4* acc_grav,
-               const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
-               float c_cfl, float4* velr_s, float2* pc_s, float* dt_out, float* dt_particle, cudaStream_t st);
+int gather_sorted_h(const float* hsml, const uint32_t* perm, int64_t n_gas, float h_max, unsigned int* status, float* h_s,
+                    cudaStream_t st);
 int gravity_share(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, int rank, int world, bool offer_sym,
                   float G, float delta, float4* acc_grav, float4* src_pk, float4* grav_part, long long* grav_acc64,
                   unsigned int* grav_flag, cudaStream_t st);   // one GPU's share of an evaluation (gravity.cu)
@@ -131,10 +143,11 @@ int gravity_finish(const float4* posm, int64_t n_total, float G, float4* acc_gra
                    const unsigned int* grav_flag, cudaStream_t st);   // after the exchange: sums -> acc_grav, if pair-symmetric
 int gravity(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, float G, float delta, float4* acc_grav,
             float4* src_pk, float4* grav_part, long long* grav_acc64, unsigned int* grav_flag, cudaStream_t st);   // targets [i0, i1) against all sources
+// dt_dev != NULL: the step is read from device memory (the adaptive step of Eq. 17), else it is `dt`
 int update_predictor(float4* posm, float4* vele, float4* vele0, const float4* acc_sph, const float4* acc_grav,
-                     int64_t n_gas, int64_t n_total, float dt, cudaStream_t st);
+                     int64_t n_gas, int64_t n_total, float dt, const float* dt_dev, cudaStream_t st);
 int update_corrector(float4* vele, const float4* vele0, const float4* acc_sph, const float4* acc_grav,
-                     int64_t n_gas, int64_t n_total, float dt, cudaStream_t st);
+                     int64_t n_gas, int64_t n_total, float dt, const float* dt_dev, cudaStream_t st);
 int bbox_gas(const float4* posm, int64_t n_gas, float* bbox_dev /*[8]*/, cudaStream_t st);
 
 }  // namespace sphb

@@ -22,6 +22,7 @@ int ensure_ws(sph_host_ctx* c, size_t need) {
     c->ws = nullptr;
     c->ws_bytes = 0;
     SPHB_CUDA(cudaMalloc(&c->ws, need));
+    SPHB_CUDA(cudaMemset(c->ws, 0, 256));   // the status word of a new workspace starts clear
     c->ws_bytes = need;
     return SPH_OK;
 }

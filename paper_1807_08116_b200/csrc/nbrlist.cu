@@ -125,7 +125,7 @@ extern "C" int sph_neighbour_lists_h(const float* posm, const float* hsml, int64
     SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
     const float* h_s = nullptr;
     if (hsml) {
-        SPHB_TRY(gather_sorted_h(hsml, perm, n_gas, w.h_s, st));
+        SPHB_TRY(gather_sorted_h(hsml, perm, n_gas, h, w.status, w.h_s, st));
         h_s = w.h_s;
     }
     k_nbr<0><<<(unsigned)cdiv(n, 128), 128, 0, st>>>(w.posm_s, perm, cell_start, n, gd, rc2, h_s, nbr_count, nullptr,

@@ -74,10 +74,15 @@ __global__ void __launch_bounds__(128) k_density(const float4* __restrict__ posm
     rho[perm[s]] = sum * norm;
 }
 
-__global__ void __launch_bounds__(256) k_gather_f32(const float* __restrict__ a, const uint32_t* __restrict__ perm, int n,
-                                                    float* __restrict__ a_s) {
+// smoothing lengths into cell order; a length above the cap h_max (which sized the cells: the 3x3x3 stencil would miss
+// neighbours) raises SPH_STATUS_HSML_ABOVE_CAP in the workspace's status word (sph_workspace_status)
+__global__ void __launch_bounds__(256) k_gather_h(const float* __restrict__ a, const uint32_t* __restrict__ perm, int n,
+                                                  float h_max, unsigned int* __restrict__ status, float* __restrict__ a_s) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s < n) a_s[s] = a[perm[s]];
+    if (s >= n) return;
+    const float v = a[perm[s]];
+    a_s[s] = v;
+    if (!(v <= h_max)) atomicOr(status, (unsigned int)SPH_STATUS_HSML_ABOVE_CAP);   // also catches NaN
 }
 
 // L82: h_i = sigma (m_i / rho_i)^(1/3), capped at h_max (reading A25).  cbrtf is within 1 ulp.
@@ -95,16 +100,17 @@ int smoothing_lengths(const float4* posm, const float* rho, int64_t n_gas, float
     return SPH_OK;
 }
 
-int gather_sorted_h(const float* hsml, const uint32_t* perm, int64_t n_gas, float* h_s, cudaStream_t st) {
+int gather_sorted_h(const float* hsml, const uint32_t* perm, int64_t n_gas, float h_max, unsigned int* status, float* h_s,
+                    cudaStream_t st) {
     if (n_gas <= 0) return SPH_OK;
-    k_gather_f32<<<(unsigned)cdiv(n_gas, 256), 256, 0, st>>>(hsml, perm, (int)n_gas, h_s);
+    k_gather_h<<<(unsigned)cdiv(n_gas, 256), 256, 0, st>>>(hsml, perm, (int)n_gas, h_max, status, h_s);
     SPHB_LAUNCHED();
     return SPH_OK;
 }
 
 int forces_dense(const float4* posm_s, const float4* velr_s, const float2* pc_s, const uint32_t* perm,
                  const uint32_t* cell_start, const sph_grid* g, float rc2, const ViscDev& q, const DenseList& dl,
-                 float4* acc_sph, cudaStream_t st);   // sph_dense.cu
+                 const CflArgs* cfl, float4* acc_sph, cudaStream_t st);   // sph_dense.cu
 
 int density_sorted(const float4* posm_s, const float* h_s /*cell order, or NULL: global h*/, const uint32_t* perm,
                    const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g, float* rho,
@@ -157,11 +163,13 @@ struct KSum {
 };
 
 // VARH: as k_density<true> — pair length h_ij = (h_i + h_j)/2 in the cutoff, in grad W_p and in mu_ij (L82, L95-97).
-template <bool VARH>
+// CFL: the per-particle terms of Eq. 17 (s^min, c^max, mu^max) are gathered in the same walk (L125-129) and the bracket is
+// formed at its end (CflArgs, common.cuh).
+template <bool VARH, bool CFL>
 __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_s, const float4* __restrict__ velr_s,
                                                 const float2* __restrict__ pc_s, const float* __restrict__ h_s,
                                                 const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start,
-                                                int n, GridDev g, float rc2, ViscDev q, uint32_t dense_min,
+                                                int n, GridDev g, float rc2, ViscDev q, uint32_t dense_min, CflArgs cfl,
                                                 float4* __restrict__ acc) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
@@ -173,6 +181,7 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
     const float2 ci = pc_s[s];
     const float h_i = VARH ? h_s[s] : 0.f;
     KSum ax, ay, az, de;
+    float d2min = __int_as_float(0x7f800000), cmax = ci.y, mumax = 0.f;   // A22: no neighbour -> s = 2h, c_i, 0
 #pragma unroll 1
     for (int r = 0; r < 9; ++r) {
         uint32_t lo, hi_;
@@ -189,7 +198,7 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
             if (d2 < rc2p && d2 > 0.f) {   // d2 == 0: self, or a coincident pair (A9) — no contribution
                 const float4 vj = velr_s[t];
                 const float2 cj = pc_s[t];
-                float f, rv;
+                float f, rv, mu, c_ij;
                 if (VARH) {
                     float rinv = rsqrtf(d2);
                     rinv = rinv * fmaf(-0.5f * d2 * rinv, rinv, 1.5f);   // one Newton step: ~1 ulp
@@ -205,14 +214,19 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
                     const float dvx = vi.x - vj.x, dvy = vi.y - vj.y, dvz = vi.z - vj.z;
                     rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
                     // mu_ij = h dr.dv / (|dr|^2 + eta h^2) if dr.dv < 0   (L97)
-                    const float mu = rv < 0.f ? (hh * rv) / (d2 + eta_h2) : 0.f;       // IEEE division
-                    const float rho_ij = 0.5f * (vi.w + vj.w), c_ij = 0.5f * (ci.y + cj.y);
+                    mu = rv < 0.f ? (hh * rv) / (d2 + eta_h2) : 0.f;                   // IEEE division
+                    const float rho_ij = 0.5f * (vi.w + vj.w);
+                    c_ij = 0.5f * (ci.y + cj.y);
                     const float nu = (mu * (q.beta * mu - q.alpha * c_ij)) / rho_ij;
                     const float Pi = ci.x + cj.x + nu;                 // p_i/rho_i^2 + p_j/rho_j^2 + nu  (L95, A2)
                     f = pj.w * Pi * gmag;                              // m_j Pi |grad Wp| / |dr|
                 } else {
-                    float mu, c_ij;
                     f = hydro_pair<false>(vi, ci, pj.w, vj, cj, dx, dy, dz, d2, q, rv, mu, c_ij);
+                }
+                if (CFL) {
+                    d2min = fminf(d2min, d2);
+                    cmax = fmaxf(cmax, c_ij);
+                    mumax = fmaxf(mumax, fabsf(mu));
                 }
                 ax.add(-f * dx);
                 ay.add(-f * dy);
@@ -221,12 +235,21 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
             }
         }
     }
-    acc[perm[s]] = make_float4(ax.s, ay.s, az.s, de.s);
+    const uint32_t i = perm[s];
+    const float4 a_own = make_float4(ax.s, ay.s, az.s, de.s);
+    if (acc) acc[i] = a_own;
+    if (CFL) {
+        const float bound = cfl_bracket(d2min, d2min == __int_as_float(0x7f800000), VARH ? 2.0f * h_i : 2.0f * q.h, cmax, mumax,
+                                        q.alpha, q.beta, cfl.q_sph ? cfl.q_sph[i] : a_own, cfl.acc_grav[i]);
+        if (cfl.dt_particle) cfl.dt_particle[i] = bound;
+        cfl_min(cfl.c_cfl * bound, cfl.dt_bits);
+    }
 }
 
 int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const float* h_s /*or NULL*/,
                   const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
-                  const DenseList* dense, float4* velr_s, float2* pc_s, float4* acc_sph, cudaStream_t st) {
+                  const DenseList* dense, const CflArgs* cfl, float4* velr_s, float2* pc_s, float4* acc_sph,
+                  cudaStream_t st) {
     if (n_gas <= 0) return SPH_OK;
     const int n = (int)n_gas;
     k_eos_gather<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(vele, rho, perm, n, p->gamma, velr_s, pc_s);
@@ -245,87 +268,31 @@ int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, co
     q.gw_unit = (float)(-45.0 / (64.0 * 3.14159265358979323846));
     q.inv_h = 1.0f / p->h;
     q.rc2 = two_h * two_h;
-    if (h_s) {
-        k_forces<true><<<(unsigned)cdiv(n, 128), 128, 0, st>>>(posm_s, velr_s, pc_s, h_s, perm, cell_start, n, to_dev(g),
-                                                               two_h * two_h, q, 0u, acc_sph);
-        SPHB_LAUNCHED();
-    } else {
-        k_forces<false><<<(unsigned)cdiv(n, 128), 128, 0, st>>>(posm_s, velr_s, pc_s, nullptr, perm, cell_start, n,
-                                                                to_dev(g), two_h * two_h, q,
-                                                                dense ? (uint32_t)kDenseMin : 0u, acc_sph);
-        SPHB_LAUNCHED();
-        if (dense) SPHB_TRY(forces_dense(posm_s, velr_s, pc_s, perm, cell_start, g, two_h * two_h, q, *dense, acc_sph, st));
-    }
+    const unsigned blocks = (unsigned)cdiv(n, 128);
+    const GridDev gd = to_dev(g);
+    const CflArgs c = cfl ? *cfl : CflArgs{};
+    const uint32_t dmin = (dense && !h_s) ? (uint32_t)kDenseMin : 0u;
+    if (h_s && cfl)
+        k_forces<true, true><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, h_s, perm, cell_start, n, gd, q.rc2, q, 0u, c, acc_sph);
+    else if (h_s)
+        k_forces<true, false><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, h_s, perm, cell_start, n, gd, q.rc2, q, 0u, c, acc_sph);
+    else if (cfl)
+        k_forces<false, true><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, nullptr, perm, cell_start, n, gd, q.rc2, q, dmin, c, acc_sph);
+    else
+        k_forces<false, false><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, nullptr, perm, cell_start, n, gd, q.rc2, q, dmin, c, acc_sph);
+    SPHB_LAUNCHED();
+    if (dmin) SPHB_TRY(forces_dense(posm_s, velr_s, pc_s, perm, cell_start, g, q.rc2, q, *dense, cfl, acc_sph, st));
     return SPH_OK;
 }
 
 // ---------------------------------------------------------------- (NEXT-1) modified CFL step, Eq. 17
-// Per gas particle: s = min |dr|, cmax = max c_ij, mumax = max |mu_ij| over its neighbours (same walk
-// and predicate as k_forces), then the bracket of Eq. 17; the global minimum by atomicMin on the bit
-// pattern (positive floats order like unsigned ints), so it is exact and order-independent.
-__global__ void k_cfl_init(float* dt_out) { *dt_out = __int_as_float(0x7f800000); }
+// The terms of Eq. 17 are gathered by the forces kernels themselves (template flag CFL above, and in sph_dense.cu); the
+// global minimum is an atomicMin on the float bit pattern (positive floats order like unsigned integers), hence exact
+// and order-independent.  This sets its starting value: the ceiling dt_max of the step, +inf for none.
+__global__ void k_cfl_init(float* dt_out, float dt_max) { *dt_out = dt_max; }
 
-__global__ void __launch_bounds__(128) k_cfl(const float4* __restrict__ posm_s, const float4* __restrict__ velr_s,
-                                             const float2* __restrict__ pc_s, const uint32_t* __restrict__ perm,
-                                             const uint32_t* __restrict__ start, const float4* __restrict__ acc_sph,
-                                             const float4* __restrict__ acc_grav, int n, GridDev g, float rc2, float h,
-                                             float eta_h2, float alpha, float beta, float c_cfl,
-                                             float* __restrict__ dt_particle, float* dt_out) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    float bound = __int_as_float(0x7f800000);
-    if (s < n) {
-        const float4 pi = posm_s[s];
-        const float4 vi = velr_s[s];
-        const float ci = pc_s[s].y;
-        int ix, iy, iz;
-        cell_of(pi, g, ix, iy, iz);
-        float d2min = rc2, cmax = ci, mumax = 0.f;   // A22: no neighbour -> s = 2h, c_i, 0
-#pragma unroll 1
-        for (int r = 0; r < 9; ++r) {
-            uint32_t lo, hi;
-            stencil_run(start, g, ix, iy, iz, r, lo, hi);
-            for (uint32_t t = lo; t < hi; ++t) {
-                const float4 pj = posm_s[t];
-                float dx, dy, dz;
-                const float d2 = dist2_f32(pi, pj, dx, dy, dz);
-                if (d2 < rc2 && d2 > 0.f) {
-                    const float4 vj = velr_s[t];
-                    const float rv = fmaf(dz, vi.z - vj.z, fmaf(dy, vi.y - vj.y, dx * (vi.x - vj.x)));
-                    const float mu = rv < 0.f ? (h * rv) / (d2 + eta_h2) : 0.f;   // L97
-                    d2min = fminf(d2min, d2);
-                    cmax = fmaxf(cmax, 0.5f * (ci + pc_s[t].y));
-                    mumax = fmaxf(mumax, fabsf(mu));
-                }
-            }
-        }
-        const uint32_t i = perm[s];
-        const float4 as = acc_sph[i], ag = acc_grav[i];
-        const float qx = as.x + ag.x, qy = as.y + ag.y, qz = as.z + ag.z;
-        const float qe = sqrtf(fmaf(qz, qz, fmaf(qy, qy, qx * qx))) + fabsf(as.w);   // |Q_i| + |E_i|
-        const float sm = d2min < rc2 ? sqrtf(d2min) : 2.0f * h;
-        bound = sm / (fmaf(cmax, 1.0f + 1.2f * alpha, 1.2f * beta * mumax) + sqrtf(sm * qe));
-        if (dt_particle) dt_particle[i] = bound;
-    }
-    float v = c_cfl * bound;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(0xffffffffu, v, o));
-    if ((threadIdx.x & 31) == 0 && v < __int_as_float(0x7f800000))
-        atomicMin(reinterpret_cast<unsigned int*>(dt_out), __float_as_uint(fmaxf(v, 0.f)));
-}
-
-int cfl_sorted(const float4* posm_s, const float4* vele, const float* rho, const float4* acc_sph, const float4* acc_grav,
-               const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
-               float c_cfl, float4* velr_s, float2* pc_s, float* dt_out, float* dt_particle, cudaStream_t st) {
-    k_cfl_init<<<1, 1, 0, st>>>(dt_out);
-    SPHB_LAUNCHED();
-    if (n_gas <= 0) return SPH_OK;
-    const int n = (int)n_gas;
-    k_eos_gather<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(vele, rho, perm, n, p->gamma, velr_s, pc_s);
-    SPHB_LAUNCHED();
-    const float two_h = 2.0f * p->h;
-    k_cfl<<<(unsigned)cdiv(n, 128), 128, 0, st>>>(posm_s, velr_s, pc_s, perm, cell_start, acc_sph, acc_grav, n, to_dev(g),
-                                                  two_h * two_h, p->h, p->eta * p->h * p->h, p->alpha, p->beta, c_cfl,
-                                                  dt_particle, dt_out);
+int cfl_init(float* dt_dev, float dt_max, cudaStream_t st) {
+    k_cfl_init<<<1, 1, 0, st>>>(dt_dev, dt_max);
     SPHB_LAUNCHED();
     return SPH_OK;
 }

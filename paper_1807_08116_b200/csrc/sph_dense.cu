@@ -52,7 +52,8 @@ struct DenseLayout {
     static constexpr int tvel = tpos + kDenseTT * 16;                   // float4 [TT]
     static constexpr int tpc = tvel + kDenseTT * 16;                    // float2 [TT]
     static constexpr int acc = tpc + kDenseTT * 8;                      // double [TT][4]
-    static constexpr int runs = acc + kDenseTT * 8 * 4;                 // uint32 [9][4]
+    static constexpr int cfl = acc + kDenseTT * 8 * 4;                  // float [TT][4]: min d2, c^max, mu^max of Eq. 17, -
+    static constexpr int runs = cfl + kDenseTT * 16;                    // uint32 [9][4]
     static constexpr int hist = runs + 9 * 4 * 4;                       // uint32 [rounds][warps][bins]
     static constexpr int bstart = hist + kRounds * kDenseWarps * kBins * 4;   // uint32 [32]: start of bin b in the sorted chunk
     static constexpr int box = bstart + 32 * 4;                         // float [bins][8]: xl, xh, yl, yh, zl, zh, -, -
@@ -60,14 +61,17 @@ struct DenseLayout {
     static constexpr int queue = tab + kDenseWarps * 4 * 8;             // uint32 [warps][kQueue]
     static constexpr int bar = queue + kDenseWarps * kQueue * 4;        // uint64
     static constexpr int item = bar + 8;                                // uint32: the work item the CTA has drawn
+    static constexpr int tnext = bar + 12;                              // uint32: next target of the chunk to hand to a warp
     static constexpr int bytes = bar + 16;
 };
 static_assert((DenseLayout::bytes + 1024) * kDenseCtasPerSm <= 227 * 1024, "shared memory per SM");
 
+// CFL: the terms of Eq. 17 (s^min, c^max, mu^max; L125-129) are reduced in the same walk, as in k_forces (sph.cu).
+template <bool CFL>
 __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
     k_dense_forces(const float4* __restrict__ posm_s, const float4* __restrict__ velr_s, const float2* __restrict__ pc_s,
             const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start, GridDev g, float cell, float rc2,
-            ViscDev q, unsigned int* __restrict__ ctl, const DenseItem* __restrict__ items,
+            ViscDev q, CflArgs cfl, unsigned int* __restrict__ ctl, const DenseItem* __restrict__ items,
             float4* __restrict__ acc_out) {
     using L = DenseLayout;
     extern __shared__ __align__(128) unsigned char smem[];
@@ -81,12 +85,14 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
     float4* t_vel = reinterpret_cast<float4*>(smem + L::tvel);
     float2* t_pc = reinterpret_cast<float2*>(smem + L::tpc);
     double* s_acc = reinterpret_cast<double*>(smem + L::acc);
+    float4* s_cfl = reinterpret_cast<float4*>(smem + L::cfl);
     uint32_t* s_runs = reinterpret_cast<uint32_t*>(smem + L::runs);
     uint32_t* s_hist = reinterpret_cast<uint32_t*>(smem + L::hist);
     uint32_t* s_bstart = reinterpret_cast<uint32_t*>(smem + L::bstart);
     float4* s_box = reinterpret_cast<float4*>(smem + L::box);
     uint64_t* s_bar = reinterpret_cast<uint64_t*>(smem + L::bar);
     uint32_t* s_item = reinterpret_cast<uint32_t*>(smem + L::item);
+    uint32_t* s_tnext = reinterpret_cast<uint32_t*>(smem + L::tnext);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned lt_mask = (1u << lane) - 1u;
@@ -162,9 +168,11 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
         for (uint32_t t = tid; t < nt; t += kDenseThreads) {
             t_pos[t] = posm_s[ts + t];
             t_vel[t] = velr_s[ts + t];
-            t_pc[t] = pc_s[ts + t];
+            const float2 pc = pc_s[ts + t];
+            t_pc[t] = pc;
 #pragma unroll
             for (int c = 0; c < 4; ++c) s_acc[4 * t + c] = 0.0;
+            if (CFL) s_cfl[t] = make_float4(__int_as_float(0x7f800000), pc.y, 0.f, 0.f);   // A22: no neighbour -> c_i, 0
         }
         __syncthreads();
 
@@ -221,6 +229,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                     if (lane >= o) inc += v;
                 }
                 s_bstart[lane] = inc - run;   // lanes >= kBins: ncand
+                if (lane == 0) *s_tnext = 0u;
             }
             if (tid >= 32 && tid < 32 + kBins) {
                 // (warp 1, after the barrier above: no warp still reads the previous chunk's boxes)
@@ -266,7 +275,14 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
             const float4 bx1 = lane < kBins ? s_box[2 * lane + 1] : make_float4(big, big, 0.f, 0.f);
             const uint32_t bs0 = s_bstart[lane];                                   // lane b: slots [bs0, bs0 + blen) of the
             const uint32_t blen = lane < kBins ? s_bstart[lane + 1] - bs0 : 0u;    // sorted chunk hold bin b
-            for (uint32_t t = warp; t < nt; t += kDenseWarps) {
+            // targets are handed to the warps one at a time from a counter: their work differs (position in the cell, the
+            // chunk's population), and the CTA waits for its slowest warp at the end of every chunk.  Which warp takes a
+            // target does not enter its sum: a target meets the chunks in a fixed order, one warp per chunk.
+            for (;;) {
+                uint32_t t = 0;
+                if (lane == 0) t = atomicAdd(s_tnext, 1u);
+                t = __shfl_sync(0xffffffffu, t, 0);
+                if (t >= nt) break;
                 const float4 pi = lds_f4(a_tpos + 16u * t);
                 // lane b: does the 2h sphere of the target reach the box of bin b?  (a lower bound of the distance)
                 const float ex = fmaxf(fmaxf(bx0.x - pi.x, pi.x - bx0.y), 0.f);
@@ -305,6 +321,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                 const float4 vi = lds_f4(a_tvel + 16u * t);
                 const float2 ci = lds_f2(a_tpc + 8u * t);
                 float ax = 0.f, ay = 0.f, az = 0.f, de = 0.f;
+                float d2min = __int_as_float(0x7f800000), cmax = 0.f, mumax = 0.f;
                 uint32_t qh = 0, qt = 0;   // ring queue of accepted candidates (byte offsets in the float4 arrays): head, tail x4
                 auto pair_term = [&](uint32_t rel) {
                     const float4 pj = lds_f4(a_pos + rel);
@@ -317,6 +334,11 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                     ay = fmaf(-f, dy, ay);
                     az = fmaf(-f, dz, az);
                     de = fmaf(0.5f * f, rv, de);   // 1/2 m_j Pi dv . grad W_p   (Eq. 11)
+                    if (CFL) {
+                        d2min = fminf(d2min, d2);
+                        cmax = fmaxf(cmax, c_ij);
+                        mumax = fmaxf(mumax, fabsf(mu));
+                    }
                 };
                 // one step: 32 flat positions, one per lane; `in` is false only for the lanes past the end in the last step
                 auto step = [&](uint32_t v16, bool in) {
@@ -362,6 +384,16 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                     k += __shfl_xor_sync(0xffffffffu, k, 2);
                     k += __shfl_xor_sync(0xffffffffu, k, 1);
                     if ((lane & 7) == 0) s_acc[4 * t + (lane >> 3)] += k;
+                    if (CFL) {   // non-negative floats order like their bit patterns
+                        const uint32_t m0 = __reduce_min_sync(0xffffffffu, __float_as_uint(d2min));
+                        const uint32_t m1 = __reduce_max_sync(0xffffffffu, __float_as_uint(cmax));
+                        const uint32_t m2 = __reduce_max_sync(0xffffffffu, __float_as_uint(mumax));
+                        if (lane == 0) {
+                            const float4 o = s_cfl[t];
+                            s_cfl[t] = make_float4(fminf(o.x, __uint_as_float(m0)), fmaxf(o.y, __uint_as_float(m1)),
+                                                   fmaxf(o.z, __uint_as_float(m2)), 0.f);
+                        }
+                    }
                 }
             }
             r = rn;
@@ -372,8 +404,17 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
         __syncthreads();
 
         for (uint32_t t = tid; t < nt; t += kDenseThreads) {
-            acc_out[perm[ts + t]] = make_float4((float)s_acc[4 * t], (float)s_acc[4 * t + 1], (float)s_acc[4 * t + 2],
-                                                (float)s_acc[4 * t + 3]);
+            const uint32_t i = perm[ts + t];
+            const float4 a_own = make_float4((float)s_acc[4 * t], (float)s_acc[4 * t + 1], (float)s_acc[4 * t + 2],
+                                             (float)s_acc[4 * t + 3]);
+            if (acc_out) acc_out[i] = a_own;
+            if (CFL) {
+                const float4 c = s_cfl[t];
+                const float bound = cfl_bracket(c.x, c.x == __int_as_float(0x7f800000), 2.0f * q.h, c.y, c.z, q.alpha, q.beta,
+                                                cfl.q_sph ? cfl.q_sph[i] : a_own, cfl.acc_grav[i]);
+                if (cfl.dt_particle) cfl.dt_particle[i] = bound;
+                cfl_min(cfl.c_cfl * bound, cfl.dt_bits);
+            }
         }
     }
 }
@@ -399,20 +440,25 @@ int dense_list_from_start(const uint32_t* cell_start, const sph_grid* g, const D
 
 int forces_dense(const float4* posm_s, const float4* velr_s, const float2* pc_s, const uint32_t* perm,
                  const uint32_t* cell_start, const sph_grid* g, float rc2, const ViscDev& q, const DenseList& dl,
-                 float4* acc_sph, cudaStream_t st) {
+                 const CflArgs* cfl, float4* acc_sph, cudaStream_t st) {
     int dev = 0;
     SPHB_CUDA(cudaGetDevice(&dev));
     static std::atomic<bool> opted[64];   // per device: the dynamic shared-memory opt-in
     if (dev < 0 || dev >= 64) return SPH_ERR_UNSUPPORTED;
     if (!opted[dev].load(std::memory_order_acquire)) {
-        SPHB_CUDA(cudaFuncSetAttribute(k_dense_forces, cudaFuncAttributeMaxDynamicSharedMemorySize, DenseLayout::bytes));
+        SPHB_CUDA(cudaFuncSetAttribute(k_dense_forces<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DenseLayout::bytes));
+        SPHB_CUDA(cudaFuncSetAttribute(k_dense_forces<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DenseLayout::bytes));
         opted[dev].store(true, std::memory_order_release);
     }
     // the faces of the cells follow the rule the keys are made with (A7: c = (x - origin) * inv_cell), so the cell
     // edge is taken from inv_cell, not from g->cell
     SPHB_CUDA(cudaMemsetAsync(dl.ctl + 1, 0, sizeof(unsigned int), st));   // the item counter
-    k_dense_forces<<<kDenseCtasPerSm * num_sms(), kDenseThreads, DenseLayout::bytes, st>>>(
-        posm_s, velr_s, pc_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, rc2, q, dl.ctl, dl.items, acc_sph);
+    if (cfl)
+        k_dense_forces<true><<<kDenseCtasPerSm * num_sms(), kDenseThreads, DenseLayout::bytes, st>>>(
+            posm_s, velr_s, pc_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, rc2, q, *cfl, dl.ctl, dl.items, acc_sph);
+    else
+        k_dense_forces<false><<<kDenseCtasPerSm * num_sms(), kDenseThreads, DenseLayout::bytes, st>>>(
+            posm_s, velr_s, pc_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, rc2, q, CflArgs{}, dl.ctl, dl.items, acc_sph);
     SPHB_LAUNCHED();
     return SPH_OK;
 }

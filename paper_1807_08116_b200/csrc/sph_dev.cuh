@@ -94,6 +94,23 @@ __device__ __forceinline__ float hydro_pair(const float4 vi /*v, rho*/, const fl
     return m_j * Pi * gmag;                              // m_j Pi |grad Wp| / |dr|
 }
 
+// Eq. 17 (L127) for one gas particle: the bracket s / (c^max (1 + 1.2 alpha) + 1.2 beta mu^max + sqrt(s (|Q| + |E|))) from
+// the squared minimum distance (>= rc2_none: no neighbour, then s = s_none, reading A22), c^max, mu^max and the
+// particle's right-hand sides Q = a_sph + a_grav (Eq. 10), E = de/dt (Eq. 11).
+__device__ __forceinline__ float cfl_bracket(float d2min, bool none, float s_none, float cmax, float mumax, float alpha,
+                                             float beta, const float4 as, const float4 ag) {
+    const float qx = as.x + ag.x, qy = as.y + ag.y, qz = as.z + ag.z;
+    const float qe = sqrtf(fmaf(qz, qz, fmaf(qy, qy, qx * qx))) + fabsf(as.w);   // |Q_i| + |E_i|
+    const float sm = none ? s_none : sqrtf(d2min);
+    return sm / (fmaf(cmax, 1.0f + 1.2f * alpha, 1.2f * beta * mumax) + sqrtf(sm * qe));
+}
+// the running minimum of c_cfl x bracket over the active lanes of the warp, then one atomicMin on the bit pattern
+__device__ __forceinline__ void cfl_min(float v, unsigned int* dt_bits) {
+    const unsigned act = __activemask();
+    const unsigned m = __reduce_min_sync(act, __float_as_uint(fmaxf(v, 0.f)));
+    if ((threadIdx.x & 31) == __ffs(act) - 1) atomicMin(dt_bits, m);
+}
+
 // ---- dense-cell work list (common.cuh: DenseItem, DenseList) ------------------------------------------------------
 __device__ __forceinline__ void dense_append(uint32_t key, uint32_t count, unsigned int* ctl, DenseItem* items) {
     const uint32_t nchunk = (count + kDenseTT - 1) / kDenseTT;

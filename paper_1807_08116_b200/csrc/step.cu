@@ -30,6 +30,7 @@ Workspace carve(void* base, int64_t n_gas, int64_t n_total, const sph_grid* g) {
     };
     const int64_t M = (g && n_gas > 0) ? grid_cells(g) : 0;
     const size_t ng = (size_t)(n_gas > 0 ? n_gas : 0), nt = (size_t)(n_total > 0 ? n_total : 0);
+    w.status = (unsigned int*)take(256);   // offset 0: the one block a caller zeroes in a new workspace
     w.bbox = (float*)take(8 * sizeof(float));
     w.key = (uint32_t*)take(ng * 4);
     w.rank_u = (uint32_t*)take(ng * 4);
@@ -59,9 +60,11 @@ Workspace carve(void* base, int64_t n_gas, int64_t n_total, const sph_grid* g) {
 // Q = a_sph + a_grav for gas, a_grav for halo (Eq. 10); E = de/dt (Eq. 11).  v(t), e(t) are saved.
 __global__ void __launch_bounds__(256) k_update_pred(float4* __restrict__ posm, float4* __restrict__ vele,
                                                      float4* __restrict__ vele0, const float4* __restrict__ acc_sph,
-                                                     const float4* __restrict__ acc_grav, int n_gas, int n, float dt) {
+                                                     const float4* __restrict__ acc_grav, int n_gas, int n, float dt_arg,
+                                                     const float* __restrict__ dt_dev) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    const float dt = dt_dev ? *dt_dev : dt_arg;
     float4 r = posm[i];
     const float4 v = vele[i];
     float4 q = acc_grav[i];
@@ -90,9 +93,11 @@ __global__ void __launch_bounds__(256) k_update_pred(float4* __restrict__ posm, 
 // Corrector, Eqs. 15-16:  v = (v(t) + v~)/2 + dt/2 Q~ ; e = (e(t) + e~)/2 + dt/2 E~.
 __global__ void __launch_bounds__(256) k_update_corr(float4* __restrict__ vele, const float4* __restrict__ vele0,
                                                      const float4* __restrict__ acc_sph,
-                                                     const float4* __restrict__ acc_grav, int n_gas, int n, float dt) {
+                                                     const float4* __restrict__ acc_grav, int n_gas, int n, float dt_arg,
+                                                     const float* __restrict__ dt_dev) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    const float dt = dt_dev ? *dt_dev : dt_arg;
     const float4 vt = vele[i], v0 = vele0[i];
     float4 q = acc_grav[i];
     float e_rate = 0.f;
@@ -113,19 +118,19 @@ __global__ void __launch_bounds__(256) k_update_corr(float4* __restrict__ vele, 
 }
 
 int update_predictor(float4* posm, float4* vele, float4* vele0, const float4* acc_sph, const float4* acc_grav,
-                     int64_t n_gas, int64_t n_total, float dt, cudaStream_t st) {
+                     int64_t n_gas, int64_t n_total, float dt, const float* dt_dev, cudaStream_t st) {
     if (n_total <= 0) return SPH_OK;
     k_update_pred<<<(unsigned)cdiv(n_total, 256), 256, 0, st>>>(posm, vele, vele0, acc_sph, acc_grav, (int)n_gas,
-                                                               (int)n_total, dt);
+                                                               (int)n_total, dt, dt_dev);
     SPHB_LAUNCHED();
     return SPH_OK;
 }
 
 int update_corrector(float4* vele, const float4* vele0, const float4* acc_sph, const float4* acc_grav, int64_t n_gas,
-                     int64_t n_total, float dt, cudaStream_t st) {
+                     int64_t n_total, float dt, const float* dt_dev, cudaStream_t st) {
     if (n_total <= 0) return SPH_OK;
     k_update_corr<<<(unsigned)cdiv(n_total, 256), 256, 0, st>>>(vele, vele0, acc_sph, acc_grav, (int)n_gas, (int)n_total,
-                                                               dt);
+                                                               dt, dt_dev);
     SPHB_LAUNCHED();
     return SPH_OK;
 }

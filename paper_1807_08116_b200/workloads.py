@@ -161,6 +161,8 @@ CONFIGS = {
     # not a BASELINE.json config: SURVEY §8(f) NEXT-3, the collisionless mode (N_g = 0; SP, DC, HFC skipped,
     # PAPER.md L150) at N = 2^22, inside the paper's range of N (L213); same halo profile and orbits as config 2
     5: dict(kind="collision", n_gas=0, n_halo=2 ** 22, h=0.05, delta=0.001, dt=1e-4, steps=5, seed=6),
+    # the same at N = 2^23, the top of the paper's range (L213)
+    6: dict(kind="collision", n_gas=0, n_halo=2 ** 23, h=0.05, delta=0.001, dt=1e-4, steps=2, seed=7),
 }
 
 

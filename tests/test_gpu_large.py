@@ -197,3 +197,19 @@ def test_full_size_collisionless_next3(cuda_lib):
     assert np.abs(p1[:, :3] - r1).max() <= 2e-6 * max(1.0, np.abs(r1).max())
     check_values(v1[:, :3], v0 + 0.5 * dt * (a0 + a1), "v(t+dt) cfg5 all", max_tol=2e-6, med_tol=2e-7)
     check_values(a1[h_idx], oracle.gravity(p1, w.G, w.delta, targets=h_idx), "a_grav(t+dt) cfg5 subset")
+
+
+def test_full_size_collisionless_2p23(cuda_lib):
+    """SURVEY §8(f) NEXT-3 at the top of the paper's range of N (L213): N = 2^23, N_g = 0.  One evaluation of Eq. 4 through
+    the pair-symmetric path (3.5e13 unordered pairs), checked on the seeded subset against the oracle, plus momentum."""
+    b = cuda_lib
+    w = wl.make_workload(6)
+    assert w.n_gas == 0 and w.n_total == 2 ** 23
+    _, h_idx = wl.subset_indices(0, w.n_halo, w.seed, n_each=1024)
+    sim = b.Simulation(w)
+    sim.evaluate()
+    assert b.sph_gravity_path(sim.ws, 0, w.n_total) == "pair_symmetric"
+    a = sim.acc_grav.cpu().numpy().astype(np.float64)[:, :3]
+    check_values(a[h_idx], oracle.gravity(w.posm, w.G, w.delta, targets=h_idx), "a_grav cfg6 (N = 2^23) subset")
+    m = w.posm[:, 3].astype(np.float64)
+    assert np.linalg.norm((m[:, None] * a).sum(0)) < 5e-7 * (m * np.linalg.norm(a, axis=1)).sum()

@@ -121,6 +121,14 @@ def _grid_case(case):
     if case == "ragged_M":
         w = _dense(4099, 6, 0.031)
         return w, None
+    if case == "huge_cell":       # 12000 particles in ONE cell (more than the shared-memory sort of the stable fix-up takes)
+        w = _dense(12000, 9, 0.03)
+        w.h = 3.0
+        return w, None
+    if case == "mixed_cells":     # one cell of 7000 (sorted in shared memory) next to thinly populated ones
+        w = _dense(9000, 10, 0.03)
+        w.posm[:7000, :3] = 0.5 + 0.02 * (w.posm[:7000, :3] - 0.5)
+        return w, None
     # ---- cases for the dense-cell walk (sph_dense.cu: cells of >= 32 particles) ----
     if case == "packed":          # 4^3 cells of ~310: several target chunks per cell, stencil rows longer than one staged chunk
         return _dense(20000, 7, 0.15), None
@@ -152,7 +160,8 @@ def _grid_case(case):
 DENSE_CASES = ("packed", "tight_clumps", "one_cell_sph", "clamped_dense")
 
 
-@pytest.mark.parametrize("case", ["galaxy", "dense", "clumps", "clamped", "one_cell", "ragged_M"])
+@pytest.mark.parametrize("case", ["galaxy", "dense", "clumps", "clamped", "one_cell", "ragged_M", "huge_cell", "mixed_cells",
+                                  "tight_clumps", "clamped_dense"])
 def test_grid_sort_bit_exact(cuda_lib, case):
     b = cuda_lib
     w, og = _grid_case(case)
@@ -200,8 +209,13 @@ def test_grid_sort_bit_exact(cuda_lib, case):
             assert tuple(runs[i, rr]) == want
     # deterministic
     perm2 = torch.zeros_like(perm)
+    b.sph_set_profiling(True)
     b.sph_build_grid(d, n, g, key, perm2, count, start, ws)
+    sort_ms = b.sph_get_stage_ms()["sort"]
+    b.sph_set_profiling(False)
     assert torch.equal(perm, perm2)
+    if case in ("huge_cell", "mixed_cells", "one_cell"):
+        assert sort_ms < 1.0, sort_ms      # a cell of 10^4 does not make the stable fix-up quadratic in wall time
 
 
 # ---------------------------------------------------------------- neighbour sets, density, forces
@@ -300,7 +314,7 @@ def test_forces_parity_oracle_own_density(cuda_lib, case):
     check_values(got[:, 3], of[:, 3], f"de/dt {case}, oracle's own rho", gross=gross[:, 1], extra_abs=2 * eps * gross[:, 1])
 
 
-@pytest.mark.parametrize("case", ["galaxy", "dense", "clumps"])
+@pytest.mark.parametrize("case", ["galaxy", "dense", "clumps", "packed", "tight_clumps"])
 def test_cfl_step_parity(cuda_lib, case):
     """NEXT-1, Eq. 17 (L125-129): per-particle bracket and the global minimum against the oracle.  Both sides
     take the same rho and the same Q, E (the GPU's verified FP32 outputs, widened), so this checks the
@@ -331,6 +345,40 @@ def test_cfl_step_parity(cuda_lib, case):
     # no gas: +inf
     b.sph_cfl_dt(None, None, None, None, None, 0, prm, None, None, None, 0.7, dt, None, ws)
     assert np.isinf(dt.item())
+
+
+@pytest.mark.parametrize("cfg,scale,steps,sigma", [(0, 1.0, 10, None), (0, 0.5, 3, 0.8)])
+def test_adaptive_step_parity(cuda_lib, cfg, scale, steps, sigma):
+    """sph_step_cfl against oracle.step(c_cfl=): the step size comes from Eq. 17 inside HFC(predictor), on the device, free
+    running.  The steps taken are compared one by one, the state at the end at the step-parity tolerances."""
+    b = cuda_lib
+    w = wl.make_workload(cfg, scale=scale)
+    ng = w.n_gas
+    sim = b.Simulation(w, sigma=sigma)
+    st = _oracle_state(w)
+    hs = None if sigma is None else np.full(ng, np.float32(w.h), dtype=np.float64)
+    nbr = oracle.position_only(st, w.h, w.G, w.delta, hs=hs)
+    dt_max = 50 * w.dt            # a ceiling Eq. 17 undercuts
+    t_gpu = t_orc = 0.0
+    for k in range(steps):
+        sim.step(dt=dt_max, c_cfl=0.6)
+        st, nbr, d = oracle.step(st, dt_max, w.h, w.G, w.delta, nbr=nbr, hs=hs, sigma=sigma or 0.0, c_cfl=0.6, gamma=w.gamma,
+                                 alpha=w.alpha, beta=w.beta, eta=w.eta)
+        hs = d["hs"]
+        got = float(sim.dt_used.item())
+        assert got < dt_max and abs(got - d["dt"]) < 2e-5 * d["dt"], (k, got, d["dt"])
+        t_gpu += got
+        t_orc += d["dt"]
+    v = sim.vele.cpu().numpy().astype(np.float64)
+    check_values(v[:, :3], st.vele[:, :3], f"v after {steps} adaptive steps", max_tol=5e-5, med_tol=2e-6)
+    assert np.abs(sim.posm.cpu().numpy()[:, :3] - st.posm[:, :3]).max() < 2e-5
+    check_density(sim.rho.cpu().numpy()[:ng], st.rho, "rho after adaptive steps")
+    # a ceiling below the criterion: the fixed step, bit for bit
+    sim_a, sim_b = b.Simulation(w), b.Simulation(w)
+    sim_a.step(dt=1e-6, c_cfl=0.6)
+    sim_b.step(dt=1e-6)
+    assert float(sim_a.dt_used.item()) == float(np.float32(1e-6))
+    assert torch.equal(sim_a.posm, sim_b.posm) and torch.equal(sim_a.vele, sim_b.vele)
 
 
 def test_coincident_gas_particles(cuda_lib):
@@ -579,6 +627,27 @@ def test_varh_sets_density_forces_parity(cuda_lib, case):
     b.sph_density_h(d, dh_eq, n, prm, g, perm, start, rho_eq, ws)
     b.sph_density(d, n, prm, g, perm, start, rho_g, ws)
     assert (rho_eq - rho_g).abs().max().item() <= 2e-6 * rho_g.max().item()
+
+
+def test_hsml_above_cap_raises_status(cuda_lib):
+    """A smoothing length above the cap that sized the cells would lose neighbours: the status word says so."""
+    b = cuda_lib
+    w = _dense(3000, 12, 0.05)
+    n = w.n_gas
+    d, g, perm, start, ws = _build(b, w)
+    prm = b.sph_params.from_workload(w)
+    rho = torch.zeros(n, device="cuda")
+    hs = torch.full((n,), float(np.float32(w.h)), device="cuda")
+    assert b.sph_workspace_status(ws, n, n, g) == 0
+    b.sph_density_h(d, hs, n, prm, g, perm, start, rho, ws)
+    assert b.sph_workspace_status(ws, n, n, g) == 0                 # h_i = h_max is allowed
+    hs[1234] = float(np.float32(w.h)) * 1.01
+    b.sph_density_h(d, hs, n, prm, g, perm, start, rho, ws)
+    assert b.sph_workspace_status(ws, n, n, g) == b.SPH_STATUS_HSML_ABOVE_CAP
+    assert b.sph_workspace_status(ws, n, n, g) == 0                 # reading clears it
+    hs[1234] = float("nan")
+    b.sph_density_h(d, hs, n, prm, g, perm, start, rho, ws)
+    assert b.sph_workspace_status(ws, n, n, g) == b.SPH_STATUS_HSML_ABOVE_CAP
 
 
 def test_varh_smoothing_lengths_and_step(cuda_lib):
