@@ -364,7 +364,10 @@ def run_ours(args, w):
 
     # ---- end-to-end arm: HOST (pinned) buffers through sph_host_ctx_step, copies inside the timing
     e2e = None
-    if not args.no_e2e:
+    if args.sigma is not None and not use_dist and not args.no_e2e:
+        # the host-buffer entry point steps with one global h: it would time a different algorithm than the arm above
+        e2e = {"value": None, "unit": "ms", "skipped": "sph_host_ctx_step has no per-particle-h variant; --sigma runs carry no end-to-end number"}
+    elif not args.no_e2e:
         hp = torch.from_numpy(w.posm.copy()).pin_memory()
         hv = torch.from_numpy(w.vele.copy()).pin_memory()
         hrho = torch.zeros(max(ng, 1), dtype=torch.float32).pin_memory()

@@ -60,7 +60,7 @@ int position_only(const float4* posm, float* hsml, float sigma, int64_t n_gas, i
         }
         {
             Span sp(ST_DENSITY, st);
-            SPHB_TRY(density_sorted(w.posm_s, hsml ? w.h_s : nullptr, w.perm, w.cell_start, n_gas, p, g, rho, st));
+            SPHB_TRY(density_sorted(w.posm_s, hsml ? w.h_s : nullptr, w.perm, w.cell_start, n_gas, p, g, &w.dense, rho, st));
             if (hsml && sigma > 0.f) {
                 SPHB_TRY(smoothing_lengths(posm, rho, n_gas, sigma, p->h, hsml, st));
                 SPHB_TRY(gather_sorted_h(hsml, w.perm, n_gas, p->h, w.status, w.h_s, st));
@@ -191,8 +191,9 @@ int sph_density(const float* posm, int64_t n_gas, const sph_params* p, const sph
     if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
+    SPHB_TRY(dense_list_from_start(cell_start, g, w.dense, st));
     Span sp(ST_DENSITY, st);
-    return density_sorted(w.posm_s, nullptr, perm, cell_start, n_gas, p, g, rho, st);
+    return density_sorted(w.posm_s, nullptr, perm, cell_start, n_gas, p, g, &w.dense, rho, st);
 }
 
 int sph_forces(const float* posm, const float* vele, const float* rho, int64_t n_gas, const sph_params* p,
@@ -505,7 +506,7 @@ int sph_density_h(const float* posm, const float* hsml, int64_t n_gas, const sph
     SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
     SPHB_TRY(gather_sorted_h(hsml, perm, n_gas, p->h, w.status, w.h_s, st));
     Span sp(ST_DENSITY, st);
-    return density_sorted(w.posm_s, w.h_s, perm, cell_start, n_gas, p, g, rho, st);
+    return density_sorted(w.posm_s, w.h_s, perm, cell_start, n_gas, p, g, nullptr, rho, st);
 }
 
 int sph_forces_h(const float* posm, const float* vele, const float* rho, const float* hsml, int64_t n_gas,

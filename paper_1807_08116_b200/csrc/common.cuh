@@ -123,10 +123,11 @@ int grid_build(const float4* posm, int64_t n_gas, const sph_grid* g, uint32_t* k
 int dense_list_from_start(const uint32_t* cell_start, const sph_grid* g, const DenseList& dl, cudaStream_t st);
 int gather_sorted_pos(const float4* posm, const uint32_t* perm, int64_t n_gas, float4* posm_s, cudaStream_t st);
 // h_s: per-particle smoothing lengths in cell order (NEXT-2), or NULL for the one global p->h
-int density_sorted(const float4* posm_s, const float* h_s, const uint32_t* perm, const uint32_t* cell_start,
-                   int64_t n_gas, const sph_params* p, const sph_grid* g, float* rho, cudaStream_t st);
 // dense: the work list of the densely populated cells, matching cell_start (global h only; NULL: every slot is walked
 // by the thread-per-slot kernel)
+int density_sorted(const float4* posm_s, const float* h_s, const uint32_t* perm, const uint32_t* cell_start,
+                   int64_t n_gas, const sph_params* p, const sph_grid* g, const DenseList* dense, float* rho,
+                   cudaStream_t st);
 int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const float* h_s, const uint32_t* perm,
                   const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
                   const DenseList* dense, const CflArgs* cfl /*or NULL*/, float4* velr_s, float2* pc_s,

@@ -42,13 +42,14 @@ template <bool VARH>
 __global__ void __launch_bounds__(128) k_density(const float4* __restrict__ posm_s, const float* __restrict__ h_s,
                                                  const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start,
                                                  int n, GridDev g, float rc2, float inv_h, float norm,
-                                                 float* __restrict__ rho) {
+                                                 uint32_t dense_min, float* __restrict__ rho) {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
     const float4 pi = posm_s[s];
     const float h_i = VARH ? h_s[s] : 0.f;
     int ix, iy, iz;
     cell_of(pi, g, ix, iy, iz);
+    if (own_cell_is_dense(start, g, ix, iy, iz, dense_min)) return;   // sph_dense_rho.cu walks that cell
     float sum = 0.f;   // includes the self term m_i W(0): j = i passes the predicate with d2 = 0 (A5)
 #pragma unroll 1
     for (int r = 0; r < 9; ++r) {
@@ -66,8 +67,8 @@ __global__ void __launch_bounds__(128) k_density(const float4* __restrict__ posm
                     sum = fmaf(pj.w, w_spline_unnorm(xi) * (inv * inv * inv), sum);
                 }
             } else if (d2 < rc2) {
-                const float xi = sqrtf(d2) * inv_h;
-                sum = fmaf(pj.w, w_spline_unnorm(xi), sum);
+                // the density is a sum of positive terms held to 1e-5: MUFU.SQRT (2^-23) and the branch-free form of W
+                sum = fmaf(pj.w, w_two_cubes(sqrt_approx(d2), -inv_h), sum);
             }
         }
     }
@@ -112,9 +113,12 @@ int forces_dense(const float4* posm_s, const float4* velr_s, const float2* pc_s,
                  const uint32_t* cell_start, const sph_grid* g, float rc2, const ViscDev& q, const DenseList& dl,
                  const CflArgs* cfl, float4* acc_sph, cudaStream_t st);   // sph_dense.cu
 
+int density_dense(const float4* posm_s, const uint32_t* perm, const uint32_t* cell_start, const sph_params* p,
+                  const sph_grid* g, const DenseList& dl, float* rho, cudaStream_t st);   // sph_dense_rho.cu
+
 int density_sorted(const float4* posm_s, const float* h_s /*cell order, or NULL: global h*/, const uint32_t* perm,
-                   const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g, float* rho,
-                   cudaStream_t st) {
+                   const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
+                   const DenseList* dense, float* rho, cudaStream_t st) {
     if (n_gas <= 0) return SPH_OK;
     const float two_h = 2.0f * p->h;
     const float rc2 = two_h * two_h;
@@ -122,13 +126,15 @@ int density_sorted(const float4* posm_s, const float* h_s /*cell order, or NULL:
     const unsigned blocks = (unsigned)cdiv(n_gas, 128);
     if (h_s) {
         k_density<true><<<blocks, 128, 0, st>>>(posm_s, h_s, perm, cell_start, (int)n_gas, to_dev(g), rc2, inv_h,
-                                                (float)(1.0 / 3.14159265358979323846), rho);
+                                                (float)(1.0 / 3.14159265358979323846), 0u, rho);
+        SPHB_LAUNCHED();
     } else {
         const float norm = (float)(1.0 / (3.14159265358979323846 * (double)p->h * (double)p->h * (double)p->h));
         k_density<false><<<blocks, 128, 0, st>>>(posm_s, nullptr, perm, cell_start, (int)n_gas, to_dev(g), rc2, inv_h,
-                                                 norm, rho);
+                                                 norm, dense ? (uint32_t)kDenseMin : 0u, rho);
+        SPHB_LAUNCHED();
+        if (dense) SPHB_TRY(density_dense(posm_s, perm, cell_start, p, g, *dense, rho, st));
     }
-    SPHB_LAUNCHED();
     return SPH_OK;
 }
 

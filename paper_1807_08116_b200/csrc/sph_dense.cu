@@ -24,8 +24,7 @@
 // calls — and are drawn from a counter by a persistent grid (kDenseCtasPerSm CTAs per SM).
 // The density pass (a7) stays on the thread-per-slot walk everywhere: its pair term is ~15 instructions, so nothing is
 // won by compacting the accepted pairs, and the staged, binned walk measured slower (46 against 31 ms at config 4).
-#include "sph_dev.cuh"
-#include "tma_dev.cuh"
+#include "sph_dense_dev.cuh"
 
 namespace sphb {
 
@@ -37,7 +36,7 @@ constexpr int kDenseCtasPerSm = 2;
 constexpr int kDenseK = 1152;             // candidate slots per staged chunk
 constexpr int kDenseKS = kDenseK + 2;     // + the even-slot alignment of the float2 array at either end
 constexpr int kRounds = (kDenseK + kDenseThreads - 1) / kDenseThreads;
-constexpr int kBins = 24;                 // (sz, sy) sub-row x (cell of the row, sx): bin = (2 sz + sy) 6 + 2 c + sx
+using dense::kBins;
 constexpr int kQueue = 64;                // ring queue entries per warp
 
 struct DenseLayout {
@@ -132,8 +131,6 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
         }
     };
 
-    const float eps = cell * 0.00390625f;   // 2^-8 of a cell: covers the rounding of the cell assignment (A7) and of the faces
-    const float half = 0.5f * cell;
     const float big = 3.0e38f;
 
     for (;;) {
@@ -149,22 +146,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
         const int ix = (int)(it.key % mx), iy = (int)((it.key / mx) % my), iz = (int)(it.key / (mx * my));
         const uint32_t ts = start[it.key] + it.chunk * kDenseTT;
         const uint32_t nt = min(start[it.key + 1u] - ts, (uint32_t)kDenseTT);
-        if (tid < 9) {
-            // row r: the cells (ix-1, ix, ix+1) at (iy + r%3 - 1, iz + r/3 - 1); boundaries b0 <= b1 <= b2 <= b3
-            const int cy = iy + (tid % 3) - 1, cz = iz + (tid / 3) - 1;
-            uint32_t b0 = 0, b1 = 0, b2 = 0, b3 = 0;
-            if (cy >= 0 && cy < g.my && cz >= 0 && cz < g.mz) {
-                const uint32_t row = mx * ((uint32_t)cy + my * (uint32_t)cz);
-                b1 = start[row + (uint32_t)ix];
-                b2 = start[row + (uint32_t)ix + 1u];
-                b0 = ix > 0 ? start[row + (uint32_t)ix - 1u] : b1;
-                b3 = ix + 1 < g.mx ? start[row + (uint32_t)ix + 2u] : b2;
-            }
-            s_runs[4 * tid] = b0;
-            s_runs[4 * tid + 1] = b1;
-            s_runs[4 * tid + 2] = b2;
-            s_runs[4 * tid + 3] = b3;
-        }
+        if (tid < 9) dense::row_bounds(start, g, ix, iy, iz, tid, s_runs);
         for (uint32_t t = tid; t < nt; t += kDenseThreads) {
             t_pos[t] = posm_s[ts + t];
             t_vel[t] = velr_s[ts + t];
@@ -184,85 +166,21 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
             const uint32_t ce = min(cs + kDenseK, s_runs[4 * r + 3]);
             const uint32_t ncand = ce - cs, roff = cs & 1u;   // candidates of this chunk; raw index of slot cs
             const uint32_t b1 = s_runs[4 * r + 1], b2 = s_runs[4 * r + 2];
-            const int cy = iy + (r % 3) - 1, cz = iz + (r / 3) - 1;
-            // mid-planes of the three cells of the row, and of the row itself
-            const float xm0 = fmaf((float)(ix - 1) + 0.5f, cell, g.ox), xm1 = xm0 + cell, xm2 = xm1 + cell;
-            const float ym = fmaf((float)cy + 0.5f, cell, g.oy), zm = fmaf((float)cz + 0.5f, cell, g.oz);
-
-            // ---- counting sort of the chunk by bin, stable (slot order inside a bin): raw -> sorted ----
-            for (int i = tid; i < kRounds * kDenseWarps * kBins; i += kDenseThreads) s_hist[i] = 0u;
-            mbar_wait(s_bar, n_staged & 1u);
-            ++n_staged;
-            __syncthreads();   // histogram zeroed; every warp is past the previous chunk's candidates
-            uint32_t my_bin[kRounds], my_rank[kRounds];
-#pragma unroll
-            for (int rd = 0; rd < kRounds; ++rd) {
-                const uint32_t i = (uint32_t)(rd * kDenseThreads + tid);
-                uint32_t bin = 31u;   // past the end of the chunk
-                if (i < ncand) {
-                    const float4 p = r_pos[roff + i];
-                    const uint32_t slot = cs + i;
-                    const uint32_t c = (slot >= b1 ? 1u : 0u) + (slot >= b2 ? 1u : 0u);
-                    const float xm = c == 0u ? xm0 : (c == 1u ? xm1 : xm2);
-                    bin = ((p.z >= zm ? 2u : 0u) + (p.y >= ym ? 1u : 0u)) * 6u + 2u * c + (p.x >= xm ? 1u : 0u);
-                }
-                const unsigned peers = __match_any_sync(0xffffffffu, bin);
-                my_bin[rd] = bin;
-                my_rank[rd] = __popc(peers & lt_mask);
-                if (bin < (uint32_t)kBins && my_rank[rd] == 0u) s_hist[(rd * kDenseWarps + warp) * kBins + bin] = __popc(peers);
-            }
-            __syncthreads();
-            if (tid < 32) {
-                // lane b: exclusive prefix of bin b over (round, warp), then the bins' starts
-                uint32_t run = 0u;
-                if (lane < kBins) {
-                    for (int j = 0; j < kRounds * kDenseWarps; ++j) {
-                        const uint32_t v = s_hist[j * kBins + lane];
-                        s_hist[j * kBins + lane] = run;
-                        run += v;
-                    }
-                }
-                uint32_t inc = run;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o);
-                    if (lane >= o) inc += v;
-                }
-                s_bstart[lane] = inc - run;   // lanes >= kBins: ncand
-                if (lane == 0) *s_tnext = 0u;
-            }
-            if (tid >= 32 && tid < 32 + kBins) {
-                // (warp 1, after the barrier above: no warp still reads the previous chunk's boxes)
-                // box of bin b: the octant, pulled out by eps; open-ended on the outside of a boundary cell, where the
-                // particles clamped into the grid sit (A7)
-                const int bb = tid - 32, k = bb % 6, sr = bb / 6, c = k >> 1, sx = k & 1, sy = sr & 1, sz = sr >> 1;
-                const int cx = ix - 1 + c;
-                const float xm = c == 0 ? xm0 : (c == 1 ? xm1 : xm2);
-                float xl = (sx ? xm : xm - half) - eps, xh = (sx ? xm + half : xm) + eps;
-                float yl = (sy ? ym : ym - half) - eps, yh = (sy ? ym + half : ym) + eps;
-                float zl = (sz ? zm : zm - half) - eps, zh = (sz ? zm + half : zm) + eps;
-                if (cx == 0 && !sx) xl = -big;
-                if (cx == g.mx - 1 && sx) xh = big;
-                if (cx < 0 || cx >= g.mx) xl = big;   // no such cell (the row ends here): out of reach, like the lanes >= kBins
-                if (cy <= 0 && !sy) yl = -big;
-                if (cy >= g.my - 1 && sy) yh = big;
-                if (cz <= 0 && !sz) zl = -big;
-                if (cz >= g.mz - 1 && sz) zh = big;
-                s_box[2 * bb] = make_float4(xl, xh, yl, yh);
-                s_box[2 * bb + 1] = make_float4(zl, zh, 0.f, 0.f);
-            }
-            __syncthreads();
-#pragma unroll
-            for (int rd = 0; rd < kRounds; ++rd) {
-                const uint32_t i = (uint32_t)(rd * kDenseThreads + tid);
-                if (i < ncand) {
-                    const uint32_t dst = s_bstart[my_bin[rd]] + s_hist[(rd * kDenseWarps + warp) * kBins + my_bin[rd]] + my_rank[rd];
-                    c_pos[dst] = r_pos[roff + i];
-                    c_vel[dst] = r_vel[roff + i];
-                    c_pc[dst] = r_pc[roff + i];
-                }
-            }
-            __syncthreads();   // the sorted chunk is complete, the landing zone is free
+            const dense::RowGeom rg = dense::row_geom(g, cell, ix, iy, iz, r);
+            // counting sort of the chunk by octant bin, stable: raw -> sorted (sph_dense_dev.cuh)
+            dense::bin_chunk<kDenseThreads, kRounds, false>(
+                r_pos, roff, ncand, cs, b1, b2, g, cell, ix, rg, s_hist, s_bstart, s_box,
+                [&]() {
+                    mbar_wait(s_bar, n_staged & 1u);
+                    ++n_staged;
+                },
+                [&]() { *s_tnext = 0u; },
+                [&](uint32_t src, uint32_t dst) {
+                    c_pos[dst] = r_pos[src];
+                    c_vel[dst] = r_vel[src];
+                    c_pc[dst] = r_pc[src];
+                },
+                [&](uint32_t) {});
 
             int rn = r;
             uint32_t csn = cs;
@@ -289,34 +207,10 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                 const float ey = fmaxf(fmaxf(bx0.z - pi.y, pi.y - bx0.w), 0.f);
                 const float ez = fmaxf(fmaxf(bx1.x - pi.z, pi.z - bx1.y), 0.f);
                 const bool reach_b = fmaf(ez, ez, fmaf(ey, ey, ex * ex)) < rc2;   // lanes >= kBins: their box is out of reach
-                const unsigned reach = __ballot_sync(0xffffffffu, reach_b);
-                // The reachable bins, in bin order, are the target's candidate list: flat position v = 0 .. T-1.  Consecutive
-                // reachable bins are one slot range (a "group").  Along a (sz, sy) sub-row the distance to the 6 x-slabs
-                // falls and rises once, so the reachable bins of a sub-row are consecutive: at most 4 groups.  Each is
-                // described by the flat position where it ends and the offset from a flat position to a slot — both
-                // kept in BYTES of the float4 array (x16), so a candidate's address is one add.
-                uint32_t incl = reach_b ? blen : 0u;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
-                    if (lane >= o) incl += v;
-                }
-                uint32_t T = __shfl_sync(0xffffffffu, incl, 31);
+                // the reachable bins, in bin order, are the target's candidate list: at most four slot ranges
+                const dense::Groups G = dense::candidate_groups(reach_b, bs0, blen, ncand, a_tab);
+                const uint32_t T = G.T;
                 if (T == 0u) continue;
-                const unsigned gstart = reach & ~(reach << 1);                           // first bin of every group
-                const int ng = __popc(gstart);
-                const int e = lane + __ffs(~(reach >> lane)) - 1;                        // (for a first bin) one past the group's last bin
-                const uint32_t gend = __shfl_sync(0xffffffffu, incl, (e - 1) & 31);
-                if (lane < 4 && lane >= ng) sts_u2(a_tab + 8u * lane, 0xffffffffu, 0u);   // no such group
-                if (((gstart >> lane) & 1u) && ng <= 4)
-                    sts_u2(a_tab + 8u * __popc(gstart & lt_mask), 16u * gend, 16u * (bs0 - (incl - blen)));
-                __syncwarp();
-                uint2 g0 = lds_u2(a_tab);
-                const uint2 g1 = lds_u2(a_tab + 8u), g2 = lds_u2(a_tab + 16u), g3 = lds_u2(a_tab + 24u);
-                if (ng > 4) {   // cannot happen for boxes in a row (see above); if it ever does, every slot of the chunk is a candidate
-                    T = ncand;
-                    g0 = make_uint2(0xffffffffu, 0u);
-                }
 
                 const float4 vi = lds_f4(a_tvel + 16u * t);
                 const float2 ci = lds_f2(a_tpc + 8u * t);
@@ -342,11 +236,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                 };
                 // one step: 32 flat positions, one per lane; `in` is false only for the lanes past the end in the last step
                 auto step = [&](uint32_t v16, bool in) {
-                    uint32_t rel = v16 + g3.y;
-                    rel = v16 < g2.x ? v16 + g2.y : rel;
-                    rel = v16 < g1.x ? v16 + g1.y : rel;
-                    rel = v16 < g0.x ? v16 + g0.y : rel;
-                    rel = in ? rel : 0u;
+                    const uint32_t rel = in ? dense::candidate_offset(G, v16) : 0u;
                     float dx, dy, dz;
                     const float d2 = dist2_f32(pi, lds_f4(a_pos + rel), dx, dy, dz);
                     // d2 == 0: self, or a coincident pair (A9) — no contribution

@@ -31,6 +31,21 @@ __device__ __forceinline__ float w_spline_unnorm(float xi) {
     return xi <= 1.0f ? inner : fmaxf(outer, 0.0f);
 }
 
+// The same piecewise cubic as the difference of two cubes,
+//   W pi h^3 = 1/4 (2 - xi)_+^3 - (1 - xi)_+^3      (xi <= 1: 1 - 3/2 xi^2 + 3/4 xi^3; 1 <= xi <= 2: 1/4 (2 - xi)^3),
+// with xi = r / h taken from r and -1/h: no branch, no second polynomial, and no cancellation (for xi <= 1 the result is
+// >= 1/4 of the larger cube).  7 operations against ~10 for the two selected branches.
+__device__ __forceinline__ float w_two_cubes(float r, float neg_inv_h) {
+    const float a = fmaxf(fmaf(r, neg_inv_h, 2.0f), 0.0f);
+    const float c = fmaxf(fmaf(r, neg_inv_h, 1.0f), 0.0f);
+    return fmaf(0.25f * a * a, a, -(c * c * c));
+}
+__device__ __forceinline__ float sqrt_approx(float x) {   // MUFU.SQRT: relative error 2^-23, sqrt(0) = 0
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
 struct ViscDev {
     float h, alpha, beta, eta_h2, gw;   // gw = -45 / (64 pi h^4): grad W_p = gw (2-xi)^2 dr/|dr|
     float inv_h2;                       // 1 / h^2
