@@ -100,8 +100,8 @@ def reduce_max_ms(ms: float, world: int, device: str = "cuda") -> float:
 
 def ncu_traffic(kernel: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed ncu --set full
-    summary profiles/traffic_r01.csv (kernel,n_total,dram_read_bytes,dram_write_bytes); None if absent."""
-    p = os.path.join(ROOT, "profiles", "traffic_r01.csv")
+    summary profiles/traffic_r02.csv (kernel,n_total,dram_read_bytes,dram_write_bytes); None if absent."""
+    p = os.path.join(ROOT, "profiles", "traffic_r02.csv")
     if not os.path.exists(p):
         return None
     for line in open(p):
@@ -431,7 +431,7 @@ def run_ours(args, w):
         lane_peak = 128 * SM_COUNT_B200 * sm_max * 1e6                 # FP32 lane-operations per second
         roofline = {"kernel": kernel, "bound": "alu", "achieved": achieved, "peak": alu_peak_tflops,
                     "unit": "TFLOP/s", "frac": achieved / alu_peak_tflops, "traffic": traffic,
-                    "traffic_note": "DRAM bytes per launch (ncu --set full, profiles/traffic_r01.csv); irrelevant to an ALU-bound kernel",
+                    "traffic_note": "DRAM bytes per launch (ncu --set full, profiles/traffic_r02.csv); irrelevant to an ALU-bound kernel",
                     "peak_source": f"2*128*148*sm_max_mhz ({peak_src} sm_max_mhz={sm_max:.0f}); 20 flops/interaction",
                     "kernel_ms": grav_ms, "launches_per_step": 1, "gravity_path": path,
                     "executed_lane_ops_per_interaction": ops,

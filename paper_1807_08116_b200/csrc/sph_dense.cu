@@ -6,7 +6,9 @@
 // (one cell, <= kDenseTT targets):
 //   * the candidates of each of the 9 stencil rows — ONE contiguous slot range per row, which is what the x-fastest cell
 //     order buys (L160, L203, L207) — are staged in shared memory by TMA bulk copies (cp.async.bulk + mbarrier), in
-//     chunks of kDenseK slots, once for all the item's targets; the copy of the next chunk runs under the work on this one;
+//     chunks of kDenseK slots, once for all the item's targets; a chunk holds a piece of one row or, where the rows are
+//     short, several whole rows (a target's queue of accepted pairs and its partial sums then live across them, and the
+//     per-chunk costs are paid once); the copy of the next chunk runs under the work on this one;
 //   * the CTA re-orders each staged chunk in shared memory by SUB-CELL (a stable counting sort over 24 bins: the
 //     three cells of the row x 2x2x2 octants, x fastest), so that the candidates a target can reach are a few contiguous
 //     ranges: a 2h sphere meets ~84 octants of h^3 against the 27 x 8 = 216 of the whole stencil — 2.6 candidates per
@@ -33,8 +35,9 @@ namespace {
 constexpr int kDenseThreads = 384;
 constexpr int kDenseWarps = kDenseThreads / 32;
 constexpr int kDenseCtasPerSm = 2;
-constexpr int kDenseK = 1152;             // candidate slots per staged chunk
-constexpr int kDenseKS = kDenseK + 2;     // + the even-slot alignment of the float2 array at either end
+constexpr int kDenseK = 1088;             // candidate slots per staged chunk
+constexpr int kMaxSeg = 6;                // pieces of stencil rows ("segments") a chunk may hold
+constexpr int kDenseKS = kDenseK + 2 * kMaxSeg;   // + the even-slot alignment of the float2 array, per segment
 constexpr int kRounds = (kDenseK + kDenseThreads - 1) / kDenseThreads;
 using dense::kBins;
 constexpr int kQueue = 64;                // ring queue entries per warp
@@ -54,11 +57,14 @@ struct DenseLayout {
     static constexpr int cfl = acc + kDenseTT * 8 * 4;                  // float [TT][4]: min d2, c^max, mu^max of Eq. 17, -
     static constexpr int runs = cfl + kDenseTT * 16;                    // uint32 [9][4]
     static constexpr int hist = runs + 9 * 4 * 4;                       // uint32 [rounds][warps][bins]
-    static constexpr int bstart = hist + kRounds * kDenseWarps * kBins * 4;   // uint32 [32]: start of bin b in the sorted chunk
-    static constexpr int box = bstart + 32 * 4;                         // float [bins][8]: xl, xh, yl, yh, zl, zh, -, -
-    static constexpr int tab = box + kBins * 8 * 4;                     // uint2 [warps][4]: a target's candidate groups
+    static constexpr int bstart = hist + kRounds * kDenseWarps * kBins * 4;   // uint32 [seg][32]: start of bin b inside its segment
+    static constexpr int box = bstart + kMaxSeg * 32 * 4;               // float [seg][bins][8]: xl, xh, yl, yh, zl, zh, -, -
+    static constexpr int tab = box + kMaxSeg * kBins * 8 * 4;           // uint2 [warps][4]: a target's candidate groups
     static constexpr int queue = tab + kDenseWarps * 4 * 8;             // uint32 [warps][kQueue]
-    static constexpr int bar = queue + kDenseWarps * kQueue * 4;        // uint64
+    static constexpr int seg = queue + kDenseWarps * kQueue * 4;        // uint4 [2][seg]: (row, first slot, end slot, raw base) of the
+                                                                        // chunk being worked on and of the one being copied
+    static constexpr int nseg = seg + 2 * kMaxSeg * 16;                 // uint32 [2] segments of those chunks, [2] (row, slot) the producer is at
+    static constexpr int bar = nseg + 16;                               // uint64
     static constexpr int item = bar + 8;                                // uint32: the work item the CTA has drawn
     static constexpr int tnext = bar + 12;                              // uint32: next target of the chunk to hand to a warp
     static constexpr int bytes = bar + 16;
@@ -89,6 +95,8 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
     uint32_t* s_hist = reinterpret_cast<uint32_t*>(smem + L::hist);
     uint32_t* s_bstart = reinterpret_cast<uint32_t*>(smem + L::bstart);
     float4* s_box = reinterpret_cast<float4*>(smem + L::box);
+    uint4* s_seg = reinterpret_cast<uint4*>(smem + L::seg);
+    uint32_t* s_nseg = reinterpret_cast<uint32_t*>(smem + L::nseg);
     uint64_t* s_bar = reinterpret_cast<uint64_t*>(smem + L::bar);
     uint32_t* s_item = reinterpret_cast<uint32_t*>(smem + L::item);
     uint32_t* s_tnext = reinterpret_cast<uint32_t*>(smem + L::tnext);
@@ -107,27 +115,42 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     uint32_t n_staged = 0;   // chunks this CTA has waited for so far: the barrier's phase parity
+    uint32_t n_chunk = 0;    // chunks this CTA has described so far: the descriptor set in use is n_chunk & 1
 
-    // stage the slots [cs, ce) of a stencil row: bulk copies need 16-byte alignment, the float2 array gives it on even
-    // slots only, so every array is staged from the even slot at or below cs (raw index = slot - (cs & ~1))
-    auto issue = [&](uint32_t cs, uint32_t ce) {
-        const uint32_t base = cs & ~1u;
-        const uint32_t cnt = (ce - base + 1u) & ~1u;   // <= kDenseKS, even
-        mbar_expect_tx(s_bar, cnt * 40u);
-        bulk_g2s(r_pos, posm_s + base, cnt * 16u, s_bar);
-        bulk_g2s(r_vel, velr_s + base, cnt * 16u, s_bar);
-        bulk_g2s(r_pc, pc_s + base, cnt * 8u, s_bar);
-    };
-    // chunk sequence of an item: rows 0..8 in order, each row [b0, b3) cut into pieces of kDenseK slots
-    auto skip_empty = [&](int& r, uint32_t& cs) {
-        while (r < 9 && s_runs[4 * r] >= s_runs[4 * r + 3]) ++r;
-        if (r < 9) cs = s_runs[4 * r];
-    };
-    auto next_chunk = [&](int& r, uint32_t& cs) {
-        cs += kDenseK;
-        if (cs >= s_runs[4 * r + 3]) {
-            ++r;
-            skip_empty(r, cs);
+    // The producer (thread 0): describe the next chunk of the item — rows in order from (s_nseg[2], s_nseg[3]); a row that
+    // does not fit what is left of the chunk starts a new one unless the chunk is empty (then it is cut) — and start
+    // its bulk copies.  Bulk copies need 16-byte alignment and the float2 array gives it on even slots only, so every
+    // segment is staged from the even slot at or below its first one, at an even raw index.
+    auto produce = [&](uint32_t set) {
+        uint32_t r = s_nseg[2], cs = s_nseg[3], ns = 0, used = 0, raw = 0;
+        while (r < 9u && ns < (uint32_t)kMaxSeg) {
+            const uint32_t left = s_runs[4 * r + 3] - cs;
+            if (left > (uint32_t)kDenseK - used && used > 0u) break;
+            const uint32_t len = min(left, (uint32_t)kDenseK - used);
+            const uint32_t base = cs & ~1u, cnt = (cs + len - base + 1u) & ~1u;
+            s_seg[set * kMaxSeg + ns] = make_uint4(r, cs, cs + len, raw);
+            raw += cnt;
+            used += len;
+            ++ns;
+            cs += len;
+            if (cs >= s_runs[4 * r + 3]) {
+                ++r;
+                while (r < 9u && s_runs[4 * r] >= s_runs[4 * r + 3]) ++r;
+                if (r < 9u) cs = s_runs[4 * r];
+            }
+            if (used == (uint32_t)kDenseK) break;
+        }
+        s_nseg[set] = ns;
+        s_nseg[2] = r;
+        s_nseg[3] = cs;
+        if (ns == 0u) return;
+        mbar_expect_tx(s_bar, raw * 40u);
+        for (uint32_t i = 0; i < ns; ++i) {
+            const uint4 sg = s_seg[set * kMaxSeg + i];
+            const uint32_t base = sg.y & ~1u, cnt = (sg.z - base + 1u) & ~1u;
+            bulk_g2s(r_pos + sg.w, posm_s + base, cnt * 16u, s_bar);
+            bulk_g2s(r_vel + sg.w, velr_s + base, cnt * 16u, s_bar);
+            bulk_g2s(r_pc + sg.w, pc_s + base, cnt * 8u, s_bar);
         }
     };
 
@@ -157,42 +180,48 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
             if (CFL) s_cfl[t] = make_float4(__int_as_float(0x7f800000), pc.y, 0.f, 0.f);   // A22: no neighbour -> c_i, 0
         }
         __syncthreads();
+        if (tid == 0) {
+            uint32_t r = 0;
+            while (r < 9u && s_runs[4 * r] >= s_runs[4 * r + 3]) ++r;
+            s_nseg[2] = r;
+            s_nseg[3] = r < 9u ? s_runs[4 * r] : 0u;
+            produce(n_chunk & 1u);
+        }
+        __syncthreads();
 
-        int r = 0;
-        uint32_t cs = 0;
-        skip_empty(r, cs);
-        if (tid == 0 && r < 9) issue(cs, min(cs + kDenseK, s_runs[4 * r + 3]));
-        while (r < 9) {
-            const uint32_t ce = min(cs + kDenseK, s_runs[4 * r + 3]);
-            const uint32_t ncand = ce - cs, roff = cs & 1u;   // candidates of this chunk; raw index of slot cs
-            const uint32_t b1 = s_runs[4 * r + 1], b2 = s_runs[4 * r + 2];
-            const dense::RowGeom rg = dense::row_geom(g, cell, ix, iy, iz, r);
-            // counting sort of the chunk by octant bin, stable: raw -> sorted (sph_dense_dev.cuh)
-            dense::bin_chunk<kDenseThreads, kRounds, false>(
-                r_pos, roff, ncand, cs, b1, b2, g, cell, ix, rg, s_hist, s_bstart, s_box,
-                [&]() {
-                    mbar_wait(s_bar, n_staged & 1u);
-                    ++n_staged;
-                },
-                [&]() { *s_tnext = 0u; },
-                [&](uint32_t src, uint32_t dst) {
-                    c_pos[dst] = r_pos[src];
-                    c_vel[dst] = r_vel[src];
-                    c_pc[dst] = r_pc[src];
-                },
-                [&](uint32_t) {});
-
-            int rn = r;
-            uint32_t csn = cs;
-            next_chunk(rn, csn);
-            if (tid == 0 && rn < 9) issue(csn, min(csn + kDenseK, s_runs[4 * rn + 3]));
+        for (;;) {
+            const uint32_t set = n_chunk & 1u;
+            const uint32_t nseg = s_nseg[set];
+            if (nseg == 0u) break;
+            ++n_chunk;
+            // ---- every segment of the chunk: counting sort by octant bin, stable: raw -> sorted (sph_dense_dev.cuh) ----
+            uint32_t soff = 0;   // sorted index where the segment starts
+            for (uint32_t sgi = 0; sgi < nseg; ++sgi) {
+                const uint4 sg = s_seg[set * kMaxSeg + sgi];   // (row, first slot, end slot, raw base)
+                const int r = (int)sg.x;
+                const dense::RowGeom rg = dense::row_geom(g, cell, ix, iy, iz, r);
+                dense::bin_chunk<kDenseThreads, kRounds, false>(
+                    r_pos, sg.w + (sg.y & 1u), sg.z - sg.y, sg.y, s_runs[4 * r + 1], s_runs[4 * r + 2], g, cell, ix, rg, s_hist,
+                    s_bstart + 32u * sgi, s_box + 2u * kBins * sgi,
+                    [&]() {
+                        if (sgi == 0u) {
+                            mbar_wait(s_bar, n_staged & 1u);
+                            ++n_staged;
+                        }
+                    },
+                    [&]() { *s_tnext = 0u; },
+                    [&](uint32_t src, uint32_t dst) {
+                        c_pos[soff + dst] = r_pos[src];
+                        c_vel[soff + dst] = r_vel[src];
+                        c_pc[soff + dst] = r_pc[src];
+                    },
+                    [&](uint32_t) {});
+                soff += sg.z - sg.y;
+            }
+            if (tid == 0) produce(n_chunk & 1u);   // the landing zone is free: the next chunk's copies run under the work below
 
             // ---- the item's targets against the chunk ----
             // (shared memory by 32-bit address from here on: byte offsets in registers, no generic-address arithmetic)
-            const float4 bx0 = lane < kBins ? s_box[2 * lane] : make_float4(big, big, big, big);
-            const float4 bx1 = lane < kBins ? s_box[2 * lane + 1] : make_float4(big, big, 0.f, 0.f);
-            const uint32_t bs0 = s_bstart[lane];                                   // lane b: slots [bs0, bs0 + blen) of the
-            const uint32_t blen = lane < kBins ? s_bstart[lane + 1] - bs0 : 0u;    // sorted chunk hold bin b
             // targets are handed to the warps one at a time from a counter: their work differs (position in the cell, the
             // chunk's population), and the CTA waits for its slowest warp at the end of every chunk.  Which warp takes a
             // target does not enter its sum: a target meets the chunks in a fixed order, one warp per chunk.
@@ -202,16 +231,6 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                 t = __shfl_sync(0xffffffffu, t, 0);
                 if (t >= nt) break;
                 const float4 pi = lds_f4(a_tpos + 16u * t);
-                // lane b: does the 2h sphere of the target reach the box of bin b?  (a lower bound of the distance)
-                const float ex = fmaxf(fmaxf(bx0.x - pi.x, pi.x - bx0.y), 0.f);
-                const float ey = fmaxf(fmaxf(bx0.z - pi.y, pi.y - bx0.w), 0.f);
-                const float ez = fmaxf(fmaxf(bx1.x - pi.z, pi.z - bx1.y), 0.f);
-                const bool reach_b = fmaf(ez, ez, fmaf(ey, ey, ex * ex)) < rc2;   // lanes >= kBins: their box is out of reach
-                // the reachable bins, in bin order, are the target's candidate list: at most four slot ranges
-                const dense::Groups G = dense::candidate_groups(reach_b, bs0, blen, ncand, a_tab);
-                const uint32_t T = G.T;
-                if (T == 0u) continue;
-
                 const float4 vi = lds_f4(a_tvel + 16u * t);
                 const float2 ci = lds_f2(a_tpc + 8u * t);
                 float ax = 0.f, ay = 0.f, az = 0.f, de = 0.f;
@@ -234,26 +253,44 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                         mumax = fmaxf(mumax, fabsf(mu));
                     }
                 };
-                // one step: 32 flat positions, one per lane; `in` is false only for the lanes past the end in the last step
-                auto step = [&](uint32_t v16, bool in) {
-                    const uint32_t rel = in ? dense::candidate_offset(G, v16) : 0u;
-                    float dx, dy, dz;
-                    const float d2 = dist2_f32(pi, lds_f4(a_pos + rel), dx, dy, dz);
-                    // d2 == 0: self, or a coincident pair (A9) — no contribution
-                    const bool ok = in && d2 < rc2 && d2 > 0.f;
-                    const unsigned m = __ballot_sync(0xffffffffu, ok);
-                    if (ok) sts_u32(a_q + ((qt + 4u * __popc(m & lt_mask)) & (4u * kQueue - 4u)), rel);
-                    qt += 4u * __popc(m);
-                    if (qt - qh >= 128u) {
-                        __syncwarp();
-                        pair_term(lds_u32(a_q + ((qh + 4u * (uint32_t)lane) & (4u * kQueue - 4u))));
-                        qh += 128u;
-                    }
-                };
-                const uint32_t T16 = 16u * T, full16 = T16 & ~511u;
-                uint32_t v16 = 16u * (uint32_t)lane;
-                for (; v16 < full16; v16 += 512u) step(v16, true);     // v16 - 16 lane < full16 for every lane: uniform
-                if (full16 != T16) step(v16, v16 < T16);
+                uint32_t first = 0;   // sorted index where the segment starts
+                for (uint32_t sgi = 0; sgi < nseg; ++sgi) {
+                    // lane b: does the 2h sphere of the target reach the box of bin b of this segment?  (a lower bound of the distance)
+                    const float4 bx0 = lane < kBins ? s_box[2u * (kBins * sgi + lane)] : make_float4(big, big, big, big);
+                    const float4 bx1 = lane < kBins ? s_box[2u * (kBins * sgi + lane) + 1u] : make_float4(big, big, 0.f, 0.f);
+                    const uint32_t bl0 = s_bstart[32u * sgi + lane];
+                    const uint32_t blen = lane < kBins ? s_bstart[32u * sgi + lane + 1] - bl0 : 0u;
+                    const uint32_t ncand = s_bstart[32u * sgi + kBins];
+                    const float ex = fmaxf(fmaxf(bx0.x - pi.x, pi.x - bx0.y), 0.f);
+                    const float ey = fmaxf(fmaxf(bx0.z - pi.y, pi.y - bx0.w), 0.f);
+                    const float ez = fmaxf(fmaxf(bx1.x - pi.z, pi.z - bx1.y), 0.f);
+                    const bool reach_b = fmaf(ez, ez, fmaf(ey, ey, ex * ex)) < rc2;   // lanes >= kBins: their box is out of reach
+                    // the reachable bins, in bin order, are the target's candidates in this segment: at most four slot ranges
+                    const dense::Groups G = dense::candidate_groups(reach_b, first + bl0, blen, first, ncand, a_tab);
+                    first += ncand;
+                    const uint32_t T = G.T;
+                    if (T == 0u) continue;
+                    // one step: 32 flat positions, one per lane; `in` is false only for the lanes past the end in the last step
+                    auto step = [&](uint32_t v16, bool in) {
+                        const uint32_t rel = in ? dense::candidate_offset(G, v16) : 0u;
+                        float dx, dy, dz;
+                        const float d2 = dist2_f32(pi, lds_f4(a_pos + rel), dx, dy, dz);
+                        // d2 == 0: self, or a coincident pair (A9) — no contribution
+                        const bool ok = in && d2 < rc2 && d2 > 0.f;
+                        const unsigned m = __ballot_sync(0xffffffffu, ok);
+                        if (ok) sts_u32(a_q + ((qt + 4u * __popc(m & lt_mask)) & (4u * kQueue - 4u)), rel);
+                        qt += 4u * __popc(m);
+                        if (qt - qh >= 128u) {
+                            __syncwarp();
+                            pair_term(lds_u32(a_q + ((qh + 4u * (uint32_t)lane) & (4u * kQueue - 4u))));
+                            qh += 128u;
+                        }
+                    };
+                    const uint32_t T16 = 16u * T, full16 = T16 & ~511u;
+                    uint32_t v16 = 16u * (uint32_t)lane;
+                    for (; v16 < full16; v16 += 512u) step(v16, true);     // v16 - 16 lane < full16 for every lane: uniform
+                    if (full16 != T16) step(v16, v16 < T16);
+                }
                 if (qt != qh) {
                     __syncwarp();
                     if (4u * (uint32_t)lane < qt - qh) pair_term(lds_u32(a_q + ((qh + 4u * (uint32_t)lane) & (4u * kQueue - 4u))));
@@ -286,10 +323,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                     }
                 }
             }
-            r = rn;
-            cs = csn;
-            // the __syncthreads() after the wait at the top of the next chunk (or the one before the write-out below)
-            // separates this chunk's reads of the sorted tile from the next re-ordering
+            __syncthreads();   // every warp is done with the sorted chunk; the next chunk's description is visible
         }
         __syncthreads();
 

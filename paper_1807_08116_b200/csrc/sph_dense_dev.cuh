@@ -108,12 +108,16 @@ __device__ __forceinline__ void bin_chunk(const float4* r_pos, uint32_t roff, ui
     __syncthreads();
     if (tid < 32) {
         // lane b: exclusive prefix of bin b over (round, warp), then the bins' starts
+        // (all the loads first: the other warps wait at the barrier below for this one)
         uint32_t run = 0u;
         if (lane < kBins) {
+            uint32_t v[ROUNDS * WARPS];
+#pragma unroll
+            for (int j = 0; j < ROUNDS * WARPS; ++j) v[j] = hist[j * kBins + lane];
+#pragma unroll
             for (int j = 0; j < ROUNDS * WARPS; ++j) {
-                const uint32_t v = hist[j * kBins + lane];
                 hist[j * kBins + lane] = run;
-                run += v;
+                run += v[j];
             }
         }
         const uint32_t len = PAD_EVEN ? (run + 1u) & ~1u : run;
@@ -148,12 +152,13 @@ __device__ __forceinline__ void bin_chunk(const float4* r_pos, uint32_t roff, ui
 // by the flat position where it ends and the offset from a flat position to a slot, both in BYTES of the float4 array
 // (x16), so a candidate's address is one add.  Warp-wide: lane b passes whether bin b is reachable and its [bs0, bs0 + blen)
 // range; the table goes through 32 bytes of shared memory at a_tab.  Returns T (0: nothing reachable); ng > 4 cannot
-// happen for boxes in a row — if it ever does, every slot of the chunk is a candidate.
+// happen for boxes in a row — if it ever does, every slot [first, first + ncand) of the staged piece is a candidate.
 struct Groups {
     uint2 g0, g1, g2, g3;
     uint32_t T;
 };
-__device__ __forceinline__ Groups candidate_groups(bool reach_b, uint32_t bs0, uint32_t blen, uint32_t ncand, uint32_t a_tab) {
+__device__ __forceinline__ Groups candidate_groups(bool reach_b, uint32_t bs0, uint32_t blen, uint32_t first, uint32_t ncand,
+                                                   uint32_t a_tab) {
     const int lane = threadIdx.x & 31;
     const unsigned lt_mask = (1u << lane) - 1u;
     const unsigned reach = __ballot_sync(0xffffffffu, reach_b);
@@ -178,9 +183,9 @@ __device__ __forceinline__ Groups candidate_groups(bool reach_b, uint32_t bs0, u
     G.g2 = lds_u2(a_tab + 16u);
     G.g3 = lds_u2(a_tab + 24u);
     __syncwarp();   // the table may be rewritten
-    if (ng > 4) {
+    if (ng > 4) {   // [first, first + ncand): the whole staged piece
         G.T = ncand;
-        G.g0 = make_uint2(0xffffffffu, 0u);
+        G.g0 = make_uint2(0xffffffffu, 16u * first);
     }
     return G;
 }
