@@ -59,8 +59,7 @@ struct DenseLayout {
     static constexpr int hist = runs + 9 * 4 * 4;                       // uint32 [rounds][warps][bins]
     static constexpr int bstart = hist + kRounds * kDenseWarps * kBins * 4;   // uint32 [seg][32]: start of bin b inside its segment
     static constexpr int box = bstart + kMaxSeg * 32 * 4;               // float [seg][bins][8]: xl, xh, yl, yh, zl, zh, -, -
-    static constexpr int tab = box + kMaxSeg * kBins * 8 * 4;           // uint2 [warps][4]: a target's candidate groups
-    static constexpr int queue = tab + kDenseWarps * 4 * 8;             // uint32 [warps][kQueue]
+    static constexpr int queue = box + kMaxSeg * kBins * 8 * 4;         // uint32 [warps][kQueue]
     static constexpr int seg = queue + kDenseWarps * kQueue * 4;        // uint4 [2][seg]: (row, first slot, end slot, raw base) of the
                                                                         // chunk being worked on and of the one being copied
     static constexpr int nseg = seg + 2 * kMaxSeg * 16;                 // uint32 [2] segments of those chunks, [2] (row, slot) the producer is at
@@ -106,7 +105,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
     const uint32_t sbase = smem_u32(smem);
     const uint32_t a_pos = sbase + L::pos, a_vel = sbase + L::vel, a_pc = sbase + L::pc;
     const uint32_t a_tpos = sbase + L::tpos, a_tvel = sbase + L::tvel, a_tpc = sbase + L::tpc;
-    const uint32_t a_tab = sbase + L::tab + 32u * (uint32_t)warp, a_q = sbase + L::queue + 4u * kQueue * (uint32_t)warp;
+    const uint32_t a_q = sbase + L::queue + 4u * kQueue * (uint32_t)warp;
     const uint32_t n_items = ctl[0];
     if (blockIdx.x >= n_items) return;   // uniform per CTA
 
@@ -114,6 +113,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
         mbar_init(s_bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    for (int i = tid; i < kRounds * kDenseWarps * kBins; i += kDenseThreads) s_hist[i] = 0u;   // dense::bin_chunk keeps it zeroed
     uint32_t n_staged = 0;   // chunks this CTA has waited for so far: the barrier's phase parity
     uint32_t n_chunk = 0;    // chunks this CTA has described so far: the descriptor set in use is n_chunk & 1
 
@@ -258,15 +258,14 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                     // lane b: does the 2h sphere of the target reach the box of bin b of this segment?  (a lower bound of the distance)
                     const float4 bx0 = lane < kBins ? s_box[2u * (kBins * sgi + lane)] : make_float4(big, big, big, big);
                     const float4 bx1 = lane < kBins ? s_box[2u * (kBins * sgi + lane) + 1u] : make_float4(big, big, 0.f, 0.f);
-                    const uint32_t bl0 = s_bstart[32u * sgi + lane];
-                    const uint32_t blen = lane < kBins ? s_bstart[32u * sgi + lane + 1] - bl0 : 0u;
                     const uint32_t ncand = s_bstart[32u * sgi + kBins];
                     const float ex = fmaxf(fmaxf(bx0.x - pi.x, pi.x - bx0.y), 0.f);
                     const float ey = fmaxf(fmaxf(bx0.z - pi.y, pi.y - bx0.w), 0.f);
                     const float ez = fmaxf(fmaxf(bx1.x - pi.z, pi.z - bx1.y), 0.f);
                     const bool reach_b = fmaf(ez, ez, fmaf(ey, ey, ex * ex)) < rc2;   // lanes >= kBins: their box is out of reach
-                    // the reachable bins, in bin order, are the target's candidates in this segment: at most four slot ranges
-                    const dense::Groups G = dense::candidate_groups(reach_b, first + bl0, blen, first, ncand, a_tab);
+                    // the reachable bins, in bin order, are the target's candidates in this segment: four slot ranges
+                    const unsigned reach = __ballot_sync(0xffffffffu, reach_b);
+                    const dense::Groups G = dense::candidate_groups(reach, s_bstart + 32u * sgi, first);
                     first += ncand;
                     const uint32_t T = G.T;
                     if (T == 0u) continue;
@@ -295,7 +294,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                     __syncwarp();
                     if (4u * (uint32_t)lane < qt - qh) pair_term(lds_u32(a_q + ((qh + 4u * (uint32_t)lane) & (4u * kQueue - 4u))));
                 }
-                __syncwarp();   // the queue and the table are rewritten for the next target
+                __syncwarp();   // the queue is rewritten for the next target
                 if (qt != 0u) {
                     // the four sums over the 32 lanes in FP64, as one butterfly: after the exchange over lane bit 4 a
                     // lane holds two of them, after bit 3 one; lanes 0, 8, 16, 24 end with a_x, a_y, a_z, de/dt

@@ -79,8 +79,8 @@ __device__ __forceinline__ void bin_box(int bb, const GridDev g, float cell, int
 // Stable counting sort of a staged chunk by bin (slot order inside a bin), all THREADS threads of the CTA:
 //   raw[roff + i], i < ncand, is the candidate of slot cs + i;  move(src raw index, dst sorted index) copies its payload;
 //   bstart[b] = first sorted index of bin b (bstart[24..31] = ncand);  box[2 b], box[2 b + 1] = the bins' boxes.
-// hist: [ROUNDS][THREADS/32][kBins] words.  `wait` is called once the histogram has been zeroed (the bulk copy's
-// mbarrier), `extra` by one thread between the barriers (per-chunk resets of the caller).  PAD_EVEN: every bin starts at
+// hist: [ROUNDS][THREADS/32][kBins] words, ZERO on entry (the caller zeroes it once, each call leaves it zeroed).  `wait` is
+// called first (the bulk copy's mbarrier), `extra` by one thread between the barriers (per-chunk resets of the caller).  PAD_EVEN: every bin starts at
 // an even sorted index — a bin of odd population is followed by one filler slot, which pad(dst) fills (a caller that
 // reads the sorted chunk two slots at a time).  Ends with a barrier: the sorted chunk is complete and the landing zone
 // is free.
@@ -91,9 +91,7 @@ __device__ __forceinline__ void bin_chunk(const float4* r_pos, uint32_t roff, ui
     constexpr int WARPS = THREADS / 32;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned lt_mask = (1u << lane) - 1u;
-    for (int i = tid; i < ROUNDS * WARPS * kBins; i += THREADS) hist[i] = 0u;
-    wait();
-    __syncthreads();   // histogram zeroed; every warp is past the previous chunk's candidates
+    wait();   // (every thread waits for the copy itself; the histogram was zeroed before the last barrier of the previous call)
     uint32_t my_bin[ROUNDS], my_rank[ROUNDS];
 #pragma unroll
     for (int rd = 0; rd < ROUNDS; ++rd) {
@@ -105,7 +103,7 @@ __device__ __forceinline__ void bin_chunk(const float4* r_pos, uint32_t roff, ui
         my_rank[rd] = __popc(peers & lt_mask);
         if (bin < (uint32_t)kBins && my_rank[rd] == 0u) hist[(rd * WARPS + warp) * kBins + bin] = __popc(peers);
     }
-    __syncthreads();
+    __syncthreads();   // counts complete; every warp is past the previous chunk's candidates
     if (tid < 32) {
         // lane b: exclusive prefix of bin b over (round, warp), then the bins' starts
         // (all the loads first: the other warps wait at the barrier below for this one)
@@ -143,50 +141,42 @@ __device__ __forceinline__ void bin_chunk(const float4* r_pos, uint32_t roff, ui
         const uint32_t i = (uint32_t)(rd * THREADS + tid);
         if (i < ncand) move(roff + i, bstart[my_bin[rd]] + hist[(rd * WARPS + warp) * kBins + my_bin[rd]] + my_rank[rd]);
     }
+    __syncwarp();
+    // zero the histogram for the next call: a warp reads only its own rows of it above
+#pragma unroll
+    for (int rd = 0; rd < ROUNDS; ++rd)
+        if (lane < kBins) hist[(rd * WARPS + warp) * kBins + lane] = 0u;
     __syncthreads();   // the sorted chunk is complete, the landing zone is free
 }
 
-// The reachable bins of a target (or of a warp of targets), in bin order, are its candidate list: flat position
-// v = 0 .. T-1.  Consecutive reachable bins are one slot range (a "group").  Along a (sz, sy) sub-row the distance to the
-// 6 x-slabs falls and rises once, so the reachable bins of a sub-row are consecutive: at most 4 groups.  Each is described
-// by the flat position where it ends and the offset from a flat position to a slot, both in BYTES of the float4 array
-// (x16), so a candidate's address is one add.  Warp-wide: lane b passes whether bin b is reachable and its [bs0, bs0 + blen)
-// range; the table goes through 32 bytes of shared memory at a_tab.  Returns T (0: nothing reachable); ng > 4 cannot
-// happen for boxes in a row — if it ever does, every slot [first, first + ncand) of the staged piece is a candidate.
+// The reachable bins of a target, in bin order, are its candidate list: flat position v = 0 .. T-1.  Along a (sz, sy)
+// sub-row the distance to the 6 x-slabs falls and rises once, so the reachable bins of a sub-row are consecutive: one
+// slot range per sub-row, from its first to its last reachable bin (if a bin in between were out of reach after all,
+// testing its candidates costs time, not correctness).  A range is described by the flat position where it ends and
+// the offset from a flat position to a slot, both in BYTES of the float4 array (x16), so a candidate's address is one
+// add.  `reach`: bit b set = bin b reachable (a ballot: uniform); bstart: the bins' starts inside the segment, which
+// begins at sorted index `first`.  All lanes compute the same four ranges: bit operations and 8 broadcast loads.
 struct Groups {
     uint2 g0, g1, g2, g3;
     uint32_t T;
 };
-__device__ __forceinline__ Groups candidate_groups(bool reach_b, uint32_t bs0, uint32_t blen, uint32_t first, uint32_t ncand,
-                                                   uint32_t a_tab) {
-    const int lane = threadIdx.x & 31;
-    const unsigned lt_mask = (1u << lane) - 1u;
-    const unsigned reach = __ballot_sync(0xffffffffu, reach_b);
-    uint32_t incl = reach_b ? blen : 0u;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += v;
-    }
+__device__ __forceinline__ Groups candidate_groups(unsigned reach, const uint32_t* bstart, uint32_t first) {
     Groups G;
-    G.T = __shfl_sync(0xffffffffu, incl, 31);
-    if (G.T == 0u) return G;
-    const unsigned gstart = reach & ~(reach << 1);                           // first bin of every group
-    const int ng = __popc(gstart);
-    const int e = lane + __ffs(~(reach >> lane)) - 1;                        // (for a first bin) one past the group's last bin
-    const uint32_t gend = __shfl_sync(0xffffffffu, incl, (e - 1) & 31);
-    if (lane < 4 && lane >= ng) sts_u2(a_tab + 8u * lane, 0xffffffffu, 0u);   // no such group
-    if (((gstart >> lane) & 1u) && ng <= 4) sts_u2(a_tab + 8u * __popc(gstart & lt_mask), 16u * gend, 16u * (bs0 - (incl - blen)));
-    __syncwarp();
-    G.g0 = lds_u2(a_tab);
-    G.g1 = lds_u2(a_tab + 8u);
-    G.g2 = lds_u2(a_tab + 16u);
-    G.g3 = lds_u2(a_tab + 24u);
-    __syncwarp();   // the table may be rewritten
-    if (ng > 4) {   // [first, first + ncand): the whole staged piece
-        G.T = ncand;
-        G.g0 = make_uint2(0xffffffffu, 16u * first);
+    uint32_t end = 0;
+    uint2* g[4] = {&G.g0, &G.g1, &G.g2, &G.g3};
+#pragma unroll
+    for (int sr = 0; sr < 4; ++sr) {
+        const unsigned m6 = (reach >> (6 * sr)) & 63u;
+        uint32_t lo = 0, hi = 0;
+        if (m6) {
+            lo = bstart[6 * sr + __ffs(m6) - 1];
+            hi = bstart[6 * sr + 32 - __clz(m6)];
+        }
+        const uint32_t off = first + lo - end;   // flat position end .. end + (hi - lo) -> slots first + lo ..
+        end += hi - lo;
+        *g[sr] = make_uint2(16u * end, 16u * off);
     }
+    G.T = end;
     return G;
 }
 // flat position (x16) -> byte offset of the candidate in the sorted float4 array

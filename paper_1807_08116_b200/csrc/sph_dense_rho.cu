@@ -87,6 +87,7 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
         mbar_init(s_bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    for (int i = tid; i < kRhoRounds * kRhoWarps * kBins; i += kRhoThreads) s_hist[i] = 0u;   // dense::bin_chunk keeps it zeroed
     uint32_t n_staged = 0;
     const float big = 3.0e38f;
     const u64 ninvh2 = pk2(neg_inv_h, neg_inv_h), two2 = pk2(2.0f, 2.0f), one2 = pk2(1.0f, 1.0f), q25 = pk2(0.25f, 0.25f);
