@@ -256,8 +256,11 @@ def test_density_and_forces_parity(cuda_lib, case):
     prm = b.sph_params.from_workload(w)
     rho = torch.zeros(n, device="cuda")
     b.sph_density(d, n, prm, g, perm, start, rho, ws)
-    if case in DENSE_CASES:      # these cases are there for the dense-cell walk: make sure it ran
+    if case in DENSE_CASES:      # these cases are there for the dense-cell walks: make sure they ran
         assert b.sph_dense_items(ws, n, n, g) > 0
+    rho2 = torch.zeros_like(rho)                 # work items and units are handed out dynamically: same bits all the same
+    b.sph_density(d, n, prm, g, perm, start, rho2, ws)
+    assert torch.equal(rho, rho2)
     ooff, oidx = oracle.neighbours(w.posm, n, w.h, method="grid")
     orho = oracle.density(w.posm, w.h, ooff, oidx)
     check_density(rho.cpu().numpy(), orho, f"rho {case}")
@@ -379,6 +382,48 @@ def test_adaptive_step_parity(cuda_lib, cfg, scale, steps, sigma):
     sim_b.step(dt=1e-6)
     assert float(sim_a.dt_used.item()) == float(np.float32(1e-6))
     assert torch.equal(sim_a.posm, sim_b.posm) and torch.equal(sim_a.vele, sim_b.vele)
+
+
+def _box_grid_case(n, dims, seed):
+    """n gas particles uniform in a box of dims cells (cell edge 0.1), on an explicit grid of exactly those cells: the
+    populations of the stencil rows are then n_per_cell x 3 (or x 2 at the faces) — chosen by the caller to sit on the
+    boundaries of the dense walks' chunking."""
+    rng = np.random.Generator(np.random.Philox(key=[seed, 0]))
+    h = np.float32(0.0499)
+    cell = np.float32(np.float32(2 * h) * np.float32(1.001953125))
+    posm = np.zeros((n, 4), np.float32)
+    vele = np.zeros((n, 4), np.float32)
+    posm[:, :3] = rng.random((n, 3)) * (np.array(dims) * float(cell) * 0.999)
+    posm[:, 3] = (0.5 + rng.random(n)) / n
+    vele[:, :3] = 0.3 * rng.standard_normal((n, 3))
+    vele[:, 3] = 0.5 + 0.5 * rng.random(n)
+    w = wl.Workload(f"box{n}", posm, vele, n, 0, float(h), 0.01, 0.0, 1e-3, 1, seed)
+    og = oracle.Grid((0.0, 0.0, 0.0), float(cell), float(np.float32(1.0) / cell), tuple(dims))
+    return w, og
+
+
+@pytest.mark.parametrize("n,dims", [(1088, (1, 1, 1)), (1089, (1, 1, 1)), (2177, (1, 1, 1)), (3264, (3, 1, 1)), (3267, (3, 1, 1)),
+                                    (1080, (3, 3, 3)), (2700, (3, 3, 3)), (9800, (3, 3, 3)), (2000, (5, 2, 1)), (33 * 8, (2, 2, 2))])
+def test_dense_walk_chunk_boundaries(cuda_lib, n, dims):
+    """The dense walks stage a stencil row in chunks of 1088 (forces) / 1152 (density) slots and pack up to six short rows
+    into one chunk: rows of exactly one chunk, one slot more, two chunks and one slot, three cells of one chunk each, many
+    short rows (six per chunk and the rest), long rows, a flat grid, cells right at the 32-particle threshold."""
+    b = cuda_lib
+    w, og = _box_grid_case(n, dims, 31 + n)
+    d, g, perm, start, ws = _build(b, w, og)
+    prm = b.sph_params.from_workload(w)
+    rho = torch.zeros(n, device="cuda")
+    b.sph_density(d, n, prm, g, perm, start, rho, ws)
+    ooff, oidx = oracle.neighbours(w.posm, n, w.h, method="grid")
+    check_density(rho.cpu().numpy(), oracle.density(w.posm, w.h, ooff, oidx), f"rho box {n} {dims}")
+    acc = torch.zeros((n, 4), device="cuda")
+    b.sph_forces(d, _t(w.vele), rho, n, prm, g, perm, start, acc, ws)
+    assert b.sph_dense_items(ws, n, n, g) > 0
+    of, gross = oracle.forces(w.posm, w.vele, rho.cpu().numpy().astype(np.float64), w.h, ooff, oidx, gamma=w.gamma,
+                              alpha=w.alpha, beta=w.beta, eta=w.eta, with_gross=True)
+    got = acc.cpu().numpy()
+    check_values(got[:, :3], of[:, :3], f"a_sph box {n} {dims}", gross=gross[:, 0])
+    check_values(got[:, 3], of[:, 3], f"de/dt box {n} {dims}", gross=gross[:, 1])
 
 
 def test_coincident_gas_particles(cuda_lib):
