@@ -3,22 +3,24 @@
 // The density pair term is ~15 instructions: nothing is won by compacting accepted pairs (the warp-per-target walk of
 // sph_dense.cu, tried on the density, lost to the thread-per-slot walk); the cost is the NUMBER of candidates tested —
 // all 27 cells of the stencil, 6 per neighbour — and the instructions per test.  Per work item (one cell, <= 384 targets):
-//   * the item's targets are ordered by the octant of their cell they lie in, so a warp of 32 targets covers one or two
-//     octants and has a small bounding box;
+//   * the item's targets are ordered by the octant of their cell they lie in, so a group of 8 consecutive targets covers
+//     one or two octants and has a small bounding box;
 //   * each stencil row is staged by TMA bulk copies and re-ordered by octant bin in shared memory (sph_dense_dev.cuh), as
 //     for the forces — positions only, and written as PAIRS (x0,x1,y0,y1)(z0,z1,m0,m1), every bin padded to an even
 //     number of slots, for the packed arithmetic below;
-//   * a warp tests the bins against ITS bounding box — lane b the box of bin b — and walks only the reachable ones
-//     (~55-65 % of the stencil, against 39 % for a single target and 100 % without bins): thread per target, every lane
-//     its own target, the candidate pair the same for all lanes — two broadcast LDS.128 per pair and warp, no bank
-//     conflict, no divergence, no reduction;
-//   * the arithmetic of a pair of candidates is packed FP32 (sub/mul/fma.f32x2, as in the gravity kernels): 13 packed
-//     operations + 2 MUFU.SQRT + 8 scalar ones for two candidates — the loop is issue-bound, and packing halves the slots;
-//   * work units: (warp of targets) x (third of the candidate pairs); a CTA's 12 warps draw the units of a chunk from a
-//     counter; a unit's partial sum lives in shared memory between chunks, the three partials of a target are added in
-//     fixed order at the end of the item.
-// Kernel value: W = 1/4 (2 - xi)_+^3 - (1 - xi)_+^3 with xi from MUFU.SQRT (sph_dev.cuh); the FP32 cutoff d2 < fl(fl(2h)^2)
-// of A8, with d2 formed by the same mul, fma, fma as everywhere, decides membership.  Fixed order: bitwise reproducible.
+//   * a work unit is one group of 8 targets on one warp, 4 lanes per target: the warp tests the bins against the GROUP's
+//     bounding box — lane b the box of bin b — and walks only the reachable ones (~65 % of the stencil; 83 % for a group
+//     of 32, 39 % for a single target, 100 % without bins); the 4 lanes of a target take the candidate pairs of a range
+//     in turn, so a warp reads 4 consecutive pairs per step — two LDS.128 of 4 distinct addresses, no bank conflict — and
+//     the 4 partial sums are added by two shuffles in a fixed order.  (2 and 8 lanes per target measured slower: 23.0
+//     and 26.2 ms against 20.9 at config 4.)
+//   * the arithmetic of a pair of candidates is packed FP32 (sub/mul/fma.f32x2, as in the gravity kernels): 14 packed
+//     operations + 2 MUFU.SQRT + 4 FMNMX + 2 LDS.128 + 3 of loop control for two candidates — 25 instructions per step
+//     of 64 lane tests; the loop is issue-bound, and packing halves the slots;
+//   * a CTA's 12 warps draw the units of a chunk from a counter; a target's running sum lives in shared memory between
+//     chunks and is touched by one warp per chunk, in chunk order.
+// Kernel value: W = 1/4 (2 - xi)_+^3 - (1 - xi)_+^3 with xi from MUFU.SQRT (sph_dev.cuh), d2 formed by the same mul, fma,
+// fma as everywhere; the clamped cubes stand in for the cutoff test (see the loop).  Fixed order: bitwise reproducible.
 #include "sph_dense_dev.cuh"
 #include "grav_dev.cuh"   // the packed-FP32 helpers pk2 / upk2 / fma2 / mul2 / sub2
 
@@ -31,9 +33,11 @@ constexpr int kRhoThreads = 384;
 constexpr int kRhoWarps = kRhoThreads / 32;
 constexpr int kRhoCtasPerSm = 3;
 constexpr int kRhoTT = 3 * kDenseTT;                        // targets per item: three consecutive entries of the work list
-constexpr int kRhoShares = 3;                               // shares of the candidate pairs
+constexpr int kRhoL = 4;                                    // lanes per target: each takes every kRhoL-th candidate pair
+constexpr int kRhoG = 32 / kRhoL;                           // targets per work unit (one warp)
 constexpr int kRhoK = 1152;                                 // candidate slots per staged chunk
 constexpr int kRhoKS = kRhoK + kBins;                       // sorted: + one filler per bin at most
+static_assert(kRhoTT == kRhoThreads, "a thread per target of the item");
 constexpr int kRhoRounds = (kRhoK + kRhoThreads - 1) / kRhoThreads;
 
 struct RhoLayout {
@@ -41,14 +45,13 @@ struct RhoLayout {
     static constexpr int pk = raw_pos + kRhoK * 16;                     // float4 [KS/2][2] the chunk in bin order, as pairs
     static constexpr int tpos = pk + kRhoKS * 16;                       // float4 [TT]    the item's targets in octant order
     static constexpr int tslot = tpos + kRhoTT * 16;                    // uint32 [TT]    their sorted slots
-    static constexpr int part = tslot + kRhoTT * 4;                     // float [shares][TT] partial sums
-    static constexpr int bbox = part + kRhoShares * kRhoTT * 4;         // float [TT/32][8] bounding boxes of the target warps
-    static constexpr int runs = bbox + (kRhoTT / 32) * 32;              // uint32 [9][4]
+    static constexpr int part = tslot + kRhoTT * 4;                     // float [TT]     the targets' running sums
+    static constexpr int bbox = part + kRhoTT * 4;                      // float [TT/G][8] bounding boxes of the target groups
+    static constexpr int runs = bbox + (kRhoTT / kRhoG) * 32;           // uint32 [9][4]
     static constexpr int hist = runs + 9 * 4 * 4;                       // uint32 [rounds][warps][bins]
     static constexpr int bstart = hist + kRhoRounds * kRhoWarps * kBins * 4;   // uint32 [32]
     static constexpr int box = bstart + 32 * 4;                         // float4 [bins][2]
-    static constexpr int tab = box + kBins * 32;                        // uint2 [warps][4]
-    static constexpr int ocnt = tab + kRhoWarps * 32;                   // uint32 [warps][8] octant counts
+    static constexpr int ocnt = box + kBins * 32;                       // uint32 [warps][8] octant counts
     static constexpr int bar = ocnt + kRhoWarps * 8 * 4;                // uint64
     static constexpr int item = bar + 8;                                // uint32
     static constexpr int unext = bar + 12;                              // uint32: next work unit of the chunk
@@ -80,7 +83,8 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned lt_mask = (1u << lane) - 1u;
     const uint32_t sbase = smem_u32(smem);
-    const uint32_t a_pk = sbase + L::pk, a_tab = sbase + L::tab + 32u * (uint32_t)warp;
+    const uint32_t a_pk = sbase + L::pk;
+    const uint32_t sub = (uint32_t)lane % kRhoL, tl = (uint32_t)lane / kRhoL;   // this lane's share and target within a unit
     const uint32_t n_items = ctl[0];
     if (blockIdx.x >= n_items) return;   // uniform per CTA
     if (tid == 0) {
@@ -136,7 +140,7 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
         if (lane < 8) s_ocnt[warp * 8 + lane] = 0u;
         __syncwarp();
         if (oct < 8u && orank == 0u) s_ocnt[warp * 8 + oct] = __popc(opeers);
-        for (int i = tid; i < kRhoShares * kRhoTT; i += kRhoThreads) s_part[i] = 0.f;
+        for (int i = tid; i < kRhoTT; i += kRhoThreads) s_part[i] = 0.f;
         __syncthreads();
         if (oct < 8u) {
             uint32_t dst = orank;
@@ -147,9 +151,8 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
             t_slot[dst] = ts + (uint32_t)tid;
         }
         __syncthreads();
-        // bounding box of every warp of targets
-        const uint32_t ntw = (nt + 31u) >> 5;
-        if ((uint32_t)warp < ntw) {
+        // bounding box of every group of kRhoG consecutive targets (the threads' targets: kRhoTT == kRhoThreads)
+        if ((uint32_t)(warp * 32) < nt) {
             const uint32_t t = (uint32_t)(warp * 32 + lane);
             const bool has = t < nt;
             const float4 p = has ? t_pos[t] : make_float4(0.f, 0.f, 0.f, 0.f);
@@ -158,17 +161,17 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
 #pragma unroll
             for (int a = 0; a < 3; ++a)
 #pragma unroll
-                for (int o = 16; o > 0; o >>= 1) {
+                for (int o = kRhoG / 2; o > 0; o >>= 1) {
                     lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
                     hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
                 }
-            if (lane == 0) {
-                s_bbox[2 * warp] = make_float4(lo[0], hi[0], lo[1], hi[1]);
-                s_bbox[2 * warp + 1] = make_float4(lo[2], hi[2], 0.f, 0.f);
+            if (lane % kRhoG == 0) {
+                s_bbox[2 * (t / kRhoG)] = make_float4(lo[0], hi[0], lo[1], hi[1]);
+                s_bbox[2 * (t / kRhoG) + 1] = make_float4(lo[2], hi[2], 0.f, 0.f);
             }
         }
         __syncthreads();
-        const uint32_t n_units = ntw * kRhoShares;   // unit u: target warp u / 3, candidate pairs = u % 3 (mod 3)
+        const uint32_t n_units = (nt + kRhoG - 1u) / kRhoG;   // unit u: targets u kRhoG .. u kRhoG + kRhoG - 1
 
         int r = 0;
         uint32_t cs = 0;
@@ -202,46 +205,35 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
 
             const float4 bx0 = lane < kBins ? s_box[2 * lane] : make_float4(big, big, big, big);
             const float4 bx1 = lane < kBins ? s_box[2 * lane + 1] : make_float4(big, big, 0.f, 0.f);
-            const uint32_t bs0 = s_bstart[lane] >> 1;                                     // in pairs (every bin starts even)
-            const uint32_t blen = lane < kBins ? (s_bstart[lane + 1] >> 1) - bs0 : 0u;
-            // units are handed to the warps from a counter (their work differs with the warp's position in the cell); a unit's
-            // partial sum is touched by one warp per chunk, chunk after chunk in a fixed order
+            // units are handed to the warps from a counter (their work differs with the group's position in the cell); a
+            // target's sum is touched by one warp per chunk, chunk after chunk in a fixed order
             for (;;) {
                 uint32_t u = 0;
                 if (lane == 0) u = atomicAdd(s_unext, 1u);
                 u = __shfl_sync(0xffffffffu, u, 0);
                 if (u >= n_units) break;
-                const uint32_t tw = u / kRhoShares, share = u - tw * kRhoShares;
-                // lane b: can any target of the warp reach bin b?  distance between the two boxes, a lower bound
-                const float4 w0 = s_bbox[2 * tw], w1 = s_bbox[2 * tw + 1];   // (xlo, xhi, ylo, yhi), (zlo, zhi)
+                // lane b: can any target of the group reach bin b?  distance between the two boxes, a lower bound
+                const float4 w0 = s_bbox[2 * u], w1 = s_bbox[2 * u + 1];   // (xlo, xhi, ylo, yhi), (zlo, zhi)
                 const float ex = fmaxf(fmaxf(bx0.x - w0.y, w0.x - bx0.y), 0.f);
                 const float ey = fmaxf(fmaxf(bx0.z - w0.w, w0.z - bx0.w), 0.f);
                 const float ez = fmaxf(fmaxf(bx1.x - w1.y, w1.x - bx1.y), 0.f);
                 const bool reach_b = fmaf(ez, ez, fmaf(ey, ey, ex * ex)) < rc2;
-                // consecutive reachable bins are one range of pairs; at most 4 ranges (sph_dense_dev.cuh)
                 const unsigned reach = __ballot_sync(0xffffffffu, reach_b) & ((1u << kBins) - 1u);
                 if (reach == 0u) continue;
-                const unsigned gstart = reach & ~(reach << 1);
-                const int e = lane + __ffs(~(reach >> lane)) - 1;                       // one past the group's last bin
-                const uint32_t gend = __shfl_sync(0xffffffffu, bs0 + blen, (e - 1) & 31);
-                const int ng = __popc(gstart);
-                if (lane < 4 && lane >= ng) sts_u2(a_tab + 8u * lane, 0u, 0u);          // no such group
-                if (((gstart >> lane) & 1u) && ng <= 4) sts_u2(a_tab + 8u * __popc(gstart & lt_mask), bs0, gend);
-                __syncwarp();
-                uint2 grp[4] = {lds_u2(a_tab), lds_u2(a_tab + 8u), lds_u2(a_tab + 16u), lds_u2(a_tab + 24u)};
-                __syncwarp();
-                if (ng > 4) {   // cannot happen for boxes in a row; if it ever does, every pair of the chunk is a candidate
-                    grp[0] = make_uint2(0u, s_bstart[kBins] >> 1);
-                    grp[1] = grp[2] = grp[3] = make_uint2(0u, 0u);
-                }
-                const uint32_t t = tw * 32u + (uint32_t)lane;
+                const uint32_t t = u * kRhoG + tl;
                 const float4 pi = t < nt ? t_pos[t] : make_float4(big, big, big, 0.f);
                 const u64 xi = pk2(pi.x, pi.x), yi = pk2(pi.y, pi.y), zi = pk2(pi.z, pi.z);
                 u64 sum2 = 0ull;   // includes the self term m_i W(0): j = i passes the predicate with d2 = 0 (A5)
+                // one range of pairs per (sz, sy) sub-row, from its first to its last reachable bin (sph_dense_dev.cuh);
+                // the kRhoL lanes of a target take the pairs of a range in turn
 #pragma unroll
-                for (int gi = 0; gi < 4; ++gi) {
-                    for (uint32_t pr = grp[gi].x + share; pr < grp[gi].y; pr += kRhoShares) {
-                        const float4 A = lds_f4(a_pk + 32u * pr), B = lds_f4(a_pk + 32u * pr + 16u);
+                for (int sr = 0; sr < 4; ++sr) {
+                    const unsigned m6 = (reach >> (6 * sr)) & 63u;
+                    if (m6 == 0u) continue;   // uniform
+                    // byte addresses of the pairs: sorted slot d is in pair d / 2 (every bin starts even), 32 bytes a pair
+                    const uint32_t hi = a_pk + 16u * s_bstart[6 * sr + 32 - __clz(m6)];
+                    for (uint32_t pa = a_pk + 16u * s_bstart[6 * sr + __ffs(m6) - 1] + 32u * sub; pa < hi; pa += 32u * kRhoL) {
+                        const float4 A = lds_f4(pa), B = lds_f4(pa + 16u);
                         const u64 dx = sub2(xi, pk2(A.x, A.y)), dy = sub2(yi, pk2(A.z, A.w)), dz = sub2(zi, pk2(B.x, B.y));
                         const u64 d2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));   // per half: the mul, fma, fma of the cutoff (A8)
                         float d2a, d2b;
@@ -253,13 +245,18 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
                         const u64 a = pk2(fmaxf(a0, 0.f), fmaxf(a1, 0.f)), c = pk2(fmaxf(c0, 0.f), fmaxf(c1, 0.f));
                         const u64 c3 = mul2(mul2(c, c), c);
                         const u64 w = sub2(mul2(mul2(mul2(a, a), a), q25), c3);   // 1/4 (2 - xi)_+^3 - (1 - xi)_+^3
-                        const u64 m = pk2(d2a < rc2 ? B.z : 0.f, d2b < rc2 ? B.w : 0.f);   // the FP32 cutoff decides; W is 0 beyond 2h anyway
-                        sum2 = fma2(m, w, sum2);
+                        // no test of the cutoff: beyond 2h the clamped cubes are 0, and where the rounding of MUFU.SQRT and of the
+                        // fma puts 2 - xi on the other side of 0 than d2 < fl(fl(2h)^2) (A8), the term is <= (2^-22)^3 / 4 of the
+                        // self term m_i W(0) that every sum holds: it does not reach the sum's last bit
+                        sum2 = fma2(pk2(B.z, B.w), w, sum2);
                     }
                 }
                 float s0, s1;
                 upk2(sum2, s0, s1);
-                if (t < nt) s_part[share * kRhoTT + t] += s0 + s1;
+                float sum = s0 + s1;
+#pragma unroll
+                for (int o = kRhoL / 2; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+                if (sub == 0u && t < nt) s_part[t] += sum;
             }
             r = rn;
             cs = csn;
@@ -268,10 +265,7 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
         }
         __syncthreads();
         if ((uint32_t)tid < nt) {
-            float tot = s_part[tid];
-#pragma unroll
-            for (int sh = 1; sh < kRhoShares; ++sh) tot += s_part[sh * kRhoTT + tid];
-            rho[perm[t_slot[tid]]] = tot * norm;
+            rho[perm[t_slot[tid]]] = s_part[tid] * norm;
         }
     }
 }
