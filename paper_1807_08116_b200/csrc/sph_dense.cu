@@ -26,6 +26,7 @@
 // calls — and are drawn from a counter by a persistent grid (kDenseCtasPerSm CTAs per SM).
 // The density pass (a7) stays on the thread-per-slot walk everywhere: its pair term is ~15 instructions, so nothing is
 // won by compacting the accepted pairs, and the staged, binned walk measured slower (46 against 31 ms at config 4).
+#include <type_traits>
 #include "sph_dense_dev.cuh"
 
 namespace sphb {
@@ -40,7 +41,7 @@ constexpr int kMaxSeg = 6;                // pieces of stencil rows ("segments")
 constexpr int kDenseKS = kDenseK + 2 * kMaxSeg;   // + the even-slot alignment of the float2 array, per segment
 constexpr int kRounds = (kDenseK + kDenseThreads - 1) / kDenseThreads;
 using dense::kBins;
-constexpr int kQueue = 64;                // ring queue entries per warp
+constexpr int kQueue = 128;               // ring queue entries per warp: <= 31 left over + 64 pushed by a step
 
 struct DenseLayout {
     // byte offsets inside the dynamic shared memory block (all multiples of 16)
@@ -269,26 +270,34 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                     first += ncand;
                     const uint32_t T = G.T;
                     if (T == 0u) continue;
-                    // one step: 32 flat positions, one per lane; `in` is false only for the lanes past the end in the last step
-                    auto step = [&](uint32_t v16, bool in) {
-                        const uint32_t rel = in ? dense::candidate_offset(G, v16) : 0u;
+                    const uint32_t T16 = 16u * T;
+                    // one step: 64 flat positions, two per lane (v16 and v16 + 32 x 16): the two tests are independent
+                    // instruction streams, and the loop control and the queue's bookkeeping are paid once for both.
+                    // FULL: every lane's two positions are inside the list; else `in` says which are (a position past the
+                    // end still reads shared memory of this CTA: nothing is done with it)
+                    auto step = [&](uint32_t v16, auto full) {
+                        const uint32_t rel0 = dense::candidate_offset(G, v16), rel1 = dense::candidate_offset(G, v16 + 512u);
                         float dx, dy, dz;
-                        const float d2 = dist2_f32(pi, lds_f4(a_pos + rel), dx, dy, dz);
+                        const float d20 = dist2_f32(pi, lds_f4(a_pos + rel0), dx, dy, dz);
+                        const float d21 = dist2_f32(pi, lds_f4(a_pos + rel1), dx, dy, dz);
                         // d2 == 0: self, or a coincident pair (A9) — no contribution
-                        const bool ok = in && d2 < rc2 && d2 > 0.f;
-                        const unsigned m = __ballot_sync(0xffffffffu, ok);
-                        if (ok) sts_u32(a_q + ((qt + 4u * __popc(m & lt_mask)) & (4u * kQueue - 4u)), rel);
-                        qt += 4u * __popc(m);
-                        if (qt - qh >= 128u) {
+                        const bool ok0 = (decltype(full)::value || v16 < T16) && d20 < rc2 && d20 > 0.f;
+                        const bool ok1 = (decltype(full)::value || v16 + 512u < T16) && d21 < rc2 && d21 > 0.f;
+                        const unsigned m0 = __ballot_sync(0xffffffffu, ok0), m1 = __ballot_sync(0xffffffffu, ok1);
+                        if (ok0) sts_u32(a_q + ((qt + 4u * __popc(m0 & lt_mask)) & (4u * kQueue - 4u)), rel0);
+                        qt += 4u * __popc(m0);
+                        if (ok1) sts_u32(a_q + ((qt + 4u * __popc(m1 & lt_mask)) & (4u * kQueue - 4u)), rel1);
+                        qt += 4u * __popc(m1);
+                        while (qt - qh >= 128u) {
                             __syncwarp();
                             pair_term(lds_u32(a_q + ((qh + 4u * (uint32_t)lane) & (4u * kQueue - 4u))));
                             qh += 128u;
                         }
                     };
-                    const uint32_t T16 = 16u * T, full16 = T16 & ~511u;
+                    const uint32_t full16 = T16 & ~1023u;
                     uint32_t v16 = 16u * (uint32_t)lane;
-                    for (; v16 < full16; v16 += 512u) step(v16, true);     // v16 - 16 lane < full16 for every lane: uniform
-                    if (full16 != T16) step(v16, v16 < T16);
+                    for (; v16 < full16; v16 += 1024u) step(v16, std::true_type{});   // v16 - 16 lane < full16 for every lane: uniform
+                    if (full16 != T16) step(v16, std::false_type{});
                 }
                 if (qt != qh) {
                     __syncwarp();
