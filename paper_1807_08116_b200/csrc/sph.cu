@@ -227,7 +227,7 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
                     const float Pi = ci.x + cj.x + nu;                 // p_i/rho_i^2 + p_j/rho_j^2 + nu  (L95, A2)
                     f = pj.w * Pi * gmag;                              // m_j Pi |grad Wp| / |dr|
                 } else {
-                    f = hydro_pair<false>(vi, ci, pj.w, vj, cj, dx, dy, dz, d2, q, rv, mu, c_ij);
+                    f = hydro_pair(vi, ci, pj.w, vj, cj, dx, dy, dz, d2, q, rv, mu, c_ij);
                 }
                 if (CFL) {
                     d2min = fminf(d2min, d2);
@@ -274,6 +274,8 @@ int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, co
     q.gw_unit = (float)(-45.0 / (64.0 * 3.14159265358979323846));
     q.inv_h = 1.0f / p->h;
     q.rc2 = two_h * two_h;
+    q.two_h2 = (float)(2.0 * h * h);
+    q.beta2 = 2.0f * p->beta;
     const unsigned blocks = (unsigned)cdiv(n, 128);
     const GridDev gd = to_dev(g);
     const CflArgs c = cfl ? *cfl : CflArgs{};

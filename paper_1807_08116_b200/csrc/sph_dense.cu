@@ -241,16 +241,16 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                     const float4 pj = lds_f4(a_pos + rel);
                     const float4 vj = lds_f4(a_vel + rel);
                     const float2 cj = lds_f2(a_pc + (rel >> 1));
-                    float dx, dy, dz, rv, mu, c_ij;
+                    float dx, dy, dz, rv, mu;
                     const float d2 = dist2_f32(pi, pj, dx, dy, dz);
-                    const float f = hydro_pair<true>(vi, ci, pj.w, vj, cj, dx, dy, dz, d2, q, rv, mu, c_ij);
+                    const float f = hydro_pair_fast(vi, ci, pj.w, vj, cj, dx, dy, dz, d2, q, rv, mu);
                     ax = fmaf(-f, dx, ax);
                     ay = fmaf(-f, dy, ay);
                     az = fmaf(-f, dz, az);
-                    de = fmaf(0.5f * f, rv, de);   // 1/2 m_j Pi dv . grad W_p   (Eq. 11)
+                    de = fmaf(f, rv, de);   // m_j Pi dv . grad W_p: twice the term of Eq. 11, halved with the warp's sum
                     if (CFL) {
                         d2min = fminf(d2min, d2);
-                        cmax = fmaxf(cmax, c_ij);
+                        cmax = fmaxf(cmax, 0.5f * (ci.y + cj.y));
                         mumax = fmaxf(mumax, fabsf(mu));
                     }
                 };
@@ -308,7 +308,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                     // the four sums over the 32 lanes in FP64, as one butterfly: after the exchange over lane bit 4 a
                     // lane holds two of them, after bit 3 one; lanes 0, 8, 16, 24 end with a_x, a_y, a_z, de/dt
                     const bool hi16 = (lane & 16) != 0, hi8 = (lane & 8) != 0;
-                    const double dxs = (double)ax, dys = (double)ay, dzs = (double)az, des = (double)de;
+                    const double dxs = (double)ax, dys = (double)ay, dzs = (double)az, des = 0.5 * (double)de;
                     double k0 = hi16 ? dzs : dxs, k1 = hi16 ? des : dys;
                     const double s0 = hi16 ? dxs : dzs, s1 = hi16 ? dys : des;
                     k0 += __shfl_xor_sync(0xffffffffu, s0, 16);

@@ -1,7 +1,10 @@
-// sph_dev.cuh — device functions shared by the two SPH walks (sph.cu: thread per sorted slot, the sparse galaxy
-// grids; sph_dense.cu: CTA per populated cell, shared-memory staged, warp per target).  Both walks evaluate a pair
-// with exactly these operation sequences, so a pair's term is the same bits whichever walk reaches it; only the
-// order of a particle's sum differs.  Internal to libsph_b200; nothing here is shared with the oracle.
+// sph_dev.cuh — device functions of the SPH walks (sph.cu: thread per sorted slot, the sparse galaxy grids;
+// sph_dense.cu / sph_dense_rho.cu: CTA per populated cell, shared-memory staged).  The cutoff predicate (dist2_f32, A8)
+// and the cell assignment (cell_of, A7) are the same operation sequence everywhere, so every walk sees the same
+// neighbour set; the pair TERM has two forms — hydro_pair (sparse walk: few terms, all near the kernel edge, so FP64
+// numerator and IEEE divisions) and hydro_pair_fast (dense walk: many terms, MUFU reciprocals) — and which one a
+// particle's sum uses is decided by its cell's population alone (kDenseMin), so results stay reproducible.
+// Internal to libsph_b200; nothing here is shared with the oracle.
 #pragma once
 #include "common.cuh"
 
@@ -53,6 +56,7 @@ struct ViscDev {
     float eta, gw_unit;                 // VARH: eta and -45 / (64 pi); the h powers are applied per pair
     float inv_h;                        // 1 / h (IEEE division on the host side of the launch)
     float rc2;                          // fl(fl(2h)^2), the FP32 cutoff of A8
+    float two_h2, beta2;                // 2 h^2 and 2 beta (hydro_pair_fast)
 };
 
 // One accepted pair (d2 < 4h^2, d2 > 0) of Eqs. 10-11 with the one global h: returns f = m_j Pi_ij |grad W_p| / |dr| and
@@ -62,51 +66,60 @@ struct ViscDev {
 //   accuracy near the kernel edge (every term of a sparsely surrounded particle sits there), so the numerator alone is
 //   taken in FP64: 3 cvt + 3 DFMA per pair.
 //   grad W_p = dWp/dxi * dr/|dr| / h,  dWp/dxi = -45/(64 pi h^3) (2-xi)^2   (L95, Eq. 9, A3)
-// a / b for b > 0 in the normal range: reciprocal by MUFU.RCP and one Newton step (~1 ulp), 4 instructions against the
-// ~17 of the IEEE division with its range check
-__device__ __forceinline__ float div_newton(float a, float b) {
-    float r;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(b));
-    r = fmaf(r, fmaf(-b, r, 1.0f), r);
-    return a * r;
-}
-// FAST (the dense walk, where a particle's sum has tens to thousands of terms spread over the whole kernel support):
-// the three divisions by div_newton, MUFU.RSQ without its Newton step (2^-22 of pseudo-random error per term), and the
-// numerator 4h^2 - |dr|^2 in FP32 — its absolute error, <= 2 ulp of 4h^2, is that of any FP32 term; only the RELATIVE
-// error of a term at the kernel edge grows, which matters where ALL of a particle's few terms sit at the edge, i.e. in
-// the sparse walk, which keeps the FP64 numerator, the refined rsqrt and the IEEE divisions.
-template <bool FAST>
 __device__ __forceinline__ float hydro_pair(const float4 vi /*v, rho*/, const float2 ci /*p/rho^2, c*/, const float m_j,
                                             const float4 vj, const float2 cj, const float dx, const float dy,
                                             const float dz, const float d2, const ViscDev& q, float& rv, float& mu,
                                             float& c_ij) {
-    float rinv;
-    if (FAST) {
-        asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(d2));   // d2 > 0 and far from the denormals (d2 ~ h^2)
-    } else {
-        rinv = rsqrtf(d2);
-        rinv = rinv * fmaf(-0.5f * d2 * rinv, rinv, 1.5f);   // one Newton step: ~1 ulp
-    }
+    float rinv = rsqrtf(d2);
+    rinv = rinv * fmaf(-0.5f * d2 * rinv, rinv, 1.5f);   // one Newton step: ~1 ulp
     const float rr = d2 * rinv;                          // |dr|
-    float num;
-    if (FAST)
-        num = q.rc2 - d2;
-    else
-        num = (float)fma(-(double)dz, (double)dz, fma(-(double)dy, (double)dy, fma(-(double)dx, (double)dx, q.rc2_64)));
+    const float num = (float)fma(-(double)dz, (double)dz, fma(-(double)dy, (double)dy, fma(-(double)dx, (double)dx, q.rc2_64)));
     const float tqn = fmaxf(num, 0.0f) * q.inv_h2, tqd = 2.0f + rr * q.inv_h;
-    const float tq = FAST ? div_newton(tqn, tqd) : tqn / tqd;   // 2 - xi
+    const float tq = tqn / tqd;                          // 2 - xi
     const float gmag = q.gw * tq * tq * rinv;            // grad W_p = gmag * dr
     const float dvx = vi.x - vj.x, dvy = vi.y - vj.y, dvz = vi.z - vj.z;
     rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
     // mu_ij = h dr.dv / (|dr|^2 + eta h^2) if dr.dv < 0   (L97)
     const float mun = q.h * rv, mud = d2 + q.eta_h2;
-    mu = rv < 0.f ? (FAST ? div_newton(mun, mud) : mun / mud) : 0.f;
+    mu = rv < 0.f ? mun / mud : 0.f;
     const float rho_ij = 0.5f * (vi.w + vj.w);
     c_ij = 0.5f * (ci.y + cj.y);
     const float nun = mu * (q.beta * mu - q.alpha * c_ij);
-    const float nu = FAST ? div_newton(nun, rho_ij) : nun / rho_ij;
+    const float nu = nun / rho_ij;
     const float Pi = ci.x + cj.x + nu;                   // p_i/rho_i^2 + p_j/rho_j^2 + nu  (L95, A2)
     return m_j * Pi * gmag;                              // m_j Pi |grad Wp| / |dr|
+}
+
+// The dense walk's pair term (a particle's sum there has tens to thousands of terms spread over the whole kernel
+// support).  The same quantities as hydro_pair, arranged for the fewest instructions:
+//   2 - xi = (4h^2 - |dr|^2) / (2h^2 + h |dr|)                 numerator and denominator in FP32: the absolute error of
+//            the numerator, <= 2 ulp of 4h^2, is that of any FP32 term; only the RELATIVE error of a term at the kernel
+//            edge grows, which matters where ALL of a particle's few terms sit at the edge, i.e. in the sparse walk,
+//            which keeps the FP64 numerator, the refined rsqrt and the IEEE divisions;
+//   nu_ij  = mu (beta mu - alpha c_ij) / rho_ij = mu (2 beta mu - alpha (c_i + c_j)) / (rho_i + rho_j)   the two halves cancel;
+//   1/x by MUFU.RCP, 1/sqrt(x) by MUFU.RSQ, unrefined: relative error <= 2^-22 per term, pseudo-random in sign.
+// The accepted pair has 0 < d2 < rc2, so the numerator needs no clamp.  Returns f = m_j Pi_ij |grad W_p| / |dr|; rv, mu as
+// in hydro_pair.
+__device__ __forceinline__ float rcp_approx(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+__device__ __forceinline__ float hydro_pair_fast(const float4 vi /*v, rho*/, const float2 ci /*p/rho^2, c*/, const float m_j,
+                                                 const float4 vj, const float2 cj, const float dx, const float dy,
+                                                 const float dz, const float d2, const ViscDev& q, float& rv, float& mu) {
+    float rinv;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(d2));   // d2 > 0 and far from the denormals (d2 ~ h^2)
+    const float rr = d2 * rinv;                                    // |dr|
+    const float tq = (q.rc2 - d2) * rcp_approx(fmaf(rr, q.h, q.two_h2));   // 2 - xi
+    const float gmag = q.gw * tq * tq * rinv;                      // grad W_p = gmag * dr
+    const float dvx = vi.x - vj.x, dvy = vi.y - vj.y, dvz = vi.z - vj.z;
+    rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
+    mu = 0.f;
+    if (rv < 0.f) mu = q.h * rv * rcp_approx(d2 + q.eta_h2);       // mu_ij = h dr.dv / (|dr|^2 + eta h^2) if dr.dv < 0   (L97)
+    const float nun = mu * fmaf(q.beta2, mu, -q.alpha * (ci.y + cj.y));
+    const float Pi = fmaf(nun, rcp_approx(vi.w + vj.w), ci.x + cj.x);   // p_i/rho_i^2 + p_j/rho_j^2 + nu  (L95, A2)
+    return m_j * Pi * gmag;
 }
 
 // Eq. 17 (L127) for one gas particle: the bracket s / (c^max (1 + 1.2 alpha) + 1.2 beta mu^max + sqrt(s (|Q| + |E|))) from
