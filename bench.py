@@ -12,7 +12,8 @@ by torchrun it takes RANK / LOCAL_RANK / WORLD_SIZE from the environment.  Every
 its SHARE of the O(N^2) gravity stage (the paper's N/k-per-GPU decomposition, L139): on the
 pair-symmetric path (every BASELINE config from config 1 up) the work items rank, rank + N, ... with one int64 SUM
 all-reduce of the fixed-point sums per evaluation; on the one-sided path target slices with one all-gather of the
-acceleration rows.  Total work is fixed ("scaling": "strong").
+acceleration rows.  The SPH passes are shared as well: every N-th tile of 128 sorted slots per rank, rho
+and acc_sph completed by an int32 SUM all-reduce of the bit patterns.  Total work is fixed ("scaling": "strong").
 """
 from __future__ import annotations
 
@@ -42,7 +43,7 @@ def _peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
-def parallelism_text(world, path=None):
+def parallelism_text(world, path=None, share_sph=True):
     """What the N > 1 run does per force evaluation, from the gravity path the device chose (sph_gravity_path)."""
     if world <= 1:
         return "single GPU"
@@ -52,9 +53,12 @@ def parallelism_text(world, path=None):
         how = (f"gravity: unordered-pair work items rank, rank+{world}, ... per GPU + 1 int64 SUM all-reduce of the "
                f"fixed-point sums (24 B x N) per evaluation")
     elif path == "none":
-        how = "no gravity (G = 0): no collective"
+        how = "no gravity (G = 0): no gravity collective"
     else:
         how = f"gravity: target slices of N/{world} per GPU + 1 all-gather of the acceleration rows (16 B x N/{world} per GPU) per evaluation"
+    if share_sph:
+        return how + (f"; SPH passes: every {world}th tile of 128 sorted slots per GPU + 1 int32 SUM all-reduce of rho (4 B x N_g) "
+                      f"and of acc_sph (16 B x N_g) per pass; O(N) stages (sort, update) replicated")
     return how + "; O(N) and SPH stages replicated"
 
 
@@ -62,7 +66,7 @@ def workload_config(args, w, grid_dims=None, cells=None, world=1, path=None):
     """The `config` object of the JSON line: identical for both arms (ours / reference)."""
     src = f"BASELINE.json configs[{args.config}]" if args.config <= 4 else "SURVEY.md 8(f) NEXT-3 (collisionless, not a BASELINE config)"
     return {"workload": f"{src} ({w.name}): N={w.n_total}, N_g={w.n_gas}, h={w.h:g}, delta={w.delta:g}, dt={w.dt:g}",
-            "grid_dims": grid_dims, "cells": cells, "parallelism": parallelism_text(world, path),
+            "grid_dims": grid_dims, "cells": cells, "parallelism": parallelism_text(world, path, share_sph=w.n_gas > 0),
             "l2": "no flush: one step streams >300 MB (cell arrays, gravity partials, particle arrays) > 126 MB L2"}
 
 

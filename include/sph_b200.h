@@ -291,6 +291,44 @@ int sph_correct(float* vele, const float* hsml /*or NULL*/, int64_t n_gas, int64
                 const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/, float dt,
                 const float* rho, float* acc_sph, const float* acc_grav, void* ws, size_t ws_bytes, void* stream);
 
+/* ---- The SPH passes shared over the GPUs as well ("SPH by i-slices over a replicated sorted gas
+ * array"; every GPU holds all particles before a kernel runs, and computes its own N/k) ----
+ * Every rank sorts (SP is O(N), and its result — keys, perm, cell_start, the sorted copies in the workspace — is what
+ * the slices are cut from), then computes DC and HFC for ITS targets only: rank `rank` of `world` takes every world-th
+ * tile of 128 sorted slots, i.e. tiles rank, rank + world, ...; a populated cell walked by the dense-cell kernels
+ * (>= 32 particles) goes, 128 targets at a time, to the rank that owns the first slot of those targets.  Cutting the
+ * SORTED order interleaves dense and sparse regions over the ranks.  A target's sum is formed by one rank with the
+ * same kernel and in the same order as on one GPU, so the values are bit for bit those of the unsharded calls.
+ * The outputs (rho, acc_sph) are written in the caller's particle order: the rank's targets get their values, every
+ * other element is ZERO, so the caller completes them with one SUM all-reduce per pass — of the 32-bit patterns as
+ * integers (x + 0 + ... + 0, exact; paper_1807_08116_b200/sharded.py does this over NCCL).
+ *   sph_position_share_sph: as sph_position_share — SP in full, the rank's share of GFC — but DC for the rank's
+ *                           targets only (rho zero elsewhere) and hsml READ only: its renewal needs the complete rho.
+ *   sph_renew_hsml:         after rho is complete: h_i = sigma (m_i / rho_i)^(1/3) capped at p->h (L82, A25), and the
+ *                           cell-order copy in the workspace that the HFC passes read.  sigma > 0.
+ *   sph_forces_share:       HFC (Eqs. 10-11) for the rank's targets from the workspace's sorted state (the last
+ *                           position call's), acc_sph zero elsewhere.  Needs the COMPLETE rho.  hsml NULL: one global h.
+ *   sph_update:             SU alone, O(N), every rank for all particles: corrector = 0: Eqs. 12-14 (posm, vele
+ *                           advanced, the time-t state kept in the workspace); corrector = 1: Eqs. 15-16 (posm unused,
+ *                           may be NULL).  Needs the COMPLETE acc_sph and acc_grav.
+ * One step on k GPUs = [first: position_share_sph, exchange] ; forces_share, exchange ; update(0) ; position_share_sph,
+ * exchange, [renew_hsml] ; forces_share, exchange ; update(1) — the stages of sph_step_h in the same order.  The step
+ * criterion of Eq. 17 is not folded into the shared HFC (a MIN over the ranks would be one more collective): the shared
+ * step takes dt from the caller.
+ * Errors as for sph_position_share; world = 1 gives the unsharded result.  Asynchronous on `stream`.                 */
+int sph_position_share_sph(const float* posm, const float* hsml /*or NULL*/, int64_t n_gas, int64_t n_halo, int rank,
+                           int world, int64_t i0, int64_t i1, const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/,
+                           float* rho, float* acc_grav, void* ws, size_t ws_bytes, void* stream);
+int sph_renew_hsml(const float* posm, float* hsml, float sigma, int64_t n_gas, int64_t n_halo,
+                   const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/, const float* rho, void* ws, size_t ws_bytes,
+                   void* stream);
+int sph_forces_share(const float* vele, const float* hsml /*or NULL*/, int64_t n_gas, int64_t n_halo, int rank, int world,
+                     const sph_params* p /*HOST*/, const sph_grid* g /*HOST*/, const float* rho, float* acc_sph,
+                     void* ws, size_t ws_bytes, void* stream);
+int sph_update(float* posm /*or NULL if corrector*/, float* vele, int64_t n_gas, int64_t n_halo,
+               const sph_grid* g /*HOST, may be NULL if n_gas == 0*/, float dt, int corrector, const float* acc_sph,
+               const float* acc_grav, void* ws, size_t ws_bytes, void* stream);
+
 /* Stage timing: after sph_set_profiling(1) every stage the calling thread enqueues is bracketed
  * by CUDA events on the call's stream; sph_get_stage_ms() returns the milliseconds summed over all
  * calls since that switch-on (at most 4096 stage spans) for

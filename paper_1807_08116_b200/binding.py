@@ -28,6 +28,7 @@ EXPORTS = (
     "nbody_pp_gravity_slice", "sph_position_slice", "sph_predict", "sph_correct",
     "sph_gravity_path", "sph_dense_items", "sph_workspace_status", "sph_position_share", "nbody_pp_gravity_share", "nbody_pp_gravity_finish",
     "sph_workspace_gravity_sums", "sph_smoothing_lengths", "sph_density_h", "sph_forces_h", "sph_evaluate_h", "sph_step_h", "sph_neighbour_lists_h", "sph_step_cfl",
+    "sph_position_share_sph", "sph_renew_hsml", "sph_forces_share", "sph_update",
 )
 
 
@@ -96,6 +97,10 @@ def load():
     L.sph_position_share.argtypes = [vp, vp, f32, i64, i64, C.c_int, C.c_int, i64, i64, pp, gp, vp, vp, vp, sz, vp]
     L.nbody_pp_gravity_share.argtypes = [vp, i64, C.c_int, C.c_int, i64, i64, f32, f32, vp, vp, sz, vp]
     L.nbody_pp_gravity_finish.argtypes = [vp, i64, i64, gp, f32, vp, vp, sz, vp]
+    L.sph_position_share_sph.argtypes = [vp, vp, i64, i64, C.c_int, C.c_int, i64, i64, pp, gp, vp, vp, vp, sz, vp]
+    L.sph_renew_hsml.argtypes = [vp, vp, f32, i64, i64, pp, gp, vp, vp, sz, vp]
+    L.sph_forces_share.argtypes = [vp, vp, i64, i64, C.c_int, C.c_int, pp, gp, vp, vp, vp, sz, vp]
+    L.sph_update.argtypes = [vp, vp, i64, i64, gp, f32, C.c_int, vp, vp, vp, sz, vp]
     L.sph_workspace_gravity_sums.argtypes = [i64, i64, gp, C.POINTER(sz), C.POINTER(sz)]
     L.sph_gravity_path.argtypes = [vp, sz, i64, i64, gp, C.POINTER(C.c_int), vp]
     L.sph_dense_items.argtypes = [vp, sz, i64, i64, gp, C.POINTER(C.c_uint32), vp]
@@ -259,6 +264,36 @@ def gravity_sums_view(ws, n_gas, n_total, grid=None) -> torch.Tensor:
     _chk("sph_workspace_gravity_sums", load().sph_workspace_gravity_sums(int(n_gas), int(n_total), g, C.byref(off),
                                                                          C.byref(nbytes)))
     return ws[off.value:off.value + nbytes.value].view(torch.int64)
+
+
+# ---- the SPH passes shared as well: include/sph_b200.h
+def sph_position_share_sph(posm, hsml, n_gas, n_halo, rank, world, i0, i1, params, grid, rho, acc_grav, ws):
+    p, nb = _ws(ws)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_position_share_sph", load().sph_position_share_sph(_ptr(posm), _ptr(hsml), int(n_gas), int(n_halo), int(rank),
+                                                                 int(world), int(i0), int(i1), C.byref(params), g, _ptr(rho),
+                                                                 _ptr(acc_grav), p, nb, _stream()))
+
+
+def sph_renew_hsml(posm, hsml, sigma, n_gas, n_halo, params, grid, rho, ws):
+    p, nb = _ws(ws)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_renew_hsml", load().sph_renew_hsml(_ptr(posm), _ptr(hsml), float(sigma), int(n_gas), int(n_halo),
+                                                 C.byref(params), g, _ptr(rho), p, nb, _stream()))
+
+
+def sph_forces_share(vele, hsml, n_gas, n_halo, rank, world, params, grid, rho, acc_sph, ws):
+    p, nb = _ws(ws)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_forces_share", load().sph_forces_share(_ptr(vele), _ptr(hsml), int(n_gas), int(n_halo), int(rank), int(world),
+                                                     C.byref(params), g, _ptr(rho), _ptr(acc_sph), p, nb, _stream()))
+
+
+def sph_update(posm, vele, n_gas, n_halo, grid, dt, corrector, acc_sph, acc_grav, ws):
+    p, nb = _ws(ws)
+    g = C.byref(grid) if grid is not None else None
+    _chk("sph_update", load().sph_update(_ptr(posm), _ptr(vele), int(n_gas), int(n_halo), g, float(dt), int(bool(corrector)),
+                                         _ptr(acc_sph), _ptr(acc_grav), p, nb, _stream()))
 
 
 def sph_position_slice(posm, hsml, sigma, n_gas, n_halo, i0, i1, params, grid, rho, acc_grav, ws):

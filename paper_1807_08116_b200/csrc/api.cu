@@ -50,7 +50,9 @@ int check_params(const sph_params* p, bool need_h) {
 // (gravity_share); the caller exchanges and then calls nbody_pp_gravity_finish.
 int position_only(const float4* posm, float* hsml, float sigma, int64_t n_gas, int64_t n_total, int64_t i0, int64_t i1,
                   const sph_params* p, const sph_grid* g, float* rho, float4* acc_grav, const Workspace& w,
-                  cudaStream_t st, int rank = 0, int world = 0) {
+                  cudaStream_t st, int rank = 0, int world = 0, bool share_dc = false) {
+    // share_dc: DC for the rank's targets only (common.cuh: Shard), rho = 0 for the others — the caller adds rho over the ranks
+    const Shard sh = share_dc ? Shard{(uint32_t)rank, (uint32_t)world} : Shard{0u, 1u};
     if (n_gas > 0) {
         {
             Span sp(ST_SORT, st);
@@ -60,7 +62,8 @@ int position_only(const float4* posm, float* hsml, float sigma, int64_t n_gas, i
         }
         {
             Span sp(ST_DENSITY, st);
-            SPHB_TRY(density_sorted(w.posm_s, hsml ? w.h_s : nullptr, w.perm, w.cell_start, n_gas, p, g, &w.dense, rho, st));
+            if (sh.world > 1u) SPHB_CUDA(cudaMemsetAsync(rho, 0, (size_t)n_gas * sizeof(float), st));
+            SPHB_TRY(density_sorted(w.posm_s, hsml ? w.h_s : nullptr, w.perm, w.cell_start, n_gas, p, g, &w.dense, rho, st, sh));
             if (hsml && sigma > 0.f) {
                 SPHB_TRY(smoothing_lengths(posm, rho, n_gas, sigma, p->h, hsml, st));
                 SPHB_TRY(gather_sorted_h(hsml, w.perm, n_gas, p->h, w.status, w.h_s, st));
@@ -79,11 +82,12 @@ int position_only(const float4* posm, float* hsml, float sigma, int64_t n_gas, i
 }
 
 int hydro(const float4* vele, const float* rho, bool varh, int64_t n_gas, const sph_params* p, const sph_grid* g,
-          float4* acc_sph, const Workspace& w, cudaStream_t st, const CflArgs* cfl = nullptr) {
+          float4* acc_sph, const Workspace& w, cudaStream_t st, const CflArgs* cfl = nullptr, Shard sh = Shard{0u, 1u}) {
     if (n_gas <= 0) return SPH_OK;
     Span sp(ST_FORCES, st);
+    if (sh.world > 1u) SPHB_CUDA(cudaMemsetAsync(acc_sph, 0, (size_t)n_gas * sizeof(float4), st));
     return forces_sorted(w.posm_s, vele, rho, varh ? w.h_s : nullptr, w.perm, w.cell_start, n_gas, p, g, &w.dense, cfl,
-                         w.velr_s, w.pc_s, acc_sph, st);
+                         w.velr_s, w.pc_s, acc_sph, st, sh);
 }
 
 int check_state_args(const void* posm, const void* vele, int64_t n_gas, int64_t n_halo, const sph_params* p,
@@ -381,6 +385,76 @@ int nbody_pp_gravity_finish(const float* posm, int64_t n_gas, int64_t n_halo, co
     Span sp(ST_GRAVITY, st);
     return gravity_finish(reinterpret_cast<const float4*>(posm), n, G, reinterpret_cast<float4*>(acc_grav), w.grav_acc64,
                           w.grav_flag, st);
+}
+
+// ---- the SPH passes shared as well ----
+int sph_position_share_sph(const float* posm, const float* hsml, int64_t n_gas, int64_t n_halo, int rank, int world,
+                           int64_t i0, int64_t i1, const sph_params* p, const sph_grid* g, float* rho, float* acc_grav,
+                           void* ws, size_t ws_bytes, void* stream) {
+    if (bad_count(n_gas) || bad_count(n_halo) || bad_count(n_gas + n_halo)) return SPH_ERR_ARG;
+    const int64_t n = n_gas + n_halo;
+    if (world < 1 || rank < 0 || rank >= world || i0 < 0 || i1 < i0 || i1 > n) return SPH_ERR_ARG;
+    SPHB_TRY(check_params(p, n_gas > 0));
+    if (n == 0) return SPH_OK;
+    if (!posm || !acc_grav || !aligned16(posm) || !aligned16(acc_grav) || (n_gas > 0 && !rho)) return SPH_ERR_ARG;
+    if (n_gas > 0) SPHB_TRY(check_grid(g, p->h));
+    if (!ws || (reinterpret_cast<uintptr_t>(ws) & 255u)) return SPH_ERR_ARG;
+    Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    // sigma = 0: hsml is read only (its renewal needs the complete rho: sph_renew_hsml, after the exchange)
+    return position_only(reinterpret_cast<const float4*>(posm), n_gas > 0 ? const_cast<float*>(hsml) : nullptr, 0.f, n_gas, n,
+                         i0, i1, p, g, rho, reinterpret_cast<float4*>(acc_grav), w, (cudaStream_t)stream, rank, world, true);
+}
+
+int sph_renew_hsml(const float* posm, float* hsml, float sigma, int64_t n_gas, int64_t n_halo, const sph_params* p,
+                   const sph_grid* g, const float* rho, void* ws, size_t ws_bytes, void* stream) {
+    if (bad_count(n_gas) || bad_count(n_halo) || bad_count(n_gas + n_halo) || !(sigma > 0.f)) return SPH_ERR_ARG;
+    SPHB_TRY(check_params(p, n_gas > 0));
+    if (n_gas == 0) return SPH_OK;
+    if (!posm || !hsml || !rho || !aligned16(posm) || !ws || (reinterpret_cast<uintptr_t>(ws) & 255u)) return SPH_ERR_ARG;
+    SPHB_TRY(check_grid(g, p->h));
+    Workspace w = carve(ws, n_gas, n_gas + n_halo, g);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    Span sp(ST_DENSITY, st);
+    SPHB_TRY(smoothing_lengths(reinterpret_cast<const float4*>(posm), rho, n_gas, sigma, p->h, hsml, st));
+    return gather_sorted_h(hsml, w.perm, n_gas, p->h, w.status, w.h_s, st);
+}
+
+int sph_forces_share(const float* vele, const float* hsml, int64_t n_gas, int64_t n_halo, int rank, int world,
+                     const sph_params* p, const sph_grid* g, const float* rho, float* acc_sph, void* ws, size_t ws_bytes,
+                     void* stream) {
+    if (bad_count(n_gas) || bad_count(n_halo) || bad_count(n_gas + n_halo) || world < 1 || rank < 0 || rank >= world)
+        return SPH_ERR_ARG;
+    SPHB_TRY(check_params(p, n_gas > 0));
+    if (n_gas == 0) return SPH_OK;
+    if (!vele || !rho || !acc_sph || !aligned16(vele) || !aligned16(acc_sph) || !ws || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return SPH_ERR_ARG;
+    SPHB_TRY(check_grid(g, p->h));
+    Workspace w = carve(ws, n_gas, n_gas + n_halo, g);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    return hydro(reinterpret_cast<const float4*>(vele), rho, hsml != nullptr, n_gas, p, g, reinterpret_cast<float4*>(acc_sph), w,
+                 (cudaStream_t)stream, nullptr, Shard{(uint32_t)rank, (uint32_t)world});
+}
+
+int sph_update(float* posm, float* vele, int64_t n_gas, int64_t n_halo, const sph_grid* g, float dt, int corrector,
+               const float* acc_sph, const float* acc_grav, void* ws, size_t ws_bytes, void* stream) {
+    if (bad_count(n_gas) || bad_count(n_halo) || bad_count(n_gas + n_halo) || (n_gas > 0 && !g)) return SPH_ERR_ARG;
+    const int64_t n = n_gas + n_halo;
+    if (n == 0) return SPH_OK;
+    if (!vele || !acc_grav || (!corrector && !posm) || (n_gas > 0 && !acc_sph) || !aligned16(vele) || !aligned16(acc_grav) ||
+        (posm && !aligned16(posm)) || (acc_sph && !aligned16(acc_sph)) || !ws || (reinterpret_cast<uintptr_t>(ws) & 255u))
+        return SPH_ERR_ARG;
+    Workspace w = carve(ws, n_gas, n, n_gas > 0 ? g : nullptr);
+    if (ws_bytes < w.bytes) return SPH_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    Span sp(ST_UPDATE, st);
+    if (corrector)
+        return update_corrector(reinterpret_cast<float4*>(vele), w.vele0, reinterpret_cast<const float4*>(acc_sph),
+                                reinterpret_cast<const float4*>(acc_grav), n_gas, n, dt, nullptr, st);   // Eqs. 15-16
+    return update_predictor(reinterpret_cast<float4*>(posm), reinterpret_cast<float4*>(vele), w.vele0,
+                            reinterpret_cast<const float4*>(acc_sph), reinterpret_cast<const float4*>(acc_grav), n_gas, n, dt,
+                            nullptr, st);                                                                 // Eqs. 12-14
 }
 
 int sph_workspace_gravity_sums(int64_t n_gas, int64_t n_total, const sph_grid* g, size_t* offset_host, size_t* bytes_host) {

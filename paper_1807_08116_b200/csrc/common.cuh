@@ -62,6 +62,14 @@ struct DenseItem {
     uint32_t key;     // cell number
     uint32_t chunk;   // targets [start[key] + chunk kDenseTT, ... + kDenseTT) of that cell
 };
+// The SPH passes shared over several GPUs (targets in slices of the sorted order over the replicated
+// sorted arrays): rank `rank` of `world` takes every world-th tile of 128 sorted slots — a thread-per-slot
+// CTA, or a dense work item by its first slot — and leaves the other targets' outputs untouched.  {0, 1}: everything.
+struct Shard {
+    uint32_t rank, world;
+    __host__ __device__ bool owns(uint32_t first_slot) const { return ((first_slot >> 7) % world) == rank; }
+};
+
 struct DenseList {
     unsigned int* ctl;   // device: ctl[0] = number of items
     DenseItem* items;    // device: [dense_capacity(n_gas)]
@@ -127,11 +135,12 @@ int gather_sorted_pos(const float4* posm, const uint32_t* perm, int64_t n_gas, f
 // by the thread-per-slot kernel)
 int density_sorted(const float4* posm_s, const float* h_s, const uint32_t* perm, const uint32_t* cell_start,
                    int64_t n_gas, const sph_params* p, const sph_grid* g, const DenseList* dense, float* rho,
-                   cudaStream_t st);
+                   cudaStream_t st, Shard sh = Shard{0u, 1u});
 int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const float* h_s, const uint32_t* perm,
                   const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
                   const DenseList* dense, const CflArgs* cfl /*or NULL*/, float4* velr_s, float2* pc_s,
-                  float4* acc_sph /*or NULL with cfl: only the step criterion is wanted*/, cudaStream_t st);
+                  float4* acc_sph /*or NULL with cfl: only the step criterion is wanted*/, cudaStream_t st,
+                  Shard sh = Shard{0u, 1u});
 int cfl_init(float* dt_dev, float dt_max, cudaStream_t st);   // *dt_dev = dt_max (+inf: no ceiling)
 int smoothing_lengths(const float4* posm, const float* rho, int64_t n_gas, float sigma, float h_max, float* hsml,
                       cudaStream_t st);

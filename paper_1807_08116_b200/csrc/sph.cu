@@ -42,8 +42,8 @@ template <bool VARH>
 __global__ void __launch_bounds__(128) k_density(const float4* __restrict__ posm_s, const float* __restrict__ h_s,
                                                  const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start,
                                                  int n, GridDev g, float rc2, float inv_h, float norm,
-                                                 uint32_t dense_min, float* __restrict__ rho) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+                                                 uint32_t dense_min, Shard sh, float* __restrict__ rho) {
+    const int s = (int)((blockIdx.x * sh.world + sh.rank) * 128u + threadIdx.x);   // the rank's tiles of 128 slots
     if (s >= n) return;
     const float4 pi = posm_s[s];
     const float h_i = VARH ? h_s[s] : 0.f;
@@ -111,29 +111,36 @@ int gather_sorted_h(const float* hsml, const uint32_t* perm, int64_t n_gas, floa
 
 int forces_dense(const float4* posm_s, const float4* velr_s, const float2* pc_s, const uint32_t* perm,
                  const uint32_t* cell_start, const sph_grid* g, float rc2, const ViscDev& q, const DenseList& dl,
-                 const CflArgs* cfl, float4* acc_sph, cudaStream_t st);   // sph_dense.cu
+                 const CflArgs* cfl, float4* acc_sph, cudaStream_t st, Shard sh);   // sph_dense.cu
 
 int density_dense(const float4* posm_s, const uint32_t* perm, const uint32_t* cell_start, const sph_params* p,
-                  const sph_grid* g, const DenseList& dl, float* rho, cudaStream_t st);   // sph_dense_rho.cu
+                  const sph_grid* g, const DenseList& dl, float* rho, cudaStream_t st, Shard sh);   // sph_dense_rho.cu
+
+// CTAs of a thread-per-slot pass: the rank's tiles rank, rank + world, ... of the cdiv(n, 128)
+static unsigned shard_blocks(int64_t n, Shard sh) {
+    const int64_t tiles = cdiv(n, 128);
+    return tiles > (int64_t)sh.rank ? (unsigned)((tiles - sh.rank + sh.world - 1) / sh.world) : 0u;
+}
 
 int density_sorted(const float4* posm_s, const float* h_s /*cell order, or NULL: global h*/, const uint32_t* perm,
                    const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
-                   const DenseList* dense, float* rho, cudaStream_t st) {
+                   const DenseList* dense, float* rho, cudaStream_t st, Shard sh) {
     if (n_gas <= 0) return SPH_OK;
     const float two_h = 2.0f * p->h;
     const float rc2 = two_h * two_h;
     const float inv_h = 1.0f / p->h;
-    const unsigned blocks = (unsigned)cdiv(n_gas, 128);
+    const unsigned blocks = shard_blocks(n_gas, sh);
+    if (blocks == 0u) return SPH_OK;
     if (h_s) {
         k_density<true><<<blocks, 128, 0, st>>>(posm_s, h_s, perm, cell_start, (int)n_gas, to_dev(g), rc2, inv_h,
-                                                (float)(1.0 / 3.14159265358979323846), 0u, rho);
+                                                (float)(1.0 / 3.14159265358979323846), 0u, sh, rho);
         SPHB_LAUNCHED();
     } else {
         const float norm = (float)(1.0 / (3.14159265358979323846 * (double)p->h * (double)p->h * (double)p->h));
         k_density<false><<<blocks, 128, 0, st>>>(posm_s, nullptr, perm, cell_start, (int)n_gas, to_dev(g), rc2, inv_h,
-                                                 norm, dense ? (uint32_t)kDenseMin : 0u, rho);
+                                                 norm, dense ? (uint32_t)kDenseMin : 0u, sh, rho);
         SPHB_LAUNCHED();
-        if (dense) SPHB_TRY(density_dense(posm_s, perm, cell_start, p, g, *dense, rho, st));
+        if (dense) SPHB_TRY(density_dense(posm_s, perm, cell_start, p, g, *dense, rho, st, sh));
     }
     return SPH_OK;
 }
@@ -176,8 +183,8 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
                                                 const float2* __restrict__ pc_s, const float* __restrict__ h_s,
                                                 const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start,
                                                 int n, GridDev g, float rc2, ViscDev q, uint32_t dense_min, CflArgs cfl,
-                                                float4* __restrict__ acc) {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+                                                Shard sh, float4* __restrict__ acc) {
+    const int s = (int)((blockIdx.x * sh.world + sh.rank) * 128u + threadIdx.x);   // the rank's tiles of 128 slots
     if (s >= n) return;
     const float4 pi = posm_s[s];
     int ix, iy, iz;
@@ -255,7 +262,7 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
 int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, const float* h_s /*or NULL*/,
                   const uint32_t* perm, const uint32_t* cell_start, int64_t n_gas, const sph_params* p, const sph_grid* g,
                   const DenseList* dense, const CflArgs* cfl, float4* velr_s, float2* pc_s, float4* acc_sph,
-                  cudaStream_t st) {
+                  cudaStream_t st, Shard sh) {
     if (n_gas <= 0) return SPH_OK;
     const int n = (int)n_gas;
     k_eos_gather<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(vele, rho, perm, n, p->gamma, velr_s, pc_s);
@@ -276,20 +283,21 @@ int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, co
     q.rc2 = two_h * two_h;
     q.two_h2 = (float)(2.0 * h * h);
     q.beta2 = 2.0f * p->beta;
-    const unsigned blocks = (unsigned)cdiv(n, 128);
+    const unsigned blocks = shard_blocks(n_gas, sh);
+    if (blocks == 0u) return SPH_OK;
     const GridDev gd = to_dev(g);
     const CflArgs c = cfl ? *cfl : CflArgs{};
     const uint32_t dmin = (dense && !h_s) ? (uint32_t)kDenseMin : 0u;
     if (h_s && cfl)
-        k_forces<true, true><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, h_s, perm, cell_start, n, gd, q.rc2, q, 0u, c, acc_sph);
+        k_forces<true, true><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, h_s, perm, cell_start, n, gd, q.rc2, q, 0u, c, sh, acc_sph);
     else if (h_s)
-        k_forces<true, false><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, h_s, perm, cell_start, n, gd, q.rc2, q, 0u, c, acc_sph);
+        k_forces<true, false><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, h_s, perm, cell_start, n, gd, q.rc2, q, 0u, c, sh, acc_sph);
     else if (cfl)
-        k_forces<false, true><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, nullptr, perm, cell_start, n, gd, q.rc2, q, dmin, c, acc_sph);
+        k_forces<false, true><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, nullptr, perm, cell_start, n, gd, q.rc2, q, dmin, c, sh, acc_sph);
     else
-        k_forces<false, false><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, nullptr, perm, cell_start, n, gd, q.rc2, q, dmin, c, acc_sph);
+        k_forces<false, false><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, nullptr, perm, cell_start, n, gd, q.rc2, q, dmin, c, sh, acc_sph);
     SPHB_LAUNCHED();
-    if (dmin) SPHB_TRY(forces_dense(posm_s, velr_s, pc_s, perm, cell_start, g, q.rc2, q, *dense, cfl, acc_sph, st));
+    if (dmin) SPHB_TRY(forces_dense(posm_s, velr_s, pc_s, perm, cell_start, g, q.rc2, q, *dense, cfl, acc_sph, st, sh));
     return SPH_OK;
 }
 

@@ -76,7 +76,7 @@ template <bool CFL>
 __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
     k_dense_forces(const float4* __restrict__ posm_s, const float4* __restrict__ velr_s, const float2* __restrict__ pc_s,
             const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start, GridDev g, float cell, float rc2,
-            ViscDev q, CflArgs cfl, unsigned int* __restrict__ ctl, const DenseItem* __restrict__ items,
+            ViscDev q, CflArgs cfl, Shard sh, unsigned int* __restrict__ ctl, const DenseItem* __restrict__ items,
             float4* __restrict__ acc_out) {
     using L = DenseLayout;
     extern __shared__ __align__(128) unsigned char smem[];
@@ -169,6 +169,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
         const uint32_t mx = (uint32_t)g.mx, my = (uint32_t)g.my;
         const int ix = (int)(it.key % mx), iy = (int)((it.key / mx) % my), iz = (int)(it.key / (mx * my));
         const uint32_t ts = start[it.key] + it.chunk * kDenseTT;
+        if (!sh.owns(ts)) continue;   // another rank's targets (common.cuh: Shard)
         const uint32_t nt = min(start[it.key + 1u] - ts, (uint32_t)kDenseTT);
         if (tid < 9) dense::row_bounds(start, g, ix, iy, iz, tid, s_runs);
         for (uint32_t t = tid; t < nt; t += kDenseThreads) {
@@ -372,7 +373,7 @@ int dense_list_from_start(const uint32_t* cell_start, const sph_grid* g, const D
 
 int forces_dense(const float4* posm_s, const float4* velr_s, const float2* pc_s, const uint32_t* perm,
                  const uint32_t* cell_start, const sph_grid* g, float rc2, const ViscDev& q, const DenseList& dl,
-                 const CflArgs* cfl, float4* acc_sph, cudaStream_t st) {
+                 const CflArgs* cfl, float4* acc_sph, cudaStream_t st, Shard sh) {
     int dev = 0;
     SPHB_CUDA(cudaGetDevice(&dev));
     static std::atomic<bool> opted[64];   // per device: the dynamic shared-memory opt-in
@@ -387,10 +388,10 @@ int forces_dense(const float4* posm_s, const float4* velr_s, const float2* pc_s,
     SPHB_CUDA(cudaMemsetAsync(dl.ctl + 1, 0, sizeof(unsigned int), st));   // the item counter
     if (cfl)
         k_dense_forces<true><<<kDenseCtasPerSm * num_sms(), kDenseThreads, DenseLayout::bytes, st>>>(
-            posm_s, velr_s, pc_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, rc2, q, *cfl, dl.ctl, dl.items, acc_sph);
+            posm_s, velr_s, pc_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, rc2, q, *cfl, sh, dl.ctl, dl.items, acc_sph);
     else
         k_dense_forces<false><<<kDenseCtasPerSm * num_sms(), kDenseThreads, DenseLayout::bytes, st>>>(
-            posm_s, velr_s, pc_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, rc2, q, CflArgs{}, dl.ctl, dl.items, acc_sph);
+            posm_s, velr_s, pc_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, rc2, q, CflArgs{}, sh, dl.ctl, dl.items, acc_sph);
     SPHB_LAUNCHED();
     return SPH_OK;
 }

@@ -61,7 +61,7 @@ static_assert((RhoLayout::bytes + 1024) * kRhoCtasPerSm <= 227 * 1024, "shared m
 
 __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
     k_dense_density(const float4* __restrict__ posm_s, const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start,
-                    GridDev g, float cell, float rc2, float neg_inv_h, float norm, unsigned int* __restrict__ ctl,
+                    GridDev g, float cell, float rc2, float neg_inv_h, float norm, Shard sh, unsigned int* __restrict__ ctl,
                     const DenseItem* __restrict__ items, float* __restrict__ rho) {
     using L = RhoLayout;
     extern __shared__ __align__(128) unsigned char smem[];
@@ -123,6 +123,7 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
         const uint32_t mx = (uint32_t)g.mx, my = (uint32_t)g.my;
         const int ix = (int)(it.key % mx), iy = (int)((it.key / mx) % my), iz = (int)(it.key / (mx * my));
         const uint32_t ts = start[it.key] + it.chunk * kDenseTT;
+        if (!sh.owns(ts)) continue;   // another rank's targets (common.cuh: Shard)
         const uint32_t nt = min(start[it.key + 1u] - ts, (uint32_t)kRhoTT);
         if (tid < 9) dense::row_bounds(start, g, ix, iy, iz, tid, s_runs);
 
@@ -273,7 +274,7 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
 }  // namespace
 
 int density_dense(const float4* posm_s, const uint32_t* perm, const uint32_t* cell_start, const sph_params* p,
-                  const sph_grid* g, const DenseList& dl, float* rho, cudaStream_t st) {
+                  const sph_grid* g, const DenseList& dl, float* rho, cudaStream_t st, Shard sh) {
     int dev = 0;
     SPHB_CUDA(cudaGetDevice(&dev));
     static std::atomic<bool> opted[64];   // per device: the dynamic shared-memory opt-in
@@ -286,7 +287,7 @@ int density_dense(const float4* posm_s, const uint32_t* perm, const uint32_t* ce
     const float norm = (float)(1.0 / (3.14159265358979323846 * (double)p->h * (double)p->h * (double)p->h));
     SPHB_CUDA(cudaMemsetAsync(dl.ctl + 1, 0, sizeof(unsigned int), st));   // the item counter
     k_dense_density<<<kRhoCtasPerSm * num_sms(), kRhoThreads, RhoLayout::bytes, st>>>(
-        posm_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, two_h * two_h, -(1.0f / p->h), norm, dl.ctl, dl.items, rho);
+        posm_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, two_h * two_h, -(1.0f / p->h), norm, sh, dl.ctl, dl.items, rho);
     SPHB_LAUNCHED();
     return SPH_OK;
 }

@@ -61,8 +61,10 @@ def test_config_is_shared_by_both_arms():
     sym = bench.workload_config(a, w, [3, 4, 5], 60, 2, "pair_symmetric")["parallelism"]
     one = bench.workload_config(a, w, [3, 4, 5], 60, 2, "one_sided_uniform")["parallelism"]
     assert "int64 SUM all-reduce" in sym and "all-gather" not in sym
-    assert "all-gather" in one and "all-reduce" not in one and "N/2 per GPU" in one
-    assert "no collective" in bench.workload_config(a, w, [3, 4, 5], 60, 2, "none")["parallelism"]
+    assert "all-gather" in one and "int64" not in one and "N/2 per GPU" in one
+    assert "no gravity collective" in bench.workload_config(a, w, [3, 4, 5], 60, 2, "none")["parallelism"]
+    # the SPH passes are shared as well: tiles of the sorted order + an all-reduce of rho and of acc_sph per pass
+    assert "int32 SUM all-reduce of rho" in sym and "int32 SUM all-reduce of rho" in one
 
 
 # ---------------------------------------------------------------- NEXT-4: slices and the exchange (host logic)
@@ -188,6 +190,27 @@ class _StubBinding:
     def sph_correct(self, *a):
         self.calls.append("correct")
 
+    # ---- the SPH passes shared as well: the rank's targets (here: every world-th element) get a rank-tagged value, the
+    # others ZERO, as the library writes them; the update call records what it was handed
+    def sph_position_share_sph(self, posm, hsml, n_gas, n_halo, rank, world, i0, i1, params, grid, rho, acc_grav, ws):
+        self.sph_position_share(posm, hsml, 0.0, n_gas, n_halo, rank, world, i0, i1, params, grid, rho, acc_grav, ws)
+        self.calls[-1] = "share_sph"
+        rho.zero_()
+        rho[rank:n_gas:world] = 10.0 + rank
+
+    def sph_forces_share(self, vele, hsml, n_gas, n_halo, rank, world, params, grid, rho, acc_sph, ws):
+        self.calls.append("forces_share")
+        self.rho_seen = rho.clone()
+        acc_sph.zero_()
+        acc_sph[rank:n_gas:world] = -1.5 - rank
+
+    def sph_update(self, posm, vele, n_gas, n_halo, grid, dt, corrector, acc_sph, acc_grav, ws):
+        self.calls.append("update1" if corrector else "update0")
+        self.acc_sph_seen = acc_sph.clone()
+
+    def sph_renew_hsml(self, *a):
+        self.calls.append("renew_hsml")
+
 
 def _sharded_worker(rank, world, port, out):
     sys.path.insert(0, ROOT)
@@ -203,10 +226,16 @@ def _sharded_worker(rank, world, port, out):
         res = {}
         for sym in (True, False):
             stub = _StubBinding(sym)
-            sim = ShardedSimulation(w, rank, world, binding=stub, device="cpu")
+            sim = ShardedSimulation(w, rank, world, binding=stub, device="cpu", share_sph=False)
             sim.step()
             sums, acc = stub.seen
             res[sym] = (stub.calls, sums.numpy(), acc[:n].numpy(), (sim.i0, sim.i1))
+        # the SPH passes shared as well (the default for world > 1), with per-particle smoothing lengths
+        stub = _StubBinding(True)
+        sim = ShardedSimulation(w, rank, world, binding=stub, device="cpu", sigma=1.3)
+        assert sim.share_sph
+        sim.step()
+        res["sph"] = (stub.calls, stub.rho_seen.numpy(), stub.acc_sph_seen.numpy(), stub.seen[0].numpy())
         out[rank] = res
     finally:
         dist.destroy_process_group()
@@ -237,6 +266,18 @@ def test_sharded_step_exchange_gloo_world2():
                 assert b0[0] == 0 and b0[1] == b1[0] and b1[1] == 2500       # the slices tile [0, n)
                 assert np.all(acc[b0[0]:b0[1]] == 1.0) and np.all(acc[b1[0]:b1[1]] == 2.0)
     assert np.array_equal(out[0][True][1], out[1][True][1]) and np.array_equal(out[0][False][2], out[1][False][2])
+    # SPH passes shared: per evaluation share -> rho completed over the ranks (-> hsml renewed, after the seeding) ->
+    # gravity exchange -> finish; per half step forces share -> acc_sph completed -> update.  What the forces and the
+    # update calls see is EVERY rank's values, bit for bit (the all-reduce adds the bit patterns to zeros)
+    for rank in range(world):
+        calls, rho_seen, acc_seen, sums = out[rank]["sph"]
+        assert calls == ["share_sph", "path", "finish", "forces_share", "update0",
+                         "share_sph", "renew_hsml", "path", "finish", "forces_share", "update1"]
+        assert np.array_equal(rho_seen[0:1000:2], np.full(500, 10.0, np.float32))
+        assert np.array_equal(rho_seen[1:1000:2], np.full(500, 11.0, np.float32))
+        assert np.array_equal(acc_seen[0:1000:2], np.full((500, 4), -1.5, np.float32))
+        assert np.array_equal(acc_seen[1:1000:2], np.full((500, 4), -2.5, np.float32))
+        assert np.array_equal(sums, 3 * k)
 
 
 # ---------------------------------------------------------------- `python bench.py --gpus N` starts its own ranks
@@ -274,5 +315,6 @@ def test_bench_launch_ranks_world2_gloo(tmp_path):
     assert len(lines) == 1                                   # rank 0 alone reports
     d = json.loads(lines[0])
     assert d["n_gpus"] == 2 and d["ranks_seen"] == [0, 1] and d["value"] == 15.0      # max over ranks of 10, 15
-    assert d["calls"] == ["share", "path", "finish", "predict", "share", "path", "finish", "correct"]
+    assert d["calls"] == ["share_sph", "path", "finish", "forces_share", "update0",
+                          "share_sph", "path", "finish", "forces_share", "update1"]
     assert d["parallelism"] == bench.parallelism_text(2, "pair_symmetric")

@@ -842,6 +842,86 @@ def test_staged_step_shares_sequential(cuda_lib, world):
             assert torch.equal(x, y)
 
 
+def _complete(reps, name, n):
+    """What sharded.allreduce_bits does, by plain copies on one GPU: SUM of the 32-bit patterns as integers.  Also checks
+    what makes that exact: every element was written (non-zero) by at most one replica."""
+    parts = [getattr(s, name)[:n] for s in reps]
+    writers = sum((p != 0).to(torch.int32) for p in parts)
+    assert int(writers.max()) <= 1
+    total = sum(p.contiguous().view(torch.int32) for p in parts).view(torch.float32)
+    for p in parts:
+        p.copy_(total)
+    return writers
+
+
+@pytest.mark.parametrize("case,world,sigma", [("galaxy1", 2, None), ("tight_clumps", 3, None), ("packed", 2, None),
+                                               ("galaxy0", 3, 1.3)])
+def test_sph_passes_shared_sequential(cuda_lib, case, world, sigma):
+    """the SPH passes shared over `world` ranks — every rank sorts, then runs DC and HFC for every world-th
+    tile of 128 sorted slots (dense-cell work items by their first slot) and writes zeros elsewhere; rho and acc_sph are
+    completed by an integer SUM of the bit patterns.  `world` replicas run one after the other on this one GPU, the
+    exchange done by copies: every target must be written by exactly one replica and the step must reproduce the
+    single-GPU step BIT FOR BIT — thread-per-slot and dense-cell walks, one global h and per-particle h."""
+    b = cuda_lib
+    from paper_1807_08116_b200.sharded import ShardedSimulation
+    if case == "galaxy1":
+        w = wl.make_workload(1, scale=0.75)
+    elif case == "galaxy0":
+        w = wl.make_workload(0)
+    else:
+        w, _ = _grid_case(case)
+    n, ng, nh = w.n_total, w.n_gas, w.n_halo
+    ref = ShardedSimulation(w, 0, 1, sigma=sigma)           # world = 1: the plain stages, no collective
+    assert not ref.share_sph
+    ref.step()
+    ref.step()
+    if case in DENSE_CASES:
+        assert b.sph_dense_items(ref.ws, ng, n, ref.grid) > 0
+    reps = [ShardedSimulation(w, r, world, sigma=sigma) for r in range(world)]
+    assert all(s.share_sph for s in reps)
+
+    def position(sg):
+        for s in reps:
+            b.sph_position_share_sph(s.posm, s.hsml, ng, nh, s.rank, world, s.i0, s.i1, s.params, s.grid, s.rho, s.acc_grav, s.ws)
+        wr = _complete(reps, "rho", ng)
+        assert int(wr.min()) == 1                          # rho > 0 everywhere (self term): every target has exactly one writer
+        if sg:
+            for s in reps:
+                b.sph_renew_hsml(s.posm, s.hsml, sg, ng, nh, s.params, s.grid, s.rho, s.ws)
+        if w.G != 0.0:
+            _exchange(reps)
+        for s in reps:
+            b.nbody_pp_gravity_finish(s.posm, ng, nh, s.grid, s.params.G, s.acc_grav, s.ws)
+
+    def hydro(corrector):
+        for s in reps:
+            b.sph_forces_share(s.vele, s.hsml, ng, nh, s.rank, world, s.params, s.grid, s.rho, s.acc_sph, s.ws)
+        # a rank's share is a real share: about 1/world of the non-zero rows
+        rows = [int((s.acc_sph[:ng] != 0).any(dim=1).sum()) for s in reps]
+        assert max(rows) < 1.5 * sum(rows) / world + 256
+        _complete(reps, "acc_sph", ng)
+        for s in reps:
+            b.sph_update(s.posm, s.vele, ng, nh, s.grid, w.dt, corrector, s.acc_sph, s.acc_grav, s.ws)
+
+    position(0.0)
+    for _ in range(2):
+        hydro(False)
+        position(sigma or 0.0)
+        hydro(True)
+    for c in reps:
+        for x, y in ((c.posm, ref.posm), (c.vele, ref.vele), (c.rho, ref.rho), (c.acc_sph, ref.acc_sph),
+                     (c.acc_grav[:n], ref.acc_grav[:n])):
+            assert torch.equal(x, y)
+        if sigma:
+            assert torch.equal(c.hsml, ref.hsml)
+    # argument checks of the new calls
+    s0 = reps[0]
+    with pytest.raises(b.SphError):
+        b.sph_forces_share(s0.vele, s0.hsml, ng, nh, world, world, s0.params, s0.grid, s0.rho, s0.acc_sph, s0.ws)
+    with pytest.raises(b.SphError):
+        b.sph_renew_hsml(s0.posm, s0.rho, 0.0, ng, nh, s0.params, s0.grid, s0.rho, s0.ws)
+
+
 @pytest.mark.parametrize("masses", ["equal", "random", "zero_mass"])
 def test_gravity_shares_add_up(cuda_lib, masses):
     """nbody_pp_gravity_share over 3 ranks + the exchange + nbody_pp_gravity_finish against the one-call evaluation:
