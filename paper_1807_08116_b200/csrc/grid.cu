@@ -7,10 +7,16 @@
 //   zero      cudaMemsetAsync of count[M]
 //   k_key_hist  per particle: cell number (A7, bit-exact FP32 op sequence) and
 //               rank_u[i] = atomicAdd(&count[k], 1) — the histogram atomics already hand every
-//               particle a unique (unstable) slot in its cell, so no second cursor array / pass
+//               particle a unique (unstable) slot in its cell, so no second cursor array / pass;
+//               four particles per thread, their loads and atomics in flight together.  On the
+//               sparse galaxy grids (N_g <= M / 8) the particles also gather the totals of the
+//               scan's tiles of 4096 cells, through a per-CTA histogram in shared memory
 //   k_scan_*    two-level exclusive scan ("in-block then across blocks", L171-172) with warp
-//               shuffles, 16 cells per thread through uint4 loads; 4 B read + 4 B read + 4 B
-//               written per cell
+//               shuffles, 16 cells per thread through uint4 loads.  Up to 8192 tiles (33.5 M cells)
+//               k_scan_apply adds up the totals of the tiles before its own by itself and, where
+//               k_key_hist gathered the totals, is the only pass over the cells: 4 B read + 4 B
+//               written per cell.  Otherwise k_scan_tile_sums (4 B read per cell more) and, above
+//               8192 tiles, k_scan_tile_offsets
 //   k_scatter   tmp[start[k_i] + rank_u[i]] = i                          (unstable, like K4)
 //   k_stable    stable fix-up: slot s holding i moves to start[k] + #{t in cell : tmp[t] < i},
 //               i.e. ascending original index inside each cell (A16).  The count costs O(n_c)
@@ -85,20 +91,65 @@ __device__ __forceinline__ uint32_t cell_key(const float4 p, const GridDev g) {
     return (uint32_t)ix + (uint32_t)g.mx * ((uint32_t)iy + (uint32_t)g.my * (uint32_t)iz);
 }
 
+// Both particle passes below are bound by the latency of their scattered accesses (an atomic with its return value; a
+// gather of start[] and a scattered store), not by bandwidth: a thread takes kPassItems particles, a CTA-stride apart
+// (coalesced), and issues their loads, then their atomics / gathers, back to back — kPassItems requests in flight per
+// thread instead of one.
+constexpr int kPassItems = 4;
+constexpr int kPassBatch = 256 * kPassItems;   // particles a CTA takes at a time
+// The scan's tile of cells (k_scan_*: 4096 cells per CTA) and the largest number of tiles for which the tile totals are
+// gathered here, by the particles, instead of by a pass over count[M] (k_scan_tile_sums): every CTA keeps a private
+// histogram over the tiles in shared memory (<= 32 KB) and adds its non-zero entries to tile_sums[] at the end — one
+// global atomic per (CTA, tile it touched), so a galaxy core or a clump does not pile its atomics on a few words (one
+// more GLOBAL atomic per particle did, and measured slower).  This drops one of the two reads of count[M].
+constexpr int kTileShift = 12;
+constexpr int kFuseTiles = 8192;
 __global__ void __launch_bounds__(256) k_key_hist(const float4* __restrict__ posm, int n, GridDev g,
                                                   uint32_t* __restrict__ key, uint32_t* __restrict__ rank_u,
-                                                  uint32_t* __restrict__ count) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    uint32_t k = cell_key(posm[i], g);
-    key[i] = k;
-    rank_u[i] = atomicAdd(count + k, 1u);
+                                                  uint32_t* __restrict__ count, uint32_t* __restrict__ tile_sums,
+                                                  int n_tiles /*0: no tile totals*/, unsigned int* dense_ctl) {
+    extern __shared__ uint32_t sh_tiles[];
+    if (dense_ctl && blockIdx.x == 0 && threadIdx.x == 0) *dense_ctl = 0u;   // the work list k_scan_apply is about to write
+    for (int t = threadIdx.x; t < n_tiles; t += 256) sh_tiles[t] = 0u;
+    if (n_tiles) __syncthreads();
+    for (int64_t b0 = (int64_t)blockIdx.x * kPassBatch; b0 < n; b0 += (int64_t)gridDim.x * kPassBatch) {
+        const int i0 = (int)b0 + threadIdx.x;
+        float4 p[kPassItems];
+#pragma unroll
+        for (int q = 0; q < kPassItems; ++q) {
+            const int i = i0 + 256 * q;
+            p[q] = i < n ? posm[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        uint32_t k[kPassItems], r[kPassItems];
+#pragma unroll
+        for (int q = 0; q < kPassItems; ++q) {
+            k[q] = cell_key(p[q], g);
+            r[q] = (i0 + 256 * q < n) ? atomicAdd(count + k[q], 1u) : 0u;
+        }
+#pragma unroll
+        for (int q = 0; q < kPassItems; ++q) {
+            const int i = i0 + 256 * q;
+            if (i < n) {
+                key[i] = k[q];
+                rank_u[i] = r[q];
+                if (n_tiles) atomicAdd(sh_tiles + (k[q] >> kTileShift), 1u);
+            }
+        }
+    }
+    if (n_tiles) {
+        __syncthreads();
+        for (int t = threadIdx.x; t < n_tiles; t += 256) {
+            const uint32_t v = sh_tiles[t];
+            if (v) atomicAdd(tile_sums + t, v);
+        }
+    }
 }
 
 // ---------------------------------------------------------------- (a3) two-level exclusive scan
 constexpr int kScanThreads = 256;
 constexpr int kScanItems = 16;
 constexpr int kScanTile = kScanThreads * kScanItems;   // 4096 cells per CTA
+static_assert(kScanTile == 1 << kTileShift, "k_key_hist's tile totals");
 
 __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* warp_sums, uint32_t& total) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -165,10 +216,8 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_tile_sums(const uint32_t*
 // slice [t*per, (t+1)*per): local sum, one block scan over the 1024 slice sums, local rescan —
 // a single pass whatever n_tiles is (the chunked version needed n_tiles/256 dependent block scans).
 constexpr int kOffThreads = 1024;
-__global__ void __launch_bounds__(kOffThreads) k_scan_tile_offsets(uint32_t* tile_sums, int n_tiles,
-                                                                  unsigned int* dense_ctl) {
+__global__ void __launch_bounds__(kOffThreads) k_scan_tile_offsets(uint32_t* tile_sums, int n_tiles) {
     __shared__ uint32_t ws[32];
-    if (dense_ctl && threadIdx.x == 0) *dense_ctl = 0u;   // the work list k_scan_apply is about to write
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int per = (n_tiles + kOffThreads - 1) / kOffThreads;
     const int lo = min(threadIdx.x * per, n_tiles), hi = min(lo + per, n_tiles);
@@ -200,19 +249,52 @@ __global__ void __launch_bounds__(kOffThreads) k_scan_tile_offsets(uint32_t* til
     }
 }
 
+// TOTALS: tile_offsets[] holds the tiles' TOTALS (k_key_hist gathered them, <= kFuseTiles of them) and the CTA adds up
+// the ones before its own itself — at most 32 KB of L2-resident reads per CTA, against one more kernel on the path.
+template <bool TOTALS>
 __global__ void __launch_bounds__(kScanThreads) k_scan_apply(const uint32_t* __restrict__ count, int64_t M,
                                                              const uint32_t* __restrict__ tile_offsets,
                                                              uint32_t* __restrict__ start, uint32_t n_gas,
                                                              unsigned int* dense_ctl, DenseItem* dense_items) {
     __shared__ uint32_t ws[kScanThreads / 32];
+    __shared__ uint32_t s_off;
     uint32_t c[kScanItems];
     const int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
     load_items(count, base, M, c);
+    uint32_t off;
+    if (TOTALS) {
+        // (16-byte loads, at most kFuseTiles / 1024 of them per thread, all in flight together; tile_offsets[] is 256-byte
+        // aligned and padded to a multiple of 4 words by the caller's allocation of n_tiles + 1 words rounded up to 256 bytes)
+        uint32_t v = 0;
+#pragma unroll
+        for (int j = 0; j < kFuseTiles / (4 * kScanThreads); ++j) {
+            const int t = 4 * (threadIdx.x + kScanThreads * j), nb = (int)blockIdx.x;
+            if (t < nb) {
+                const uint4 q = *reinterpret_cast<const uint4*>(tile_offsets + t);
+                v += q.x + (t + 1 < nb ? q.y : 0u) + (t + 2 < nb ? q.z : 0u) + (t + 3 < nb ? q.w : 0u);
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = v;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            uint32_t t = 0;
+#pragma unroll
+            for (int q = 0; q < kScanThreads / 32; ++q) t += ws[q];
+            s_off = t;
+        }
+        __syncthreads();
+        off = s_off;
+        __syncthreads();   // ws is reused by the scan below
+    } else {
+        off = tile_offsets[blockIdx.x];
+    }
     uint32_t s = 0;
 #pragma unroll
     for (int q = 0; q < kScanItems; ++q) s += c[q];
     uint32_t total;
-    uint32_t run = tile_offsets[blockIdx.x] + block_exclusive_scan(s, ws, total);
+    uint32_t run = off + block_exclusive_scan(s, ws, total);
     uint32_t out[kScanItems];
 #pragma unroll
     for (int q = 0; q < kScanItems; ++q) {
@@ -240,9 +322,21 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_apply(const uint32_t* __r
 // ---------------------------------------------------------------- (a4) scatter and stable fix-up
 __global__ void __launch_bounds__(256) k_scatter(const uint32_t* __restrict__ key, const uint32_t* __restrict__ rank_u,
                                                  const uint32_t* __restrict__ start, int n, uint32_t* __restrict__ tmp) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    tmp[start[key[i]] + rank_u[i]] = (uint32_t)i;
+    const int i0 = blockIdx.x * (256 * kPassItems) + threadIdx.x;
+    uint32_t k[kPassItems], r[kPassItems], a[kPassItems];
+#pragma unroll
+    for (int q = 0; q < kPassItems; ++q) {
+        const int i = i0 + 256 * q;
+        k[q] = i < n ? key[i] : 0u;
+        r[q] = i < n ? rank_u[i] : 0u;
+    }
+#pragma unroll
+    for (int q = 0; q < kPassItems; ++q) a[q] = start[k[q]];
+#pragma unroll
+    for (int q = 0; q < kPassItems; ++q) {
+        const int i = i0 + 256 * q;
+        if (i < n) tmp[a[q] + r[q]] = (uint32_t)i;
+    }
 }
 
 // slot s of the unstable order holds i = tmp[s]; its stable slot is start[k] + #{t in cell k : tmp[t] < i}.
@@ -311,21 +405,47 @@ int grid_build(const float4* posm, int64_t n_gas, const sph_grid* g, uint32_t* k
                float4* posm_s, const DenseList* dense, cudaStream_t st) {
     const int64_t M = grid_cells(g);
     const int n = (int)n_gas;
-    SPHB_CUDA(cudaMemsetAsync(cell_count, 0, (size_t)M * sizeof(uint32_t), st));          // K0
-    if (n > 0) {
-        k_key_hist<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(posm, n, to_dev(g), key, rank_u, cell_count);   // K1
+    const int n_tiles = (int)cdiv(M, kScanTile);
+    // Few tiles (M <= 33.5 M cells): k_scan_apply adds up the totals of the tiles before its own by itself, one kernel less
+    // on the path; and where the particles are few against the cells (the galaxy grids: N_g <= M / 8) they gather the tile
+    // totals themselves in k_key_hist, which drops the pass that reads count[M] only to add it up.
+    const bool own_offsets = n_tiles <= kFuseTiles;
+    const bool by_particles = own_offsets && (int64_t)n * 8 <= M;
+    unsigned int* ctl = dense ? dense->ctl : nullptr;
+    DenseItem* items = dense ? dense->items : nullptr;
+    {   // K0; tile_sums[] lies right behind count[M] in a workspace (step.cu: carve): one memset then zeroes both
+        const char* c_end = reinterpret_cast<const char*>(cell_count + M);
+        const char* t_beg = reinterpret_cast<const char*>(tile_sums);
+        const char* t_end = reinterpret_cast<const char*>(tile_sums + n_tiles);
+        if (by_particles && t_beg >= c_end && t_beg - c_end < 4096) {
+            SPHB_CUDA(cudaMemsetAsync(cell_count, 0, (size_t)(t_end - reinterpret_cast<const char*>(cell_count)), st));
+        } else {
+            SPHB_CUDA(cudaMemsetAsync(cell_count, 0, (size_t)M * sizeof(uint32_t), st));
+            if (by_particles) SPHB_CUDA(cudaMemsetAsync(tile_sums, 0, (size_t)n_tiles * sizeof(uint32_t), st));
+        }
+    }
+    {
+        const int64_t batches = cdiv(n, kPassBatch), cap = (int64_t)num_sms() * 8;
+        const unsigned blocks = (unsigned)(batches < 1 ? 1 : (by_particles && batches > cap ? cap : batches));
+        k_key_hist<<<blocks, 256, by_particles ? (size_t)n_tiles * sizeof(uint32_t) : 0, st>>>(
+            posm, n, to_dev(g), key, rank_u, cell_count, tile_sums, by_particles ? n_tiles : 0, ctl);   // K1
         SPHB_LAUNCHED();
     }
-    const int n_tiles = (int)cdiv(M, kScanTile);
-    k_scan_tile_sums<<<n_tiles, kScanThreads, 0, st>>>(cell_count, M, tile_sums);          // K2 (in-block)
-    SPHB_LAUNCHED();
-    k_scan_tile_offsets<<<1, kOffThreads, 0, st>>>(tile_sums, n_tiles, dense ? dense->ctl : nullptr);   // K2 (across blocks)
-    SPHB_LAUNCHED();
-    k_scan_apply<<<n_tiles, kScanThreads, 0, st>>>(cell_count, M, tile_sums, cell_start, (uint32_t)n,
-                                                   dense ? dense->ctl : nullptr, dense ? dense->items : nullptr);   // K3
-    SPHB_LAUNCHED();
+    if (!by_particles) {
+        k_scan_tile_sums<<<n_tiles, kScanThreads, 0, st>>>(cell_count, M, tile_sums);          // K2 (in-block)
+        SPHB_LAUNCHED();
+    }
+    if (own_offsets) {
+        k_scan_apply<true><<<n_tiles, kScanThreads, 0, st>>>(cell_count, M, tile_sums, cell_start, (uint32_t)n, ctl, items);   // K2 (across blocks) + K3
+        SPHB_LAUNCHED();
+    } else {
+        k_scan_tile_offsets<<<1, kOffThreads, 0, st>>>(tile_sums, n_tiles);                     // K2 (across blocks)
+        SPHB_LAUNCHED();
+        k_scan_apply<false><<<n_tiles, kScanThreads, 0, st>>>(cell_count, M, tile_sums, cell_start, (uint32_t)n, ctl, items);   // K3
+        SPHB_LAUNCHED();
+    }
     if (n > 0) {
-        k_scatter<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(key, rank_u, cell_start, n, tmp);                 // K4
+        k_scatter<<<(unsigned)cdiv(n, 256 * kPassItems), 256, 0, st>>>(key, rank_u, cell_start, n, tmp);                 // K4
         SPHB_LAUNCHED();
         k_stable<<<(unsigned)cdiv(n, 256), 256, 0, st>>>(tmp, to_dev(g), cell_start, posm, n, perm, posm_s);
         SPHB_LAUNCHED();

@@ -37,8 +37,8 @@ Workspace carve(void* base, int64_t n_gas, int64_t n_total, const sph_grid* g) {
     w.tmp = (uint32_t*)take(ng * 4);
     w.perm = (uint32_t*)take(ng * 4);
     w.cell_count = (uint32_t*)take((size_t)M * 4);
+    w.tile_sums = (uint32_t*)take((size_t)(cdiv(M > 0 ? M : 1, 4096) + 1) * 4);   // right behind count[M]: one memset zeroes both (grid.cu)
     w.cell_start = (uint32_t*)take((size_t)(M + 1) * 4);
-    w.tile_sums = (uint32_t*)take((size_t)(cdiv(M > 0 ? M : 1, 4096) + 1) * 4);
     w.posm_s = (float4*)take(ng * 16);
     w.velr_s = (float4*)take(ng * 16);
     w.pc_s = (float2*)take(ng * 8);
