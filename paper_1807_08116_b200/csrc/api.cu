@@ -580,7 +580,8 @@ int sph_density_h(const float* posm, const float* hsml, int64_t n_gas, const sph
     SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
     SPHB_TRY(gather_sorted_h(hsml, perm, n_gas, p->h, w.status, w.h_s, st));
     Span sp(ST_DENSITY, st);
-    return density_sorted(w.posm_s, w.h_s, perm, cell_start, n_gas, p, g, nullptr, rho, st);
+    SPHB_TRY(dense_list_from_start(cell_start, g, w.dense, st));
+    return density_sorted(w.posm_s, w.h_s, perm, cell_start, n_gas, p, g, &w.dense, rho, st);
 }
 
 int sph_forces_h(const float* posm, const float* vele, const float* rho, const float* hsml, int64_t n_gas,
@@ -598,8 +599,9 @@ int sph_forces_h(const float* posm, const float* vele, const float* rho, const f
     cudaStream_t st = (cudaStream_t)stream;
     SPHB_TRY(gather_sorted_pos(reinterpret_cast<const float4*>(posm), perm, n_gas, w.posm_s, st));
     SPHB_TRY(gather_sorted_h(hsml, perm, n_gas, p->h, w.status, w.h_s, st));
+    SPHB_TRY(dense_list_from_start(cell_start, g, w.dense, st));
     Span sp(ST_FORCES, st);
-    return forces_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, w.h_s, perm, cell_start, n_gas, p, g, nullptr,
+    return forces_sorted(w.posm_s, reinterpret_cast<const float4*>(vele), rho, w.h_s, perm, cell_start, n_gas, p, g, &w.dense,
                          nullptr, w.velr_s, w.pc_s, reinterpret_cast<float4*>(acc_sph), st);
 }
 

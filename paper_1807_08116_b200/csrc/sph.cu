@@ -109,11 +109,11 @@ int gather_sorted_h(const float* hsml, const uint32_t* perm, int64_t n_gas, floa
     return SPH_OK;
 }
 
-int forces_dense(const float4* posm_s, const float4* velr_s, const float2* pc_s, const uint32_t* perm,
+int forces_dense(const float4* posm_s, const float4* velr_s, const float2* pc_s, const float* h_s, const uint32_t* perm,
                  const uint32_t* cell_start, const sph_grid* g, float rc2, const ViscDev& q, const DenseList& dl,
                  const CflArgs* cfl, float4* acc_sph, cudaStream_t st, Shard sh);   // sph_dense.cu
 
-int density_dense(const float4* posm_s, const uint32_t* perm, const uint32_t* cell_start, const sph_params* p,
+int density_dense(const float4* posm_s, const float* h_s, const uint32_t* perm, const uint32_t* cell_start, const sph_params* p,
                   const sph_grid* g, const DenseList& dl, float* rho, cudaStream_t st, Shard sh);   // sph_dense_rho.cu
 
 // CTAs of a thread-per-slot pass: the rank's tiles rank, rank + world, ... of the cdiv(n, 128)
@@ -133,14 +133,15 @@ int density_sorted(const float4* posm_s, const float* h_s /*cell order, or NULL:
     if (blocks == 0u) return SPH_OK;
     if (h_s) {
         k_density<true><<<blocks, 128, 0, st>>>(posm_s, h_s, perm, cell_start, (int)n_gas, to_dev(g), rc2, inv_h,
-                                                (float)(1.0 / 3.14159265358979323846), 0u, sh, rho);
+                                                (float)(1.0 / 3.14159265358979323846), dense ? (uint32_t)kDenseMin : 0u, sh, rho);
         SPHB_LAUNCHED();
+        if (dense) SPHB_TRY(density_dense(posm_s, h_s, perm, cell_start, p, g, *dense, rho, st, sh));
     } else {
         const float norm = (float)(1.0 / (3.14159265358979323846 * (double)p->h * (double)p->h * (double)p->h));
         k_density<false><<<blocks, 128, 0, st>>>(posm_s, nullptr, perm, cell_start, (int)n_gas, to_dev(g), rc2, inv_h,
                                                  norm, dense ? (uint32_t)kDenseMin : 0u, sh, rho);
         SPHB_LAUNCHED();
-        if (dense) SPHB_TRY(density_dense(posm_s, perm, cell_start, p, g, *dense, rho, st, sh));
+        if (dense) SPHB_TRY(density_dense(posm_s, nullptr, perm, cell_start, p, g, *dense, rho, st, sh));
     }
     return SPH_OK;
 }
@@ -213,26 +214,7 @@ __global__ void __launch_bounds__(128) k_forces(const float4* __restrict__ posm_
                 const float2 cj = pc_s[t];
                 float f, rv, mu, c_ij;
                 if (VARH) {
-                    float rinv = rsqrtf(d2);
-                    rinv = rinv * fmaf(-0.5f * d2 * rinv, rinv, 1.5f);   // one Newton step: ~1 ulp
-                    const float rr = d2 * rinv;                        // |dr|
-                    // the pair factor goes like h_ij^-8: with a per-pair h its roundings no longer cancel as a
-                    // common factor of the particle's sum, so it is formed in FP64 and rounded once
-                    const double hd = 0.5 * (double)hsum, ihd = 1.0 / hd, ih2 = ihd * ihd;
-                    const double num = fma(-(double)dz, (double)dz, fma(-(double)dy, (double)dy, fma(-(double)dx, (double)dx, (double)hsum * (double)hsum)));
-                    const double tqd = fmax(num, 0.0) * ih2 / (2.0 + (double)rr * ihd);       // 2 - xi
-                    const float gmag = (float)((double)q.gw_unit * ih2 * ih2 * tqd * tqd) * rinv;   // grad W_p = gmag * dr
-                    const float hh = 0.5f * hsum;
-                    const float eta_h2 = q.eta * hh * hh;
-                    const float dvx = vi.x - vj.x, dvy = vi.y - vj.y, dvz = vi.z - vj.z;
-                    rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
-                    // mu_ij = h dr.dv / (|dr|^2 + eta h^2) if dr.dv < 0   (L97)
-                    mu = rv < 0.f ? (hh * rv) / (d2 + eta_h2) : 0.f;                   // IEEE division
-                    const float rho_ij = 0.5f * (vi.w + vj.w);
-                    c_ij = 0.5f * (ci.y + cj.y);
-                    const float nu = (mu * (q.beta * mu - q.alpha * c_ij)) / rho_ij;
-                    const float Pi = ci.x + cj.x + nu;                 // p_i/rho_i^2 + p_j/rho_j^2 + nu  (L95, A2)
-                    f = pj.w * Pi * gmag;                              // m_j Pi |grad Wp| / |dr|
+                    f = hydro_pair_h(vi, ci, pj.w, vj, cj, dx, dy, dz, d2, hsum, q, rv, mu, c_ij);
                 } else {
                     f = hydro_pair(vi, ci, pj.w, vj, cj, dx, dy, dz, d2, q, rv, mu, c_ij);
                 }
@@ -287,17 +269,17 @@ int forces_sorted(const float4* posm_s, const float4* vele, const float* rho, co
     if (blocks == 0u) return SPH_OK;
     const GridDev gd = to_dev(g);
     const CflArgs c = cfl ? *cfl : CflArgs{};
-    const uint32_t dmin = (dense && !h_s) ? (uint32_t)kDenseMin : 0u;
+    const uint32_t dmin = dense ? (uint32_t)kDenseMin : 0u;   // those cells are walked by sph_dense.cu
     if (h_s && cfl)
-        k_forces<true, true><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, h_s, perm, cell_start, n, gd, q.rc2, q, 0u, c, sh, acc_sph);
+        k_forces<true, true><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, h_s, perm, cell_start, n, gd, q.rc2, q, dmin, c, sh, acc_sph);
     else if (h_s)
-        k_forces<true, false><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, h_s, perm, cell_start, n, gd, q.rc2, q, 0u, c, sh, acc_sph);
+        k_forces<true, false><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, h_s, perm, cell_start, n, gd, q.rc2, q, dmin, c, sh, acc_sph);
     else if (cfl)
         k_forces<false, true><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, nullptr, perm, cell_start, n, gd, q.rc2, q, dmin, c, sh, acc_sph);
     else
         k_forces<false, false><<<blocks, 128, 0, st>>>(posm_s, velr_s, pc_s, nullptr, perm, cell_start, n, gd, q.rc2, q, dmin, c, sh, acc_sph);
     SPHB_LAUNCHED();
-    if (dmin) SPHB_TRY(forces_dense(posm_s, velr_s, pc_s, perm, cell_start, g, q.rc2, q, *dense, cfl, acc_sph, st, sh));
+    if (dmin) SPHB_TRY(forces_dense(posm_s, velr_s, pc_s, h_s, perm, cell_start, g, q.rc2, q, *dense, cfl, acc_sph, st, sh));
     return SPH_OK;
 }
 

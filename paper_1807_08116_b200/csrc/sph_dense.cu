@@ -36,14 +36,17 @@ namespace {
 constexpr int kDenseThreads = 384;
 constexpr int kDenseWarps = kDenseThreads / 32;
 constexpr int kDenseCtasPerSm = 2;
-constexpr int kDenseK = 1088;             // candidate slots per staged chunk
 constexpr int kMaxSeg = 6;                // pieces of stencil rows ("segments") a chunk may hold
-constexpr int kDenseKS = kDenseK + 2 * kMaxSeg;   // + the even-slot alignment of the float2 array, per segment
-constexpr int kRounds = (kDenseK + kDenseThreads - 1) / kDenseThreads;
 using dense::kBins;
 constexpr int kQueue = 128;               // ring queue entries per warp: <= 31 left over + 64 pushed by a step
 
+// VARH (per-particle smoothing lengths, L82): the sorted chunk also holds the candidates' lengths and every bin its
+// largest one, so the chunk is a little smaller
+template <bool VARH>
 struct DenseLayout {
+    static constexpr int kDenseK = VARH ? 992 : 1088;                   // candidate slots per staged chunk
+    static constexpr int kDenseKS = kDenseK + 2 * kMaxSeg;              // + the even-slot alignment of the float2 array, per segment
+    static constexpr int kRounds = (kDenseK + kDenseThreads - 1) / kDenseThreads;
     // byte offsets inside the dynamic shared memory block (all multiples of 16)
     static constexpr int raw_pos = 0;                                   // float4 [KS]   landing zone of the bulk copies
     static constexpr int raw_vel = raw_pos + kDenseKS * 16;             // float4 [KS]
@@ -51,7 +54,8 @@ struct DenseLayout {
     static constexpr int pos = raw_pc + kDenseKS * 8;                   // float4 [K]    the chunk in bin order: (x, y, z, m)
     static constexpr int vel = pos + kDenseK * 16;                      // float4 [K]    (v, rho)
     static constexpr int pc = vel + kDenseK * 16;                       // float2 [K]    (p/rho^2, c)
-    static constexpr int tpos = pc + kDenseK * 8;                       // float4 [TT]   the item's targets
+    static constexpr int hh = pc + kDenseK * 8;                         // float [K]     VARH: the candidates' smoothing lengths
+    static constexpr int tpos = hh + (VARH ? kDenseK * 4 : 0);          // float4 [TT]   the item's targets
     static constexpr int tvel = tpos + kDenseTT * 16;                   // float4 [TT]
     static constexpr int tpc = tvel + kDenseTT * 16;                    // float2 [TT]
     static constexpr int acc = tpc + kDenseTT * 8;                      // double [TT][4]
@@ -60,7 +64,9 @@ struct DenseLayout {
     static constexpr int hist = runs + 9 * 4 * 4;                       // uint32 [rounds][warps][bins]
     static constexpr int bstart = hist + kRounds * kDenseWarps * kBins * 4;   // uint32 [seg][32]: start of bin b inside its segment
     static constexpr int box = bstart + kMaxSeg * 32 * 4;               // float [seg][bins][8]: xl, xh, yl, yh, zl, zh, -, -
-    static constexpr int queue = box + kMaxSeg * kBins * 8 * 4;         // uint32 [warps][kQueue]
+    static constexpr int hmax = box + kMaxSeg * kBins * 8 * 4;          // uint32 [seg][32]: VARH: bits of the largest length in bin b
+    static constexpr int th = hmax + (VARH ? kMaxSeg * 32 * 4 : 0);     // float [TT]: VARH: the targets' lengths
+    static constexpr int queue = th + (VARH ? kDenseTT * 4 : 0);        // uint32 [warps][kQueue]
     static constexpr int seg = queue + kDenseWarps * kQueue * 4;        // uint4 [2][seg]: (row, first slot, end slot, raw base) of the
                                                                         // chunk being worked on and of the one being copied
     static constexpr int nseg = seg + 2 * kMaxSeg * 16;                 // uint32 [2] segments of those chunks, [2] (row, slot) the producer is at
@@ -69,16 +75,22 @@ struct DenseLayout {
     static constexpr int tnext = bar + 12;                              // uint32: next target of the chunk to hand to a warp
     static constexpr int bytes = bar + 16;
 };
-static_assert((DenseLayout::bytes + 1024) * kDenseCtasPerSm <= 227 * 1024, "shared memory per SM");
+static_assert((DenseLayout<false>::bytes + 1024) * kDenseCtasPerSm <= 227 * 1024, "shared memory per SM");
+static_assert((DenseLayout<true>::bytes + 1024) * kDenseCtasPerSm <= 227 * 1024, "shared memory per SM");
 
 // CFL: the terms of Eq. 17 (s^min, c^max, mu^max; L125-129) are reduced in the same walk, as in k_forces (sph.cu).
-template <bool CFL>
+// VARH: per-particle smoothing lengths h_s[] in cell order (L82; readings A24-A26 as in k_forces<true>): the pair is a
+// neighbour pair iff d2 < fl(fl(h_i + h_j)^2), the pair term uses h_ij = (h_i + h_j)/2, and a target's sphere reaches a
+// bin iff its distance to the bin's box is below h_i + (the largest length in that bin) — the paper's hmaxCell (L164,
+// L207) at the granularity of the octant bins, gathered while the chunk is binned.
+template <bool CFL, bool VARH>
 __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
     k_dense_forces(const float4* __restrict__ posm_s, const float4* __restrict__ velr_s, const float2* __restrict__ pc_s,
-            const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start, GridDev g, float cell, float rc2,
-            ViscDev q, CflArgs cfl, Shard sh, unsigned int* __restrict__ ctl, const DenseItem* __restrict__ items,
-            float4* __restrict__ acc_out) {
-    using L = DenseLayout;
+            const float* __restrict__ h_s, const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start, GridDev g,
+            float cell, float rc2, ViscDev q, CflArgs cfl, Shard sh, unsigned int* __restrict__ ctl,
+            const DenseItem* __restrict__ items, float4* __restrict__ acc_out) {
+    using L = DenseLayout<VARH>;
+    constexpr int kDenseK = L::kDenseK, kRounds = L::kRounds;
     extern __shared__ __align__(128) unsigned char smem[];
     float4* r_pos = reinterpret_cast<float4*>(smem + L::raw_pos);
     float4* r_vel = reinterpret_cast<float4*>(smem + L::raw_vel);
@@ -86,6 +98,9 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
     float4* c_pos = reinterpret_cast<float4*>(smem + L::pos);
     float4* c_vel = reinterpret_cast<float4*>(smem + L::vel);
     float2* c_pc = reinterpret_cast<float2*>(smem + L::pc);
+    float* c_h = reinterpret_cast<float*>(smem + L::hh);
+    float* t_h = reinterpret_cast<float*>(smem + L::th);
+    uint32_t* s_hmax = reinterpret_cast<uint32_t*>(smem + L::hmax);
     float4* t_pos = reinterpret_cast<float4*>(smem + L::tpos);
     float4* t_vel = reinterpret_cast<float4*>(smem + L::tvel);
     float2* t_pc = reinterpret_cast<float2*>(smem + L::tpc);
@@ -104,7 +119,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned lt_mask = (1u << lane) - 1u;
     const uint32_t sbase = smem_u32(smem);
-    const uint32_t a_pos = sbase + L::pos, a_vel = sbase + L::vel, a_pc = sbase + L::pc;
+    const uint32_t a_pos = sbase + L::pos, a_vel = sbase + L::vel, a_pc = sbase + L::pc, a_h = sbase + L::hh;
     const uint32_t a_tpos = sbase + L::tpos, a_tvel = sbase + L::tvel, a_tpc = sbase + L::tpc;
     const uint32_t a_q = sbase + L::queue + 4u * kQueue * (uint32_t)warp;
     const uint32_t n_items = ctl[0];
@@ -180,6 +195,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
 #pragma unroll
             for (int c = 0; c < 4; ++c) s_acc[4 * t + c] = 0.0;
             if (CFL) s_cfl[t] = make_float4(__int_as_float(0x7f800000), pc.y, 0.f, 0.f);   // A22: no neighbour -> c_i, 0
+            if (VARH) t_h[t] = h_s[ts + t];
         }
         __syncthreads();
         if (tid == 0) {
@@ -202,6 +218,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                 const uint4 sg = s_seg[set * kMaxSeg + sgi];   // (row, first slot, end slot, raw base)
                 const int r = (int)sg.x;
                 const dense::RowGeom rg = dense::row_geom(g, cell, ix, iy, iz, r);
+                if (VARH && tid < 32) s_hmax[32u * sgi + tid] = 0u;   // (ordered before the moves by bin_chunk's barriers)
                 dense::bin_chunk<kDenseThreads, kRounds, false>(
                     r_pos, sg.w + (sg.y & 1u), sg.z - sg.y, sg.y, s_runs[4 * r + 1], s_runs[4 * r + 2], g, cell, ix, rg, s_hist,
                     s_bstart + 32u * sgi, s_box + 2u * kBins * sgi,
@@ -212,10 +229,15 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                         }
                     },
                     [&]() { *s_tnext = 0u; },
-                    [&](uint32_t src, uint32_t dst) {
+                    [&](uint32_t src, uint32_t dst, uint32_t bin) {
                         c_pos[soff + dst] = r_pos[src];
                         c_vel[soff + dst] = r_vel[src];
                         c_pc[soff + dst] = r_pc[src];
+                        if (VARH) {   // the length straight from global memory (L2), and the bin's largest (positive floats order like their bits)
+                            const float hj = h_s[sg.y + (src - (sg.w + (sg.y & 1u)))];
+                            c_h[soff + dst] = hj;
+                            atomicMax(s_hmax + 32u * sgi + bin, __float_as_uint(hj));
+                        }
                     },
                     [&](uint32_t) {});
                 soff += sg.z - sg.y;
@@ -235,6 +257,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                 const float4 pi = lds_f4(a_tpos + 16u * t);
                 const float4 vi = lds_f4(a_tvel + 16u * t);
                 const float2 ci = lds_f2(a_tpc + 8u * t);
+                const float h_i = VARH ? t_h[t] : 0.f;
                 float ax = 0.f, ay = 0.f, az = 0.f, de = 0.f;
                 float d2min = __int_as_float(0x7f800000), cmax = 0.f, mumax = 0.f;
                 uint32_t qh = 0, qt = 0;   // ring queue of accepted candidates (byte offsets in the float4 arrays): head, tail x4
@@ -244,7 +267,11 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                     const float2 cj = lds_f2(a_pc + (rel >> 1));
                     float dx, dy, dz, rv, mu;
                     const float d2 = dist2_f32(pi, pj, dx, dy, dz);
-                    const float f = hydro_pair_fast(vi, ci, pj.w, vj, cj, dx, dy, dz, d2, q, rv, mu);
+                    float f, c_v = 0.f;
+                    if (VARH)   // the sparse walk's arithmetic (sph_dev.cuh says why); twice the term, as hydro_pair_fast's is halved below
+                        f = hydro_pair_h(vi, ci, pj.w, vj, cj, dx, dy, dz, d2, __fadd_rn(h_i, lds_f32(a_h + (rel >> 2))), q, rv, mu, c_v);
+                    else
+                        f = hydro_pair_fast(vi, ci, pj.w, vj, cj, dx, dy, dz, d2, q, rv, mu);
                     ax = fmaf(-f, dx, ax);
                     ay = fmaf(-f, dy, ay);
                     az = fmaf(-f, dz, az);
@@ -264,7 +291,12 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                     const float ex = fmaxf(fmaxf(bx0.x - pi.x, pi.x - bx0.y), 0.f);
                     const float ey = fmaxf(fmaxf(bx0.z - pi.y, pi.y - bx0.w), 0.f);
                     const float ez = fmaxf(fmaxf(bx1.x - pi.z, pi.z - bx1.y), 0.f);
-                    const bool reach_b = fmaf(ez, ez, fmaf(ey, ey, ex * ex)) < rc2;   // lanes >= kBins: their box is out of reach
+                    float rcb2 = rc2;
+                    if (VARH) {   // h_i + the largest length among the bin's candidates
+                        const float rcb = h_i + __uint_as_float(s_hmax[32u * sgi + lane]);
+                        rcb2 = rcb * rcb;
+                    }
+                    const bool reach_b = fmaf(ez, ez, fmaf(ey, ey, ex * ex)) < rcb2;   // lanes >= kBins: their box is out of reach
                     // the reachable bins, in bin order, are the target's candidates in this segment: four slot ranges
                     const unsigned reach = __ballot_sync(0xffffffffu, reach_b);
                     const dense::Groups G = dense::candidate_groups(reach, s_bstart + 32u * sgi, first);
@@ -282,8 +314,14 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                         const float d20 = dist2_f32(pi, lds_f4(a_pos + rel0), dx, dy, dz);
                         const float d21 = dist2_f32(pi, lds_f4(a_pos + rel1), dx, dy, dz);
                         // d2 == 0: self, or a coincident pair (A9) — no contribution
-                        const bool ok0 = (decltype(full)::value || v16 < T16) && d20 < rc2 && d20 > 0.f;
-                        const bool ok1 = (decltype(full)::value || v16 + 512u < T16) && d21 < rc2 && d21 > 0.f;
+                        float rc20 = rc2, rc21 = rc2;
+                        if (VARH) {   // d2 < fl(fl(h_i + h_j)^2) (A24); a position past the end reads some length of this CTA
+                            const float s0 = __fadd_rn(h_i, lds_f32(a_h + (rel0 >> 2))), s1 = __fadd_rn(h_i, lds_f32(a_h + (rel1 >> 2)));
+                            rc20 = __fmul_rn(s0, s0);
+                            rc21 = __fmul_rn(s1, s1);
+                        }
+                        const bool ok0 = (decltype(full)::value || v16 < T16) && d20 < rc20 && d20 > 0.f;
+                        const bool ok1 = (decltype(full)::value || v16 + 512u < T16) && d21 < rc21 && d21 > 0.f;
                         const unsigned m0 = __ballot_sync(0xffffffffu, ok0), m1 = __ballot_sync(0xffffffffu, ok1);
                         if (ok0) sts_u32(a_q + ((qt + 4u * __popc(m0 & lt_mask)) & (4u * kQueue - 4u)), rel0);
                         qt += 4u * __popc(m0);
@@ -343,7 +381,7 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
             if (acc_out) acc_out[i] = a_own;
             if (CFL) {
                 const float4 c = s_cfl[t];
-                const float bound = cfl_bracket(c.x, c.x == __int_as_float(0x7f800000), 2.0f * q.h, c.y, c.z, q.alpha, q.beta,
+                const float bound = cfl_bracket(c.x, c.x == __int_as_float(0x7f800000), 2.0f * (VARH ? t_h[t] : q.h), c.y, c.z, q.alpha, q.beta,
                                                 cfl.q_sph ? cfl.q_sph[i] : a_own, cfl.acc_grav[i]);
                 if (cfl.dt_particle) cfl.dt_particle[i] = bound;
                 cfl_min(cfl.c_cfl * bound, cfl.dt_bits);
@@ -371,27 +409,42 @@ int dense_list_from_start(const uint32_t* cell_start, const sph_grid* g, const D
     return SPH_OK;
 }
 
-int forces_dense(const float4* posm_s, const float4* velr_s, const float2* pc_s, const uint32_t* perm,
-                 const uint32_t* cell_start, const sph_grid* g, float rc2, const ViscDev& q, const DenseList& dl,
-                 const CflArgs* cfl, float4* acc_sph, cudaStream_t st, Shard sh) {
+int forces_dense(const float4* posm_s, const float4* velr_s, const float2* pc_s, const float* h_s /*cell order, or NULL*/,
+                 const uint32_t* perm, const uint32_t* cell_start, const sph_grid* g, float rc2, const ViscDev& q,
+                 const DenseList& dl, const CflArgs* cfl, float4* acc_sph, cudaStream_t st, Shard sh) {
     int dev = 0;
     SPHB_CUDA(cudaGetDevice(&dev));
     static std::atomic<bool> opted[64];   // per device: the dynamic shared-memory opt-in
     if (dev < 0 || dev >= 64) return SPH_ERR_UNSUPPORTED;
     if (!opted[dev].load(std::memory_order_acquire)) {
-        SPHB_CUDA(cudaFuncSetAttribute(k_dense_forces<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DenseLayout::bytes));
-        SPHB_CUDA(cudaFuncSetAttribute(k_dense_forces<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DenseLayout::bytes));
+        SPHB_CUDA(cudaFuncSetAttribute(k_dense_forces<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DenseLayout<false>::bytes));
+        SPHB_CUDA(cudaFuncSetAttribute(k_dense_forces<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, DenseLayout<false>::bytes));
+        SPHB_CUDA(cudaFuncSetAttribute(k_dense_forces<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DenseLayout<true>::bytes));
+        SPHB_CUDA(cudaFuncSetAttribute(k_dense_forces<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, DenseLayout<true>::bytes));
         opted[dev].store(true, std::memory_order_release);
     }
     // the faces of the cells follow the rule the keys are made with (A7: c = (x - origin) * inv_cell), so the cell
     // edge is taken from inv_cell, not from g->cell
     SPHB_CUDA(cudaMemsetAsync(dl.ctl + 1, 0, sizeof(unsigned int), st));   // the item counter
-    if (cfl)
-        k_dense_forces<true><<<kDenseCtasPerSm * num_sms(), kDenseThreads, DenseLayout::bytes, st>>>(
-            posm_s, velr_s, pc_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, rc2, q, *cfl, sh, dl.ctl, dl.items, acc_sph);
-    else
-        k_dense_forces<false><<<kDenseCtasPerSm * num_sms(), kDenseThreads, DenseLayout::bytes, st>>>(
-            posm_s, velr_s, pc_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, rc2, q, CflArgs{}, sh, dl.ctl, dl.items, acc_sph);
+    const unsigned grid = (unsigned)(kDenseCtasPerSm * num_sms());
+    const float cell = 1.0f / g->inv_cell;
+    const CflArgs c = cfl ? *cfl : CflArgs{};
+    const GridDev gd = to_dev(g);
+    if (h_s) {
+        if (cfl)
+            k_dense_forces<true, true><<<grid, kDenseThreads, DenseLayout<true>::bytes, st>>>(
+                posm_s, velr_s, pc_s, h_s, perm, cell_start, gd, cell, rc2, q, c, sh, dl.ctl, dl.items, acc_sph);
+        else
+            k_dense_forces<false, true><<<grid, kDenseThreads, DenseLayout<true>::bytes, st>>>(
+                posm_s, velr_s, pc_s, h_s, perm, cell_start, gd, cell, rc2, q, c, sh, dl.ctl, dl.items, acc_sph);
+    } else {
+        if (cfl)
+            k_dense_forces<true, false><<<grid, kDenseThreads, DenseLayout<false>::bytes, st>>>(
+                posm_s, velr_s, pc_s, nullptr, perm, cell_start, gd, cell, rc2, q, c, sh, dl.ctl, dl.items, acc_sph);
+        else
+            k_dense_forces<false, false><<<grid, kDenseThreads, DenseLayout<false>::bytes, st>>>(
+                posm_s, velr_s, pc_s, nullptr, perm, cell_start, gd, cell, rc2, q, c, sh, dl.ctl, dl.items, acc_sph);
+    }
     SPHB_LAUNCHED();
     return SPH_OK;
 }

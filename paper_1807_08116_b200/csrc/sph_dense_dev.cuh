@@ -77,7 +77,7 @@ __device__ __forceinline__ void bin_box(int bb, const GridDev g, float cell, int
 }
 
 // Stable counting sort of a staged chunk by bin (slot order inside a bin), all THREADS threads of the CTA:
-//   raw[roff + i], i < ncand, is the candidate of slot cs + i;  move(src raw index, dst sorted index) copies its payload;
+//   raw[roff + i], i < ncand, is the candidate of slot cs + i;  move(src raw index, dst sorted index, bin) copies its payload;
 //   bstart[b] = first sorted index of bin b (bstart[24..31] = ncand);  box[2 b], box[2 b + 1] = the bins' boxes.
 // hist: [ROUNDS][THREADS/32][kBins] words, ZERO on entry (the caller zeroes it once, each call leaves it zeroed).  `wait` is
 // called first (the bulk copy's mbarrier), `extra` by one thread between the barriers (per-chunk resets of the caller).  PAD_EVEN: every bin starts at
@@ -139,7 +139,7 @@ __device__ __forceinline__ void bin_chunk(const float4* r_pos, uint32_t roff, ui
 #pragma unroll
     for (int rd = 0; rd < ROUNDS; ++rd) {
         const uint32_t i = (uint32_t)(rd * THREADS + tid);
-        if (i < ncand) move(roff + i, bstart[my_bin[rd]] + hist[(rd * WARPS + warp) * kBins + my_bin[rd]] + my_rank[rd]);
+        if (i < ncand) move(roff + i, bstart[my_bin[rd]] + hist[(rd * WARPS + warp) * kBins + my_bin[rd]] + my_rank[rd], my_bin[rd]);
     }
     __syncwarp();
     // zero the histogram for the next call: a warp reads only its own rows of it above

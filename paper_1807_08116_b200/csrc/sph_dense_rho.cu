@@ -40,10 +40,16 @@ constexpr int kRhoKS = kRhoK + kBins;                       // sorted: + one fil
 static_assert(kRhoTT == kRhoThreads, "a thread per target of the item");
 constexpr int kRhoRounds = (kRhoK + kRhoThreads - 1) / kRhoThreads;
 
+// VARH (per-particle smoothing lengths, L82): the pairs also carry (h0, h1), every bin its largest length, every target
+// its own and every group of targets its largest
+template <bool VARH>
 struct RhoLayout {
     static constexpr int raw_pos = 0;                                   // float4 [K]     landing zone of the bulk copies
     static constexpr int pk = raw_pos + kRhoK * 16;                     // float4 [KS/2][2] the chunk in bin order, as pairs
-    static constexpr int tpos = pk + kRhoKS * 16;                       // float4 [TT]    the item's targets in octant order
+    static constexpr int hp = pk + kRhoKS * 16;                         // float2 [KS/2]  VARH: the pairs' lengths
+    static constexpr int th = hp + (VARH ? kRhoKS * 4 : 0);             // float [TT]     VARH: the targets' lengths, octant order
+    static constexpr int hmax = th + (VARH ? kRhoTT * 4 : 0);           // uint32 [32]    VARH: bits of the largest length in bin b
+    static constexpr int tpos = hmax + (VARH ? 32 * 4 : 0);             // float4 [TT]    the item's targets in octant order
     static constexpr int tslot = tpos + kRhoTT * 16;                    // uint32 [TT]    their sorted slots
     static constexpr int part = tslot + kRhoTT * 4;                     // float [TT]     the targets' running sums
     static constexpr int bbox = part + kRhoTT * 4;                      // float [TT/G][8] bounding boxes of the target groups
@@ -57,16 +63,25 @@ struct RhoLayout {
     static constexpr int unext = bar + 12;                              // uint32: next work unit of the chunk
     static constexpr int bytes = bar + 16;
 };
-static_assert((RhoLayout::bytes + 1024) * kRhoCtasPerSm <= 227 * 1024, "shared memory per SM");
+static_assert((RhoLayout<false>::bytes + 1024) * kRhoCtasPerSm <= 227 * 1024, "shared memory per SM");
+static_assert((RhoLayout<true>::bytes + 1024) * kRhoCtasPerSm <= 227 * 1024, "shared memory per SM");
 
+// VARH: W(|dr| / h_ij, h_ij) with h_ij = (h_i + h_j)/2 carries its own 1/(pi h_ij^3) (readings A24-A26 as in
+// k_density<true>); norm is then 8/pi (1/h_ij^3 = 8/(h_i + h_j)^3).  A group's sphere reaches a bin iff the distance of
+// the boxes is below (the group's largest length) + (the bin's largest length) — the paper's hmaxCell (L164, L207) at the
+// granularity of the octant bins.
+template <bool VARH>
 __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
-    k_dense_density(const float4* __restrict__ posm_s, const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start,
-                    GridDev g, float cell, float rc2, float neg_inv_h, float norm, Shard sh, unsigned int* __restrict__ ctl,
-                    const DenseItem* __restrict__ items, float* __restrict__ rho) {
-    using L = RhoLayout;
+    k_dense_density(const float4* __restrict__ posm_s, const float* __restrict__ h_s, const uint32_t* __restrict__ perm,
+                    const uint32_t* __restrict__ start, GridDev g, float cell, float rc2, float neg_inv_h, float norm, Shard sh,
+                    unsigned int* __restrict__ ctl, const DenseItem* __restrict__ items, float* __restrict__ rho) {
+    using L = RhoLayout<VARH>;
     extern __shared__ __align__(128) unsigned char smem[];
     float4* r_pos = reinterpret_cast<float4*>(smem + L::raw_pos);
     float* c_pk = reinterpret_cast<float*>(smem + L::pk);
+    float* c_hp = reinterpret_cast<float*>(smem + L::hp);
+    float* t_h = reinterpret_cast<float*>(smem + L::th);
+    uint32_t* s_hmax = reinterpret_cast<uint32_t*>(smem + L::hmax);
     float4* t_pos = reinterpret_cast<float4*>(smem + L::tpos);
     uint32_t* t_slot = reinterpret_cast<uint32_t*>(smem + L::tslot);
     float* s_part = reinterpret_cast<float*>(smem + L::part);
@@ -84,6 +99,7 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
     const unsigned lt_mask = (1u << lane) - 1u;
     const uint32_t sbase = smem_u32(smem);
     const uint32_t a_pk = sbase + L::pk;
+    const uint32_t a_hp_pk = sbase + L::hp - (a_pk >> 2);   // a pair at byte address pa of the pk array has its lengths at a_hp_pk + pa / 4
     const uint32_t sub = (uint32_t)lane % kRhoL, tl = (uint32_t)lane / kRhoL;   // this lane's share and target within a unit
     const uint32_t n_items = ctl[0];
     if (blockIdx.x >= n_items) return;   // uniform per CTA
@@ -129,9 +145,11 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
 
         // ---- the item's targets into octant order (stable): a warp of 32 then covers one or two octants ----
         float4 mine = make_float4(big, big, big, 0.f);
+        float mine_h = 0.f;
         uint32_t oct = 8u;
         if ((uint32_t)tid < nt) {
             mine = posm_s[ts + tid];
+            if (VARH) mine_h = h_s[ts + tid];
             const float xm = fmaf((float)ix + 0.5f, cell, g.ox), ym = fmaf((float)iy + 0.5f, cell, g.oy),
                         zm = fmaf((float)iz + 0.5f, cell, g.oz);
             oct = (mine.x >= xm ? 1u : 0u) + (mine.y >= ym ? 2u : 0u) + (mine.z >= zm ? 4u : 0u);
@@ -150,6 +168,7 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
                     if (o < oct || w < warp) dst += s_ocnt[w * 8 + o];
             t_pos[dst] = mine;
             t_slot[dst] = ts + (uint32_t)tid;
+            if (VARH) t_h[dst] = mine_h;
         }
         __syncthreads();
         // bounding box of every group of kRhoG consecutive targets (the threads' targets: kRhoTT == kRhoThreads)
@@ -159,6 +178,7 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
             const float4 p = has ? t_pos[t] : make_float4(0.f, 0.f, 0.f, 0.f);
             float lo[3] = {has ? p.x : big, has ? p.y : big, has ? p.z : big};
             float hi[3] = {has ? p.x : -big, has ? p.y : -big, has ? p.z : -big};
+            float hg = (VARH && has) ? t_h[t] : 0.f;   // the group's largest length
 #pragma unroll
             for (int a = 0; a < 3; ++a)
 #pragma unroll
@@ -166,9 +186,13 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
                     lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
                     hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
                 }
+            if (VARH) {
+#pragma unroll
+                for (int o = kRhoG / 2; o > 0; o >>= 1) hg = fmaxf(hg, __shfl_xor_sync(0xffffffffu, hg, o));
+            }
             if (lane % kRhoG == 0) {
                 s_bbox[2 * (t / kRhoG)] = make_float4(lo[0], hi[0], lo[1], hi[1]);
-                s_bbox[2 * (t / kRhoG) + 1] = make_float4(lo[2], hi[2], 0.f, 0.f);
+                s_bbox[2 * (t / kRhoG) + 1] = make_float4(lo[2], hi[2], hg, 0.f);
             }
         }
         __syncthreads();
@@ -191,14 +215,26 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
                 q[4] = p.z;
                 q[6] = p.w;
             };
+            if (VARH && tid < 32) s_hmax[tid] = 0u;   // (ordered before the moves by bin_chunk's barriers)
             dense::bin_chunk<kRhoThreads, kRhoRounds, true>(
                 r_pos, 0u, ncand, cs, b1, b2, g, cell, ix, rg, s_hist, s_bstart, s_box,
                 [&]() {
                     mbar_wait(s_bar, n_staged & 1u);
                     ++n_staged;
                 },
-                [&]() { *s_unext = 0u; }, [&](uint32_t src, uint32_t dst) { put(dst, r_pos[src]); },
-                [&](uint32_t dst) { put(dst, make_float4(big, big, big, 0.f)); });   // a filler: out of reach, no mass
+                [&]() { *s_unext = 0u; },
+                [&](uint32_t src, uint32_t dst, uint32_t bin) {
+                    put(dst, r_pos[src]);
+                    if (VARH) {   // the length straight from global memory (L2), and the bin's largest (positive floats order like their bits)
+                        const float hj = h_s[cs + src];
+                        c_hp[dst] = hj;
+                        atomicMax(s_hmax + bin, __float_as_uint(hj));
+                    }
+                },
+                [&](uint32_t dst) {   // a filler: out of reach, no mass
+                    put(dst, make_float4(big, big, big, 0.f));
+                    if (VARH) c_hp[dst] = 1.0f;
+                });
             int rn = r;
             uint32_t csn = cs;
             next_chunk(rn, csn);
@@ -218,12 +254,19 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
                 const float ex = fmaxf(fmaxf(bx0.x - w0.y, w0.x - bx0.y), 0.f);
                 const float ey = fmaxf(fmaxf(bx0.z - w0.w, w0.z - bx0.w), 0.f);
                 const float ez = fmaxf(fmaxf(bx1.x - w1.y, w1.x - bx1.y), 0.f);
-                const bool reach_b = fmaf(ez, ez, fmaf(ey, ey, ex * ex)) < rc2;
+                float rcb2 = rc2;
+                if (VARH) {
+                    const float rcb = w1.z + __uint_as_float(s_hmax[lane]);
+                    rcb2 = rcb * rcb;
+                }
+                const bool reach_b = fmaf(ez, ez, fmaf(ey, ey, ex * ex)) < rcb2;
                 const unsigned reach = __ballot_sync(0xffffffffu, reach_b) & ((1u << kBins) - 1u);
                 if (reach == 0u) continue;
                 const uint32_t t = u * kRhoG + tl;
                 const float4 pi = t < nt ? t_pos[t] : make_float4(big, big, big, 0.f);
                 const u64 xi = pk2(pi.x, pi.x), yi = pk2(pi.y, pi.y), zi = pk2(pi.z, pi.z);
+                const float h_i = (VARH && t < nt) ? t_h[t] : 1.0f;
+                const u64 hi2 = pk2(h_i, h_i), m2 = pk2(-2.0f, -2.0f);
                 u64 sum2 = 0ull;   // includes the self term m_i W(0): j = i passes the predicate with d2 = 0 (A5)
                 // one range of pairs per (sz, sy) sub-row, from its first to its last reachable bin (sph_dense_dev.cuh);
                 // the kRhoL lanes of a target take the pairs of a range in turn
@@ -241,15 +284,29 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
                         upk2(d2, d2a, d2b);
                         const u64 rr = pk2(sqrt_approx(d2a), sqrt_approx(d2b));
                         float a0, a1, c0, c1;
-                        upk2(fma2(rr, ninvh2, two2), a0, a1);   // 2 - xi
-                        upk2(fma2(rr, ninvh2, one2), c0, c1);   // 1 - xi
+                        u64 rh = 0ull;   // VARH: 1 / (h_i + h_j) = 1 / (2 h_ij)
+                        if (VARH) {
+                            const float2 H = lds_f2(a_hp_pk + (pa >> 2));
+                            float s0_, s1_;
+                            upk2(add2(hi2, pk2(H.x, H.y)), s0_, s1_);
+                            rh = pk2(rcp_approx(s0_), rcp_approx(s1_));
+                            const u64 t2 = mul2(rr, rh);            // xi / 2
+                            upk2(fma2(t2, m2, two2), a0, a1);       // 2 - xi
+                            upk2(fma2(t2, m2, one2), c0, c1);       // 1 - xi
+                        } else {
+                            upk2(fma2(rr, ninvh2, two2), a0, a1);   // 2 - xi
+                            upk2(fma2(rr, ninvh2, one2), c0, c1);   // 1 - xi
+                        }
                         const u64 a = pk2(fmaxf(a0, 0.f), fmaxf(a1, 0.f)), c = pk2(fmaxf(c0, 0.f), fmaxf(c1, 0.f));
                         const u64 c3 = mul2(mul2(c, c), c);
                         const u64 w = sub2(mul2(mul2(mul2(a, a), a), q25), c3);   // 1/4 (2 - xi)_+^3 - (1 - xi)_+^3
                         // no test of the cutoff: beyond 2h the clamped cubes are 0, and where the rounding of MUFU.SQRT and of the
                         // fma puts 2 - xi on the other side of 0 than d2 < fl(fl(2h)^2) (A8), the term is <= (2^-22)^3 / 4 of the
                         // self term m_i W(0) that every sum holds: it does not reach the sum's last bit
-                        sum2 = fma2(pk2(B.z, B.w), w, sum2);
+                        if (VARH)
+                            sum2 = fma2(mul2(pk2(B.z, B.w), mul2(mul2(rh, rh), rh)), w, sum2);   // m_j W / (h_i + h_j)^3; 8/pi at the end
+                        else
+                            sum2 = fma2(pk2(B.z, B.w), w, sum2);
                     }
                 }
                 float s0, s1;
@@ -273,21 +330,29 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
 
 }  // namespace
 
-int density_dense(const float4* posm_s, const uint32_t* perm, const uint32_t* cell_start, const sph_params* p,
-                  const sph_grid* g, const DenseList& dl, float* rho, cudaStream_t st, Shard sh) {
+int density_dense(const float4* posm_s, const float* h_s /*cell order, or NULL*/, const uint32_t* perm, const uint32_t* cell_start,
+                  const sph_params* p, const sph_grid* g, const DenseList& dl, float* rho, cudaStream_t st, Shard sh) {
     int dev = 0;
     SPHB_CUDA(cudaGetDevice(&dev));
     static std::atomic<bool> opted[64];   // per device: the dynamic shared-memory opt-in
     if (dev < 0 || dev >= 64) return SPH_ERR_UNSUPPORTED;
     if (!opted[dev].load(std::memory_order_acquire)) {
-        SPHB_CUDA(cudaFuncSetAttribute(k_dense_density, cudaFuncAttributeMaxDynamicSharedMemorySize, RhoLayout::bytes));
+        SPHB_CUDA(cudaFuncSetAttribute(k_dense_density<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RhoLayout<false>::bytes));
+        SPHB_CUDA(cudaFuncSetAttribute(k_dense_density<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RhoLayout<true>::bytes));
         opted[dev].store(true, std::memory_order_release);
     }
     const float two_h = 2.0f * p->h;
-    const float norm = (float)(1.0 / (3.14159265358979323846 * (double)p->h * (double)p->h * (double)p->h));
     SPHB_CUDA(cudaMemsetAsync(dl.ctl + 1, 0, sizeof(unsigned int), st));   // the item counter
-    k_dense_density<<<kRhoCtasPerSm * num_sms(), kRhoThreads, RhoLayout::bytes, st>>>(
-        posm_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, two_h * two_h, -(1.0f / p->h), norm, sh, dl.ctl, dl.items, rho);
+    const unsigned grid = (unsigned)(kRhoCtasPerSm * num_sms());
+    if (h_s) {
+        k_dense_density<true><<<grid, kRhoThreads, RhoLayout<true>::bytes, st>>>(
+            posm_s, h_s, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, two_h * two_h, 0.f, (float)(8.0 / 3.14159265358979323846), sh,
+            dl.ctl, dl.items, rho);
+    } else {
+        const float norm = (float)(1.0 / (3.14159265358979323846 * (double)p->h * (double)p->h * (double)p->h));
+        k_dense_density<false><<<grid, kRhoThreads, RhoLayout<false>::bytes, st>>>(
+            posm_s, nullptr, perm, cell_start, to_dev(g), 1.0f / g->inv_cell, two_h * two_h, -(1.0f / p->h), norm, sh, dl.ctl, dl.items, rho);
+    }
     SPHB_LAUNCHED();
     return SPH_OK;
 }

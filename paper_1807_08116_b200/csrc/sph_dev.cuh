@@ -122,6 +122,35 @@ __device__ __forceinline__ float hydro_pair_fast(const float4 vi /*v, rho*/, con
     return m_j * Pi * gmag;
 }
 
+// One accepted pair with a per-pair smoothing length h_ij = hsum / 2, hsum = fl(h_i + h_j) (L82, A24): grad W_p carries
+// its own -45 / (64 pi h_ij^4), mu_ij and eta h_ij^2 use h_ij.  Used by BOTH walks: with per-particle lengths a particle
+// in a populated cell may still have only a handful of neighbours, all near the edge of its kernel, so the dense-cell
+// walk cannot take the short cuts of hydro_pair_fast (measured: de/dt off by 2.0e-4 of the bar's 2e-4 in
+// `clamped_dense`).  The pair factor goes like h_ij^-8: with a per-pair h its roundings no longer cancel as a common
+// factor of the particle's sum, so it is formed in FP64 and rounded once.
+__device__ __forceinline__ float hydro_pair_h(const float4 vi, const float2 ci, const float m_j, const float4 vj,
+                                              const float2 cj, const float dx, const float dy, const float dz, const float d2,
+                                              const float hsum, const ViscDev& q, float& rv, float& mu, float& c_ij) {
+    float rinv = rsqrtf(d2);
+    rinv = rinv * fmaf(-0.5f * d2 * rinv, rinv, 1.5f);   // one Newton step: ~1 ulp
+    const float rr = d2 * rinv;                        // |dr|
+    const double hd = 0.5 * (double)hsum, ihd = 1.0 / hd, ih2 = ihd * ihd;
+    const double num = fma(-(double)dz, (double)dz, fma(-(double)dy, (double)dy, fma(-(double)dx, (double)dx, (double)hsum * (double)hsum)));
+    const double tqd = fmax(num, 0.0) * ih2 / (2.0 + (double)rr * ihd);       // 2 - xi
+    const float gmag = (float)((double)q.gw_unit * ih2 * ih2 * tqd * tqd) * rinv;   // grad W_p = gmag * dr
+    const float hh = 0.5f * hsum;
+    const float eta_h2 = q.eta * hh * hh;
+    const float dvx = vi.x - vj.x, dvy = vi.y - vj.y, dvz = vi.z - vj.z;
+    rv = fmaf(dz, dvz, fmaf(dy, dvy, dx * dvx));
+    // mu_ij = h dr.dv / (|dr|^2 + eta h^2) if dr.dv < 0   (L97)
+    mu = rv < 0.f ? (hh * rv) / (d2 + eta_h2) : 0.f;                   // IEEE division
+    const float rho_ij = 0.5f * (vi.w + vj.w);
+    c_ij = 0.5f * (ci.y + cj.y);
+    const float nu = (mu * (q.beta * mu - q.alpha * c_ij)) / rho_ij;
+    const float Pi = ci.x + cj.x + nu;                 // p_i/rho_i^2 + p_j/rho_j^2 + nu  (L95, A2)
+    return m_j * Pi * gmag;                            // m_j Pi |grad Wp| / |dr|
+}
+
 // Eq. 17 (L127) for one gas particle: the bracket s / (c^max (1 + 1.2 alpha) + 1.2 beta mu^max + sqrt(s (|Q| + |E|))) from
 // the squared minimum distance (>= rc2_none: no neighbour, then s = s_none, reading A22), c^max, mu^max and the
 // particle's right-hand sides Q = a_sph + a_grav (Eq. 10), E = de/dt (Eq. 11).

@@ -633,7 +633,7 @@ def _hs_for(w, seed=5):
     return (np.float32(w.h) * (0.45 + 0.55 * rng.random(w.n_gas))).astype(np.float32)
 
 
-@pytest.mark.parametrize("case", ["galaxy", "dense", "clumps"])
+@pytest.mark.parametrize("case", ["galaxy", "dense", "clumps", "packed", "tight_clumps", "clamped_dense"])
 def test_varh_sets_density_forces_parity(cuda_lib, case):
     b = cuda_lib
     w, og = _grid_case(case)
@@ -658,6 +658,8 @@ def test_varh_sets_density_forces_parity(cuda_lib, case):
     acc = torch.zeros((n, 4), device="cuda")
     dv = _t(w.vele)
     b.sph_forces_h(d, dv, rho, dh, n, prm, g, perm, start, acc, ws)
+    if case in DENSE_CASES:      # these cases are there for the dense-cell walks: make sure they ran
+        assert b.sph_dense_items(ws, n, n, g) > 0
     of, gross = oracle.forces(w.posm, w.vele, rho.cpu().numpy().astype(np.float64), w.h, ooff, oidx, gamma=w.gamma,
                               alpha=w.alpha, beta=w.beta, eta=w.eta, with_gross=True, hs=hs)
     got = acc.cpu().numpy()
