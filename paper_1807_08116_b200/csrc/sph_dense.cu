@@ -16,16 +16,16 @@
 //   * a WARP takes a target: lane b finds out whether the sphere reaches bin b (distance to the octant's box, pulled out
 //     by eps and open-ended on the outside of boundary cells, where clamped particles sit); the reachable bins, in bin
 //     order, are the target's candidate list, addressed by a flat position through at most four slot ranges, so the 32
-//     lanes test 32 candidates per step with every lane busy whatever the bins' sizes;
+//     lanes test 64 candidates per step (two per lane) with every lane busy whatever the bins' sizes;
 //   * accepted candidates are compacted by ballot + popc into a per-warp ring queue and the pair term (sph_dev.cuh:
-//     hydro_pair) runs on full warps, its operands read from the staged tile;
+//     hydro_pair_fast; hydro_pair_h with per-particle lengths) runs on full warps, its operands read from the staged tile;
 //   * a lane's partial sum over one chunk (<= kDenseK/32 candidates) is plain FP32; the 32 partials are added across the
 //     warp in FP64 (one butterfly for the four sums) and accumulated per target in FP64 shared memory, so a target's sum
 //     has a fixed order (bitwise reproducible) and is at least as accurate as the compensated FP32 sum of the sparse walk.
 // Work items come from the list the grid build writes (grid.cu: k_scan_apply) — or k_dense_list for the stand-alone
 // calls — and are drawn from a counter by a persistent grid (kDenseCtasPerSm CTAs per SM).
-// The density pass (a7) stays on the thread-per-slot walk everywhere: its pair term is ~15 instructions, so nothing is
-// won by compacting the accepted pairs, and the staged, binned walk measured slower (46 against 31 ms at config 4).
+// The density pass (a7) of these cells is sph_dense_rho.cu: the same staging and binning, but four lanes per target and
+// no compaction — its pair term is ~15 instructions.
 #include <type_traits>
 #include "sph_dense_dev.cuh"
 
