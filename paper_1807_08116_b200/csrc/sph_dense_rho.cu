@@ -215,14 +215,19 @@ __global__ void __launch_bounds__(kRhoThreads, kRhoCtasPerSm)
                 q[4] = p.z;
                 q[6] = p.w;
             };
-            if (VARH && tid < 32) s_hmax[tid] = 0u;   // (ordered before the moves by bin_chunk's barriers)
             dense::bin_chunk<kRhoThreads, kRhoRounds, true>(
                 r_pos, 0u, ncand, cs, b1, b2, g, cell, ix, rg, s_hist, s_bstart, s_box,
                 [&]() {
                     mbar_wait(s_bar, n_staged & 1u);
                     ++n_staged;
                 },
-                [&]() { *s_unext = 0u; },
+                [&]() {   // one thread, after every warp has left the previous chunk and before the moves
+                    *s_unext = 0u;
+                    if (VARH) {
+#pragma unroll
+                        for (int bq = 0; bq < 32; ++bq) s_hmax[bq] = 0u;
+                    }
+                },
                 [&](uint32_t src, uint32_t dst, uint32_t bin) {
                     put(dst, r_pos[src]);
                     if (VARH) {   // the length straight from global memory (L2), and the bin's largest (positive floats order like their bits)

@@ -857,7 +857,7 @@ def _complete(reps, name, n):
 
 
 @pytest.mark.parametrize("case,world,sigma", [("galaxy1", 2, None), ("tight_clumps", 3, None), ("packed", 2, None),
-                                               ("galaxy0", 3, 1.3)])
+                                               ("galaxy0", 3, 1.3), ("packed", 3, 1.3)])
 def test_sph_passes_shared_sequential(cuda_lib, case, world, sigma):
     """the SPH passes shared over `world` ranks — every rank sorts, then runs DC and HFC for every world-th
     tile of 128 sorted slots (dense-cell work items by their first slot) and writes zeros elsewhere; rho and acc_sph are
