@@ -350,12 +350,14 @@ def test_cfl_step_parity(cuda_lib, case):
     assert np.isinf(dt.item())
 
 
-@pytest.mark.parametrize("cfg,scale,steps,sigma", [(0, 1.0, 10, None), (0, 0.5, 3, 0.8)])
+@pytest.mark.parametrize("cfg,scale,steps,sigma", [(0, 1.0, 10, None), (0, 0.5, 3, 0.8), ("packed", None, 2, 1.3),
+                                                   ("tight_clumps", None, 2, None)])
 def test_adaptive_step_parity(cuda_lib, cfg, scale, steps, sigma):
     """sph_step_cfl against oracle.step(c_cfl=): the step size comes from Eq. 17 inside HFC(predictor), on the device, free
     running.  The steps taken are compared one by one, the state at the end at the step-parity tolerances."""
     b = cuda_lib
-    w = wl.make_workload(cfg, scale=scale)
+    # (the named cases have populated cells: Eq. 17 gathered by the dense-cell walk, with one global h and with per-particle h)
+    w = wl.make_workload(cfg, scale=scale) if isinstance(cfg, int) else _grid_case(cfg)[0]
     ng = w.n_gas
     sim = b.Simulation(w, sigma=sigma)
     st = _oracle_state(w)
@@ -369,13 +371,19 @@ def test_adaptive_step_parity(cuda_lib, cfg, scale, steps, sigma):
                                  alpha=w.alpha, beta=w.beta, eta=w.eta)
         hs = d["hs"]
         got = float(sim.dt_used.item())
-        assert got < dt_max and abs(got - d["dt"]) < 2e-5 * d["dt"], (k, got, d["dt"])
+        # the bracket of Eq. 17 holds sqrt(s (|Q| + |E|)): a relative error e of the particle's right-hand sides (bar 2e-4)
+        # is at most e / 2 on dt.  At config 0 the sound-speed term dominates and 2e-5 holds; in the packed / clumped cases
+        # the acceleration term does, and the bound itself is the tolerance
+        tol_dt = 2e-5 if isinstance(cfg, int) else 1e-4
+        assert got < dt_max and abs(got - d["dt"]) < tol_dt * d["dt"], (k, got, d["dt"])
         t_gpu += got
         t_orc += d["dt"]
     v = sim.vele.cpu().numpy().astype(np.float64)
     check_values(v[:, :3], st.vele[:, :3], f"v after {steps} adaptive steps", max_tol=5e-5, med_tol=2e-6)
     assert np.abs(sim.posm.cpu().numpy()[:, :3] - st.posm[:, :3]).max() < 2e-5
     check_density(sim.rho.cpu().numpy()[:ng], st.rho, "rho after adaptive steps")
+    if not isinstance(cfg, int):
+        assert b.sph_dense_items(sim.ws, ng, w.n_total, sim.grid) > 0
     # a ceiling below the criterion: the fixed step, bit for bit
     sim_a, sim_b = b.Simulation(w), b.Simulation(w)
     sim_a.step(dt=1e-6, c_cfl=0.6)
