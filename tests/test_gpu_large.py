@@ -173,6 +173,35 @@ def test_full_size_sph_only_config4(cuda_lib):
     assert nn.max() > 500           # the clump cores
 
 
+def test_full_size_sph_only_config4_varh(cuda_lib):
+    """config 4 with per-particle smoothing lengths (NEXT-2, L82): seeded lengths in [0.3, 1] of the cap, spatially
+    uncorrelated (the hardest case for the pair cutoff and for the largest-length-per-bin pruning of the dense-cell
+    walks) — density and forces on the subset against the oracle's h_ij sums, the launch configuration bench.py
+    --sigma times (dense-cell walks with VARH + thread-per-slot walks)."""
+    b = cuda_lib
+    w = wl.make_workload(4)
+    ng = w.n_gas
+    rng = np.random.Generator(np.random.Philox(key=[44, 9]))
+    hs = (np.float32(w.h) * (0.3 + 0.7 * rng.random(ng))).astype(np.float32)
+    sim = b.Simulation(w, sigma=0.0)                      # sigma = 0: the lengths are kept as given
+    sim.hsml.copy_(torch.from_numpy(hs))
+    og, okey, ocount, ostart, operm = _check_structures(b, sim, w)
+    g_idx, _ = _subset(w, okey, ocount)
+    sim.evaluate()
+    assert b.sph_dense_items(sim.ws, ng, w.n_total, sim.grid) > 50000
+    assert b.sph_workspace_status(sim.ws, ng, w.n_total, sim.grid) == 0
+    sort = (okey, ostart, operm)
+    off, idx = oracle.neighbours(w.posm, ng, w.h, targets=g_idx, method="grid", grid=og, sort=sort, hs=hs)
+    rho_gpu = sim.rho.cpu().numpy()
+    check_density(rho_gpu[g_idx], oracle.density(w.posm, w.h, off, idx, targets=g_idx, hs=hs), "rho subset varh")
+    of, gross = oracle.forces(w.posm, w.vele, rho_gpu.astype(np.float64), w.h, off, idx, targets=g_idx, gamma=w.gamma,
+                              alpha=w.alpha, beta=w.beta, eta=w.eta, with_gross=True, hs=hs)
+    acc = sim.acc_sph.cpu().numpy()
+    check_values(acc[g_idx, :3], of[:, :3], "a_sph subset varh", gross=gross[:, 0])
+    check_values(acc[g_idx, 3], of[:, 3], "de/dt subset varh", gross=gross[:, 1])
+    assert np.diff(off).max() > 100
+
+
 def test_full_size_collisionless_next3(cuda_lib):
     """N_g = 0 (SP, DC, HFC skipped, L150) at N = 2^22.  One step: Eqs. 12-16 reduce to
     velocity Verlet (pin P8), checked on ALL particles from the GPU's own accelerations; the accelerations
