@@ -299,6 +299,10 @@ __global__ void __launch_bounds__(kDenseThreads, kDenseCtasPerSm)
                     const bool reach_b = fmaf(ez, ez, fmaf(ey, ey, ex * ex)) < rcb2;   // lanes >= kBins: their box is out of reach
                     // the reachable bins, in bin order, are the target's candidates in this segment: four slot ranges
                     const unsigned reach = __ballot_sync(0xffffffffu, reach_b);
+                    if (reach == 0u) {   // nothing of this segment in reach (with per-particle lengths: most segments)
+                        first += ncand;
+                        continue;
+                    }
                     const dense::Groups G = dense::candidate_groups(reach, s_bstart + 32u * sgi, first);
                     first += ncand;
                     const uint32_t T = G.T;
