@@ -329,6 +329,21 @@ int sph_update(float* posm /*or NULL if corrector*/, float* vele, int64_t n_gas,
                const sph_grid* g /*HOST, may be NULL if n_gas == 0*/, float dt, int corrector, const float* acc_sph,
                const float* acc_grav, void* ws, size_t ws_bytes, void* stream);
 
+/* ---- Eq. 4 without any allocation: for callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, serving loops, harnesses that forbid it) ----
+ * nbody_pp_gravity_static is nbody_pp_gravity with the workspace replaced by a fixed device array inside the library
+ * (csrc/noalloc.cu: 12 MiB, held by every GPU that loads the library until the process exits): the caller passes inputs
+ * and outputs only, and the call makes no cudaMalloc / cudaFree / allocating library call.  Same kernels, same results
+ * bit for bit as nbody_pp_gravity on the same input.
+ *   posm     DEVICE [n_total][4] (x, y, z, m), 16-byte aligned      acc_grav  DEVICE [n_total][4] out, 16-byte aligned
+ *   n_total  <= nbody_pp_gravity_static_max() (65536); more returns SPH_ERR_WORKSPACE — the fixed scratch is too small,
+ *            use nbody_pp_gravity with a caller-owned workspace.
+ * ALL calls on a device share the one array: it keeps the last call's contents (what must start at zero is cleared by
+ * every call, on its stream), and calls that overlap on the GPU — two streams, two host threads on one device — RACE on
+ * it: serialise them.  Other errors: SPH_ERR_ARG, SPH_ERR_UNSUPPORTED (delta < 0), SPH_ERR_CUDA.  Asynchronous on `stream`. */
+int64_t nbody_pp_gravity_static_max(void);
+int nbody_pp_gravity_static(const float* posm, int64_t n_total, float G, float delta, float* acc_grav, void* stream);
+
 /* Stage timing: after sph_set_profiling(1) every stage the calling thread enqueues is bracketed
  * by CUDA events on the call's stream; sph_get_stage_ms() returns the milliseconds summed over all
  * calls since that switch-on (at most 4096 stage spans) for

@@ -29,6 +29,7 @@ EXPORTS = (
     "sph_gravity_path", "sph_dense_items", "sph_workspace_status", "sph_position_share", "nbody_pp_gravity_share", "nbody_pp_gravity_finish",
     "sph_workspace_gravity_sums", "sph_smoothing_lengths", "sph_density_h", "sph_forces_h", "sph_evaluate_h", "sph_step_h", "sph_neighbour_lists_h", "sph_step_cfl",
     "sph_position_share_sph", "sph_renew_hsml", "sph_forces_share", "sph_update",
+    "nbody_pp_gravity_static", "nbody_pp_gravity_static_max",
 )
 
 
@@ -101,6 +102,8 @@ def load():
     L.sph_renew_hsml.argtypes = [vp, vp, f32, i64, i64, pp, gp, vp, vp, sz, vp]
     L.sph_forces_share.argtypes = [vp, vp, i64, i64, C.c_int, C.c_int, pp, gp, vp, vp, vp, sz, vp]
     L.sph_update.argtypes = [vp, vp, i64, i64, gp, f32, C.c_int, vp, vp, vp, sz, vp]
+    L.nbody_pp_gravity_static.argtypes = [vp, i64, f32, f32, vp, vp]
+    L.nbody_pp_gravity_static_max.restype = i64
     L.sph_workspace_gravity_sums.argtypes = [i64, i64, gp, C.POINTER(sz), C.POINTER(sz)]
     L.sph_gravity_path.argtypes = [vp, sz, i64, i64, gp, C.POINTER(C.c_int), vp]
     L.sph_dense_items.argtypes = [vp, sz, i64, i64, gp, C.POINTER(C.c_uint32), vp]
@@ -226,6 +229,17 @@ def sph_evaluate(posm, vele, n_gas, n_halo, params, grid, rho, acc_sph, acc_grav
     g = C.byref(grid) if grid is not None else None
     _chk("sph_evaluate", load().sph_evaluate(_ptr(posm), _ptr(vele), int(n_gas), int(n_halo), C.byref(params), g,
                                              _ptr(rho), _ptr(acc_sph), _ptr(acc_grav), p, nb, _stream()))
+
+
+def nbody_pp_gravity_static(posm, n_total, G, delta, acc_grav):
+    """Eq. 4 with the library's own fixed scratch: no workspace, no allocation; n_total <= nbody_pp_gravity_static_max().
+    Calls on one device share that scratch and must not overlap on the GPU (include/sph_b200.h)."""
+    _chk("nbody_pp_gravity_static", load().nbody_pp_gravity_static(_ptr(posm), int(n_total), float(G), float(delta),
+                                                                   _ptr(acc_grav), _stream()))
+
+
+def nbody_pp_gravity_static_max() -> int:
+    return int(load().nbody_pp_gravity_static_max())
 
 
 # ------------------------------------------------------------------ NEXT-4: stages of a step, target slices

@@ -12,7 +12,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 PKG = os.path.dirname(HERE)
 LIB = os.path.join(PKG, "libsph_b200.so")
-SOURCES = ["api.cu", "gravity.cu", "gravity_sym.cu", "grid.cu", "sph.cu", "sph_dense.cu", "sph_dense_rho.cu", "step.cu", "host.cu", "nbrlist.cu"]
+SOURCES = ["api.cu", "gravity.cu", "gravity_sym.cu", "grid.cu", "sph.cu", "sph_dense.cu", "sph_dense_rho.cu", "step.cu", "host.cu", "nbrlist.cu", "noalloc.cu"]
 DEPS = SOURCES + ["common.cuh", "grav_dev.cuh", "sph_dev.cuh", "sph_dense_dev.cuh", "tma_dev.cuh", os.path.join("..", "..", "include", "sph_b200.h")]
 
 
