@@ -932,6 +932,38 @@ def test_sph_passes_shared_sequential(cuda_lib, case, world, sigma):
         b.sph_renew_hsml(s0.posm, s0.rho, 0.0, ng, nh, s0.params, s0.grid, s0.rho, s0.ws)
 
 
+def test_sharded_step_through_nccl_world1(cuda_lib):
+    """The collectives of sharded.py as NCCL runs them (a process group of ONE rank — the box has one GPU): the int64 SUM
+    all-reduce of the fixed-point sums and the int32 SUM all-reduces of the bit patterns of rho and acc_sph, on the views
+    ShardedSimulation hands them, with the SPH passes shared.  Two steps reproduce the plain step bit for bit."""
+    import socket
+    import torch.distributed as dist
+    from paper_1807_08116_b200.sharded import ShardedSimulation
+    b = cuda_lib
+    w = wl.make_workload(1, scale=0.75)
+    n = w.n_total
+    ref = b.Simulation(w)
+    ref.step()
+    ref.step()
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    assert not dist.is_initialized()
+    dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1,
+                            device_id=torch.device("cuda", torch.cuda.current_device()))
+    try:
+        sim = ShardedSimulation(w, 0, 1, share_sph=True)
+        sim.step()
+        sim.step()
+        torch.cuda.synchronize()
+        assert sim.path == "pair_symmetric" and sim.exchanged_bytes > 0
+        for x, y in ((sim.posm, ref.posm), (sim.vele, ref.vele), (sim.rho, ref.rho), (sim.acc_sph, ref.acc_sph),
+                     (sim.acc_grav[:n], ref.acc_grav)):
+            assert torch.equal(x, y)
+    finally:
+        dist.destroy_process_group()
+
+
 @pytest.mark.parametrize("masses", ["equal", "random", "zero_mass"])
 def test_gravity_shares_add_up(cuda_lib, masses):
     """nbody_pp_gravity_share over 3 ranks + the exchange + nbody_pp_gravity_finish against the one-call evaluation:
