@@ -470,6 +470,22 @@ def run_ours(args, w):
         # accepted force pair ~60 more; one density pass and two forces passes per step
         cand, acc = pairs["candidate_pairs"], pairs["accepted_pairs"]
         lane_ops = (cand * 7 + acc * 12) + 2 * (cand * 7 + acc * 60)
+        if roofline is None:
+            # no gravity (config 4): the dominant kernel is the hydro-force walk, bound by instruction issue / FP32 ALU.
+            # ALGORITHMIC lane-operations of ONE forces pass (27-cell candidates x 7 + accepted pairs x 60, an FMA counted
+            # once) x 2 flops, over the forces stage's time per pass (EOS gather + thread-per-slot walk of the
+            # sparse cells + dense-cell walk; the dense-cell walk is ~90 % of it, profiles/launches_c4_r02.md)
+            f_ops = 2.0 * (cand * 7 + acc * 60)
+            f_ach = f_ops / (0.5 * forc_ms * 1e-3) / 1e12
+            roofline = {"kernel": "k_dense_forces" if pairs.get("dense_walk_items") else "k_forces", "bound": "alu",
+                        "achieved": f_ach, "peak": alu_peak_tflops, "unit": "TFLOP/s", "frac": f_ach / alu_peak_tflops,
+                        "traffic": None, "kernel_ms": 0.5 * forc_ms, "launches_per_step": 2,
+                        "peak_source": f"2*128*148*sm_max_mhz ({peak_src} sm_max_mhz={sm_max:.0f})",
+                        "note": "achieved = 2 x ALGORITHMIC FP32 lane-operations of one hydro-force pass (27-cell candidate "
+                                "tests x 7 + accepted pairs x 60) / forces stage time per pass; the dense-cell walk tests ~2.5 "
+                                "candidates per neighbour instead of the 27-cell count's 6 (octant binning), so the executed "
+                                "operations are fewer than the algorithmic ones; DRAM traffic is irrelevant to this kernel "
+                                "(profiles/sph_dense_r02.md: 2.6 GB per launch)"}
         stages.update({
             "sph_pairs": pairs,
             "sph_candidate_pairs_per_s": 3 * cand / ((dens_ms + forc_ms) * 1e-3),
