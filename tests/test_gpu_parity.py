@@ -434,6 +434,49 @@ def test_dense_walk_chunk_boundaries(cuda_lib, n, dims):
     check_values(got[:, 3], of[:, 3], f"de/dt box {n} {dims}", gross=gross[:, 1])
 
 
+@pytest.mark.parametrize("seed", range(12))
+def test_dense_walk_random_sweep(cuda_lib, seed):
+    """Seeded random grids and populations (compute-sanitizer is closed on this pool: memory safety of the dense walks
+    rests on many shapes): 1-6 cells per axis, 40-700 particles per cell on average with a clump that overfills some cells,
+    every second case with per-particle smoothing lengths; density and forces of ALL particles against the oracle, and
+    the arrays around the outputs untouched."""
+    b = cuda_lib
+    rng = np.random.Generator(np.random.Philox(key=[seed, 77]))
+    dims = tuple(int(x) for x in rng.integers(1, 7, size=3))
+    per_cell = int(rng.integers(40, 700))
+    n = min(int(np.prod(dims)) * per_cell, 16000)
+    w, og = _box_grid_case(n, dims, 500 + seed)
+    k = n // 4                                     # a clump in one corner region: cells far above the average
+    w.posm[:k, :3] = (w.posm[:k, :3] * 0.35).astype(np.float32)
+    varh = seed % 2 == 1
+    hs = (np.float32(w.h) * (0.4 + 0.6 * rng.random(n))).astype(np.float32) if varh else None
+    d, g, perm, start, ws = _build(b, w, og)
+    prm = b.sph_params.from_workload(w)
+    guard = 64
+    rho_buf = torch.full((n + 2 * guard,), -7.0, device="cuda")
+    acc_buf = torch.full((n + 2 * guard, 4), -7.0, device="cuda")
+    rho, acc = rho_buf[guard:guard + n], acc_buf[guard:guard + n]
+    dv = _t(w.vele)
+    if varh:
+        dh = _t(hs)
+        b.sph_density_h(d, dh, n, prm, g, perm, start, rho, ws)
+        b.sph_forces_h(d, dv, rho, dh, n, prm, g, perm, start, acc, ws)
+    else:
+        b.sph_density(d, n, prm, g, perm, start, rho, ws)
+        b.sph_forces(d, dv, rho, n, prm, g, perm, start, acc, ws)
+    assert b.sph_dense_items(ws, n, n, g) > 0
+    for buf in (rho_buf, acc_buf):
+        assert torch.all(buf[:guard] == -7.0) and torch.all(buf[guard + n:] == -7.0)
+    ooff, oidx = oracle.neighbours(w.posm, n, w.h, method="grid", hs=hs)
+    tag = f"sweep {seed} {dims} n={n}{' varh' if varh else ''}"
+    check_density(rho.cpu().numpy(), oracle.density(w.posm, w.h, ooff, oidx, hs=hs), f"rho {tag}")
+    of, gross = oracle.forces(w.posm, w.vele, rho.cpu().numpy().astype(np.float64), w.h, ooff, oidx, gamma=w.gamma,
+                              alpha=w.alpha, beta=w.beta, eta=w.eta, with_gross=True, hs=hs)
+    got = acc.cpu().numpy()
+    check_values(got[:, :3], of[:, :3], f"a_sph {tag}", gross=gross[:, 0])
+    check_values(got[:, 3], of[:, 3], f"de/dt {tag}", gross=gross[:, 1])
+
+
 def test_coincident_gas_particles(cuda_lib):
     b = cuda_lib
     w = _dense(2000, 8, 0.08)
