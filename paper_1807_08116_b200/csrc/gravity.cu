@@ -136,8 +136,8 @@ constexpr int kStages = 2;
 
 // One CTA: THREADS*I targets (i-tile blockIdx.x) against the sources of chunk blockIdx.y.
 // UNIFORM: all masses are equal (*nonuniform == 0): the factor m_j leaves the loop (11 instead of 12 packed FP32
-// operations per interaction pair) and is applied once, with G, in grav_reduce.  Each variant returns immediately
-// when the flag says the other one applies, so launching both costs one empty grid (~20 us) and no synchronisation.
+// operations per interaction pair) and is applied once, with G, in grav_reduce.  The variant is chosen by the flag on
+// the device (grav_pp_kernel below says how), without synchronisation.
 // Diagonal mode (dg.tiles > 0): the part of the pair-symmetric path that kernel leaves out — each CTA's sources are the
 // column block of dg.tiles tiles that holds its targets; only the blocks c with c % dg.world == dg.rank are done (one
 // GPU's share, NEXT-4), and the FP32 sums are added, in fixed point, to the accumulators dg.acc64 of gravity_sym.cu.
@@ -145,17 +145,13 @@ struct GravDiag {
     int tiles, rank, world;
     long long* acc64;
 };
-template <int I, int THREADS, int MINB, bool ZERO_SOFT, int UNROLL = 2, bool UNIFORM = false>
-__global__ void __launch_bounds__(THREADS, MINB)
-    grav_pp_kernel(const float4* __restrict__ posm /*targets*/, const float4* __restrict__ pk, int n, int tiles_total,
-                   int tiles_per_chunk, const GravDiag dg, float eps2, float4* __restrict__ part,
-                   const GravCtl* __restrict__ ctl) {
+template <int I, int THREADS, bool ZERO_SOFT, int UNROLL, bool UNIFORM>
+__device__ __forceinline__ void grav_pp_body(const float4* __restrict__ posm /*targets*/, const float4* __restrict__ pk, int n,
+                                             int tiles_total, int tiles_per_chunk, const GravDiag dg, float eps2,
+                                             float4* __restrict__ part, const GravCtl* __restrict__ ctl) {
     const int diag_tiles = dg.tiles;
     extern __shared__ __align__(128) float4 tiles[];   // [kStages][2 * kTilePairs]
     __shared__ __align__(8) uint64_t full_bar[kStages];
-    // uniform over the grid: this variant runs iff the masses are (not) uniform and, diag_tiles > 0 (the diagonal
-    // blocks that the pair-symmetric kernel leaves out), iff that kernel takes the rest of the evaluation
-    if ((ctl->nonuniform == 0u) != UNIFORM || (ctl->sym != 0u) != (diag_tiles > 0)) return;
 
     const int tid = threadIdx.x;
     // diag_tiles > 0: the sources are the column block of `diag_tiles` tiles that holds this CTA's targets
@@ -278,6 +274,29 @@ __global__ void __launch_bounds__(THREADS, MINB)
     }
 }
 
+// UNIFORM: 1 / 0 = the body without / with the per-source mass factor, a no-op when the flag says the other applies (two
+// launches, one of them empty: the large-N shape, where an empty grid is < 0.01 % of the evaluation); 2 = both bodies
+// behind one branch on the flag in a single launch (the small-N shape: no empty grid on the path).
+template <int I, int THREADS, int MINB, bool ZERO_SOFT, int UNROLL = 2, int UNIFORM = 0>
+__global__ void __launch_bounds__(THREADS, MINB)
+    grav_pp_kernel(const float4* __restrict__ posm /*targets*/, const float4* __restrict__ pk, int n, int tiles_total,
+                   int tiles_per_chunk, const GravDiag dg, float eps2, float4* __restrict__ part,
+                   const GravCtl* __restrict__ ctl) {
+    // uniform over the grid: a variant runs iff the masses are (not) uniform and, dg.tiles > 0 (the diagonal blocks that
+    // the pair-symmetric kernel leaves out), iff that kernel takes the rest of the evaluation
+    const bool uni = ctl->nonuniform == 0u;
+    if ((ctl->sym != 0u) != (dg.tiles > 0)) return;
+    if (UNIFORM == 2) {
+        if (uni)
+            grav_pp_body<I, THREADS, ZERO_SOFT, UNROLL, true>(posm, pk, n, tiles_total, tiles_per_chunk, dg, eps2, part, ctl);
+        else
+            grav_pp_body<I, THREADS, ZERO_SOFT, UNROLL, false>(posm, pk, n, tiles_total, tiles_per_chunk, dg, eps2, part, ctl);
+    } else {
+        if (uni != (UNIFORM == 1)) return;
+        grav_pp_body<I, THREADS, ZERO_SOFT, UNROLL, UNIFORM == 1>(posm, pk, n, tiles_total, tiles_per_chunk, dg, eps2, part, ctl);
+    }
+}
+
 // acc[i] = G [m_0] * sum (dx was r_j - r_i, so the sign of Eq. 4 is in).  Two modes, each a no-op when the device chose the
 // other path.  SYM = false, one-sided path: the S chunk partials of the slice's targets, s = 0..S-1 in fixed order.
 // SYM = true, pair-symmetric path: the fixed-point sums acc64 — exact integers whatever the order, and whichever GPUs,
@@ -344,7 +363,7 @@ int grav_splits(int64_t n_total) {
     return S;
 }
 
-template <int I, int THREADS, int MINB, bool ZERO_SOFT, int UNROLL, bool UNIFORM>
+template <int I, int THREADS, int MINB, bool ZERO_SOFT, int UNROLL, int UNIFORM>
 static int launch_one(dim3 grid, const float4* targets, const float4* pk, int n, int tiles, int tpc, const GravDiag& dg,
                       float eps2, float4* part, const GravCtl* ctl, cudaStream_t st) {
     const size_t smem = (size_t)kStages * kTileBytes;
@@ -361,12 +380,17 @@ template <int I, int THREADS, int MINB, int UNROLL>
 static int launch_grav(const float4* targets, const float4* pk, int n, int tiles, int tpc, int S, const GravDiag& dg,
                        float eps2, bool zero_soft, float4* part, const GravCtl* ctl, cudaStream_t st) {
     dim3 grid((unsigned)cdiv(n, (int64_t)I * THREADS), (unsigned)S);
-    if (zero_soft) {
-        SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, true>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
-        SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, false>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
+    if constexpr (I == 1) {   // the small-N shape: one launch holds both mass variants
+        if (zero_soft)
+            SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, 2>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
+        else
+            SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, 2>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
+    } else if (zero_soft) {
+        SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, 1>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
+        SPHB_TRY((launch_one<I, THREADS, MINB, true, UNROLL, 0>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
     } else {
-        SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, true>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
-        SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, false>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
+        SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, 1>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
+        SPHB_TRY((launch_one<I, THREADS, MINB, false, UNROLL, 0>(grid, targets, pk, n, tiles, tpc, dg, eps2, part, ctl, st)));
     }
     return SPH_OK;
 }
@@ -444,7 +468,10 @@ int gravity(const float4* posm, int64_t n_total, int64_t i0, int64_t i1, float G
     if (n_total <= 0 || i1 <= i0) return SPH_OK;
     const bool whole = (i0 == 0 && i1 == n_total);
     SPHB_TRY(gravity_share(posm, n_total, i0, i1, 0, 1, whole, G, delta, acc_grav, src_pk, grav_part, grav_acc64, grav_flag, st));
-    if (whole) SPHB_TRY(gravity_finish(posm, n_total, G, acc_grav, grav_acc64, grav_flag, st));
+    // (the pair-symmetric path is offered only with softening and from kSymMinN particles on: below that there is nothing
+    // for the finish to do, and no empty grid is launched)
+    if (whole && delta * delta > 0.f && n_total >= kSymMinN)
+        SPHB_TRY(gravity_finish(posm, n_total, G, acc_grav, grav_acc64, grav_flag, st));
     return SPH_OK;
 }
 
