@@ -252,20 +252,21 @@ __global__ void __launch_bounds__(kOffThreads) k_scan_tile_offsets(uint32_t* til
 // TOTALS: tile_offsets[] holds the tiles' TOTALS (k_key_hist gathered them, <= kFuseTiles of them) and the CTA adds up
 // the ones before its own itself — at most 32 KB of L2-resident reads per CTA, against one more kernel on the path.
 template <bool TOTALS>
-__global__ void __launch_bounds__(kScanThreads) k_scan_apply(const uint32_t* __restrict__ count, int64_t M,
-                                                             const uint32_t* __restrict__ tile_offsets,
-                                                             uint32_t* __restrict__ start, uint32_t n_gas,
-                                                             unsigned int* dense_ctl, DenseItem* dense_items) {
-    __shared__ uint32_t ws[kScanThreads / 32];
-    __shared__ uint32_t s_off;
+__global__ void __launch_bounds__(kScanThreads, TOTALS ? 6 : 4) k_scan_apply(const uint32_t* __restrict__ count, int64_t M,
+                                                                const uint32_t* __restrict__ tile_offsets,
+                                                                uint32_t* __restrict__ start, uint32_t n_gas,
+                                                                unsigned int* dense_ctl, DenseItem* dense_items) {
+    constexpr int kWarps = kScanThreads / 32;
+    __shared__ uint32_t ws[kWarps], wv[kWarps];   // per warp: its cells' total; its share of the totals of the tiles before this one
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     uint32_t c[kScanItems];
     const int64_t base = (int64_t)blockIdx.x * kScanTile + (int64_t)threadIdx.x * kScanItems;
     load_items(count, base, M, c);
-    uint32_t off;
+    uint32_t v = 0;
     if (TOTALS) {
-        // (16-byte loads, at most kFuseTiles / 1024 of them per thread, all in flight together; tile_offsets[] is 256-byte
-        // aligned and padded to a multiple of 4 words by the caller's allocation of n_tiles + 1 words rounded up to 256 bytes)
-        uint32_t v = 0;
+        // (16-byte loads, at most kFuseTiles / 1024 of them per thread, all in flight together with the cells' loads;
+        // tile_offsets[] is 256-byte aligned and padded to a multiple of 4 words by the caller's allocation of n_tiles + 1
+        // words rounded up to 256 bytes)
 #pragma unroll
         for (int j = 0; j < kFuseTiles / (4 * kScanThreads); ++j) {
             const int t = 4 * (threadIdx.x + kScanThreads * j), nb = (int)blockIdx.x;
@@ -274,27 +275,29 @@ __global__ void __launch_bounds__(kScanThreads) k_scan_apply(const uint32_t* __r
                 v += q.x + (t + 1 < nb ? q.y : 0u) + (t + 2 < nb ? q.z : 0u) + (t + 3 < nb ? q.w : 0u);
             }
         }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = v;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            uint32_t t = 0;
-#pragma unroll
-            for (int q = 0; q < kScanThreads / 32; ++q) t += ws[q];
-            s_off = t;
-        }
-        __syncthreads();
-        off = s_off;
-        __syncthreads();   // ws is reused by the scan below
-    } else {
-        off = tile_offsets[blockIdx.x];
     }
+    const uint32_t off = TOTALS ? 0u : tile_offsets[blockIdx.x];   // (every thread: the load is in flight with the cells')
     uint32_t s = 0;
 #pragma unroll
     for (int q = 0; q < kScanItems; ++q) s += c[q];
-    uint32_t total;
-    uint32_t run = off + block_exclusive_scan(s, ws, total);
+    // ONE barrier: inclusive scan of s inside the warp, the warp's sum of v; then every thread adds up the (at most 8 + 8)
+    // per-warp words it needs
+    uint32_t inc = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 31) ws[w] = inc;
+    if (lane == 0) wv[w] = v;
+    __syncthreads();
+    uint32_t part = lane < kWarps ? ((lane < w ? ws[lane] : 0u) + wv[lane]) : 0u;
+#pragma unroll
+    for (int o = kWarps / 2; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+    part = __shfl_sync(0xffffffffu, part, 0);
+    uint32_t run = off + part + inc - s;
     uint32_t out[kScanItems];
 #pragma unroll
     for (int q = 0; q < kScanItems; ++q) {
