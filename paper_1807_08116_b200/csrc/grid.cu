@@ -151,31 +151,6 @@ constexpr int kScanItems = 16;
 constexpr int kScanTile = kScanThreads * kScanItems;   // 4096 cells per CTA
 static_assert(kScanTile == 1 << kTileShift, "k_key_hist's tile totals");
 
-__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* warp_sums, uint32_t& total) {
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    uint32_t inc = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= o) inc += t;
-    }
-    if (lane == 31) warp_sums[w] = inc;
-    __syncthreads();
-    if (w == 0) {
-        uint32_t s = lane < (kScanThreads / 32) ? warp_sums[lane] : 0u;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            uint32_t t = __shfl_up_sync(0xffffffffu, s, o);
-            if (lane >= o) s += t;
-        }
-        if (lane < (kScanThreads / 32)) warp_sums[lane] = s;   // inclusive over warps
-    }
-    __syncthreads();
-    total = warp_sums[kScanThreads / 32 - 1];
-    uint32_t base = w > 0 ? warp_sums[w - 1] : 0u;
-    return base + inc - v;
-}
-
 // tile layout: thread t owns cells [tile*4096 + 16 t, +16) — four uint4 loads, fully coalesced per warp
 __device__ __forceinline__ void load_items(const uint32_t* __restrict__ count, int64_t base, int64_t M,
                                            uint32_t (&c)[kScanItems]) {
